@@ -1,0 +1,175 @@
+/*
+ * nf.h — C ABI of the B200-native low-bit gradient-bucket aggregation library (libnf.so).
+ *
+ * The library implements the per-bucket hot path of NEURON-Fabric's DDP communication hook
+ * (§3.3, §5.2, §6.1), with the W workers' flat FP32 gradient
+ * buckets emulated as W replicas resident in one GPU's HBM (BASELINE.json north_star).
+ *
+ * Conventions (all entry points):
+ *  - Every pointer is a DEVICE pointer unless the argument is marked "host". The caller owns
+ *    every buffer; the library never allocates device memory and never synchronises.
+ *  - Every call only ENQUEUES work on `stream` (a cudaStream_t passed as void*; NULL = default
+ *    stream) and returns. Calls on one stream compose in order without host synchronisation.
+ *  - Return value: NF_OK (0) or a negative nf_status. Host-checkable errors (ranges, NULLs,
+ *    alignment, plan size) are detected before anything is launched. The bucket layout lives in
+ *    device memory, so layout errors (overlap, out of range, unsorted) are detected ON THE
+ *    DEVICE by nf_route_bucket: it writes NF_ERR_ARG into summary[NF_SUM_STATUS] and into the
+ *    plan, and every later call given that plan does nothing.
+ *  - Layout of a bucket: `n` FP32 elements per worker; worker w's bucket starts at
+ *    g + w*worker_stride (worker_stride >= n, in elements). Tensor t occupies
+ *    [off[t], off[t]+len[t]); tensors are in ascending order, non-overlapping, gaps allowed
+ *    (gap positions are never read or written). len[t] >= 0.
+ *  - Alignment: g, out, P, N must be 16-byte aligned (else NF_ERR_ALIGN). Tensor offsets and
+ *    strides may be arbitrary; tensors whose rows are not 16-byte aligned take a scalar path.
+ *  - Packed planes (reading #10): uint32 words, LSB = lowest element index, each L tensor starts
+ *    at word woff[t] and is padded with 0 bits to a word boundary; worker w's plane starts at
+ *    P + w*plane_stride (plane_stride >= Wd words).
+ *  - Outputs that accumulate (abs_sum, sumsq, nan_cnt, inf_cnt) are zeroed by the callee on the
+ *    same stream. `out` is written only at positions owned by the call (L tensors for
+ *    nf_sign_count_reduce, P/F tensors for nf_fp32_reduce), so the calls compose into one buffer.
+ *  - 1 <= W <= 255 (uint8 counts), 0 <= margin <= 255, 0 <= T <= NF_MAX_TENSORS; else NF_ERR_RANGE.
+ */
+#ifndef NF_H_
+#define NF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum nf_status {
+    NF_OK = 0,
+    NF_ERR_ARG = -1,    /* NULL where a pointer is required, bad mode, bad bucket layout, plan too small */
+    NF_ERR_ALIGN = -2,  /* a base pointer is not 16-byte aligned */
+    NF_ERR_RANGE = -3,  /* W, margin, T or n outside the supported range */
+    NF_ERR_CUDA = -4    /* a CUDA runtime call or kernel launch failed */
+} nf_status;
+
+/* Route codes: L = low-bit executed, F = FP32 fallback of an admitted route under
+ * veto / guard reject, P = plain FP32. */
+typedef enum nf_route { NF_ROUTE_P = 0, NF_ROUTE_L = 1, NF_ROUTE_F = 2 } nf_route;
+
+/* Low-bit payload formats: G-Binary = one-bit sign-count route; G-Ternary adds the
+ * zero-gating plane. */
+typedef enum nf_mode { NF_MODE_GBINARY = 1, NF_MODE_GTERNARY = 2 } nf_mode;
+
+/* Per-step controller state read by the hook, PAPER L143 steps (4) and (6): Commander admission,
+ * Supervisor veto, endpoint-capacity guard verdict. */
+typedef struct nf_state { int32_t admitted, veto, capacity_ok; } nf_state;
+
+#define NF_MAX_TENSORS 8192
+/* summary[] slots written by nf_route_bucket (8 x int64, device) */
+enum { NF_SUM_WD = 0, NF_SUM_NL = 1, NF_SUM_NF = 2, NF_SUM_NP = 3, NF_SUM_E = 4, NF_SUM_F = 5,
+       NF_SUM_TILES = 6, NF_SUM_STATUS = 7, NF_SUM_LEN = 8 };
+
+typedef void *nf_stream; /* cudaStream_t */
+
+const char *nf_status_string(int status);
+/* library version, e.g. 100 = 0.1.0 */
+int nf_version(void);
+
+/* Bytes of the device "plan" buffer nf_route_bucket fills for a bucket of T tensors (host call).
+ * The plan holds the route-dependent tile map the streaming kernels walk plus small scratch
+ * (per-tensor scales); it depends only on T. 16-byte aligned buffer required. */
+size_t nf_plan_bytes(int T);
+
+/* Bytes of the device workspace nf_aggregate_bucket needs for a bucket of n elements (host call):
+ * the 2-bit aggregate directions of the low-bit positions between its two passes. */
+size_t nf_workspace_bytes(int T, int64_t n);
+
+/*
+ * a1 Route — PAPER L108, L132, L143, L205, L229 (oracle O1).
+ * For each tensor: !admitted -> P; elig==0 -> P; veto or !capacity_ok -> F; else L.
+ * Outputs: route[T] (uint8 nf_route), woff[T] (first packed word of an L tensor = running sum of
+ * ceil(len/32) over L tensors in bucket order; -1 if not L), summary[NF_SUM_LEN] =
+ * {Wd, nL, nF, nP, e, f, n_tiles, status}, and the plan. One single-CTA kernel.
+ */
+int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
+                    nf_state state, uint8_t *route, int64_t *woff, int64_t *summary,
+                    void *plan, size_t plan_bytes, nf_stream stream);
+
+/*
+ * a2 Pack — PAPER L144, L211 (write-side payload materialisation; oracle O2).
+ * For each worker w and L tensor t: P bit = (x > tau_t), G-Ternary N bit = (x < -tau_t)
+ * (tau == NULL means 0; tau[t] >= 0 is the caller's contract), abs_sum[w*T+t] = sum |x| (FP64).
+ * abs_sum of non-L tensors is 0. N may be NULL iff mode == NF_MODE_GBINARY. Reads g once.
+ */
+int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
+                 const int64_t *off, const int64_t *len, const uint8_t *route, const int64_t *woff,
+                 int T, int mode, const float *tau,
+                 uint32_t *P, uint32_t *N, int64_t plane_stride, double *abs_sum,
+                 void *plan, nf_stream stream);
+
+/*
+ * a3 Sign-count reduce + decode — PAPER L211, L243, L247 (read-side aggregation; oracle O3).
+ * Per L element: cpos = popcount over the W pos-plane bits, cneg likewise over the neg plane
+ * (G-Binary: cneg = W - cpos); D = cpos - cneg; d = (D > margin) - (D < -margin);
+ * s_wt = (float)(abs_sum[w*T+t]/len_t); S_t = (float)(sum_w (double)s_wt / W);
+ * out[off_t+i] = S_t * (float)d. Optional: cpos/cneg [n] uint8 at bucket positions (L positions
+ * only are written), scale_out[T] (0 for non-L tensors).
+ */
+int nf_sign_count_reduce(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int W, int64_t n,
+                         const int64_t *off, const int64_t *len, const uint8_t *route,
+                         const int64_t *woff, int T, int mode, int margin, const double *abs_sum,
+                         float *out, uint8_t *cpos, uint8_t *cneg, float *scale_out,
+                         void *plan, nf_stream stream);
+
+/*
+ * a4a FP32 route — PAPER L50, L66, L144 (oracle O4a). For every P/F tensor:
+ * out[i] = alpha * (((g_0[i] + g_1[i]) + g_2[i]) + ... + g_{W-1}[i]) in FP32, fixed worker order.
+ */
+int nf_fp32_reduce(const float *g, int64_t worker_stride, int W, int64_t n,
+                   const int64_t *off, const int64_t *len, const uint8_t *route, int T,
+                   float alpha, float *out, void *plan, nf_stream stream);
+
+/*
+ * a4b Health statistics — BASELINE.json north_star step (4); consumer PAPER L158, L177 (oracle O4b).
+ * For every replica r < R and tensor t (any route): sumsq[r*T+t] = sum of x*x over finite x
+ * (FP64), nan_cnt = #NaN, inf_cnt = #+-Inf. L2 norm = sqrt(sumsq). R >= 1 (no upper bound).
+ */
+int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
+                    const int64_t *off, const int64_t *len, int T,
+                    double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                    void *plan, nf_stream stream);
+
+/*
+ * Fused path (the one the target is measured on) — same results as
+ * nf_route_bucket -> nf_sign_pack -> nf_sign_count_reduce -> nf_fp32_reduce -> nf_health_stats(g),
+ * with the W x n gradients read ONCE: pass A routes, packs, counts, votes, sums the FP32 tensors
+ * and gathers abs-sums and health statistics from a single read; pass B expands the 2-bit
+ * directions by the per-tensor scale. P and N may both be NULL (planes not materialised);
+ * sumsq/nan_cnt/inf_cnt may all be NULL (no health statistics); scale_out may be NULL.
+ * route/woff/summary/plan are outputs exactly as in nf_route_bucket.
+ */
+int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
+                        const int64_t *off, const int64_t *len, const uint8_t *elig, int T,
+                        nf_state state, int mode, const float *tau, int margin, float alpha,
+                        uint8_t *route, int64_t *woff, int64_t *summary,
+                        uint32_t *P, uint32_t *N, int64_t plane_stride,
+                        double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                        float *out, float *scale_out,
+                        void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
+                        nf_stream stream);
+
+/*
+ * End-to-end convenience with HOST buffers (used for the e2e measurement): copies W x n floats
+ * from pinned/pageable host memory `g_host` (worker stride = worker_stride elements) into the
+ * caller's device staging buffer `g_dev` (same stride), runs nf_aggregate_bucket with device
+ * metadata/outputs as above, and copies `out` (n floats) back to `out_host`. All copies are
+ * cudaMemcpyAsync on `stream`; the caller synchronises the stream.
+ */
+int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t worker_stride, int W,
+                             int64_t n, const int64_t *off, const int64_t *len, const uint8_t *elig,
+                             int T, nf_state state, int mode, const float *tau, int margin, float alpha,
+                             uint8_t *route, int64_t *woff, int64_t *summary,
+                             double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                             float *out, float *out_host /*host*/,
+                             void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
+                             nf_stream stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NF_H_ */

@@ -1,0 +1,177 @@
+"""Thin Python binding of libnf.so (include/nf.h): argument marshalling only.
+
+Every function has the name and argument order of its C entry point and takes torch CUDA
+tensors (or None for optional pointers); PyTorch is used for device memory and streams only.
+There is NO CPU fallback: if libnf.so is missing or fails to load, the first call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnf.so")
+
+NF_OK, NF_ERR_ARG, NF_ERR_ALIGN, NF_ERR_RANGE, NF_ERR_CUDA = 0, -1, -2, -3, -4
+ROUTE_P, ROUTE_L, ROUTE_F = 0, 1, 2
+MODE_GBINARY, MODE_GTERNARY = 1, 2
+SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = range(9)
+
+EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
+           "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host")
+
+
+class NfState(C.Structure):
+    _fields_ = [("admitted", C.c_int32), ("veto", C.c_int32), ("capacity_ok", C.c_int32)]
+
+
+class NfError(RuntimeError):
+    def __init__(self, fn: str, status: int):
+        self.status = status
+        super().__init__(f"{fn}: {status_string(status)} ({status})")
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libnf.so. Fails loudly: the product has no other implementation to fall back to."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_25759_b200.build` "
+                           "(there is no CPU or PyTorch fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, i32, sz, f32 = C.c_void_p, C.c_int64, C.c_int, C.c_size_t, C.c_float
+    L.nf_status_string.restype = C.c_char_p
+    L.nf_status_string.argtypes = [i32]
+    L.nf_version.restype = i32
+    L.nf_plan_bytes.restype = sz
+    L.nf_plan_bytes.argtypes = [i32]
+    L.nf_workspace_bytes.restype = sz
+    L.nf_workspace_bytes.argtypes = [i32, i64]
+    L.nf_route_bucket.restype = i32
+    L.nf_route_bucket.argtypes = [vp, vp, vp, i32, i64, NfState, vp, vp, vp, vp, sz, vp]
+    L.nf_sign_pack.restype = i32
+    L.nf_sign_pack.argtypes = [vp, i64, i32, i64, vp, vp, vp, vp, i32, i32, vp, vp, vp, i64, vp, vp, vp]
+    L.nf_sign_count_reduce.restype = i32
+    L.nf_sign_count_reduce.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, vp, i32, i32, i32, vp,
+                                       vp, vp, vp, vp, vp, vp]
+    L.nf_fp32_reduce.restype = i32
+    L.nf_fp32_reduce.argtypes = [vp, i64, i32, i64, vp, vp, vp, i32, f32, vp, vp, vp]
+    L.nf_health_stats.restype = i32
+    L.nf_health_stats.argtypes = [vp, i64, i32, i64, vp, vp, i32, vp, vp, vp, vp, vp]
+    L.nf_aggregate_bucket.restype = i32
+    L.nf_aggregate_bucket.argtypes = [vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32, f32,
+                                      vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp,
+                                      vp, sz, vp, sz, vp]
+    L.nf_aggregate_bucket_host.restype = i32
+    L.nf_aggregate_bucket_host.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32,
+                                           f32, vp, vp, vp, vp, vp, vp, vp, vp, vp,
+                                           vp, sz, vp, sz, vp]
+    _lib = L
+    return L
+
+
+def status_string(status: int) -> str:
+    return lib().nf_status_string(int(status)).decode()
+
+
+def _ptr(t: Optional[torch.Tensor], cuda: bool = True) -> Optional[int]:
+    if t is None:
+        return None
+    if cuda and not t.is_cuda:
+        raise TypeError("expected a CUDA tensor")
+    if not t.is_contiguous():
+        raise TypeError("expected a contiguous tensor")
+    return t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream or None
+    return int(stream) or None
+
+
+def _state(state) -> NfState:
+    if isinstance(state, NfState):
+        return state
+    a, v, c = state
+    return NfState(int(a), int(v), int(c))
+
+
+def _check(fn: str, rc: int):
+    if rc != NF_OK:
+        raise NfError(fn, rc)
+
+
+def nf_plan_bytes(T: int) -> int:
+    return int(lib().nf_plan_bytes(int(T)))
+
+
+def nf_workspace_bytes(T: int, n: int) -> int:
+    return int(lib().nf_workspace_bytes(int(T), int(n)))
+
+
+def nf_route_bucket(off, length, elig, T, n, state, route, woff, summary, plan, stream=None):
+    _check("nf_route_bucket", lib().nf_route_bucket(
+        _ptr(off), _ptr(length), _ptr(elig), int(T), int(n), _state(state), _ptr(route), _ptr(woff),
+        _ptr(summary), _ptr(plan), plan.numel() * plan.element_size(), _stream(stream)))
+
+
+def nf_sign_pack(g, worker_stride, W, n, off, length, route, woff, T, mode, tau, P, N, plane_stride,
+                 abs_sum, plan, stream=None):
+    _check("nf_sign_pack", lib().nf_sign_pack(
+        _ptr(g), int(worker_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(route), _ptr(woff),
+        int(T), int(mode), _ptr(tau), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(plan),
+        _stream(stream)))
+
+
+def nf_sign_count_reduce(P, N, plane_stride, W, n, off, length, route, woff, T, mode, margin, abs_sum,
+                         out, cpos, cneg, scale_out, plan, stream=None):
+    _check("nf_sign_count_reduce", lib().nf_sign_count_reduce(
+        _ptr(P), _ptr(N), int(plane_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(route),
+        _ptr(woff), int(T), int(mode), int(margin), _ptr(abs_sum), _ptr(out), _ptr(cpos), _ptr(cneg),
+        _ptr(scale_out), _ptr(plan), _stream(stream)))
+
+
+def nf_fp32_reduce(g, worker_stride, W, n, off, length, route, T, alpha, out, plan, stream=None):
+    _check("nf_fp32_reduce", lib().nf_fp32_reduce(
+        _ptr(g), int(worker_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(route), int(T),
+        float(alpha), _ptr(out), _ptr(plan), _stream(stream)))
+
+
+def nf_health_stats(x, replica_stride, R, n, off, length, T, sumsq, nan_cnt, inf_cnt, plan, stream=None):
+    _check("nf_health_stats", lib().nf_health_stats(
+        _ptr(x), int(replica_stride), int(R), int(n), _ptr(off), _ptr(length), int(T), _ptr(sumsq),
+        _ptr(nan_cnt), _ptr(inf_cnt), _ptr(plan), _stream(stream)))
+
+
+def nf_aggregate_bucket(g, worker_stride, W, n, off, length, elig, T, state, mode, tau, margin, alpha,
+                        route, woff, summary, P, N, plane_stride, abs_sum, sumsq, nan_cnt, inf_cnt,
+                        out, scale_out, plan, workspace, stream=None):
+    _check("nf_aggregate_bucket", lib().nf_aggregate_bucket(
+        _ptr(g), int(worker_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(elig), int(T),
+        _state(state), int(mode), _ptr(tau), int(margin), float(alpha), _ptr(route), _ptr(woff),
+        _ptr(summary), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt),
+        _ptr(inf_cnt), _ptr(out), _ptr(scale_out), _ptr(plan), plan.numel() * plan.element_size(),
+        _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, elig, T, state, mode, tau,
+                             margin, alpha, route, woff, summary, abs_sum, sumsq, nan_cnt, inf_cnt, out,
+                             out_host, plan, workspace, stream=None):
+    _check("nf_aggregate_bucket_host", lib().nf_aggregate_bucket_host(
+        _ptr(g_host, cuda=False), _ptr(g_dev), int(worker_stride), int(W), int(n), _ptr(off),
+        _ptr(length), _ptr(elig), int(T), _state(state), int(mode), _ptr(tau), int(margin), float(alpha),
+        _ptr(route), _ptr(woff), _ptr(summary), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt), _ptr(inf_cnt),
+        _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
+        _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))

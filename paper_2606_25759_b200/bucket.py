@@ -1,0 +1,83 @@
+"""Device-side buffers of one gradient bucket (memory plumbing only, no arithmetic).
+
+`BucketBuffers` owns the metadata tensors (off/len/elig), the outputs and the plan/workspace
+scratch that the C-ABI calls need for one bucket layout, so tests and bench.py do not repeat the
+allocation boilerplate. Every computation is done by the calls in `binding`.
+"""
+from __future__ import annotations
+
+from typing import Sequence
+
+import torch
+
+from . import binding as nf
+
+
+class BucketBuffers:
+    def __init__(self, off: Sequence[int], length: Sequence[int], elig: Sequence[int], n: int, W: int,
+                 device="cuda", planes: bool = True, counts: bool = False, health: bool = True,
+                 plane_stride: int | None = None):
+        dev = torch.device(device)
+        self.T, self.n, self.W = len(off), int(n), int(W)
+        T = max(self.T, 1)
+        self.off = torch.tensor(list(off), dtype=torch.int64, device=dev)
+        self.len = torch.tensor(list(length), dtype=torch.int64, device=dev)
+        self.elig = torch.tensor(list(elig), dtype=torch.uint8, device=dev)
+        self.route = torch.zeros(T, dtype=torch.uint8, device=dev)
+        self.woff = torch.zeros(T, dtype=torch.int64, device=dev)
+        self.summary = torch.zeros(nf.SUM_LEN, dtype=torch.int64, device=dev)
+        self.plan = torch.zeros(nf.nf_plan_bytes(self.T), dtype=torch.uint8, device=dev)
+        self.workspace = torch.zeros(nf.nf_workspace_bytes(self.T, self.n), dtype=torch.uint8, device=dev)
+        self.Wd_max = sum((int(l) + 31) // 32 for l in length)
+        ps = plane_stride if plane_stride is not None else (self.Wd_max + 3) // 4 * 4
+        self.plane_stride = max(ps, 4)
+        self.P = self.N = None
+        if planes:
+            self.P = torch.zeros((W, self.plane_stride), dtype=torch.int32, device=dev)
+            self.N = torch.zeros((W, self.plane_stride), dtype=torch.int32, device=dev)
+        self.abs_sum = torch.zeros((W, T), dtype=torch.float64, device=dev)
+        self.sumsq = self.nan_cnt = self.inf_cnt = None
+        if health:
+            self.sumsq = torch.zeros((W, T), dtype=torch.float64, device=dev)
+            self.nan_cnt = torch.zeros((W, T), dtype=torch.int64, device=dev)
+            self.inf_cnt = torch.zeros((W, T), dtype=torch.int64, device=dev)
+        self.out = torch.zeros(max(self.n, 4), dtype=torch.float32, device=dev)
+        self.scale = torch.zeros(T, dtype=torch.float32, device=dev)
+        self.cpos = self.cneg = None
+        if counts:
+            self.cpos = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=dev)
+            self.cneg = torch.zeros(max(self.n, 1), dtype=torch.uint8, device=dev)
+
+    # -- the five calls + the fused call, with this bucket's buffers filled in --------------------
+    def route_bucket(self, state, stream=None):
+        nf.nf_route_bucket(self.off, self.len, self.elig, self.T, self.n, state, self.route, self.woff,
+                           self.summary, self.plan, stream)
+
+    def sign_pack(self, g, worker_stride, mode, tau=None, stream=None):
+        nf.nf_sign_pack(g, worker_stride, self.W, self.n, self.off, self.len, self.route, self.woff,
+                        self.T, mode, tau, self.P, self.N if mode == nf.MODE_GTERNARY else None,
+                        self.plane_stride, self.abs_sum, self.plan, stream)
+
+    def sign_count_reduce(self, mode, margin=0, stream=None):
+        nf.nf_sign_count_reduce(self.P, self.N if mode == nf.MODE_GTERNARY else None, self.plane_stride,
+                                self.W, self.n, self.off, self.len, self.route, self.woff, self.T, mode,
+                                margin, self.abs_sum, self.out, self.cpos, self.cneg, self.scale,
+                                self.plan, stream)
+
+    def fp32_reduce(self, g, worker_stride, alpha=1.0, stream=None):
+        nf.nf_fp32_reduce(g, worker_stride, self.W, self.n, self.off, self.len, self.route, self.T,
+                          alpha, self.out, self.plan, stream)
+
+    def health_stats(self, x, replica_stride, R=None, stream=None):
+        nf.nf_health_stats(x, replica_stride, self.W if R is None else R, self.n, self.off, self.len,
+                           self.T, self.sumsq, self.nan_cnt, self.inf_cnt, self.plan, stream)
+
+    def aggregate(self, g, worker_stride, state=(1, 0, 1), mode=nf.MODE_GTERNARY, tau=None, margin=0,
+                  alpha=1.0, planes=None, stream=None):
+        use_planes = (self.P is not None) if planes is None else planes
+        nf.nf_aggregate_bucket(g, worker_stride, self.W, self.n, self.off, self.len, self.elig, self.T,
+                               state, mode, tau, margin, alpha, self.route, self.woff, self.summary,
+                               self.P if use_planes else None,
+                               self.N if (use_planes and mode == nf.MODE_GTERNARY) else None,
+                               self.plane_stride, self.abs_sum, self.sumsq, self.nan_cnt, self.inf_cnt,
+                               self.out, self.scale, self.plan, self.workspace, stream)

@@ -1,0 +1,218 @@
+// nf_api.cu — the extern "C" entry points declared in include/nf.h: argument checks that can be
+// made on the host, then kernel launches on the caller's stream. No allocation, no sync.
+#include "nf_internal.cuh"
+
+using namespace nf;
+
+namespace {
+
+inline bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NF_OK : NF_ERR_CUDA; }
+
+int check_common(int W, int64_t n, int T) {
+    if (W < 1 || W > 255) return NF_ERR_RANGE;
+    if (T < 0 || T > NF_MAX_TENSORS) return NF_ERR_RANGE;
+    if (n < 0 || n > ((int64_t)1 << 40)) return NF_ERR_RANGE;
+    return NF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *nf_status_string(int status) {
+    switch (status) {
+        case NF_OK: return "NF_OK";
+        case NF_ERR_ARG: return "NF_ERR_ARG: bad argument or bucket layout";
+        case NF_ERR_ALIGN: return "NF_ERR_ALIGN: base pointer not 16-byte aligned";
+        case NF_ERR_RANGE: return "NF_ERR_RANGE: W, margin, T or n out of range";
+        case NF_ERR_CUDA: return "NF_ERR_CUDA: CUDA runtime / launch failure";
+        default: return "unknown nf_status";
+    }
+}
+
+int nf_version(void) { return 100; }
+
+size_t nf_plan_bytes(int T) {
+    if (T < 0) T = 0;
+    return plan_layout(T).total;
+}
+
+size_t nf_workspace_bytes(int T, int64_t n) {
+    if (T < 0) T = 0;
+    if (n < 0) n = 0;
+    // one byte per 4 low-bit elements, each L tensor padded to a 32-element word: (n/32 + T) * 8
+    return align_up((size_t)(n / 32 + T + 1) * 8, 256);
+}
+
+int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
+                    nf_state state, uint8_t *route, int64_t *woff, int64_t *summary,
+                    void *plan, size_t plan_bytes, nf_stream stream) {
+    int rc = check_common(1, n, T);
+    if (rc != NF_OK) return rc;
+    if (!summary || !plan || plan_bytes < nf_plan_bytes(T)) return NF_ERR_ARG;
+    if (T > 0 && (!off || !len || !elig || !route || !woff)) return NF_ERR_ARG;
+    if (misaligned16(plan)) return NF_ERR_ALIGN;
+    return cuda_rc(launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
+                                nullptr, nullptr, nullptr, nullptr, 0, (cudaStream_t)stream));
+}
+
+int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
+                 const int64_t *off, const int64_t *len, const uint8_t *route, const int64_t *woff,
+                 int T, int mode, const float *tau,
+                 uint32_t *P, uint32_t *N, int64_t plane_stride, double *abs_sum,
+                 void *plan, nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!plan || !abs_sum || worker_stride < n || plane_stride < 0) return NF_ERR_ARG;
+    if (T > 0 && (!g || !off || !len || !route || !woff || !P)) return NF_ERR_ARG;
+    if (mode == NF_MODE_GTERNARY && T > 0 && !N) return NF_ERR_ARG;
+    if (misaligned16(g) || misaligned16(P) || misaligned16(N) || misaligned16(plan)) return NF_ERR_ALIGN;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (T == 0) return NF_OK;
+    if (cudaMemsetAsync(abs_sum, 0, sizeof(double) * (size_t)W * T, s) != cudaSuccess) return NF_ERR_CUDA;
+    StreamParams p{};
+    p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
+    p.off = off; p.len = len; p.route = route; p.woff = woff;
+    p.ternary = (mode == NF_MODE_GTERNARY); p.tau = tau;
+    p.P = P; p.N = N; p.plane_stride = plane_stride; p.abs_sum = abs_sum; p.plan = plan;
+    return cuda_rc(launch_stream(kFPack, p, n, s));
+}
+
+int nf_sign_count_reduce(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int W, int64_t n,
+                         const int64_t *off, const int64_t *len, const uint8_t *route,
+                         const int64_t *woff, int T, int mode, int margin, const double *abs_sum,
+                         float *out, uint8_t *cpos, uint8_t *cneg, float *scale_out,
+                         void *plan, nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (margin < 0 || margin > 255) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!plan || plane_stride < 0) return NF_ERR_ARG;
+    if (T > 0 && (!P || !off || !len || !route || !woff || !abs_sum || !out)) return NF_ERR_ARG;
+    if (mode == NF_MODE_GTERNARY && T > 0 && !N) return NF_ERR_ARG;
+    if (misaligned16(P) || misaligned16(N) || misaligned16(out) || misaligned16(plan)) return NF_ERR_ALIGN;
+    if (T == 0) return NF_OK;
+    ReduceParams p{};
+    p.P = P; p.N = N; p.plane_stride = plane_stride; p.W = W; p.T = T;
+    p.off = off; p.len = len; p.route = route; p.woff = woff;
+    p.ternary = (mode == NF_MODE_GTERNARY); p.margin = margin; p.abs_sum = abs_sum;
+    p.out = out; p.cpos = cpos; p.cneg = cneg; p.scale_out = scale_out; p.plan = plan;
+    return cuda_rc(launch_count_reduce(p, n, (cudaStream_t)stream));
+}
+
+int nf_fp32_reduce(const float *g, int64_t worker_stride, int W, int64_t n,
+                   const int64_t *off, const int64_t *len, const uint8_t *route, int T,
+                   float alpha, float *out, void *plan, nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (!plan || worker_stride < n) return NF_ERR_ARG;
+    if (T > 0 && (!g || !off || !len || !route || !out)) return NF_ERR_ARG;
+    if (misaligned16(g) || misaligned16(out) || misaligned16(plan)) return NF_ERR_ALIGN;
+    if (T == 0) return NF_OK;
+    StreamParams p{};
+    p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
+    p.off = off; p.len = len; p.route = route; p.alpha = alpha; p.out = out; p.plan = plan;
+    return cuda_rc(launch_stream(kFFp32, p, n, (cudaStream_t)stream));
+}
+
+int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
+                    const int64_t *off, const int64_t *len, int T,
+                    double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                    void *plan, nf_stream stream) {
+    if (R < 1 || R > (1 << 20)) return NF_ERR_RANGE;
+    int rc = check_common(1, n, T);
+    if (rc != NF_OK) return rc;
+    if (!plan || replica_stride < n || !sumsq || !nan_cnt || !inf_cnt) return NF_ERR_ARG;
+    if (T > 0 && (!x || !off || !len)) return NF_ERR_ARG;
+    if (misaligned16(x) || misaligned16(plan)) return NF_ERR_ALIGN;
+    if (T == 0) return NF_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t cnt = (size_t)R * T;
+    if (cudaMemsetAsync(sumsq, 0, sizeof(double) * cnt, s) != cudaSuccess ||
+        cudaMemsetAsync(nan_cnt, 0, sizeof(uint64_t) * cnt, s) != cudaSuccess ||
+        cudaMemsetAsync(inf_cnt, 0, sizeof(uint64_t) * cnt, s) != cudaSuccess)
+        return NF_ERR_CUDA;
+    StreamParams p{};
+    p.g = x; p.worker_stride = replica_stride; p.W = R; p.T = T;
+    p.off = off; p.len = len; p.route = nullptr;
+    p.sumsq = sumsq; p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
+    p.plan = plan;
+    return cuda_rc(launch_stream(kFHealth, p, n, s));
+}
+
+int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
+                        const int64_t *off, const int64_t *len, const uint8_t *elig, int T,
+                        nf_state state, int mode, const float *tau, int margin, float alpha,
+                        uint8_t *route, int64_t *woff, int64_t *summary,
+                        uint32_t *P, uint32_t *N, int64_t plane_stride,
+                        double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                        float *out, float *scale_out,
+                        void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
+                        nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (margin < 0 || margin > 255) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!summary || !plan || plan_bytes < nf_plan_bytes(T)) return NF_ERR_ARG;
+    if (!workspace || workspace_bytes < nf_workspace_bytes(T, n)) return NF_ERR_ARG;
+    if (worker_stride < n || plane_stride < 0 || !abs_sum) return NF_ERR_ARG;
+    if (T > 0 && (!g || !off || !len || !elig || !route || !woff || !out)) return NF_ERR_ARG;
+    if (P && mode == NF_MODE_GTERNARY && !N) return NF_ERR_ARG;
+    const bool health = sumsq || nan_cnt || inf_cnt;
+    if (health && !(sumsq && nan_cnt && inf_cnt)) return NF_ERR_ARG;
+    if (misaligned16(g) || misaligned16(out) || misaligned16(P) || misaligned16(N) ||
+        misaligned16(plan) || misaligned16(workspace))
+        return NF_ERR_ALIGN;
+    cudaStream_t s = (cudaStream_t)stream;
+    // a1 (+ zeroing of the accumulators, so no memset nodes sit on the stream)
+    cudaError_t e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
+                                 abs_sum, sumsq, (unsigned long long *)nan_cnt,
+                                 (unsigned long long *)inf_cnt, (int64_t)W * T, s);
+    if (e != cudaSuccess) return NF_ERR_CUDA;
+    if (T == 0 || n == 0) return NF_OK;
+    // pass A: one read of the W x n gradients
+    StreamParams p{};
+    p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
+    p.off = off; p.len = len; p.route = route; p.woff = woff;
+    p.ternary = (mode == NF_MODE_GTERNARY); p.tau = tau; p.margin = margin; p.alpha = alpha;
+    p.P = P; p.N = N; p.plane_stride = plane_stride;
+    p.abs_sum = abs_sum; p.sumsq = sumsq;
+    p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
+    p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
+    e = launch_stream(health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32), p, n, s);
+    if (e != cudaSuccess) return NF_ERR_CUDA;
+    // pass B: scale x direction for the low-bit positions
+    ReduceParams r{};
+    r.W = W; r.T = T; r.off = off; r.len = len; r.route = route; r.woff = woff;
+    r.abs_sum = abs_sum; r.out = out; r.scale_out = scale_out;
+    r.dirs = (const uint8_t *)workspace; r.plan = plan;
+    return cuda_rc(launch_decode(r, n, s));
+}
+
+int nf_aggregate_bucket_host(const float *g_host, float *g_dev, int64_t worker_stride, int W,
+                             int64_t n, const int64_t *off, const int64_t *len, const uint8_t *elig,
+                             int T, nf_state state, int mode, const float *tau, int margin, float alpha,
+                             uint8_t *route, int64_t *woff, int64_t *summary,
+                             double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                             float *out, float *out_host,
+                             void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
+                             nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (!g_host || !g_dev || !out_host || worker_stride < n) return NF_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (cudaMemcpyAsync(g_dev, g_host, sizeof(float) * (size_t)worker_stride * W,
+                        cudaMemcpyHostToDevice, s) != cudaSuccess)
+        return NF_ERR_CUDA;
+    rc = nf_aggregate_bucket(g_dev, worker_stride, W, n, off, len, elig, T, state, mode, tau, margin,
+                             alpha, route, woff, summary, nullptr, nullptr, 0, abs_sum, sumsq, nan_cnt,
+                             inf_cnt, out, nullptr, plan, plan_bytes, workspace, workspace_bytes, stream);
+    if (rc != NF_OK) return rc;
+    if (cudaMemcpyAsync(out_host, out, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return NF_ERR_CUDA;
+    return NF_OK;
+}
+
+}  // extern "C"

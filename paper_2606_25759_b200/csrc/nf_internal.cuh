@@ -1,0 +1,173 @@
+// nf_internal.cuh — internal declarations shared by the libnf translation units (sm_100a).
+// Not part of the public ABI (that is include/nf.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "nf.h"
+
+namespace nf {
+
+// ---------------------------------------------------------------------------------------------
+// Work decomposition. A *tile* is NF_TILE consecutive elements of ONE tensor, in tensor-relative
+// index space (so bit j of packed word k is always lane-aligned, whatever off[t] is). The plan's
+// tile_prefix[t] is the exclusive prefix of ceil(len[t]/NF_TILE) over ALL tensors in bucket order;
+// persistent CTAs walk tiles blockIdx.x, blockIdx.x+gridDim.x, ... and find the tensor of a tile
+// by binary search in tile_prefix (T+1 ints, L1/L2 resident).
+// ---------------------------------------------------------------------------------------------
+constexpr int kThreads = 256;              // threads per CTA of the streaming kernels
+constexpr int kRows = 2;                   // float4 rows per thread per tile
+constexpr int kRowElems = kThreads * 4;    // 1024 elements per row
+constexpr int kTile = kRows * kRowElems;   // 2048 elements per tile
+constexpr int kGroup = 8;                  // workers per register group (8 x 4-bit nibbles = 32 bits)
+constexpr uint32_t kPlanMagic = 0x4e46504cu;  // "NFPL"
+
+struct PlanHeader {                        // 64 bytes, at plan + 0
+    uint32_t magic;
+    int32_t status;                        // NF_OK or NF_ERR_ARG (bad layout): later kernels no-op
+    int32_t T;
+    int32_t nL;
+    int64_t n;
+    int64_t Wd;                            // total packed words per worker plane
+    int32_t n_tiles;
+    int32_t pad0;
+    int64_t pad1[3];
+};
+
+// Offsets (bytes) of the plan arrays for a bucket of T tensors.
+struct PlanLayout {
+    size_t tile_prefix;                    // int32 [T+1]
+    size_t lt_index;                       // int32 [T]     ids of the L tensors, in order
+    size_t lt_woff;                        // int64 [T+1]   woff of the L tensors, lt_woff[nL] = Wd
+    size_t scale;                          // float [T]     per-tensor scale scratch
+    size_t total;
+};
+
+__host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+__host__ __device__ inline PlanLayout plan_layout(int T) {
+    PlanLayout L;
+    size_t o = sizeof(PlanHeader);
+    L.tile_prefix = o; o = align_up(o + sizeof(int32_t) * (size_t)(T + 1), 16);
+    L.lt_index = o;    o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
+    L.lt_woff = o;     o = align_up(o + sizeof(int64_t) * (size_t)(T + 1), 16);
+    L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
+    L.total = o;
+    return L;
+}
+
+struct PlanView {
+    const PlanHeader *hdr;
+    const int32_t *tile_prefix;
+    const int32_t *lt_index;
+    const int64_t *lt_woff;
+    float *scale;
+};
+
+__host__ __device__ inline PlanView plan_view(void *plan, int T) {
+    PlanLayout L = plan_layout(T);
+    char *p = (char *)plan;
+    PlanView v;
+    v.hdr = (const PlanHeader *)p;
+    v.tile_prefix = (const int32_t *)(p + L.tile_prefix);
+    v.lt_index = (const int32_t *)(p + L.lt_index);
+    v.lt_woff = (const int64_t *)(p + L.lt_woff);
+    v.scale = (float *)(p + L.scale);
+    return v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Parameters of the streaming kernel family (pack / fp32 / health / fused pass A).
+// ---------------------------------------------------------------------------------------------
+struct StreamParams {
+    const float *g;            // [W][worker_stride]
+    int64_t worker_stride;
+    int W;
+    int T;
+    const int64_t *off;
+    const int64_t *len;
+    const uint8_t *route;      // NULL for health-only (all tensors processed, no route semantics)
+    const int64_t *woff;
+    int ternary;               // mode == NF_MODE_GTERNARY
+    const float *tau;          // [T] or NULL
+    int margin;
+    float alpha;
+    uint32_t *P;               // may be NULL (planes not materialised)
+    uint32_t *N;
+    int64_t plane_stride;
+    double *abs_sum;           // [W][T]
+    double *sumsq;             // [W][T] or NULL
+    unsigned long long *nan_cnt;
+    unsigned long long *inf_cnt;
+    float *out;                // [n]
+    uint8_t *dirs;             // workspace: one byte per 4 low-bit elements (lo nibble +, hi nibble -)
+    void *plan;
+};
+
+enum : int {
+    kFPack = 1,     // L tiles: bit planes + abs-sum
+    kFCount = 2,    // L tiles: per-position counts -> majority direction -> dirs
+    kFFp32 = 4,     // non-L tiles: fixed-order FP32 sum -> out
+    kFHealth = 8    // all tiles: sum of squares over finite values, NaN / Inf tallies
+};
+
+struct ReduceParams {
+    const uint32_t *P;
+    const uint32_t *N;
+    int64_t plane_stride;
+    int W;
+    int T;
+    const int64_t *off;
+    const int64_t *len;
+    const uint8_t *route;
+    const int64_t *woff;
+    int ternary;
+    int margin;
+    const double *abs_sum;
+    float *out;
+    uint8_t *cpos;
+    uint8_t *cneg;
+    float *scale_out;
+    const uint8_t *dirs;       // decode pass of the fused path
+    void *plan;
+};
+
+// launchers (each returns a cudaError_t from the launch)
+cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
+                         nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
+                         double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
+                         int64_t zcount, cudaStream_t s);
+cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStream_t s);
+cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s);
+cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s);
+int device_sm_count();
+
+// ---------------------------------------------------------------------------------------------
+// Device helpers
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+// largest t in [0,T) with prefix[t] <= x  (prefix is non-decreasing, prefix[0] = 0, x < prefix[T])
+template <typename I>
+__device__ __forceinline__ int upper_tensor(const I *__restrict__ prefix, int T, I x) {
+    int lo = 0, hi = T;                    // invariant: prefix[lo] <= x < prefix[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(prefix + mid) <= x) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// S_t = (float)( sum_w (double)(float)(A[w][t]/len_t) / W )   — PAPER L211 "mean-absolute scale",
+// combined over workers by a fixed-order FP64 mean (readings #7, #8).
+__device__ __forceinline__ float tensor_scale(const double *__restrict__ abs_sum, int W, int T, int t,
+                                              int64_t len_t) {
+    double s = 0.0;
+    const double dl = (double)len_t;
+    for (int w = 0; w < W; ++w) {
+        float swt = (float)(abs_sum[(size_t)w * T + t] / dl);
+        s += (double)swt;
+    }
+    return (float)(s / (double)W);
+}
+#endif
+
+}  // namespace nf

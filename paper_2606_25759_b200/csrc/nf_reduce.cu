@@ -1,0 +1,274 @@
+// nf_reduce.cu — step a3 (reducer-side compact sign-count aggregation + decode) and pass B of the
+// fused path (expand 2-bit directions by the per-tensor scale). PAPER §5.2 L211 ("sum these
+// indicators across workers ... majority voting ... writes the scaled aggregate direction back"),
+// §6.1 L247 ("recovering per-coordinate sign counts rather than numerically adding packed
+// machine words"), L76 (endpoint service = counting compact updates under fan-in W).
+//
+// a3 is a positional popcount over the W packed words of each word position. One thread owns one
+// word position (32 elements): it streams the W words (coalesced across the warp, 8 independent
+// loads in flight) through a bit-sliced carry-save adder tree (Harley-Seal style: 7 full adders
+// per 8 words, ~3 LOP3 per word), which leaves the per-element counts as 8 bit-planes; the
+// majority test with margin is then a bit-sliced compare that decides 32 elements at once.
+// The FP32 output is written warp-cooperatively (lane = element) so stores are 128-byte coalesced.
+#include "nf_internal.cuh"
+
+namespace nf {
+
+constexpr int kRThreads = 256;
+
+// full adder on 32 bit-lanes: 2 LOP3
+__device__ __forceinline__ void csa(uint32_t &carry, uint32_t &sum, uint32_t a, uint32_t b, uint32_t c) {
+    sum = a ^ b ^ c;
+    carry = (a & b) | (a & c) | (b & c);
+}
+
+// Bit-sliced counter: c[b] is the 2^b digit of 32 independent counts (<= 255).
+struct SlicedCounter {
+    uint32_t c[8];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int b = 0; b < 8; ++b) c[b] = 0u;
+    }
+    // add `x` (a bit-plane of weight 2^from) with ripple carry into planes from..7
+    template <int FROM>
+    __device__ __forceinline__ void add_plane(uint32_t x) {
+#pragma unroll
+        for (int b = FROM; b < 8; ++b) {
+            const uint32_t t = c[b] & x;
+            c[b] ^= x;
+            x = t;
+        }
+    }
+    // add 8 one-bit words: 7 CSAs down to one weight-8 plane (+ the running 1/2/4 planes)
+    __device__ __forceinline__ void add8(const uint32_t (&x)[8]) {
+        uint32_t t2a, t2b, t2c, t2d, t4a, t4b, t8;
+        csa(t2a, c[0], c[0], x[0], x[1]);
+        csa(t2b, c[0], c[0], x[2], x[3]);
+        csa(t4a, c[1], c[1], t2a, t2b);
+        csa(t2c, c[0], c[0], x[4], x[5]);
+        csa(t2d, c[0], c[0], x[6], x[7]);
+        csa(t4b, c[1], c[1], t2c, t2d);
+        csa(t8, c[2], c[2], t4a, t4b);
+        add_plane<3>(t8);
+    }
+};
+
+// gt = (a > b) bitwise over 32 lanes; a has 8 planes, b has 9 planes (b may exceed 255)
+__device__ __forceinline__ uint32_t sliced_gt(const uint32_t (&a)[8], const uint32_t (&b)[9]) {
+    uint32_t gt = 0u, eq = ~b[8];            // a's plane 8 is zero: if b[8] is set, a < b
+#pragma unroll
+    for (int k = 7; k >= 0; --k) {
+        gt |= eq & a[k] & ~b[k];
+        eq &= ~(a[k] ^ b[k]);
+    }
+    return gt;
+}
+
+// b = a + m (m <= 255 constant across lanes), 9 planes
+__device__ __forceinline__ void sliced_add_const(const uint32_t (&a)[8], int m, uint32_t (&b)[9]) {
+    uint32_t carry = 0u;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const uint32_t mk = ((m >> k) & 1) ? 0xffffffffu : 0u;
+        b[k] = a[k] ^ mk ^ carry;
+        carry = (a[k] & mk) | (a[k] & carry) | (mk & carry);
+    }
+    b[8] = carry;
+}
+
+__device__ __forceinline__ void const_planes(int v, uint32_t (&b)[9]) {
+#pragma unroll
+    for (int k = 0; k < 9; ++k) b[k] = ((v >> k) & 1) ? 0xffffffffu : 0u;
+}
+
+// Stream the W words of word position k of one plane into a sliced counter.
+__device__ __forceinline__ void count_words(const uint32_t *__restrict__ base, int64_t stride, int W,
+                                            SlicedCounter &sc) {
+    sc.clear();
+    int w = 0;
+    for (; w + 8 <= W; w += 8) {
+        uint32_t x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = __ldcs(base + (size_t)(w + i) * stride);
+        sc.add8(x);
+    }
+    if (w < W) {
+        uint32_t x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = (w + i < W) ? __ldcs(base + (size_t)(w + i) * stride) : 0u;
+        sc.add8(x);
+    }
+}
+
+// every CTA computes the scales of the L tensors it may touch into shared memory; CTA 0 publishes
+__device__ __forceinline__ void compute_scales(const ReduceParams &p, const PlanView &pv, float *s_scale) {
+    for (int t = threadIdx.x; t < p.T; t += blockDim.x) {
+        float S = 0.f;
+        if (p.route[t] == NF_ROUTE_L) S = tensor_scale(p.abs_sum, p.W, p.T, t, p.len[t]);
+        s_scale[t] = S;
+        if (blockIdx.x == 0) {
+            pv.scale[t] = S;
+            if (p.scale_out) p.scale_out[t] = S;
+        }
+    }
+    __syncthreads();
+}
+
+template <bool WRITE_COUNTS>
+__global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReduceParams p) {
+    extern __shared__ float s_scale[];
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    compute_scales(p, pv, s_scale);
+    const int64_t Wd = pv.hdr->Wd;
+    const int nL = pv.hdr->nL;
+    const int lane = threadIdx.x & 31;
+    const int W = p.W;
+    const int64_t n_chunks = (Wd + kRThreads - 1) / kRThreads;
+
+    for (int64_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+        const int64_t k = chunk * kRThreads + threadIdx.x;      // global word position
+        uint32_t dpos = 0u, dneg = 0u;
+        int nvalid = 0;
+        int64_t obase = 0;
+        float S = 0.f;
+        SlicedCounter cpv, cnv;
+        cpv.clear(); cnv.clear();
+        if (k < Wd) {
+            const int li = upper_tensor<int64_t>(pv.lt_woff, nL, k);
+            const int t = __ldg(pv.lt_index + li);
+            const int64_t i0 = (k - __ldg(pv.lt_woff + li)) * 32;  // tensor-relative first element
+            const int64_t rem = __ldg(p.len + t) - i0;
+            nvalid = rem >= 32 ? 32 : (int)rem;
+            obase = __ldg(p.off + t) + i0;
+            S = s_scale[t];
+            count_words(p.P + k, p.plane_stride, W, cpv);
+            if (p.ternary) {
+                count_words(p.N + k, p.plane_stride, W, cnv);
+                // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
+                uint32_t b[9];
+                sliced_add_const(cnv.c, p.margin, b);
+                dpos = sliced_gt(cpv.c, b);
+                sliced_add_const(cpv.c, p.margin, b);
+                dneg = sliced_gt(cnv.c, b);
+            } else {
+                // G-Binary: cneg = W - cpos; D = 2 cpos - W.  d+ : cpos > floor((W+m)/2);
+                // d- : cpos < ceil((W-m)/2)  (never if W <= m)
+                uint32_t b[9], a9[9];
+                const_planes((W + p.margin) >> 1, b);
+                dpos = sliced_gt(cpv.c, b);
+                const int k2 = (W > p.margin) ? (W - p.margin + 1) >> 1 : 0;
+                // k2 > cpos  <=>  const(k2) > cpos : compare with roles swapped
+                uint32_t ka[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) { ka[q] = ((k2 >> q) & 1) ? 0xffffffffu : 0u; a9[q] = cpv.c[q]; }
+                a9[8] = 0u;
+                dneg = sliced_gt(ka, a9);
+            }
+            const uint32_t vmask = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+            dpos &= vmask;
+            dneg &= vmask;
+        }
+        // warp-cooperative, coalesced write-back: iteration j handles the word of lane j
+#pragma unroll 4
+        for (int j = 0; j < 32; ++j) {
+            const int nv = __shfl_sync(0xffffffffu, nvalid, j);
+            if (nv == 0) continue;                               // warp-uniform
+            const uint32_t dp = __shfl_sync(0xffffffffu, dpos, j);
+            const uint32_t dn = __shfl_sync(0xffffffffu, dneg, j);
+            const int64_t ob = __shfl_sync(0xffffffffu, obase, j);
+            const float Sj = __shfl_sync(0xffffffffu, S, j);
+            const int d = (int)((dp >> lane) & 1u) - (int)((dn >> lane) & 1u);
+            if (lane < nv) p.out[ob + lane] = __fmul_rn(Sj, (float)d);
+            if (WRITE_COUNTS) {
+                uint32_t c1 = 0u, c2 = 0u;
+#pragma unroll
+                for (int b = 0; b < 8; ++b) {
+                    c1 |= ((__shfl_sync(0xffffffffu, cpv.c[b], j) >> lane) & 1u) << b;
+                    c2 |= ((__shfl_sync(0xffffffffu, cnv.c[b], j) >> lane) & 1u) << b;
+                }
+                if (!p.ternary) c2 = (uint32_t)W - c1;
+                if (lane < nv) {
+                    if (p.cpos) p.cpos[ob + lane] = (uint8_t)c1;
+                    if (p.cneg) p.cneg[ob + lane] = (uint8_t)c2;
+                }
+            }
+        }
+    }
+}
+
+// Pass B of the fused path: out[off_t+i] = S_t * d for every low-bit element, d from the 2-bit
+// directions pass A left in the workspace (one byte per 4 elements: low nibble +, high nibble -).
+__global__ void __launch_bounds__(kRThreads) decode_kernel(const ReduceParams p) {
+    extern __shared__ float s_scale[];
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    compute_scales(p, pv, s_scale);
+    const int n_tiles = pv.hdr->n_tiles;
+    int t = -1, tile_b = 0, tile_e = 0;
+    int64_t off_t = 0, len_t = 0, woff_t = 0;
+    bool isL = false;
+    float S = 0.f;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (tile >= tile_e) {
+            t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
+            tile_b = __ldg(pv.tile_prefix + t);
+            tile_e = __ldg(pv.tile_prefix + t + 1);
+            off_t = __ldg(p.off + t);
+            len_t = __ldg(p.len + t);
+            isL = __ldg(p.route + t) == NF_ROUTE_L;
+            woff_t = isL ? __ldg(p.woff + t) : 0;
+            S = s_scale[t];
+        }
+        if (!isL) continue;
+        const int64_t tb = (int64_t)(tile - tile_b) * kTile;
+        const bool al = (off_t & 3) == 0;
+#pragma unroll
+        for (int u = 0; u < kTile / (kRThreads * 4); ++u) {
+            const int64_t i = tb + (int64_t)u * kRThreads * 4 + threadIdx.x * 4;
+            const int64_t rem = len_t - i;
+            if (rem <= 0) continue;
+            const uint32_t d = __ldcs(p.dirs + (size_t)woff_t * 8 + (size_t)(i >> 2));
+            float4 r;
+            r.x = __fmul_rn(S, (float)((int)(d & 1u) - (int)((d >> 4) & 1u)));
+            r.y = __fmul_rn(S, (float)((int)((d >> 1) & 1u) - (int)((d >> 5) & 1u)));
+            r.z = __fmul_rn(S, (float)((int)((d >> 2) & 1u) - (int)((d >> 6) & 1u)));
+            r.w = __fmul_rn(S, (float)((int)((d >> 3) & 1u) - (int)((d >> 7) & 1u)));
+            float *o = p.out + off_t + i;
+            if (rem >= 4 && al) {
+                __stcs(reinterpret_cast<float4 *>(o), r);
+            } else {
+                o[0] = r.x;
+                if (rem > 1) o[1] = r.y;
+                if (rem > 2) o[2] = r.z;
+                if (rem > 3) o[3] = r.w;
+            }
+        }
+    }
+}
+
+static int grid_for(int64_t units, int per_sm) {
+    int64_t g = (int64_t)device_sm_count() * per_sm;
+    if (g > units) g = units;
+    return (int)(g < 1 ? 1 : g);
+}
+
+cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s) {
+    const int64_t max_words = n / 32 + p.T;
+    const int64_t chunks = (max_words + kRThreads - 1) / kRThreads;
+    const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
+    const int grid = grid_for(chunks, 8);
+    if (p.cpos || p.cneg) count_reduce_kernel<true><<<grid, kRThreads, smem, s>>>(p);
+    else count_reduce_kernel<false><<<grid, kRThreads, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s) {
+    const int64_t max_tiles = n / kTile + p.T;
+    const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
+    const int grid = grid_for(max_tiles, 8);
+    decode_kernel<<<grid, kRThreads, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace nf

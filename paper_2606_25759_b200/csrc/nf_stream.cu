@@ -1,0 +1,380 @@
+// nf_stream.cu — the streaming kernel family: steps a2 (pack), a4a (FP32 route), a4b (health) and
+// pass A of the fused path (route-aware pack + sign count + majority vote + FP32 sum + health from
+// ONE read of the W x n gradients). PAPER §5.2, §3.3; SURVEY §8(a).
+//
+// HBM-bound elementwise streaming (no contraction -> no tensor cores). Design for sm_100a:
+//  * persistent grid (multiple of the SM count), CTAs walk tiles of ONE tensor (tensor-relative
+//    index space), so packed bit j of word k is lane-aligned for any tensor offset;
+//  * each thread owns 4 consecutive elements per row and loads them from up to 8 workers with
+//    128-bit streaming loads (16 independent 16-byte requests in flight per thread);
+//  * sign bits are built as one 4-bit nibble per worker in a single register (8 workers x 4 bits);
+//    per-position counts are popcounts of that register under a 0x11111111 mask, and the packed
+//    32-bit plane words come from an 8x8 nibble transpose across 8 lanes (3 shuffles);
+//  * per-(worker,tensor) abs-sum / sum-of-squares run in FP32 over 8 elements, then FP64 per
+//    thread, one block reduce-scatter + FP64 atomics per tensor change.
+#include <float.h>
+#include "nf_internal.cuh"
+
+namespace nf {
+
+__device__ __forceinline__ float4 ld_stream4(const float *p) {
+    return __ldcs(reinterpret_cast<const float4 *>(p));
+}
+
+// Load 4 consecutive floats of which the first `valid` exist; missing ones read as +0.
+__device__ __forceinline__ float4 load4(const float *p, int valid, bool aligned) {
+    if (valid == 4 && aligned) return ld_stream4(p);
+    float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (valid > 0) r.x = __ldcs(p);
+    if (valid > 1) r.y = __ldcs(p + 1);
+    if (valid > 2) r.z = __ldcs(p + 2);
+    if (valid > 3) r.w = __ldcs(p + 3);
+    return r;
+}
+
+// 8x8 transpose of 4-bit elements held one row per lane across each aligned group of 8 lanes:
+// in : lane q holds nibble u = M[q][u];   out: lane q holds nibble q' = M[q'][q].
+__device__ __forceinline__ uint32_t nibble_transpose8(uint32_t v, int lane) {
+    uint32_t t = __shfl_xor_sync(0xffffffffu, v, 4);
+    v = (lane & 4) ? ((v & 0xffff0000u) | (t >> 16)) : ((v & 0x0000ffffu) | (t << 16));
+    t = __shfl_xor_sync(0xffffffffu, v, 2);
+    v = (lane & 2) ? ((v & 0xff00ff00u) | ((t & 0xff00ff00u) >> 8))
+                   : ((v & 0x00ff00ffu) | ((t & 0x00ff00ffu) << 8));
+    t = __shfl_xor_sync(0xffffffffu, v, 1);
+    v = (lane & 1) ? ((v & 0xf0f0f0f0u) | ((t & 0xf0f0f0f0u) >> 4))
+                   : ((v & 0x0f0f0f0fu) | ((t & 0x0f0f0f0fu) << 4));
+    return v;
+}
+
+// Warp reduce-scatter of 16 doubles: on return v[0] of lane l holds the warp total of value
+// idx(l) = 8*bit4 + 4*bit3 + 2*bit2 + bit1 (lanes l and l^1 hold the same value). Fixed order.
+__device__ __forceinline__ void warp_reduce_scatter16(double (&v)[16], int lane) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const bool hi = lane & 16;
+        double send = hi ? v[i] : v[i + 8], keep = hi ? v[i + 8] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const bool hi = lane & 8;
+        double send = hi ? v[i] : v[i + 4], keep = hi ? v[i + 4] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const bool hi = lane & 4;
+        double send = hi ? v[i] : v[i + 2], keep = hi ? v[i + 2] : v[i];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    {
+        const bool hi = lane & 2;
+        double send = hi ? v[0] : v[1], keep = hi ? v[1] : v[0];
+        v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+    }
+    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+}
+
+struct FlushCtx {
+    double (*s_red)[16];
+    unsigned int *s_nan;
+    unsigned int *s_inf;
+};
+
+// Block-reduce the per-thread FP64 partials of one worker group and add them to the global
+// per-(worker,tensor) accumulators. CTA-uniform call.
+template <int FLAGS>
+__device__ __forceinline__ void flush_stats(const StreamParams &p, const FlushCtx &c, double (&a)[8],
+                                            double (&q)[8], int w0, int nw, int t, bool isL) {
+    constexpr bool PACK = FLAGS & kFPack, HEALTH = FLAGS & kFHealth;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double v[16];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { v[i] = a[i]; v[i + 8] = q[i]; a[i] = 0.0; q[i] = 0.0; }
+    warp_reduce_scatter16(v, lane);
+    const int idx = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+    if ((lane & 1) == 0) c.s_red[warp][idx] = v[0];
+    __syncthreads();
+    if (threadIdx.x < 16) {
+        const int j = threadIdx.x, w = j & 7;
+        double tot = 0.0;
+#pragma unroll
+        for (int k = 0; k < kThreads / 32; ++k) tot += c.s_red[k][j];
+        if (w < nw) {
+            const size_t o = (size_t)(w0 + w) * p.T + t;
+            if (j < 8) {
+                if (PACK && isL && p.abs_sum && tot != 0.0) atomicAdd(p.abs_sum + o, tot);
+            } else {
+                if (HEALTH && p.sumsq && tot != 0.0) atomicAdd(p.sumsq + o, tot);
+            }
+        }
+    } else if (HEALTH && threadIdx.x >= 32 && threadIdx.x < 40) {
+        const int w = threadIdx.x - 32;
+        const unsigned int cn = c.s_nan[w], ci = c.s_inf[w];
+        if (w < nw && p.nan_cnt) {
+            const size_t o = (size_t)(w0 + w) * p.T + t;
+            if (cn) atomicAdd(p.nan_cnt + o, (unsigned long long)cn);
+            if (ci) atomicAdd(p.inf_cnt + o, (unsigned long long)ci);
+        }
+        c.s_nan[w] = 0u;
+        c.s_inf[w] = 0u;
+    }
+    __syncthreads();
+}
+
+template <int FLAGS>
+__global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams p) {
+    constexpr bool PACK = FLAGS & kFPack, COUNT = FLAGS & kFCount, FP32 = FLAGS & kFFp32,
+                   HEALTH = FLAGS & kFHealth;
+    __shared__ double s_red[kThreads / 32][16];
+    __shared__ unsigned int s_nan[8], s_inf[8];
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    const int n_tiles = pv.hdr->n_tiles;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid < 8) { s_nan[tid] = 0u; s_inf[tid] = 0u; }
+    __syncthreads();
+    const FlushCtx fc{s_red, s_nan, s_inf};
+
+    const int W = p.W;
+    const bool multi = W > kGroup;           // more than one register group of workers
+    double a[8], q[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = 0.0; q[i] = 0.0; }
+    int acc_t = -1;                          // tensor the accumulators belong to (single-group mode)
+    bool acc_isL = false;
+
+    // cached properties of the current tensor
+    int t = -1, tile_b = 0, tile_e = 0;
+    int64_t off_t = 0, len_t = 0, woff_t = 0;
+    bool isL = false, aligned = false;
+    float tau = 0.f;
+
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        if (tile >= tile_e) {
+            t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
+            tile_b = __ldg(pv.tile_prefix + t);
+            tile_e = __ldg(pv.tile_prefix + t + 1);
+            off_t = __ldg(p.off + t);
+            len_t = __ldg(p.len + t);
+            isL = p.route ? (__ldg(p.route + t) == NF_ROUTE_L) : false;
+            woff_t = (isL && p.woff) ? __ldg(p.woff + t) : 0;
+            tau = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
+            aligned = (((off_t | p.worker_stride) & 3) == 0);
+        }
+        const bool do_tile = HEALTH || (isL ? (PACK || COUNT) : FP32);
+        if (!do_tile) continue;
+        if (!multi && acc_t != t) {
+            if (acc_t >= 0) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
+            acc_t = t;
+            acc_isL = isL;
+        }
+        const int64_t i0 = (int64_t)(tile - tile_b) * kTile + tid * 4;   // tensor-relative, row 0
+        int valid[kRows];
+#pragma unroll
+        for (int u = 0; u < kRows; ++u) {
+            int64_t rem = len_t - (i0 + (int64_t)u * kRowElems);
+            valid[u] = rem >= 4 ? 4 : (rem > 0 ? (int)rem : 0);
+        }
+        uint32_t cp[kRows], cn[kRows];       // byte-packed per-position counts (4 positions each)
+        float4 acc[kRows];                   // FP32-route running sums
+#pragma unroll
+        for (int u = 0; u < kRows; ++u) { cp[u] = 0u; cn[u] = 0u; acc[u] = make_float4(0.f, 0.f, 0.f, 0.f); }
+
+        for (int w0 = 0; w0 < W; w0 += kGroup) {
+            const int nw = min(kGroup, W - w0);
+            const float *gb = p.g + (size_t)w0 * p.worker_stride + off_t + i0;
+            float4 x[kRows][kGroup];
+#pragma unroll
+            for (int u = 0; u < kRows; ++u)
+#pragma unroll
+                for (int w = 0; w < kGroup; ++w)
+                    x[u][w] = (w < nw) ? load4(gb + (size_t)w * p.worker_stride + (size_t)u * kRowElems,
+                                               valid[u], aligned)
+                                       : make_float4(0.f, 0.f, 0.f, 0.f);
+
+            uint32_t posR[kRows], negR[kRows];
+#pragma unroll
+            for (int u = 0; u < kRows; ++u) { posR[u] = 0u; negR[u] = 0u; }
+
+#pragma unroll
+            for (int w = 0; w < kGroup; ++w) {
+                if (w < nw) {
+                    if (PACK || HEALTH) {
+                        // FP32 over this thread's 8 elements of worker w, then FP64
+                        float af = 0.f, qf = 0.f;
+#pragma unroll
+                        for (int u = 0; u < kRows; ++u) {
+                            const float4 v = x[u][w];
+                            af += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
+                            if (HEALTH) {
+                                qf = fmaf(v.x, v.x, qf); qf = fmaf(v.y, v.y, qf);
+                                qf = fmaf(v.z, v.z, qf); qf = fmaf(v.w, v.w, qf);
+                            }
+                        }
+                        // fast path: everything finite and the FP32 squares did not underflow
+                        const bool ok = HEALTH ? ((qf < FLT_MAX) && (qf >= 1e-30f || af == 0.f))
+                                               : (af < FLT_MAX);
+                        if (ok) {
+                            a[w] += (double)af;
+                            if (HEALTH) q[w] += (double)qf;
+                        } else {
+#pragma unroll
+                            for (int u = 0; u < kRows; ++u) {
+                                const float e4[4] = {x[u][w].x, x[u][w].y, x[u][w].z, x[u][w].w};
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) {
+                                    const float v = e4[j];
+                                    a[w] += (double)fabsf(v);
+                                    if (HEALTH) {
+                                        if (v != v) atomicAdd(&s_nan[w], 1u);
+                                        else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[w], 1u);
+                                        else q[w] += (double)v * (double)v;
+                                    }
+                                }
+                            }
+                        }
+                    }
+                    if (isL) {
+                        if (PACK || COUNT) {
+#pragma unroll
+                            for (int u = 0; u < kRows; ++u) {
+                                const float4 v = x[u][w];
+                                uint32_t pb = (v.x > tau ? 1u : 0u) | (v.y > tau ? 2u : 0u) |
+                                              (v.z > tau ? 4u : 0u) | (v.w > tau ? 8u : 0u);
+                                posR[u] |= pb << (4 * w);
+                                if (p.ternary) {
+                                    const float nt = -tau;
+                                    uint32_t nb = (v.x < nt ? 1u : 0u) | (v.y < nt ? 2u : 0u) |
+                                                  (v.z < nt ? 4u : 0u) | (v.w < nt ? 8u : 0u);
+                                    negR[u] |= nb << (4 * w);
+                                }
+                            }
+                        }
+                    } else if (FP32) {
+                        // fixed worker order, plain FP32 adds
+#pragma unroll
+                        for (int u = 0; u < kRows; ++u) {
+                            const float4 v = x[u][w];
+                            if (w0 == 0 && w == 0) acc[u] = v;
+                            else {
+                                acc[u].x = __fadd_rn(acc[u].x, v.x); acc[u].y = __fadd_rn(acc[u].y, v.y);
+                                acc[u].z = __fadd_rn(acc[u].z, v.z); acc[u].w = __fadd_rn(acc[u].w, v.w);
+                            }
+                        }
+                    }
+                }
+            }
+
+            if (isL && (PACK || COUNT)) {
+#pragma unroll
+                for (int u = 0; u < kRows; ++u) {
+                    if (COUNT) {
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            cp[u] += (uint32_t)__popc(posR[u] & (0x11111111u << j)) << (8 * j);
+                            if (p.ternary) cn[u] += (uint32_t)__popc(negR[u] & (0x11111111u << j)) << (8 * j);
+                        }
+                    }
+                    if (PACK && p.P) {
+                        const int64_t wi = ((int64_t)(tile - tile_b) * kTile + (int64_t)u * kRowElems) / 32 +
+                                           warp * 4 + (lane >> 3);
+                        const int wq = lane & 7;
+                        const bool st = (wq < nw) && (wi < (len_t + 31) / 32);
+                        const size_t o = (size_t)(w0 + wq) * p.plane_stride + woff_t + wi;
+                        const uint32_t pw = nibble_transpose8(posR[u], lane);
+                        if (st) p.P[o] = pw;
+                        if (p.ternary) {
+                            const uint32_t nwd = nibble_transpose8(negR[u], lane);
+                            if (st) p.N[o] = nwd;
+                        }
+                    }
+                }
+            }
+            if (multi && (PACK || HEALTH)) flush_stats<FLAGS>(p, fc, a, q, w0, nw, t, isL);
+        }
+
+        if (isL) {
+            if (COUNT) {
+                // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
+#pragma unroll
+                for (int u = 0; u < kRows; ++u) {
+                    if (valid[u] > 0) {
+                        uint32_t d = 0u;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const int c_p = (cp[u] >> (8 * j)) & 0xff;
+                            const int c_n = p.ternary ? (int)((cn[u] >> (8 * j)) & 0xff) : (W - c_p);
+                            const int D = c_p - c_n;
+                            d |= (D > p.margin ? 1u : 0u) << j;
+                            d |= (D < -p.margin ? 1u : 0u) << (4 + j);
+                        }
+                        p.dirs[(size_t)woff_t * 8 + (size_t)((i0 + (int64_t)u * kRowElems) >> 2)] = (uint8_t)d;
+                    }
+                }
+            }
+        } else if (FP32) {
+#pragma unroll
+            for (int u = 0; u < kRows; ++u) {
+                float *o = p.out + off_t + i0 + (int64_t)u * kRowElems;
+                float4 r = acc[u];
+                r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
+                r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
+                if (valid[u] == 4 && ((off_t & 3) == 0)) {
+                    __stcs(reinterpret_cast<float4 *>(o), r);
+                } else {
+                    if (valid[u] > 0) o[0] = r.x;
+                    if (valid[u] > 1) o[1] = r.y;
+                    if (valid[u] > 2) o[2] = r.z;
+                    if (valid[u] > 3) o[3] = r.w;
+                }
+            }
+        }
+    }
+    if (!multi && acc_t >= 0 && (PACK || HEALTH)) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+int device_sm_count() {
+    static int sms = 0;
+    if (sms == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    }
+    return sms;
+}
+
+template <int FLAGS>
+static cudaError_t launch_stream_t(const StreamParams &p, int64_t n, cudaStream_t s) {
+    static int per_sm = 0;
+    if (per_sm == 0) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stream_kernel<FLAGS>, kThreads, 0) !=
+                cudaSuccess || per_sm <= 0)
+            per_sm = 1;
+    }
+    // upper bound of the tile count known on the host: every tensor adds at most one ragged tile
+    const int64_t max_tiles = n / kTile + p.T;
+    if (max_tiles <= 0) return cudaSuccess;
+    int64_t grid = (int64_t)device_sm_count() * per_sm;     // persistent: a multiple of the SM count
+    if (grid > max_tiles) grid = max_tiles;
+    stream_kernel<FLAGS><<<(unsigned)grid, kThreads, 0, s>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStream_t s) {
+    switch (flags) {
+        case kFPack: return launch_stream_t<kFPack>(p, n, s);
+        case kFFp32: return launch_stream_t<kFFp32>(p, n, s);
+        case kFHealth: return launch_stream_t<kFHealth>(p, n, s);
+        case kFPack | kFCount | kFFp32: return launch_stream_t<kFPack | kFCount | kFFp32>(p, n, s);
+        case kFPack | kFCount | kFFp32 | kFHealth:
+            return launch_stream_t<kFPack | kFCount | kFFp32 | kFHealth>(p, n, s);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace nf

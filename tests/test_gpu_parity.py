@@ -1,0 +1,133 @@
+"""`-m gpu` parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs. Sizes span several tiles (tile = 2048 elements) and ragged
+tails; full-size configs are in test_gpu_fullsize.py."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import nf_oracle as O
+from paper_2606_25759_b200 import BucketBuffers, binding as nf
+from tests.parity import run_both, compare, _np
+from tests.util import read_golden, layout
+from workloads import shapes, gen
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda"
+
+
+def _dev(g_np, pad_to4=True):
+    W, n = g_np.shape
+    s = (n + 3) // 4 * 4 if pad_to4 else n
+    g = torch.zeros((W, max(s, 4)), dtype=torch.float32, device=DEV)
+    g[:, :n] = torch.from_numpy(g_np)
+    return g
+
+
+def test_handworked_bucket_on_gpu():
+    d = read_golden("handworked_w4.txt")
+    W = int(d["W"][0])
+    off, ln, n = layout([int(x) for x in d["len"]])
+    elig = [int(x) for x in d["elig"]]
+    g = np.array([[float(x) for x in d[f"g{w}"]] for w in range(W)], np.float32)
+    for mode, dkey in ((O.MODE_GTERNARY, "d_ternary"), (O.MODE_GBINARY, "d_binary")):
+        ref = run_both(_dev(g), off, ln, elig, mode=mode, what="handworked")
+        S = np.float32(float(d["scale"][0]))
+        assert np.array_equal(ref.out[:8], np.array([S * int(x) for x in d[dkey]], np.float32))
+
+
+@pytest.mark.parametrize("W", [1, 2, 3, 4, 8, 9, 17, 255])
+@pytest.mark.parametrize("mode", [O.MODE_GBINARY, O.MODE_GTERNARY])
+def test_adversarial_lengths_and_offsets(W, mode):
+    """Lengths 1, 31, 32, 33, 4099, a multi-tile tensor, offsets that are not multiples of 4,
+    gaps between tensors, -0.0, denormals, +-Inf, a tensor that is entirely NaN."""
+    rng = np.random.default_rng(1000 + W)
+    lens = [1, 31, 32, 33, 4099, 2048 * 3 + 5, 7, 2048, 64]
+    off, o = [], 3                                            # first tensor starts at 3: misaligned
+    for i, l in enumerate(lens):
+        off.append(o)
+        o += l + (2 if i % 3 == 0 else 0)                     # gaps
+    n = o + 1
+    off, ln = np.array(off, np.int64), np.array(lens, np.int64)
+    elig = [1, 1, 0, 1, 1, 1, 0, 1, 1]
+    g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-6, 2, (1, n))).astype(np.float32)
+    g[rng.random((W, n)) < 0.1] = 0.0
+    g[0, off[4] + 5] = -0.0
+    g[W - 1, off[4] + 6] = 1e-42                              # denormal
+    g[0, off[5] + 100] = np.inf
+    g[W - 1, off[5] + 101] = -np.inf
+    g[:, off[8]:off[8] + 64] = np.nan                         # tensor entirely NaN
+    g[0, off[2] + 3] = np.nan                                 # NaN on the FP32 route
+    tau = (rng.random(len(lens)) * 1e-3).astype(np.float32)
+    gd = _dev(g)
+    run_both(gd, off, ln, elig, mode=mode, what=f"adv W={W}")
+    run_both(gd, off, ln, elig, mode=mode, tau=tau, margin=1, alpha=1.0 / W, what=f"adv tau W={W}")
+
+
+@pytest.mark.parametrize("state", [(0, 0, 1), (1, 1, 1), (1, 0, 0), (1, 0, 1)])
+def test_three_state_preflight(state):
+    """warm-up / admitted / forced veto (and guard reject) over the same binding."""
+    cfg = shapes.tiny()
+    b = cfg.buckets[0]
+    g = gen.gen_bucket(cfg, b, DEV)
+    ref = run_both(g, b.off, b.length, b.elig, state=state, what=f"tiny state={state}")
+    if state != (1, 0, 1):
+        plain = O.fp32_reduce(_np(g)[:, :b.n].copy(), b.off, b.length, np.zeros(len(b.off), np.uint8))
+        assert np.array_equal(ref.out, plain)
+
+
+def test_no_L_and_no_P_buckets_and_empty():
+    rng = np.random.default_rng(5)
+    off, ln, n = layout([5000, 333])
+    g = _dev(rng.standard_normal((4, n)).astype(np.float32))
+    run_both(g, off, ln, [0, 0], what="zero L")
+    run_both(g, off, ln, [1, 1], what="zero P")
+    # zero-length tensor in the middle, and T = 0
+    off2, ln2 = np.array([0, 100, 100], np.int64), np.array([100, 0, 200], np.int64)
+    run_both(g, off2, ln2, [1, 1, 0], what="empty tensor")
+    bb = BucketBuffers([], [], [], 0, 4, DEV)
+    bb.aggregate(g, g.shape[1])
+    torch.cuda.synchronize()
+    assert int(bb.summary[nf.SUM_STATUS]) == 0 and int(bb.summary[nf.SUM_WD]) == 0
+
+
+def test_bad_layout_is_flagged_on_device_and_nothing_runs():
+    g = torch.ones((2, 64), device=DEV)
+    bb = BucketBuffers([0, 8], [16, 8], [1, 1], 32, 2, DEV)   # overlap
+    bb.out.fill_(5.0)
+    bb.aggregate(g, 64)
+    torch.cuda.synchronize()
+    assert int(bb.summary[nf.SUM_STATUS]) == nf.NF_ERR_ARG
+    assert bool((bb.out == 5.0).all())
+
+
+@pytest.mark.parametrize("name", ["tiny", "resnet50", "vit_b16", "gpt2_1p3b", "sweep_w2", "sweep_w32", "sweep_w128"])
+def test_config_shapes_small(name):
+    """The five BASELINE configs, structurally identical but scaled down (tiny is full size)."""
+    cfg = shapes.get(name, small=True)
+    for b in cfg.buckets:
+        g = gen.gen_bucket(cfg, b, DEV)
+        ref = run_both(g, b.off, b.length, b.elig, what=f"{cfg.name} bucket {b.index}")
+        if cfg.nan_frac and b.index == cfg.nan_bucket:
+            assert ref.nan_cnt[cfg.nan_worker].sum() > 0 and ref.nan_cnt.sum() == ref.nan_cnt[cfg.nan_worker].sum()
+
+
+def test_gpu_invariants_without_oracle():
+    """Properties that hold at any size, checked on the GPU's own outputs."""
+    cfg = shapes.tiny()
+    b = cfg.buckets[0]
+    g = gen.gen_bucket(cfg, b, DEV)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, counts=True)
+    bb.route_bucket((1, 0, 1))
+    bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+    bb.sign_count_reduce(nf.MODE_GTERNARY)
+    torch.cuda.synchronize()
+    assert not bool((bb.P & bb.N).any())
+    cz = cfg.W - bb.cpos.to(torch.int32) - bb.cneg.to(torch.int32)
+    assert int(cz.min()) >= 0
+    # permuting workers leaves counts unchanged
+    cp0 = bb.cpos.clone()
+    g2 = g[torch.tensor([2, 0, 3, 1], device=DEV)].contiguous()
+    bb.sign_pack(g2, g2.shape[1], nf.MODE_GTERNARY)
+    bb.sign_count_reduce(nf.MODE_GTERNARY)
+    torch.cuda.synchronize()
+    assert torch.equal(cp0, bb.cpos)
