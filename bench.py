@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the fused low-bit bucket-aggregation hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config NAME]
+
+A "step" is one pass of the whole hot path (route + pack + sign-count + decode + FP32 route +
+health statistics, i.e. nf_aggregate_bucket) over every DDP bucket of the workload, W emulated
+workers resident in HBM. Default workload: BASELINE.json configs[3], the GPT-2-1.3B-shaped model
+(W=8, 1.31 G params, 37 buckets, 42 GB of FP32 gradients) — the config the metric is quoted on.
+Prints ONE JSON line. Metric: FP32-gradient input bytes consumed per second, 4*W*n/t, in GB/s.
+
+N > 1 (torchrun): the path does not shard across GPUs in this build (BASELINE.json: one GPU, no
+collectives): every rank runs an independent replica ("replicas only"),
+value = N * per-replica bytes / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "bucket FP32-grad GB/s aggregated (W emulated workers, 1 B200), % HBM peak"
+UNIT = "GB/s"
+HBM_FALLBACK_GBS = 6650.0      # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+HBM_NOMINAL_GBS = 8000.0       # BASELINE.json "~8 TB/s peak"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="nf", choices=["nf", "reference"])
+    ap.add_argument("--config", default="gpt2_1p3b")
+    ap.add_argument("--small", action="store_true", help="scaled-down shapes (debug only; invalid as a bench number)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-planes", action="store_true", help="do not materialise the packed planes")
+    ap.add_argument("--mode", default="ternary", choices=["ternary", "binary"])
+    ap.add_argument("--max-buckets", type=int, default=0, help="profiling aid: only the first K buckets "
+                    "(invalid as a bench number)")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy)"
+    except Exception:
+        return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    try:
+        with open(p) as f:
+            return json.load(f)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                   "samples": len(sm)}
+        return out
+
+
+def dist_setup(n_gpus):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend=backend)
+    return rank, world, local
+
+
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Barrier-bracketed timing is taken as the MAX over ranks (replicas run independently)."""
+    if world <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+# ------------------------------------------------------------------------------------------------
+def algorithmic_bytes(cfg, planes: bool, ternary: bool):
+    """fused path moves 4*W*n (in) + 4*n (out) + e/4 + e/4 (2-bit directions written
+    by pass A and read by pass B) + p*W*e/8 (planes, when materialised) bytes per bucket."""
+    p = 2 if ternary else 1
+    tot_in = tot_all = passA = 0
+    for b in cfg.buckets:
+        e, n = b.n_eligible, b.n
+        f = n - e
+        inp = 4 * cfg.W * n
+        pl = (p * cfg.W * e) // 8 if planes else 0
+        a = inp + pl + e // 4 + 4 * f          # pass A: read all, write planes + dirs + FP32-route out
+        bb = e // 4 + 4 * e                    # pass B: read dirs, write low-bit out
+        tot_in += inp
+        passA += a
+        tot_all += a + bb
+    return tot_in, tot_all, passA
+
+
+def run_nf(args):
+    import torch
+    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from paper_2606_25759_b200 import build as nf_build
+    from workloads import shapes, gen
+
+    rank, world, local = dist_setup(args.gpus)
+    nf_build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    cfg = shapes.get(args.config, small=args.small)
+    if args.max_buckets > 0:
+        cfg.buckets = cfg.buckets[:args.max_buckets]
+    W = cfg.W
+    ternary = args.mode == "ternary"
+    mode = nf.MODE_GTERNARY if ternary else nf.MODE_GBINARY
+    planes = not args.no_planes
+
+    # ---- resident inputs: every bucket's [W][stride] gradients in HBM (42 GB for the GPT config)
+    t0 = time.time()
+    G, BB = [], []
+    max_ps = max((sum((l + 31) // 32 for l in b.length) + 3) // 4 * 4 for b in cfg.buckets)
+    max_n = max(b.n for b in cfg.buckets)
+    P = torch.zeros((W, max_ps), dtype=torch.int32, device=dev) if planes else None
+    N = torch.zeros((W, max_ps), dtype=torch.int32, device=dev) if (planes and ternary) else None
+    ws = torch.zeros(nf.nf_workspace_bytes(max(len(b.tensors) for b in cfg.buckets), max_n),
+                     dtype=torch.uint8, device=dev)
+    for b in cfg.buckets:
+        G.append(gen.gen_bucket(cfg, b, dev))
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, W, dev, planes=False, health=True)
+        bb.P, bb.N, bb.plane_stride, bb.workspace = P, N, max_ps, ws
+        BB.append(bb)
+    torch.cuda.synchronize()
+    gen_s = time.time() - t0
+    stream = torch.cuda.current_stream()
+
+    def step():
+        for g, bb in zip(G, BB):
+            bb.aggregate(g, g.shape[1], (1, 0, 1), mode, None, 0, 1.0, planes=planes)
+
+    in_bytes, all_bytes, passA_bytes = algorithmic_bytes(cfg, planes, ternary)
+    n_total = cfg.n_params
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    # ---- timed region: device-resident inputs (inputs are 42 GB >> 126 MB L2: no flush needed)
+    barrier(world)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    clocks = sampler.stop() if sampler else None
+    ms_per_step = ms / args.steps
+    value = world * in_bytes / (ms_per_step * 1e-3) / 1e9
+
+    # ---- per-kernel durations of the same steps (events recorded inside the C call)
+    nb = len(cfg.buckets)
+    prof_steps = min(args.steps, 5)
+    nf.nf_prof_enable(nb * prof_steps)
+    for _ in range(prof_steps):
+        step()
+    torch.cuda.synchronize()
+    recs = nf.nf_prof_collect(nb * prof_steps)
+    nf.nf_prof_enable(0)
+    route_ms = sum(r[0] for r in recs) / prof_steps
+    passA_ms = sum(r[1] for r in recs) / prof_steps
+    passB_ms = sum(r[2] for r in recs) / prof_steps
+    peak, peak_src = measured_peak()
+    achieved = passA_bytes / (passA_ms * 1e-3) / 1e9
+    traffic = ncu_traffic()
+    roofline = {"bound": "hbm", "kernel": "nf::stream_kernel<pack|count|fp32|health> (fused pass A)",
+                "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "peak_source": peak_src,
+                "frac_of_nominal_8TBs": round(achieved / HBM_NOMINAL_GBS, 4),
+                "algorithmic_bytes_per_step": passA_bytes, "launches_per_step": nb,
+                "avg_launch_ms": round(passA_ms / nb, 4),
+                "traffic": (traffic or {}).get("dram_bytes_per_launch_avg"),
+                "traffic_note": (traffic or {}).get("note"),
+                "whole_path": {"algorithmic_bytes_per_step": all_bytes,
+                               "achieved": round(all_bytes / (ms_per_step * 1e-3) / 1e9, 1),
+                               "frac": round(all_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4)},
+                "kernel_ms_per_step": {"route": round(route_ms, 4), "passA": round(passA_ms, 4),
+                                       "passB": round(passB_ms, 4)}}
+
+    # ---- e2e: same metric through the C-ABI call with HOST buffers (H2D + D2H inside the region)
+    e2e = None
+    if not args.no_e2e:
+        e2e = run_e2e(args, cfg, BB, mode, dev, world)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(cfg, G, budget_s=20.0)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": round(ms_per_step, 4),
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic", "impl": "nf",
+                "config": {"workload": f"{cfg.name}: W={W} emulated workers, {cfg.n_params} FP32 params, "
+                                       f"{nb} DDP buckets, {cfg.n_tensors} tensors, mode=G-"
+                                       f"{'Ternary' if ternary else 'Binary'}, planes={'on' if planes else 'off'}",
+                           "W": W, "n_params": n_total, "buckets": nb, "input_bytes_per_step": in_bytes,
+                           "l2": "inputs (42 GB) are larger than L2 (126 MB); no flush",
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "small": bool(args.small), "max_buckets": args.max_buckets},
+                "elements_per_s": round(world * n_total / (ms_per_step * 1e-3), 1),
+                "input_elements_per_s": round(world * n_total * W / (ms_per_step * 1e-3), 1),
+                "pct_hbm_peak_measured": round(100 * all_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 2),
+                "pct_hbm_peak_nominal_8TBs": round(100 * all_bytes / (ms_per_step * 1e-3) / 1e9 / HBM_NOMINAL_GBS, 2),
+                "gpu_launches": args.steps * nb * 3,
+                "roofline": roofline, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu,
+                "setup_s": round(gen_s, 1)}
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+def run_e2e(args, cfg, BB, mode, dev, world):
+    """nf_aggregate_bucket_host per bucket: H2D of the bucket's W x n floats from pinned host memory,
+    the fused path, D2H of the n aggregated floats. The pinned pool holds one bucket's worth of
+    gradients (the largest), reused for every bucket: the bytes cross PCIe every step."""
+    import torch
+    from paper_2606_25759_b200 import binding as nf
+    W = cfg.W
+    max_stride = max((b.n + 3) // 4 * 4 for b in cfg.buckets)
+    g_dev = torch.empty(W * max_stride, dtype=torch.float32, device=dev)
+    g_dev.normal_(0.0, 1e-3)
+    g_host = torch.empty(W * max_stride, dtype=torch.float32, pin_memory=True)
+    g_host.copy_(g_dev)
+    out_host = torch.empty(max_stride, dtype=torch.float32, pin_memory=True)
+    torch.cuda.synchronize()
+    stream = torch.cuda.current_stream()
+    steps = max(1, min(args.steps, 2))
+
+    def step():
+        for b, bb in zip(cfg.buckets, BB):
+            s = (b.n + 3) // 4 * 4
+            nf.nf_aggregate_bucket_host(g_host, g_dev, s, W, b.n, bb.off, bb.len, bb.elig, bb.T, (1, 0, 1),
+                                        mode, None, 0, 1.0, bb.route, bb.woff, bb.summary, bb.abs_sum,
+                                        bb.sumsq, bb.nan_cnt, bb.inf_cnt, bb.out, out_host, bb.plan,
+                                        bb.workspace)
+    step()
+    torch.cuda.synchronize()
+    barrier(world)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev) / steps
+    h2d = sum(4 * W * ((b.n + 3) // 4 * 4) for b in cfg.buckets)
+    d2h = sum(4 * b.n for b in cfg.buckets)
+    in_bytes = sum(4 * W * b.n for b in cfg.buckets)
+    del g_dev, g_host, out_host
+    return {"value": round(world * in_bytes / (ms * 1e-3) / 1e9, 2), "unit": UNIT,
+            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "ms_per_step": round(ms, 2),
+            "steps": steps, "api": "nf_aggregate_bucket_host (pinned host buffers, cudaMemcpyAsync)"}
+
+
+def cpu_baseline(cfg, G, budget_s=20.0):
+    """The oracle as it stands, single-threaded, on a bounded sample of the same workload: whole
+    buckets in order until ~budget_s of CPU work. Input values are the device-resident ones."""
+    from oracle import nf_oracle as O
+    done_bytes, t_total, used, last = 0, 0.0, [], 0.0
+    for b, g in zip(cfg.buckets, G):
+        if used and t_total + last > budget_s:
+            break
+        if b.n * cfg.W > 600_000_000:            # keep the host copy of one bucket under ~2.4 GB
+            continue
+        gh = g.cpu().numpy()[:, :b.n].copy()
+        t0 = time.perf_counter()
+        O.aggregate_bucket(gh, b.off, b.length, b.elig, (1, 0, 1), O.MODE_GTERNARY)
+        last = time.perf_counter() - t0
+        t_total += last
+        done_bytes += 4 * cfg.W * b.n
+        used.append(b.index)
+        del gh
+    if not used:
+        return None
+    return {"value": round(done_bytes / t_total / 1e9, 4), "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"buckets {used} of {cfg.name} ({done_bytes / 1e9:.2f} GB of FP32 gradient input, "
+                      f"{t_total:.1f} s single-threaded, host has {os.cpu_count()} cores)"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (oracle/), as it stands, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    import torch
+    from oracle import nf_oracle as O
+    from workloads import shapes, gen
+    cfg = shapes.get(args.config, small=args.small)
+    # bounded sample: the first mixed low-bit bucket of the workload (bucket 1: 33.6 M elements x W)
+    b = cfg.buckets[min(1, len(cfg.buckets) - 1)]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    gh = gen.gen_bucket(cfg, b, dev).cpu().numpy()[:, :b.n].copy()
+    in_bytes = 4 * cfg.W * b.n
+
+    def step():
+        O.aggregate_bucket(gh, b.off, b.length, b.elig, (1, 0, 1), O.MODE_GTERNARY)
+    for _ in range(min(args.warmup, 1)):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    val = round(in_bytes / dt / 1e9, 4)
+    sample = (f"bucket {b.index} of {cfg.name} per step ({in_bytes / 1e9:.2f} GB of FP32 gradient input, "
+              f"{b.n} elements x W={cfg.W}); single-threaded C oracle; host has {os.cpu_count()} cores")
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
+                      "n_gpus": args.gpus, "steps": args.steps, "warmup": min(args.warmup, 1),
+                      "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{cfg.name}: W={cfg.W}, bounded sample = {sample}"},
+                      "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}))
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_nf(a)

@@ -169,6 +169,17 @@ int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t
                              void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
                              nf_stream stream);
 
+/*
+ * Instrumentation (host calls, not part of the data path). nf_prof_enable(k > 0) creates CUDA
+ * events for up to k nf_aggregate_bucket calls and makes each such call record four events on
+ * its stream (before route, before pass A, after pass A, after pass B); nf_prof_enable(0) frees
+ * them. nf_prof_collect synchronises on the recorded events, writes 3 floats per recorded call
+ * (route ms, pass A ms, pass B ms) to the HOST array `ms` (room for 3*max_records floats), resets
+ * the record counter and returns the number of calls written (or a negative nf_status).
+ */
+int nf_prof_enable(int max_records);
+int nf_prof_collect(float *ms /*host*/, int max_records);
+
 #ifdef __cplusplus
 }
 #endif

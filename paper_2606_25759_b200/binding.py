@@ -23,7 +23,7 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
-           "nf_aggregate_bucket", "nf_aggregate_bucket_host")
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect")
 
 
 class NfState(C.Structure):
@@ -75,6 +75,10 @@ def lib() -> C.CDLL:
     L.nf_aggregate_bucket_host.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32,
                                            f32, vp, vp, vp, vp, vp, vp, vp, vp, vp,
                                            vp, sz, vp, sz, vp]
+    L.nf_prof_enable.restype = i32
+    L.nf_prof_enable.argtypes = [i32]
+    L.nf_prof_collect.restype = i32
+    L.nf_prof_collect.argtypes = [vp, i32]
     _lib = L
     return L
 
@@ -175,3 +179,16 @@ def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, el
         _ptr(route), _ptr(woff), _ptr(summary), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt), _ptr(inf_cnt),
         _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_prof_enable(max_records: int):
+    _check("nf_prof_enable", lib().nf_prof_enable(int(max_records)))
+
+
+def nf_prof_collect(max_records: int):
+    """Returns a list of (route_ms, passA_ms, passB_ms), one per recorded nf_aggregate_bucket call."""
+    buf = (C.c_float * (3 * max(max_records, 1)))()
+    k = lib().nf_prof_collect(C.cast(buf, C.c_void_p), int(max_records))
+    if k < 0:
+        raise NfError("nf_prof_collect", k)
+    return [(buf[3 * i], buf[3 * i + 1], buf[3 * i + 2]) for i in range(k)]

@@ -6,6 +6,13 @@ using namespace nf;
 
 namespace {
 
+// instrumentation state (nf_prof_*): 4 events per recorded nf_aggregate_bucket call
+cudaEvent_t *g_prof_ev = nullptr;
+int g_prof_cap = 0, g_prof_n = 0;
+inline void prof_mark(int slot, cudaStream_t s) {
+    if (g_prof_ev && g_prof_n < g_prof_cap) cudaEventRecord(g_prof_ev[4 * g_prof_n + slot], s);
+}
+
 inline bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NF_OK : NF_ERR_CUDA; }
 
@@ -166,12 +173,14 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
         misaligned16(plan) || misaligned16(workspace))
         return NF_ERR_ALIGN;
     cudaStream_t s = (cudaStream_t)stream;
+    prof_mark(0, s);
     // a1 (+ zeroing of the accumulators, so no memset nodes sit on the stream)
     cudaError_t e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
                                  abs_sum, sumsq, (unsigned long long *)nan_cnt,
                                  (unsigned long long *)inf_cnt, (int64_t)W * T, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
     if (T == 0 || n == 0) return NF_OK;
+    prof_mark(1, s);
     // pass A: one read of the W x n gradients
     StreamParams p{};
     p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
@@ -183,12 +192,44 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
     e = launch_stream(health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32), p, n, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
+    prof_mark(2, s);
     // pass B: scale x direction for the low-bit positions
     ReduceParams r{};
     r.W = W; r.T = T; r.off = off; r.len = len; r.route = route; r.woff = woff;
     r.abs_sum = abs_sum; r.out = out; r.scale_out = scale_out;
     r.dirs = (const uint8_t *)workspace; r.plan = plan;
-    return cuda_rc(launch_decode(r, n, s));
+    e = launch_decode(r, n, s);
+    prof_mark(3, s);
+    if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;
+    return cuda_rc(e);
+}
+
+int nf_prof_enable(int max_records) {
+    if (g_prof_ev) {
+        for (int i = 0; i < 4 * g_prof_cap; ++i) cudaEventDestroy(g_prof_ev[i]);
+        delete[] g_prof_ev;
+        g_prof_ev = nullptr;
+    }
+    g_prof_cap = g_prof_n = 0;
+    if (max_records <= 0) return NF_OK;
+    g_prof_ev = new cudaEvent_t[4 * (size_t)max_records];
+    for (int i = 0; i < 4 * max_records; ++i)
+        if (cudaEventCreate(&g_prof_ev[i]) != cudaSuccess) return NF_ERR_CUDA;
+    g_prof_cap = max_records;
+    return NF_OK;
+}
+
+int nf_prof_collect(float *ms, int max_records) {
+    if (!ms || max_records < 0) return NF_ERR_ARG;
+    int k = g_prof_n < max_records ? g_prof_n : max_records;
+    for (int i = 0; i < k; ++i) {
+        if (cudaEventSynchronize(g_prof_ev[4 * i + 3]) != cudaSuccess) return NF_ERR_CUDA;
+        for (int j = 0; j < 3; ++j)
+            if (cudaEventElapsedTime(&ms[3 * i + j], g_prof_ev[4 * i + j], g_prof_ev[4 * i + j + 1]) != cudaSuccess)
+                return NF_ERR_CUDA;
+    }
+    g_prof_n = 0;
+    return k;
 }
 
 int nf_aggregate_bucket_host(const float *g_host, float *g_dev, int64_t worker_stride, int W,

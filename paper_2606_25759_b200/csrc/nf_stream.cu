@@ -122,10 +122,26 @@ __device__ __forceinline__ void flush_stats(const StreamParams &p, const FlushCt
     __syncthreads();
 }
 
+// pos/neg indicator bits: one compare + one predicated OR per element and plane
+__device__ __forceinline__ void or_if_gt(uint32_t &r, float x, float t, uint32_t bit) {
+    asm("{\n\t.reg .pred p;\n\tsetp.gt.f32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}" : "+r"(r) : "f"(x), "f"(t), "r"(bit));
+}
+__device__ __forceinline__ void or_if_lt(uint32_t &r, float x, float t, uint32_t bit) {
+    asm("{\n\t.reg .pred p;\n\tsetp.lt.f32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}" : "+r"(r) : "f"(x), "f"(t), "r"(bit));
+}
+
+template <bool B> struct BoolTag { static constexpr bool value = B; };
+
+// Element owned by (warp, lane) in row u of a tile: each warp covers 256 consecutive elements per
+// tile (two rows of 128), so its packed words of one worker are 8 consecutive words = one 32-byte
+// sector, its direction bytes one sector per row, and every load/store instruction is 512 B wide.
+__device__ __forceinline__ int tile_elem(int warp, int lane, int u) { return warp * (kRows * 128) + u * 128 + lane * 4; }
+
 template <int FLAGS>
 __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams p) {
     constexpr bool PACK = FLAGS & kFPack, COUNT = FLAGS & kFCount, FP32 = FLAGS & kFFp32,
                    HEALTH = FLAGS & kFHealth;
+    constexpr bool STATS = PACK || HEALTH;
     __shared__ double s_red[kThreads / 32][16];
     __shared__ unsigned int s_nan[8], s_inf[8];
     const PlanView pv = plan_view(p.plan, p.T);
@@ -138,6 +154,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
 
     const int W = p.W;
     const bool multi = W > kGroup;           // more than one register group of workers
+    const bool ternary = p.ternary != 0;
     double a[8], q[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) { a[i] = 0.0; q[i] = 0.0; }
@@ -148,7 +165,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
     int t = -1, tile_b = 0, tile_e = 0;
     int64_t off_t = 0, len_t = 0, woff_t = 0;
     bool isL = false, aligned = false;
-    float tau = 0.f;
+    float tau = 0.f, ntau = -0.f;
 
     for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         if (tile >= tile_e) {
@@ -160,47 +177,54 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
             isL = p.route ? (__ldg(p.route + t) == NF_ROUTE_L) : false;
             woff_t = (isL && p.woff) ? __ldg(p.woff + t) : 0;
             tau = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
+            ntau = -tau;
             aligned = (((off_t | p.worker_stride) & 3) == 0);
         }
         const bool do_tile = HEALTH || (isL ? (PACK || COUNT) : FP32);
         if (!do_tile) continue;
-        if (!multi && acc_t != t) {
+        if (STATS && !multi && acc_t != t) {
             if (acc_t >= 0) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
             acc_t = t;
             acc_isL = isL;
         }
-        const int64_t i0 = (int64_t)(tile - tile_b) * kTile + tid * 4;   // tensor-relative, row 0
+        const int64_t tile_base = (int64_t)(tile - tile_b) * kTile;   // tensor-relative
+        const bool full_tile = aligned && (len_t - tile_base >= kTile);
+        int64_t irel[kRows];
         int valid[kRows];
 #pragma unroll
         for (int u = 0; u < kRows; ++u) {
-            int64_t rem = len_t - (i0 + (int64_t)u * kRowElems);
+            irel[u] = tile_base + tile_elem(warp, lane, u);
+            const int64_t rem = len_t - irel[u];
             valid[u] = rem >= 4 ? 4 : (rem > 0 ? (int)rem : 0);
         }
-        uint32_t cp[kRows], cn[kRows];       // byte-packed per-position counts (4 positions each)
+        uint32_t cp[kRows], cn[kRows];       // multi-group: byte-packed per-position counts
+        uint32_t posR[kRows], negR[kRows];
         float4 acc[kRows];                   // FP32-route running sums
 #pragma unroll
         for (int u = 0; u < kRows; ++u) { cp[u] = 0u; cn[u] = 0u; acc[u] = make_float4(0.f, 0.f, 0.f, 0.f); }
 
         for (int w0 = 0; w0 < W; w0 += kGroup) {
             const int nw = min(kGroup, W - w0);
-            const float *gb = p.g + (size_t)w0 * p.worker_stride + off_t + i0;
-            float4 x[kRows][kGroup];
-#pragma unroll
-            for (int u = 0; u < kRows; ++u)
-#pragma unroll
-                for (int w = 0; w < kGroup; ++w)
-                    x[u][w] = (w < nw) ? load4(gb + (size_t)w * p.worker_stride + (size_t)u * kRowElems,
-                                               valid[u], aligned)
-                                       : make_float4(0.f, 0.f, 0.f, 0.f);
-
-            uint32_t posR[kRows], negR[kRows];
+            const float *gb = p.g + (size_t)w0 * p.worker_stride + off_t;
 #pragma unroll
             for (int u = 0; u < kRows; ++u) { posR[u] = 0u; negR[u] = 0u; }
 
+            auto body = [&](auto full_tag) {
+                constexpr bool FULL = decltype(full_tag)::value;   // 8 workers, whole aligned tile
+                float4 x[kRows][kGroup];
 #pragma unroll
-            for (int w = 0; w < kGroup; ++w) {
-                if (w < nw) {
-                    if (PACK || HEALTH) {
+                for (int u = 0; u < kRows; ++u)
+#pragma unroll
+                    for (int w = 0; w < kGroup; ++w) {
+                        const float *src = gb + (size_t)w * p.worker_stride + irel[u];
+                        if (FULL) x[u][w] = ld_stream4(src);
+                        else x[u][w] = (w < nw) ? load4(src, valid[u], aligned) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                uint32_t badmask = 0u;
+#pragma unroll
+                for (int w = 0; w < kGroup; ++w) {
+                    if (!FULL && w >= nw) continue;
+                    if (STATS) {
                         // FP32 over this thread's 8 elements of worker w, then FP64
                         float af = 0.f, qf = 0.f;
 #pragma unroll
@@ -213,41 +237,26 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                             }
                         }
                         // fast path: everything finite and the FP32 squares did not underflow
-                        const bool ok = HEALTH ? ((qf < FLT_MAX) && (qf >= 1e-30f || af == 0.f))
+                        const bool ok = HEALTH ? (((qf >= 1e-30f) && (qf < FLT_MAX)) || af == 0.f)
                                                : (af < FLT_MAX);
-                        if (ok) {
-                            a[w] += (double)af;
-                            if (HEALTH) q[w] += (double)qf;
-                        } else {
-#pragma unroll
-                            for (int u = 0; u < kRows; ++u) {
-                                const float e4[4] = {x[u][w].x, x[u][w].y, x[u][w].z, x[u][w].w};
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) {
-                                    const float v = e4[j];
-                                    a[w] += (double)fabsf(v);
-                                    if (HEALTH) {
-                                        if (v != v) atomicAdd(&s_nan[w], 1u);
-                                        else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[w], 1u);
-                                        else q[w] += (double)v * (double)v;
-                                    }
-                                }
-                            }
-                        }
+                        a[w] += (double)(ok ? af : 0.f);
+                        if (HEALTH) q[w] += (double)(ok ? qf : 0.f);
+                        badmask |= ok ? 0u : (1u << w);
                     }
                     if (isL) {
                         if (PACK || COUNT) {
 #pragma unroll
                             for (int u = 0; u < kRows; ++u) {
                                 const float4 v = x[u][w];
-                                uint32_t pb = (v.x > tau ? 1u : 0u) | (v.y > tau ? 2u : 0u) |
-                                              (v.z > tau ? 4u : 0u) | (v.w > tau ? 8u : 0u);
-                                posR[u] |= pb << (4 * w);
-                                if (p.ternary) {
-                                    const float nt = -tau;
-                                    uint32_t nb = (v.x < nt ? 1u : 0u) | (v.y < nt ? 2u : 0u) |
-                                                  (v.z < nt ? 4u : 0u) | (v.w < nt ? 8u : 0u);
-                                    negR[u] |= nb << (4 * w);
+                                or_if_gt(posR[u], v.x, tau, 1u << (4 * w));
+                                or_if_gt(posR[u], v.y, tau, 2u << (4 * w));
+                                or_if_gt(posR[u], v.z, tau, 4u << (4 * w));
+                                or_if_gt(posR[u], v.w, tau, 8u << (4 * w));
+                                if (ternary) {
+                                    or_if_lt(negR[u], v.x, ntau, 1u << (4 * w));
+                                    or_if_lt(negR[u], v.y, ntau, 2u << (4 * w));
+                                    or_if_lt(negR[u], v.z, ntau, 4u << (4 * w));
+                                    or_if_lt(negR[u], v.w, ntau, 8u << (4 * w));
                                 }
                             }
                         }
@@ -256,7 +265,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
 #pragma unroll
                         for (int u = 0; u < kRows; ++u) {
                             const float4 v = x[u][w];
-                            if (w0 == 0 && w == 0) acc[u] = v;
+                            if (w == 0 && w0 == 0) acc[u] = v;
                             else {
                                 acc[u].x = __fadd_rn(acc[u].x, v.x); acc[u].y = __fadd_rn(acc[u].y, v.y);
                                 acc[u].z = __fadd_rn(acc[u].z, v.z); acc[u].w = __fadd_rn(acc[u].w, v.w);
@@ -264,34 +273,59 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                         }
                     }
                 }
-            }
+                if (STATS && badmask) {
+                    // rare: NaN / Inf / FP32 over- or underflow in this thread's elements -> FP64, exact tallies
+#pragma unroll
+                    for (int w = 0; w < kGroup; ++w) {
+                        if (!((badmask >> w) & 1u)) continue;
+#pragma unroll
+                        for (int u = 0; u < kRows; ++u) {
+                            const float e4[4] = {x[u][w].x, x[u][w].y, x[u][w].z, x[u][w].w};
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                const float v = e4[j];
+                                a[w] += (double)fabsf(v);
+                                if (HEALTH) {
+                                    if (v != v) atomicAdd(&s_nan[w], 1u);
+                                    else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[w], 1u);
+                                    else q[w] += (double)v * (double)v;
+                                }
+                            }
+                        }
+                    }
+                }
+            };
+            if (full_tile && nw == kGroup) body(BoolTag<true>{});
+            else body(BoolTag<false>{});
 
             if (isL && (PACK || COUNT)) {
+                if (COUNT && multi) {
 #pragma unroll
-                for (int u = 0; u < kRows; ++u) {
-                    if (COUNT) {
+                    for (int u = 0; u < kRows; ++u)
 #pragma unroll
                         for (int j = 0; j < 4; ++j) {
                             cp[u] += (uint32_t)__popc(posR[u] & (0x11111111u << j)) << (8 * j);
-                            if (p.ternary) cn[u] += (uint32_t)__popc(negR[u] & (0x11111111u << j)) << (8 * j);
+                            if (ternary) cn[u] += (uint32_t)__popc(negR[u] & (0x11111111u << j)) << (8 * j);
                         }
-                    }
-                    if (PACK && p.P) {
-                        const int64_t wi = ((int64_t)(tile - tile_b) * kTile + (int64_t)u * kRowElems) / 32 +
-                                           warp * 4 + (lane >> 3);
-                        const int wq = lane & 7;
-                        const bool st = (wq < nw) && (wi < (len_t + 31) / 32);
+                }
+                if (PACK && p.P) {
+                    const int wq = lane & 7;
+                    const int64_t nwords = (len_t + 31) >> 5;
+#pragma unroll
+                    for (int u = 0; u < kRows; ++u) {
+                        const int64_t wi = (tile_base >> 5) + warp * (kRows * 4) + u * 4 + (lane >> 3);
+                        const bool st = (wq < nw) && (wi < nwords);
                         const size_t o = (size_t)(w0 + wq) * p.plane_stride + woff_t + wi;
                         const uint32_t pw = nibble_transpose8(posR[u], lane);
                         if (st) p.P[o] = pw;
-                        if (p.ternary) {
+                        if (ternary) {
                             const uint32_t nwd = nibble_transpose8(negR[u], lane);
                             if (st) p.N[o] = nwd;
                         }
                     }
                 }
             }
-            if (multi && (PACK || HEALTH)) flush_stats<FLAGS>(p, fc, a, q, w0, nw, t, isL);
+            if (multi && STATS) flush_stats<FLAGS>(p, fc, a, q, w0, nw, t, isL);
         }
 
         if (isL) {
@@ -299,24 +333,29 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                 // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
 #pragma unroll
                 for (int u = 0; u < kRows; ++u) {
-                    if (valid[u] > 0) {
-                        uint32_t d = 0u;
+                    uint32_t d = 0u;
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int c_p = (cp[u] >> (8 * j)) & 0xff;
-                            const int c_n = p.ternary ? (int)((cn[u] >> (8 * j)) & 0xff) : (W - c_p);
-                            const int D = c_p - c_n;
-                            d |= (D > p.margin ? 1u : 0u) << j;
-                            d |= (D < -p.margin ? 1u : 0u) << (4 + j);
+                    for (int j = 0; j < 4; ++j) {
+                        int c_p, c_n;
+                        if (multi) {
+                            c_p = (cp[u] >> (8 * j)) & 0xff;
+                            c_n = (cn[u] >> (8 * j)) & 0xff;
+                        } else {
+                            c_p = __popc(posR[u] & (0x11111111u << j));
+                            c_n = __popc(negR[u] & (0x11111111u << j));
                         }
-                        p.dirs[(size_t)woff_t * 8 + (size_t)((i0 + (int64_t)u * kRowElems) >> 2)] = (uint8_t)d;
+                        if (!ternary) c_n = W - c_p;
+                        const int D = c_p - c_n;
+                        d |= (D > p.margin ? 1u : 0u) << j;
+                        d |= (D < -p.margin ? 1u : 0u) << (4 + j);
                     }
+                    if (valid[u] > 0) p.dirs[(size_t)woff_t * 8 + (size_t)(irel[u] >> 2)] = (uint8_t)d;
                 }
             }
         } else if (FP32) {
 #pragma unroll
             for (int u = 0; u < kRows; ++u) {
-                float *o = p.out + off_t + i0 + (int64_t)u * kRowElems;
+                float *o = p.out + off_t + irel[u];
                 float4 r = acc[u];
                 r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
                 r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
@@ -331,7 +370,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
             }
         }
     }
-    if (!multi && acc_t >= 0 && (PACK || HEALTH)) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
+    if (STATS && !multi && acc_t >= 0) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
 }
 
 // ---------------------------------------------------------------------------------------------
