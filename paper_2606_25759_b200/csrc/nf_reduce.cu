@@ -199,49 +199,82 @@ __global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReducePar
 
 // Pass B of the fused path: out[off_t+i] = S_t * d for every low-bit element, d from the 2-bit
 // directions pass A left in the workspace (one byte per 4 elements: low nibble +, high nibble -).
-__global__ void __launch_bounds__(kRThreads) decode_kernel(const ReduceParams p) {
+// Write-bound (4 B/element out, 0.25 B/element in). 128-thread CTAs; a warp owns 512 consecutive
+// elements of a tile: each lane loads one 32-bit word of directions (16 elements), the bytes are
+// redistributed by shuffle so that every store instruction writes 512 contiguous bytes; 4 tiles
+// are in flight per thread to cover the load latency.
+constexpr int kDThreads = 128;
+constexpr int kDUnroll = 4;
+
+struct DecodeTensor {
+    int tile_b, tile_e;
+    int64_t off_t, len_t, woff_t;
+    bool isL;
+    float S;
+};
+
+__global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p) {
     extern __shared__ float s_scale[];
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     compute_scales(p, pv, s_scale);
     const int n_tiles = pv.hdr->n_tiles;
-    int t = -1, tile_b = 0, tile_e = 0;
-    int64_t off_t = 0, len_t = 0, woff_t = 0;
-    bool isL = false;
-    float S = 0.f;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        if (tile >= tile_e) {
-            t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
-            tile_b = __ldg(pv.tile_prefix + t);
-            tile_e = __ldg(pv.tile_prefix + t + 1);
-            off_t = __ldg(p.off + t);
-            len_t = __ldg(p.len + t);
-            isL = __ldg(p.route + t) == NF_ROUTE_L;
-            woff_t = isL ? __ldg(p.woff + t) : 0;
-            S = s_scale[t];
-        }
-        if (!isL) continue;
-        const int64_t tb = (int64_t)(tile - tile_b) * kTile;
-        const bool al = (off_t & 3) == 0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    DecodeTensor c{0, 0, 0, 0, 0, false, 0.f};
+    for (int base = blockIdx.x * kDUnroll; base < n_tiles; base += gridDim.x * kDUnroll) {
+        uint32_t dw[kDUnroll];
+        int64_t obase[kDUnroll], rem[kDUnroll];
+        float S[kDUnroll];
 #pragma unroll
-        for (int u = 0; u < kTile / (kRThreads * 4); ++u) {
-            const int64_t i = tb + (int64_t)u * kRThreads * 4 + threadIdx.x * 4;
-            const int64_t rem = len_t - i;
-            if (rem <= 0) continue;
-            const uint32_t d = __ldcs(p.dirs + (size_t)woff_t * 8 + (size_t)(i >> 2));
-            float4 r;
-            r.x = __fmul_rn(S, (float)((int)(d & 1u) - (int)((d >> 4) & 1u)));
-            r.y = __fmul_rn(S, (float)((int)((d >> 1) & 1u) - (int)((d >> 5) & 1u)));
-            r.z = __fmul_rn(S, (float)((int)((d >> 2) & 1u) - (int)((d >> 6) & 1u)));
-            r.w = __fmul_rn(S, (float)((int)((d >> 3) & 1u) - (int)((d >> 7) & 1u)));
-            float *o = p.out + off_t + i;
-            if (rem >= 4 && al) {
-                __stcs(reinterpret_cast<float4 *>(o), r);
-            } else {
-                o[0] = r.x;
-                if (rem > 1) o[1] = r.y;
-                if (rem > 2) o[2] = r.z;
-                if (rem > 3) o[3] = r.w;
+        for (int k = 0; k < kDUnroll; ++k) {
+            const int tile = base + k;
+            rem[k] = 0; dw[k] = 0u; obase[k] = 0; S[k] = 0.f;
+            if (tile >= n_tiles) continue;
+            if (tile >= c.tile_e || tile < c.tile_b) {
+                const int t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
+                c.tile_b = __ldg(pv.tile_prefix + t);
+                c.tile_e = __ldg(pv.tile_prefix + t + 1);
+                c.off_t = __ldg(p.off + t);
+                c.len_t = __ldg(p.len + t);
+                c.isL = __ldg(p.route + t) == NF_ROUTE_L;
+                c.woff_t = c.isL ? __ldg(p.woff + t) : 0;
+                c.S = s_scale[t];
+            }
+            if (!c.isL) continue;
+            const int64_t wbase = (int64_t)(tile - c.tile_b) * kTile + warp * 512;   // tensor-relative
+            const int64_t i = wbase + lane * 16;
+            if (i < c.len_t)
+                dw[k] = __ldcs(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)c.woff_t * 8 + (size_t)(i >> 2)));
+            obase[k] = c.off_t + wbase;
+            rem[k] = c.len_t - wbase;           // elements of this warp's 512 that exist (may be <= 0)
+            S[k] = c.S;
+        }
+#pragma unroll
+        for (int k = 0; k < kDUnroll; ++k) {
+            if (rem[k] <= 0) continue;          // warp-uniform
+            const bool al = (obase[k] & 3) == 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
+                const uint32_t w32 = __shfl_sync(0xffffffffu, dw[k], j * 8 + (lane >> 2));
+                const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
+                const int64_t e0 = j * 128 + lane * 4;
+                const int64_t r = rem[k] - e0;
+                if (r <= 0) continue;
+                float4 v;
+                v.x = __fmul_rn(S[k], (float)((int)(d & 1u) - (int)((d >> 4) & 1u)));
+                v.y = __fmul_rn(S[k], (float)((int)((d >> 1) & 1u) - (int)((d >> 5) & 1u)));
+                v.z = __fmul_rn(S[k], (float)((int)((d >> 2) & 1u) - (int)((d >> 6) & 1u)));
+                v.w = __fmul_rn(S[k], (float)((int)((d >> 3) & 1u) - (int)((d >> 7) & 1u)));
+                float *o = p.out + obase[k] + e0;
+                if (r >= 4 && al) {
+                    __stcs(reinterpret_cast<float4 *>(o), v);
+                } else {
+                    o[0] = v.x;
+                    if (r > 1) o[1] = v.y;
+                    if (r > 2) o[2] = v.z;
+                    if (r > 3) o[3] = v.w;
+                }
             }
         }
     }
@@ -266,8 +299,8 @@ cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s
 cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s) {
     const int64_t max_tiles = n / kTile + p.T;
     const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
-    const int grid = grid_for(max_tiles, 8);
-    decode_kernel<<<grid, kRThreads, smem, s>>>(p);
+    const int grid = grid_for((max_tiles + kDUnroll - 1) / kDUnroll, 16);
+    decode_kernel<<<grid, kDThreads, smem, s>>>(p);
     return cudaGetLastError();
 }
 

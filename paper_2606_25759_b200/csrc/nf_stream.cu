@@ -131,6 +131,7 @@ __device__ __forceinline__ void or_if_lt(uint32_t &r, float x, float t, uint32_t
 }
 
 template <bool B> struct BoolTag { static constexpr bool value = B; };
+template <int I> struct IntTag { static constexpr int value = I; };
 
 // Element owned by (warp, lane) in row u of a tile: each warp covers 256 consecutive elements per
 // tile (two rows of 128), so its packed words of one worker are 8 consecutive words = one 32-byte
@@ -209,8 +210,9 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
 #pragma unroll
             for (int u = 0; u < kRows; ++u) { posR[u] = 0u; negR[u] = 0u; }
 
-            auto body = [&](auto full_tag) {
+            auto body = [&](auto full_tag, auto kind_tag) {
                 constexpr bool FULL = decltype(full_tag)::value;   // 8 workers, whole aligned tile
+                constexpr int KIND = decltype(kind_tag)::value;    // 0: non-L tile, 1: L G-Binary, 2: L G-Ternary
                 float4 x[kRows][kGroup];
 #pragma unroll
                 for (int u = 0; u < kRows; ++u)
@@ -243,7 +245,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                         if (HEALTH) q[w] += (double)(ok ? qf : 0.f);
                         badmask |= ok ? 0u : (1u << w);
                     }
-                    if (isL) {
+                    if (KIND != 0) {
                         if (PACK || COUNT) {
 #pragma unroll
                             for (int u = 0; u < kRows; ++u) {
@@ -252,7 +254,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                                 or_if_gt(posR[u], v.y, tau, 2u << (4 * w));
                                 or_if_gt(posR[u], v.z, tau, 4u << (4 * w));
                                 or_if_gt(posR[u], v.w, tau, 8u << (4 * w));
-                                if (ternary) {
+                                if (KIND == 2) {
                                     or_if_lt(negR[u], v.x, ntau, 1u << (4 * w));
                                     or_if_lt(negR[u], v.y, ntau, 2u << (4 * w));
                                     or_if_lt(negR[u], v.z, ntau, 4u << (4 * w));
@@ -295,8 +297,16 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                     }
                 }
             };
-            if (full_tile && nw == kGroup) body(BoolTag<true>{});
-            else body(BoolTag<false>{});
+            const int kind = isL ? (ternary ? 2 : 1) : 0;
+            if (full_tile && nw == kGroup) {
+                if (kind == 2) body(BoolTag<true>{}, IntTag<2>{});
+                else if (kind == 1) body(BoolTag<true>{}, IntTag<1>{});
+                else body(BoolTag<true>{}, IntTag<0>{});
+            } else {
+                if (kind == 2) body(BoolTag<false>{}, IntTag<2>{});
+                else if (kind == 1) body(BoolTag<false>{}, IntTag<1>{});
+                else body(BoolTag<false>{}, IntTag<0>{});
+            }
 
             if (isL && (PACK || COUNT)) {
                 if (COUNT && multi) {
