@@ -34,16 +34,25 @@ __device__ __forceinline__ float4 load4(const float *p, int valid, bool aligned)
 
 // 8x8 transpose of 4-bit elements held one row per lane across each aligned group of 8 lanes:
 // in : lane q holds nibble u = M[q][u];   out: lane q holds nibble q' = M[q'][q].
-__device__ __forceinline__ uint32_t nibble_transpose8(uint32_t v, int lane) {
+// Three butterfly stages; the 16-bit and 8-bit stages are single byte-permutes (PRMT) with a
+// per-lane selector, the 4-bit stage is a rotate + bit-select.
+struct TransposeCtl { uint32_t sel4, sel2, rot1, mask1; };
+__device__ __forceinline__ TransposeCtl make_transpose_ctl(int lane) {
+    TransposeCtl c;
+    c.sel4 = (lane & 4) ? 0x3276u : 0x5410u;     // [t2 t3 v2 v3] : [v0 v1 t0 t1]
+    c.sel2 = (lane & 2) ? 0x3715u : 0x6240u;     // [t1 v1 t3 v3] : [v0 t0 v2 t2]
+    c.rot1 = (lane & 1) ? 28u : 4u;              // t >> 4 : t << 4 (as a rotate)
+    c.mask1 = (lane & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
+    return c;
+}
+__device__ __forceinline__ uint32_t nibble_transpose8(uint32_t v, const TransposeCtl &c) {
     uint32_t t = __shfl_xor_sync(0xffffffffu, v, 4);
-    v = (lane & 4) ? ((v & 0xffff0000u) | (t >> 16)) : ((v & 0x0000ffffu) | (t << 16));
+    v = __byte_perm(v, t, c.sel4);
     t = __shfl_xor_sync(0xffffffffu, v, 2);
-    v = (lane & 2) ? ((v & 0xff00ff00u) | ((t & 0xff00ff00u) >> 8))
-                   : ((v & 0x00ff00ffu) | ((t & 0x00ff00ffu) << 8));
+    v = __byte_perm(v, t, c.sel2);
     t = __shfl_xor_sync(0xffffffffu, v, 1);
-    v = (lane & 1) ? ((v & 0xf0f0f0f0u) | ((t & 0xf0f0f0f0u) >> 4))
-                   : ((v & 0x0f0f0f0fu) | ((t & 0x0f0f0f0fu) << 4));
-    return v;
+    t = __funnelshift_l(t, t, c.rot1);
+    return (v & c.mask1) | (t & ~c.mask1);
 }
 
 // Warp reduce-scatter of 16 doubles: on return v[0] of lane l holds the warp total of value
@@ -152,6 +161,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
     if (tid < 8) { s_nan[tid] = 0u; s_inf[tid] = 0u; }
     __syncthreads();
     const FlushCtx fc{s_red, s_nan, s_inf};
+    const TransposeCtl tctl = make_transpose_ctl(lane);
 
     const int W = p.W;
     const bool multi = W > kGroup;           // more than one register group of workers
@@ -222,6 +232,20 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                         if (FULL) x[u][w] = ld_stream4(src);
                         else x[u][w] = (w < nw) ? load4(src, valid[u], aligned) : make_float4(0.f, 0.f, 0.f, 0.f);
                     }
+                if (FULL) {
+                    // pull the unit this CTA visits next into L2 while this one is being computed:
+                    // 8 workers x 1 KB per warp = 64 lines, two per lane
+                    const float *nb = nullptr;
+                    if (w0 + 2 * kGroup <= W) nb = gb + (size_t)kGroup * p.worker_stride + tile_base;
+                    else if (w0 + kGroup >= W && tile + (int)gridDim.x < tile_e &&
+                             len_t - (tile_base + (int64_t)gridDim.x * kTile) >= kTile)
+                        nb = p.g + off_t + tile_base + (int64_t)gridDim.x * kTile;
+                    if (nb) {
+                        const float *l = nb + (size_t)(lane >> 2) * p.worker_stride + warp * (kRows * 128) + (lane & 3) * 32;
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(l));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(l + 128));
+                    }
+                }
                 uint32_t badmask = 0u;
 #pragma unroll
                 for (int w = 0; w < kGroup; ++w) {
@@ -326,10 +350,10 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                         const int64_t wi = (tile_base >> 5) + warp * (kRows * 4) + u * 4 + (lane >> 3);
                         const bool st = (wq < nw) && (wi < nwords);
                         const size_t o = (size_t)(w0 + wq) * p.plane_stride + woff_t + wi;
-                        const uint32_t pw = nibble_transpose8(posR[u], lane);
+                        const uint32_t pw = nibble_transpose8(posR[u], tctl);
                         if (st) p.P[o] = pw;
                         if (ternary) {
-                            const uint32_t nwd = nibble_transpose8(negR[u], lane);
+                            const uint32_t nwd = nibble_transpose8(negR[u], tctl);
                             if (st) p.N[o] = nwd;
                         }
                     }
