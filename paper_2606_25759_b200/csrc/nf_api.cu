@@ -1,5 +1,6 @@
 // nf_api.cu — the extern "C" entry points declared in include/nf.h: argument checks that can be
 // made on the host, then kernel launches on the caller's stream. No allocation, no sync.
+#include <stdlib.h>
 #include "nf_internal.cuh"
 
 using namespace nf;
@@ -61,7 +62,7 @@ int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig,
     if (T > 0 && (!off || !len || !elig || !route || !woff)) return NF_ERR_ARG;
     if (misaligned16(plan)) return NF_ERR_ALIGN;
     return cuda_rc(launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
-                                nullptr, nullptr, nullptr, nullptr, 0, (cudaStream_t)stream));
+                                nullptr, nullptr, nullptr, nullptr, 0, 0, (cudaStream_t)stream));
 }
 
 int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
@@ -177,7 +178,7 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     // a1 (+ zeroing of the accumulators, so no memset nodes sit on the stream)
     cudaError_t e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
                                  abs_sum, sumsq, (unsigned long long *)nan_cnt,
-                                 (unsigned long long *)inf_cnt, (int64_t)W * T, s);
+                                 (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
     if (T == 0 || n == 0) return NF_OK;
     prof_mark(1, s);
@@ -190,7 +191,16 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.abs_sum = abs_sum; p.sumsq = sumsq;
     p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
     p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
-    e = launch_stream(health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32), p, n, s);
+    // W <= 8: full tiles of aligned tensors go through the TMA-ring kernel (nf_fused.cu); the LDG
+    // streaming kernel takes the rest (ragged tails, unaligned tensors) or, for W > 8, everything.
+    static const bool use_ldg = getenv("NF_PASSA_LDG") != nullptr;   // A/B aid
+    const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);
+    if (W <= 8 && !use_ldg) {
+        e = launch_fused_passA(health, p, n, s);
+        if (e != cudaSuccess) return NF_ERR_CUDA;
+        p.skip_fast = 1;
+    }
+    e = launch_stream(flags, p, n, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
     prof_mark(2, s);
     // pass B: scale x direction for the low-bit positions

@@ -29,7 +29,7 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     int64_t n;
     int64_t Wd;                            // total packed words per worker plane
     int32_t n_tiles;
-    int32_t pad0;
+    int32_t n_unaligned;                   // non-empty tensors whose rows are not 16-byte aligned
     int64_t pad1[3];
 };
 
@@ -101,6 +101,7 @@ struct StreamParams {
     float *out;                // [n]
     uint8_t *dirs;             // workspace: one byte per 4 low-bit elements (lo nibble +, hi nibble -)
     void *plan;
+    int skip_fast;             // LDG kernel: leave the 16-byte-aligned tensors to the TMA-ring kernel
 };
 
 enum : int {
@@ -135,8 +136,9 @@ struct ReduceParams {
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
                          nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
                          double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, cudaStream_t s);
+                         int64_t zcount, int64_t worker_stride, cudaStream_t s);
 cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStream_t s);
+cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s);
 int device_sm_count();

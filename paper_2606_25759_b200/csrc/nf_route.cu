@@ -59,7 +59,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
              const uint8_t *__restrict__ elig, int T, int64_t n, nf_state st,
              uint8_t *__restrict__ route, int64_t *__restrict__ woff, int64_t *__restrict__ summary,
              void *plan, double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-             int64_t zcount) {
+             int64_t zcount, int64_t worker_stride) {
     __shared__ Scan3 s_scan[33];
     PlanLayout L = plan_layout(T);
     char *pb = (char *)plan;
@@ -78,6 +78,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
 
     Scan3 carry{0, 0, 0};
     long long nF = 0, nP = 0, e = 0, tot = 0;   // per-thread partials, reduced at the end
+    int unal = 0;
     int bad = 0;
     for (int base = 0; base < T; base += kRouteThreads) {
         const int t = base + threadIdx.x;
@@ -96,6 +97,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
             else if (st.veto || !st.capacity_ok) r = NF_ROUTE_F;
             else r = NF_ROUTE_L;
             v.tiles = (l + kTile - 1) / kTile;
+            if (l > 0 && (((o | worker_stride) & 3) != 0)) ++unal;
             tot += l;
             if (r == NF_ROUTE_L) { v.words = (l + 31) / 32; v.nl = 1; e += l; }
             else if (r == NF_ROUTE_F) ++nF;
@@ -114,14 +116,15 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     }
     // block-reduce the small tallies through shared memory atomics
     __shared__ unsigned long long s_tal[4];
-    __shared__ int s_bad;
-    if (threadIdx.x == 0) { s_tal[0] = s_tal[1] = s_tal[2] = s_tal[3] = 0ull; s_bad = 0; }
+    __shared__ int s_bad, s_unal;
+    if (threadIdx.x == 0) { s_tal[0] = s_tal[1] = s_tal[2] = s_tal[3] = 0ull; s_bad = 0; s_unal = 0; }
     __syncthreads();
     if (nF) atomicAdd(&s_tal[0], (unsigned long long)nF);
     if (nP) atomicAdd(&s_tal[1], (unsigned long long)nP);
     if (e) atomicAdd(&s_tal[2], (unsigned long long)e);
     if (tot) atomicAdd(&s_tal[3], (unsigned long long)tot);
     if (bad) atomicOr(&s_bad, 1);
+    if (unal) atomicAdd(&s_unal, unal);
     __syncthreads();
     if (threadIdx.x == 0) {
         int status = NF_OK;
@@ -135,7 +138,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
         hdr->n = n;
         hdr->Wd = carry.words;
         hdr->n_tiles = (status == NF_OK) ? (int32_t)carry.tiles : 0;
-        hdr->pad0 = 0;
+        hdr->n_unaligned = s_unal;
         summary[NF_SUM_WD] = carry.words;
         summary[NF_SUM_NL] = carry.nl;
         summary[NF_SUM_NF] = (int64_t)s_tal[0];
@@ -150,9 +153,9 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
                          nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
                          double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, cudaStream_t s) {
+                         int64_t zcount, int64_t worker_stride, cudaStream_t s) {
     route_kernel<<<1, kRouteThreads, 0, s>>>(off, len, elig, T, n, st, route, woff, summary, plan,
-                                             z0, z1, z2, z3, zcount);
+                                             z0, z1, z2, z3, zcount, worker_stride);
     return cudaGetLastError();
 }
 

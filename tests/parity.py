@@ -100,5 +100,17 @@ def run_both(g: torch.Tensor, off, length, elig, state=(1, 0, 1), mode=O.MODE_GT
     cover = np.zeros(n, bool)
     for o, l in zip(off, length):
         cover[o:o + l] = True
-    assert np.array_equal(a[m & cover], b[m & cover]), what + " fused vs 5-call out"
+    # same directions everywhere; magnitudes (the per-tensor scale, summed in a different order by
+    # the two paths) within twice the oracle tolerance of each other; FP32-route values identical
+    sel = m & cover
+    assert np.array_equal(np.sign(a[sel]), np.sign(b[sel])), what + " fused vs 5-call directions"
+    fin = sel & np.isfinite(a) & np.isfinite(b)
+    assert np.all(np.abs(a[fin] - b[fin]) <= 2 * RTOL_OUT * np.abs(b[fin])), what + " fused vs 5-call out"
+    inf = sel & ~np.isfinite(a)
+    assert np.array_equal(a[inf], b[inf]), what + " fused vs 5-call inf"
+    isP = cover.copy()
+    for o, l, r in zip(off, length, ref.route.route):
+        if r == O.ROUTE_L:
+            isP[o:o + l] = False
+    assert np.array_equal(a[m & isP], b[m & isP]), what + " fused vs 5-call FP32 route"
     return ref
