@@ -14,6 +14,7 @@ inline void prof_mark(int slot, cudaStream_t s) {
     if (g_prof_ev && g_prof_n < g_prof_cap) cudaEventRecord(g_prof_ev[4 * g_prof_n + slot], s);
 }
 
+unsigned long long *g_trace = nullptr;   // debug (nf_debug_trace): per-CTA time stamps of the fused kernel
 inline bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NF_OK : NF_ERR_CUDA; }
 
@@ -62,7 +63,7 @@ int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig,
     if (T > 0 && (!off || !len || !elig || !route || !woff)) return NF_ERR_ARG;
     if (misaligned16(plan)) return NF_ERR_ALIGN;
     return cuda_rc(launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
-                                nullptr, nullptr, nullptr, nullptr, 0, 0, (cudaStream_t)stream));
+                                nullptr, nullptr, nullptr, nullptr, 0, 0, 0, (cudaStream_t)stream));
 }
 
 int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
@@ -173,12 +174,15 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     if (misaligned16(g) || misaligned16(out) || misaligned16(P) || misaligned16(N) ||
         misaligned16(plan) || misaligned16(workspace))
         return NF_ERR_ALIGN;
+    static const bool use_ldg = getenv("NF_PASSA_LDG") != nullptr;   // A/B aid: register-staged pass A + decode kernel
+    static const bool use_pdl = getenv("NF_NO_PDL") == nullptr;            // A/B aid: plain stream-ordered launches
+    static const bool sep_decode = getenv("NF_DECODE_SEPARATE") != nullptr;   // A/B aid: pass B as its own kernel
     cudaStream_t s = (cudaStream_t)stream;
     prof_mark(0, s);
     // a1 (+ zeroing of the accumulators, so no memset nodes sit on the stream)
     cudaError_t e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
                                  abs_sum, sumsq, (unsigned long long *)nan_cnt,
-                                 (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, s);
+                                 (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, use_pdl ? 1 : 0, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
     if (T == 0 || n == 0) return NF_OK;
     prof_mark(1, s);
@@ -191,16 +195,20 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.abs_sum = abs_sum; p.sumsq = sumsq;
     p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
     p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
+    p.scale_out = scale_out;
+    p.trace = g_trace;
+    p.separate_decode = sep_decode ? 1 : 0;
+    p.pdl = use_pdl ? 1 : 0;
     // W <= 8: full tiles of aligned tensors go through the TMA-ring kernel (nf_fused.cu); the LDG
     // streaming kernel takes the rest (ragged tails, unaligned tensors) or, for W > 8, everything.
-    static const bool use_ldg = getenv("NF_PASSA_LDG") != nullptr;   // A/B aid
     const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);
     if (W <= 8 && !use_ldg) {
         e = launch_fused_passA(health, p, n, s);
         if (e != cudaSuccess) return NF_ERR_CUDA;
         p.skip_fast = 1;
     }
-    e = launch_stream(flags, p, n, s);
+    static const bool skip_ldg = getenv("NF_SKIP_LDG") != nullptr;   // timing aid only (wrong results for unaligned tensors)
+    if (!(skip_ldg && p.skip_fast)) e = launch_stream(flags, p, n, s);
     if (e != cudaSuccess) return NF_ERR_CUDA;
     prof_mark(2, s);
     // pass B: scale x direction for the low-bit positions
@@ -208,10 +216,22 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     r.W = W; r.T = T; r.off = off; r.len = len; r.route = route; r.woff = woff;
     r.abs_sum = abs_sum; r.out = out; r.scale_out = scale_out;
     r.dirs = (const uint8_t *)workspace; r.plan = plan;
+    r.worker_stride = worker_stride;
+    r.pdl = use_pdl ? 1 : 0;
+    r.only_unaligned = (W <= 8 && !use_ldg && !sep_decode) ? 1 : 0;      // the TMA-ring kernel decoded the aligned tensors itself
     e = launch_decode(r, n, s);
     prof_mark(3, s);
     if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;
     return cuda_rc(e);
+}
+
+// debug, not in nf.h: enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;
+// with `out` != NULL the stamps are copied to the host (synchronises).
+int nf_debug_trace(int on, unsigned long long *out) {
+    if (on && !g_trace) { if (cudaMalloc(&g_trace, 256 * 8 * 8) != cudaSuccess) return NF_ERR_CUDA; cudaMemset(g_trace, 0, 256 * 8 * 8); }
+    if (out && g_trace && cudaMemcpy(out, g_trace, 256 * 8 * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return NF_ERR_CUDA;
+    if (!on && g_trace) { cudaFree(g_trace); g_trace = nullptr; }
+    return NF_OK;
 }
 
 int nf_prof_enable(int max_records) {

@@ -25,7 +25,9 @@ namespace nf {
 
 constexpr int kCW = 16;                          // consumer warps
 constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = one tile
-constexpr int kFThreads = kCThreads + 64;         // + producer warp + tail warp
+constexpr int kDW = 2;                           // decode warps (pass B inside the kernel)
+constexpr int kFThreads = kCThreads + 64 + kDW * 32;   // + producer warp + housekeeping warp + decode warps
+constexpr int kDU = 4;                           // decode: tiles in flight per warp
 constexpr int kStageFloats = kGroup * kTile;     // 8 workers x 2048 elements
 constexpr int kStageBytes = kStageFloats * 4;    // 64 KB
 constexpr int kKTiles = 4;                       // tiles of FP32 partial accumulation
@@ -131,14 +133,18 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 // shared-memory carve-up (dynamic). Everything the hot loop touches sits at a compile-time offset:
 //   [0, 64)      mbarriers full[4], empty[4]
 //   [64, 2112)   NaN / Inf tallies, 256 workers each
-//   [4096, ...)  ring [stages][8][kTile] floats
+//   [3072, 3088) tile index carried by each ring stage (dynamic tile scheduling)
+//   [4096, 8192) decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
+//   [8192, ...)  ring [stages][8][kTile] floats
 //   after ring   per-warp FP64 totals {abs, sq} per worker: [kCW][2*W] doubles
 // ---------------------------------------------------------------------------------------------
-constexpr int kSmemHdr = 4096;
+constexpr int kSmemHdr = 8192;
 struct FusedSmem {
     float *ring;
     uint64_t *full, *empty;
     unsigned int *nan, *inf;
+    int *tile_of;                // [kMaxStages] tile held by a stage, -1 = no more tiles
+    float4 *dtab;                // [256]
     double *wacc;
 };
 __host__ __device__ inline size_t fused_smem_bytes(int stages, int W) {
@@ -150,6 +156,8 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.empty = s.full + kMaxStages;
     s.nan = (unsigned int *)(base + 64);
     s.inf = s.nan + 256;
+    s.tile_of = (int *)(base + 3072);
+    s.dtab = (float4 *)(base + 4096);
     s.ring = (float *)(base + kSmemHdr);
     s.wacc = (double *)(base + kSmemHdr + (size_t)stages * kStageBytes);
     return s;
@@ -174,29 +182,50 @@ __device__ __forceinline__ void tensor_lookup(const StreamParams &p, const PlanV
     c.tau = (p.tau && c.isL) ? __ldg(p.tau + t) : 0.f;
     c.aligned = (((c.off | p.worker_stride) & 3) == 0);
 }
-// Exact FP64 re-read of one thread's elements of worker `wg` over the last `cnt` bulk tiles of the
-// current tensor (rare: NaN / Inf / FP32 range trouble in the FP32 partials). Returns
+// Exact FP64 re-read of one thread's elements of worker `wg` over the last `cnt` (<= 4) tiles of the
+// current tensor (`recent`, most recent first) (rare: NaN / Inf / FP32 range trouble in the FP32 partials). Returns
 // {sum |x|, sum of x^2 over finite x}; NaN / Inf are tallied in shared memory slot `slot`.
 template <bool HEALTH>
 __device__ __noinline__ double2 exact_redo(const float *__restrict__ g, int64_t worker_stride, int wg,
-                                           int64_t off_t, int64_t len_t, int tile_b, int last_tile, int cnt,
-                                           int tile_step, int ctid, unsigned int *s_nan, unsigned int *s_inf,
-                                           int slot) {
+                                           int64_t off_t, int64_t len_t, int tile_b, int4 recent, int cnt, int ctid,
+                                           unsigned int *s_nan, unsigned int *s_inf, int slot) {
     double da = 0.0, dq = 0.0;
     const float *row = g + (size_t)wg * worker_stride + off_t;
-    for (int j = 0; j < cnt; ++j) {
-        const int64_t base = (int64_t)(last_tile - j * tile_step - tile_b) * kTile + 4 * ctid;
+    // all loads first (independent, one round trip), then the arithmetic
+    float x[4][4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int tl = j == 0 ? recent.x : (j == 1 ? recent.y : (j == 2 ? recent.z : recent.w));
+        const int64_t base = (int64_t)(tl - tile_b) * kTile + 4 * ctid;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) x[j][k] = 0.f;
+        if (j < cnt) {
+            if (base + 4 <= len_t) {                         // rows of the ring tiles are 16-byte aligned
+                const float4 v = __ldg(reinterpret_cast<const float4 *>(row + base));
+                x[j][0] = v.x; x[j][1] = v.y; x[j][2] = v.z; x[j][3] = v.w;
+            } else {
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+                    if (base + k < len_t) x[j][k] = __ldg(row + base + k);
+            }
+        }
+    }
+    unsigned cn = 0u, ci = 0u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
         for (int k = 0; k < 4; ++k) {
-            const int64_t i = base + k;
-            if (i >= len_t) break;
-            const float v = __ldg(row + i);
+            const float v = x[j][k];                         // padding zeros add nothing
             da += (double)fabsf(v);
             if (HEALTH) {
-                if (v != v) atomicAdd(&s_nan[slot], 1u);
-                else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[slot], 1u);
+                if (v != v) ++cn;
+                else if (fabsf(v) == INFINITY) ++ci;
                 else dq += (double)v * (double)v;
             }
         }
+    if (HEALTH) {
+        if (cn) atomicAdd(&s_nan[slot], cn);
+        if (ci) atomicAdd(&s_inf[slot], ci);
     }
     return make_double2(da, dq);
 }
@@ -261,6 +290,44 @@ __device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)
     }
     return acc;
 }
+// Ragged last tile of a tensor (need < kTile elements): the ring holds the whole float4s; the one
+// thread that owns the partial float4 reads its 1..3 elements from global memory; threads past the
+// end see zeros. One instantiation, uniform branches on the tile kind.
+template <bool HEALTH>
+__device__ __forceinline__ void ragged_tile(const float *sb, const float *grow, int64_t worker_stride, int nw, int valid,
+                                            bool isL, bool ternary, float tau, float ntau, float (&af)[8],
+                                            float (&qf)[8], uint32_t &posR, uint32_t &negR, float4 &acc) {
+#pragma unroll
+    for (int w = 0; w < kGroup; ++w) {
+        if (w >= nw) break;
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (valid == 4) {
+            v = *reinterpret_cast<const float4 *>(sb + w * kTile);
+        } else if (valid > 0) {
+            const float *g = grow + (size_t)w * worker_stride;
+            v.x = __ldg(g);
+            if (valid > 1) v.y = __ldg(g + 1);
+            if (valid > 2) v.z = __ldg(g + 2);
+        }
+        if (isL || HEALTH) {
+            af[w] += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
+            if (HEALTH) {
+                qf[w] = fmaf(v.x, v.x, qf[w]); qf[w] = fmaf(v.y, v.y, qf[w]);
+                qf[w] = fmaf(v.z, v.z, qf[w]); qf[w] = fmaf(v.w, v.w, qf[w]);
+            }
+        }
+        if (isL) {
+            posR |= ((v.x > tau ? 1u : 0u) | (v.y > tau ? 2u : 0u) | (v.z > tau ? 4u : 0u) | (v.w > tau ? 8u : 0u)) << (4 * w);
+            if (ternary)
+                negR |= ((v.x < ntau ? 1u : 0u) | (v.y < ntau ? 2u : 0u) | (v.z < ntau ? 4u : 0u) | (v.w < ntau ? 8u : 0u)) << (4 * w);
+        } else if (w == 0) {
+            acc = v;
+        } else {
+            acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
+            acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
+        }
+    }
+}
 // majority vote of one thread's 4 positions, single worker group (readings #3, #5, #6):
 // low nibble = "+" flags, high nibble = "-" flags
 template <bool TERNARY>
@@ -284,7 +351,7 @@ __device__ __forceinline__ uint32_t vote4(uint32_t posR, uint32_t negR, int W, i
 template <bool HEALTH>
 __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, float (&af)[8], float (&qf)[8],
                                            int64_t off_t, int64_t len_t, int tile_b, int w0, int nw, int cnt,
-                                           int last_tile, int tile_step, int ctid) {
+                                           int4 recent, int ctid) {
     const int lane = ctid & 31, warp = ctid >> 5, W = p.W;
     float v16[16];
 #pragma unroll
@@ -312,8 +379,8 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
                                          : (a_t <= FLT_MAX);
                 double2 e = make_double2((double)a_t, (double)q_t);
                 if (!ok_t)
-                    e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, last_tile, cnt,
-                                           tile_step, ctid, sm.nan, sm.inf, w0 + w);
+                    e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, recent, cnt, ctid, sm.nan,
+                                           sm.inf, w0 + w);
                 const double ea = warp_sum(e.x), eq = warp_sum(e.y);
                 if (lane == 0) { slot[w * 2] += ea; slot[w * 2 + 1] += eq; }
             } else if ((lane & 1) == 0 && wl == w) {
@@ -326,98 +393,117 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
     __syncwarp();
 }
 
+__device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
+    if (p.trace) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        p.trace[(size_t)blockIdx.x * 8 + slot] = t;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
-// tail warp: the LAST tile of every 16-byte-aligned tensor (the only tile that can be ragged),
-// straight from global memory, one warp per tile, 128 elements per step. Runs beside the
-// consumers; statistics are exact FP64 and go to the global accumulators with one warp-reduced
-// atomic per worker. Same arithmetic as the fast path (oracle O2-O4b).
+// pass B inside the kernel: out[off_t+i] = S_t * d for the low-bit tiles this CTA owns, as soon as
+// tensor t is complete (all its tiles published by every CTA: plan.done[t] == tiles of t). A unit
+// is half a tile (1024 elements); warps take kDU units at a time from a per-CTA cursor in shared
+// memory, in tile order, so the wait is always on the earliest unfinished tensor. The dedicated
+// decode warps overlap their stores with the consumers' reads of later tensors; the consumers
+// join when their own tiles are done. Every store instruction writes 512 contiguous bytes.
 // ---------------------------------------------------------------------------------------------
-template <bool HEALTH>
-__device__ __forceinline__ void tail_tile_warp(const StreamParams &p, const TensorCur &c, int lane) {
-    const int W = p.W, T = p.T;
-    const bool ternary = p.ternary != 0;
-    const TCtl tctl = make_tctl(lane);
-    const float tau = c.tau, ntau = -c.tau;
-    const int64_t tile_base = (int64_t)(c.tile_e - 1 - c.tile_b) * kTile;
-    const int need = (int)(c.len - tile_base);                 // 1..kTile
-    const int64_t nwords = (c.len + 31) >> 5;
-    double a[kGroup], q[kGroup];
-    unsigned cnan[kGroup], cinf[kGroup];
+__device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const float4 *dtab,
+                                             int n_tiles, int lane) {
+    const int W = p.W;
+    const int total_units = n_tiles * 2;
+    int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
+    int t_cur = -1, tile_b = 0, tile_e = 0;
+    int64_t off_t = 0, len_t = 0, woff_t = 0;
+    bool dec = false;
+    float S_t = 0.f;
+    const bool trace_me = p.trace && threadIdx.x == 0;
+    bool first_wait = true;
+    unsigned long long nunits = 0;
+    for (;;) {
+        int u0 = 0;
+        if (lane == 0) u0 = atomicAdd(cursor, kDU);
+        u0 = __shfl_sync(0xffffffffu, u0, 0);
+        if (u0 >= total_units) break;
+        uint32_t dv[kDU][2];
+        int64_t obase[kDU], rem[kDU];
+        float S[kDU];
 #pragma unroll
-    for (int w = 0; w < kGroup; ++w) { a[w] = 0.0; q[w] = 0.0; cnan[w] = 0u; cinf[w] = 0u; }
-    for (int e0 = 0; e0 < need; e0 += 128) {
-        const int rem = need - e0 - 4 * lane;
-        const int valid = rem >= 4 ? 4 : (rem > 0 ? rem : 0);
-        const int64_t irel = tile_base + e0 + 4 * lane;
-        uint32_t posR = 0u, negR = 0u;
-        float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-        for (int w = 0; w < kGroup; ++w) {
-            if (w >= W) break;
-            const float *row = p.g + (size_t)w * p.worker_stride + c.off + irel;
-            float x[4] = {0.f, 0.f, 0.f, 0.f};
-            if (valid == 4) {
-                const float4 v = __ldcs(reinterpret_cast<const float4 *>(row));
-                x[0] = v.x; x[1] = v.y; x[2] = v.z; x[3] = v.w;
-            } else {
-#pragma unroll
-                for (int k = 0; k < 3; ++k)
-                    if (k < valid) x[k] = __ldcs(row + k);
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const float v = x[k];
-                if (c.isL || HEALTH) a[w] += (double)fabsf(v);
-                if (HEALTH) {
-                    if (v != v) ++cnan[w];
-                    else if (fabsf(v) == INFINITY) ++cinf[w];
-                    else q[w] += (double)v * (double)v;
+        for (int k = 0; k < kDU; ++k) {
+            const int u = u0 + k;
+            rem[k] = 0; obase[k] = 0; S[k] = 0.f; dv[k][0] = 0u; dv[k][1] = 0u;
+            if (u >= total_units) continue;
+            const int tile = u >> 1;
+            if (tile >= tile_e) {
+                t_cur = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
+                tile_b = __ldg(pv.tile_prefix + t_cur);
+                tile_e = __ldg(pv.tile_prefix + t_cur + 1);
+                off_t = __ldg(p.off + t_cur);
+                len_t = __ldg(p.len + t_cur);
+                dec = (__ldg(p.route + t_cur) == NF_ROUTE_L) && (((off_t | p.worker_stride) & 3) == 0);
+                if (dec) {
+                    woff_t = __ldg(p.woff + t_cur);
+                    const int total = tile_e - tile_b;
+                    const int *dp = pv.done + t_cur;
+                    int seen;
+                    for (unsigned spins = 0;; ++spins) {
+                        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(dp) : "memory");
+                        if (seen >= total) break;
+                        __nanosleep(4000);
+                        if (spins > (1u << 20)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
+                    }
+                    S_t = tensor_scale(p.abs_sum, W, p.T, t_cur, len_t);
+                    if (trace_me) { trace_stamp(p, first_wait ? 5 : 7); first_wait = false; }
                 }
-                if (c.isL) {
-                    if (v > tau) posR |= (1u << k) << (4 * w);
-                    if (ternary && v < ntau) negR |= (1u << k) << (4 * w);
-                } else {
-                    acc[k] = (w == 0) ? v : __fadd_rn(acc[k], v);
-                }
             }
+            if (!dec) continue;
+            ++nunits;
+            if (tile == tile_b && (u & 1) == 0 && lane == 0) {
+                pv.scale[t_cur] = S_t;
+                if (p.scale_out) p.scale_out[t_cur] = S_t;
+            }
+            const int64_t wbase = (int64_t)(tile - tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int64_t i = wbase + h * 512 + lane * 16;
+                if (i < len_t)
+                    dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)woff_t * 8 + (size_t)(i >> 2)));
+            }
+            obase[k] = off_t + wbase;
+            rem[k] = len_t - wbase;
+            S[k] = S_t;
         }
-        if (c.isL) {
-            if (p.P) {
-                const int64_t wi = (irel >> 5);                 // same word for the 8 lanes of an octet
-                const bool stp = ((lane & 7) < W) && (wi < nwords) && (e0 + 32 * (lane >> 3) < need);
-                const size_t o = (size_t)(lane & 7) * p.plane_stride + c.woff + wi;
-                const uint32_t pw = nib_transpose8(posR, tctl);
-                if (stp) p.P[o] = pw;
-                if (ternary) {
-                    const uint32_t nwd = nib_transpose8(negR, tctl);
-                    if (stp) p.N[o] = nwd;
+#pragma unroll
+        for (int k = 0; k < kDU; ++k) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int64_t rh = rem[k] - h * 512;
+                if (rh <= 0) continue;                       // warp-uniform
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
+                    const uint32_t w32 = __shfl_sync(0xffffffffu, dv[k][h], j * 8 + (lane >> 2));
+                    const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
+                    const int64_t e0 = j * 128 + lane * 4;
+                    const int64_t r = rh - e0;
+                    if (r <= 0) continue;
+                    float4 v = dtab[d];
+                    v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
+                    v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
+                    float *o = p.out + obase[k] + h * 512 + e0;
+                    if (r >= 4) {
+                        __stcs(reinterpret_cast<float4 *>(o), v);
+                    } else {
+                        o[0] = v.x;
+                        if (r > 1) o[1] = v.y;
+                        if (r > 2) o[2] = v.z;
+                    }
                 }
             }
-            const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
-            if (valid > 0) p.dirs[(size_t)c.woff * 8 + (size_t)(irel >> 2)] = (uint8_t)d;
-        } else {
-            float *o = p.out + c.off + irel;
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (k < valid) o[k] = __fmul_rn(p.alpha, acc[k]);
         }
     }
-#pragma unroll
-    for (int w = 0; w < kGroup; ++w) {
-        if (w >= W) break;
-        const double da = warp_sum(a[w]);
-        const size_t o = (size_t)w * T + c.t;
-        if (HEALTH) {
-            const double dq = warp_sum(q[w]);
-            const unsigned n1 = warp_sum(cnan[w]), n2 = warp_sum(cinf[w]);
-            if (lane == 0) {
-                if (dq != 0.0) atomicAdd(p.sumsq + o, dq);
-                if (n1) atomicAdd(p.nan_cnt + o, (unsigned long long)n1);
-                if (n2) atomicAdd(p.inf_cnt + o, (unsigned long long)n2);
-            }
-        }
-        if (lane == 0 && c.isL && da != 0.0) atomicAdd(p.abs_sum + o, da);
-    }
+    if (trace_me) p.trace[(size_t)blockIdx.x * 8 + 6] = nunits;
 }
 
 extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -427,21 +513,28 @@ extern __shared__ __align__(128) unsigned char smem_raw[];
 // ---------------------------------------------------------------------------------------------
 template <bool HEALTH>
 __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ StreamParams p) {
-    const PlanView pv = plan_view(p.plan, p.T);
-    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     constexpr int stages = kStages;
     const FusedSmem sm = carve(smem_raw, stages);
-    const int n_tiles = pv.hdr->n_tiles;
     const int W = p.W;                          // 1..8: one worker group (launch_fused_passA)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_launch_dependents();
 
     if (tid == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(sm.full + s, 1); mbar_init(sm.empty + s, kCW); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < 256; i += kFThreads) { sm.nan[i] = 0u; sm.inf[i] = 0u; }
+    for (int i = tid; i < 256; i += kFThreads)
+        sm.dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
+                                 (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
     for (int i = tid; i < kCW * 2 * W; i += kFThreads) sm.wacc[i] = 0.0;
     __syncthreads();
+    // everything above touched shared memory only and overlapped the route kernel (PDL); the plan
+    // and the zeroed accumulators are visible after this point
+    pdl_wait();
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    const int n_tiles = pv.hdr->n_tiles;
 
     // =========================================================================================
     // producer: one elected lane issues the bulk copies of every fast tile
@@ -453,41 +546,63 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         uint32_t ph = 0;
         TensorCur c{};
         c.tile_e = 0;
-        // full tiles of aligned tensors (the consumers walk exactly the same sequence)
-        {
-            for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-                if (tile >= c.tile_e) tensor_lookup(p, pv, tile, c);
-                if (!c.aligned || tile + 1 >= c.tile_e) continue;
-                const float *src = p.g + c.off + (int64_t)(tile - c.tile_b) * kTile;
+        // Dynamic tile scheduling: tiles are handed out by a device-wide cursor, so a CTA that runs
+        // ahead (SM position, co-running decode warps) simply takes more. Every tile of an aligned
+        // tensor enters the ring; the stage carries its tile index to the consumers.
+        int32_t *cursor = const_cast<int32_t *>(&pv.hdr->tile_cursor);
+        for (;;) {
+            const int tile = atomicAdd(cursor, 1);
+            if (tile >= n_tiles) {
                 mbar_wait(sm.empty + st, ph ^ 1u);
-                mbar_expect_tx(sm.full + st, (uint32_t)(W * kTile * 4));
+                sm.tile_of[st] = -1;                               // sentinel: the consumers stop
+                mbar_arrive(sm.full + st);
+                break;
+            }
+            if (tile >= c.tile_e) tensor_lookup(p, pv, tile, c);
+            if (!c.aligned) continue;                              // LDG kernel + decode kernel
+            const int64_t tile_base = (int64_t)(tile - c.tile_b) * kTile;
+            const int64_t rem = c.len - tile_base;
+            // whole float4s only (a partial one is read from global memory by its owner thread)
+            const uint32_t bytes = rem >= kTile ? (uint32_t)(kTile * 4) : (uint32_t)((rem & ~(int64_t)3) * 4);
+            const float *src = p.g + c.off + tile_base;
+            mbar_wait(sm.empty + st, ph ^ 1u);
+            sm.tile_of[st] = tile;
+            if (bytes) {
+                mbar_expect_tx(sm.full + st, (uint32_t)W * bytes);
                 float *dst = sm.ring + (size_t)st * kStageFloats;
                 for (int w = 0; w < W; ++w)
-                    bulk_g2s(dst + w * kTile, src + (size_t)w * p.worker_stride, (uint32_t)(kTile * 4), sm.full + st, pol);
-                if (++st == stages) { st = 0; ph ^= 1u; }
+                    bulk_g2s(dst + w * kTile, src + (size_t)w * p.worker_stride, bytes, sm.full + st, pol);
+            } else {
+                mbar_arrive(sm.full + st);
             }
+            if (++st == stages) { st = 0; ph ^= 1u; }
         }
         return;
     }
     // =========================================================================================
-    // tail warp: last tile of every aligned tensor, tensors dealt round-robin over the CTAs
+    // housekeeping warp: scales of the tensors nobody decodes (0 for the FP32 route; the oracle's
+    // 0/0 for an empty low-bit tensor, abs_sum having been zeroed by the route kernel)
     // =========================================================================================
     if (warp == kCW + 1) {
-        for (int t = blockIdx.x; t < p.T; t += gridDim.x) {
-            TensorCur c;
-            c.t = t;
-            c.tile_b = __ldg(pv.tile_prefix + t);
-            c.tile_e = __ldg(pv.tile_prefix + t + 1);
-            if (c.tile_e == c.tile_b) continue;                  // empty tensor
-            c.off = __ldg(p.off + t);
-            c.len = __ldg(p.len + t);
-            if (((c.off | p.worker_stride) & 3) != 0) continue;  // unaligned rows: LDG kernel
-            c.isL = __ldg(p.route + t) == NF_ROUTE_L;
-            c.woff = c.isL ? __ldg(p.woff + t) : 0;
-            c.tau = (p.tau && c.isL) ? __ldg(p.tau + t) : 0.f;
-            c.aligned = true;
-            tail_tile_warp<HEALTH>(p, c, lane);
+        for (int t = blockIdx.x * 32 + lane; t < p.T; t += (int)gridDim.x * 32) {
+            const int64_t off_t = __ldg(p.off + t), len_t = __ldg(p.len + t);
+            if (((off_t | p.worker_stride) & 3) != 0) continue;  // unaligned rows: decode kernel
+            const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
+            if (isL && len_t > 0) continue;                       // published by the decode
+            const float S = isL ? tensor_scale(p.abs_sum, W, p.T, t, len_t) : 0.f;
+            pv.scale[t] = S;
+            if (p.scale_out) p.scale_out[t] = S;
         }
+        return;
+    }
+
+    // =========================================================================================
+    // decode warps (pass B inside the kernel): see decode_units(). The consumers join them once
+    // their own tiles are done.
+    // =========================================================================================
+    if (warp >= kCW + 2) {
+        if (!p.separate_decode) decode_units(p, pv, sm.dtab, n_tiles, lane);
+        if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
         return;
     }
 
@@ -495,26 +610,27 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // consumers
     // =========================================================================================
     const int ctid = tid;                       // 0..511
+    if (ctid == 0) trace_stamp(p, 0);
     const TCtl tctl = make_tctl(lane);
     const bool ternary = p.ternary != 0;
-    const int tile_step = (int)gridDim.x;
     float af[8], qf[8];                         // FP32 partials of the current worker group
 #pragma unroll
     for (int i = 0; i < 8; ++i) { af[i] = 0.f; qf[i] = 0.f; }
-    int kcnt = 0, last_bulk = 0;
+    int kcnt = 0;
+    int4 recent = make_int4(0, 0, 0, 0);        // the last tiles accumulated in af/qf, most recent first
     int st = 0;
     uint32_t ph = 0;
     TensorCur c{};
     c.tile_e = 0;
     c.t = -1;
     bool touched = false;                       // this CTA accumulated something for tensor c.t
-    bool fastT = false;                         // current tensor qualifies for the fast path
+    int ntile_acc = 0;                          // tiles of tensor c.t this CTA has finished
     uint32_t *pP = nullptr, *pN = nullptr;      // this thread's plane-word / direction / output slots
     uint8_t *pD = nullptr;                      //   of tile 0 of the current tensor
     float *pO = nullptr;
 
     auto flush_tensor = [&]() __attribute__((always_inline)) {
-        if (kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, last_bulk, tile_step, ctid); kcnt = 0; }
+        if (kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
         consumer_sync();
         for (int j = ctid; j < 2 * W; j += kCThreads) {
             double tot = 0.0;
@@ -534,30 +650,69 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 if (ci_) { atomicAdd(p.inf_cnt + o, (unsigned long long)ci_); sm.inf[w] = 0u; }
             }
         }
+        // publish: every consumer's direction bytes / plane words / atomics of this tensor are ordered
+        // before the counter the decode warps (of any CTA) acquire
+        __threadfence();
         consumer_sync();
+        if (ctid == 0 && c.isL) {
+            __threadfence();
+            atomicAdd(pv.done + c.t, ntile_acc);
+        }
+        ntile_acc = 0;
     };
 
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    for (;;) {
+        mbar_wait(sm.full + st, ph);
+        const int tile = sm.tile_of[st];
+        if (tile < 0) break;
         if (tile >= c.tile_e) {
             if (touched) flush_tensor();
             tensor_lookup(p, pv, tile, c);
             touched = false;
-            fastT = c.aligned;
             const size_t pl = (size_t)(lane & 7) * p.plane_stride + c.woff + warp * 4 + (lane >> 3);
             pP = (c.isL && p.P) ? p.P + pl : nullptr;
             pN = (c.isL && p.P && ternary) ? p.N + pl : nullptr;
             pD = c.isL ? p.dirs + (size_t)c.woff * 8 + ctid : nullptr;
             pO = p.out + c.off + 4 * ctid;
         }
-        if (!fastT || tile + 1 >= c.tile_e) continue;                        // left to the LDG kernel
         {
-            // ---- fast path: full tile, aligned rows, one worker group, data in the ring ----------
             const int rel = tile - c.tile_b;
-            mbar_wait(sm.full + st, ph);
             const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
             uint64_t *const empty_bar = sm.empty + st;
             if (++st == stages) { st = 0; ph ^= 1u; }
-            if (c.isL) {
+            const int64_t rem_t = c.len - (int64_t)rel * kTile;
+            if (rem_t < kTile) {
+                // ---- ragged last tile of the tensor ------------------------------------------------
+                const int need = (int)rem_t;
+                const int valid = min(max(need - 4 * ctid, 0), 4);
+                uint32_t posR = 0u, negR = 0u;
+                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+                ragged_tile<HEALTH>(sb, p.g + c.off + (int64_t)rel * kTile + 4 * ctid, p.worker_stride, W, valid, c.isL,
+                                    ternary, c.tau, -c.tau, af, qf, posR, negR, acc);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar);
+                if (c.isL) {
+                    if (pP) {
+                        const bool stp = ((lane & 7) < W) && (32 * (warp * 4 + (lane >> 3)) < need);
+                        const uint32_t pw = nib_transpose8(posR, tctl);
+                        if (stp) pP[(size_t)rel * (kTile / 32)] = pw;
+                        if (ternary) {
+                            const uint32_t nwd = nib_transpose8(negR, tctl);
+                            if (stp) pN[(size_t)rel * (kTile / 32)] = nwd;
+                        }
+                    }
+                    const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
+                    if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
+                } else {
+                    float *o = pO + (size_t)rel * kTile;
+                    const float r4[4] = {__fmul_rn(p.alpha, acc.x), __fmul_rn(p.alpha, acc.y), __fmul_rn(p.alpha, acc.z),
+                                         __fmul_rn(p.alpha, acc.w)};
+#pragma unroll
+                    for (int k = 0; k < 4; ++k)
+                        if (k < valid) o[k] = r4[k];
+                }
+            } else if (c.isL) {
+                // ---- full tile, aligned rows, one worker group, data in the ring -----------------
                 uint32_t posR = 0u, negR = 0u;
                 const float tau = c.tau, ntau = -c.tau;
                 if (ternary) {
@@ -589,12 +744,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 __stcs(reinterpret_cast<float4 *>(pO + (size_t)rel * kTile), r);
             }
             touched = true;
-            last_bulk = tile;
-            if (++kcnt == kKTiles) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, tile, tile_step, ctid); kcnt = 0; }
+            ++ntile_acc;
+            recent = make_int4(tile, recent.x, recent.y, recent.z);
+            if (++kcnt == kKTiles) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
         }
     }
+    if (ctid == 0) trace_stamp(p, 1);
     if (touched) flush_tensor();
-
+    if (ctid == 0) trace_stamp(p, 2);
+    if (!p.separate_decode) decode_units(p, pv, sm.dtab, n_tiles, lane);     // help finish pass B
+    if (ctid == 0) trace_stamp(p, 3);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -609,11 +768,12 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    int64_t work = n / kTile > p.T ? n / kTile : p.T;        // full tiles (consumers) or tensors (tail warp)
+    int64_t work = n / kTile + p.T;                          // upper bound of the tile count
     if (work <= 0) return cudaSuccess;
     int64_t grid = device_sm_count();                        // persistent: one CTA per SM
     if (grid > work) grid = work;
-    fused_passA_kernel<HEALTH><<<(unsigned)grid, kFThreads, smem, s>>>(p);
+    cudaError_t e = launch_kernel(fused_passA_kernel<HEALTH>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0, p);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 

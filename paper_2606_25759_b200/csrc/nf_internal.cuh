@@ -30,7 +30,9 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     int64_t Wd;                            // total packed words per worker plane
     int32_t n_tiles;
     int32_t n_unaligned;                   // non-empty tensors whose rows are not 16-byte aligned
-    int64_t pad1[3];
+    int32_t tile_cursor;                   // fused path: next pass-A tile (dynamic scheduling over the CTAs)
+    int32_t unit_cursor;                   // fused path: next pass-B unit (half tile)
+    int64_t pad1[2];
 };
 
 // Offsets (bytes) of the plan arrays for a bucket of T tensors.
@@ -39,6 +41,7 @@ struct PlanLayout {
     size_t lt_index;                       // int32 [T]     ids of the L tensors, in order
     size_t lt_woff;                        // int64 [T+1]   woff of the L tensors, lt_woff[nL] = Wd
     size_t scale;                          // float [T]     per-tensor scale scratch
+    size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
     size_t total;
 };
 
@@ -51,6 +54,7 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
     L.lt_index = o;    o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
     L.lt_woff = o;     o = align_up(o + sizeof(int64_t) * (size_t)(T + 1), 16);
     L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
+    L.done = o;        o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
     L.total = o;
     return L;
 }
@@ -61,6 +65,7 @@ struct PlanView {
     const int32_t *lt_index;
     const int64_t *lt_woff;
     float *scale;
+    int32_t *done;
 };
 
 __host__ __device__ inline PlanView plan_view(void *plan, int T) {
@@ -72,6 +77,7 @@ __host__ __device__ inline PlanView plan_view(void *plan, int T) {
     v.lt_index = (const int32_t *)(p + L.lt_index);
     v.lt_woff = (const int64_t *)(p + L.lt_woff);
     v.scale = (float *)(p + L.scale);
+    v.done = (int32_t *)(p + L.done);
     return v;
 }
 
@@ -99,8 +105,12 @@ struct StreamParams {
     unsigned long long *nan_cnt;
     unsigned long long *inf_cnt;
     float *out;                // [n]
+    float *scale_out;          // [T] or NULL (fused path: the in-kernel decode publishes the scales)
     uint8_t *dirs;             // workspace: one byte per 4 low-bit elements (lo nibble +, hi nibble -)
     void *plan;
+    int separate_decode;       // A/B aid: 1 = no decode inside nf_fused.cu (decode_kernel does everything)
+    unsigned long long *trace; // debug: per-CTA globaltimer stamps [grid][8], or NULL
+    int pdl;                   // launch with programmatic stream serialization (fused path)
     int skip_fast;             // LDG kernel: leave the 16-byte-aligned tensors to the TMA-ring kernel
 };
 
@@ -129,6 +139,9 @@ struct ReduceParams {
     uint8_t *cneg;
     float *scale_out;
     const uint8_t *dirs;       // decode pass of the fused path
+    int64_t worker_stride;     // decode pass: alignment test (with only_unaligned)
+    int pdl;                   // launch with programmatic stream serialization (fused path)
+    int only_unaligned;        // decode pass: the aligned tensors were decoded inside nf_fused.cu
     void *plan;
 };
 
@@ -136,12 +149,40 @@ struct ReduceParams {
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
                          nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
                          double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, int64_t worker_stride, cudaStream_t s);
+                         int64_t zcount, int64_t worker_stride, int pdl, cudaStream_t s);
 cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s);
 int device_sm_count();
+
+
+// ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch (PDL): the kernels of one nf_aggregate_bucket call (and of
+// back-to-back calls) are chained so that a kernel's launch latency and prologue overlap the tail
+// of its predecessor. Every kernel executes pdl_wait() before touching global memory (a no-op
+// when it was launched without the attribute), so completion is transitive along the chain.
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s,
+                                 bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+#endif
 
 // ---------------------------------------------------------------------------------------------
 // Device helpers
@@ -165,7 +206,7 @@ __device__ __forceinline__ float tensor_scale(const double *__restrict__ abs_sum
     double s = 0.0;
     const double dl = (double)len_t;
     for (int w = 0; w < W; ++w) {
-        float swt = (float)(abs_sum[(size_t)w * T + t] / dl);
+        float swt = (float)(__ldcg(abs_sum + (size_t)w * T + t) / dl);
         s += (double)swt;
     }
     return (float)(s / (double)W);

@@ -10,6 +10,7 @@
 // per 8 words, ~3 LOP3 per word), which leaves the per-element counts as 8 bit-planes; the
 // majority test with margin is then a bit-sliced compare that decides 32 elements at once.
 // The FP32 output is written warp-cooperatively (lane = element) so stores are 128-byte coalesced.
+#include <stdlib.h>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -106,7 +107,8 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
         float S = 0.f;
         if (p.route[t] == NF_ROUTE_L) S = tensor_scale(p.abs_sum, p.W, p.T, t, p.len[t]);
         s_scale[t] = S;
-        if (blockIdx.x == 0) {
+        const bool mine = !p.only_unaligned || (((p.off[t] | p.worker_stride) & 3) != 0);
+        if (blockIdx.x == 0 && mine) {
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
@@ -215,8 +217,11 @@ struct DecodeTensor {
 
 __global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p) {
     extern __shared__ float s_scale[];
+    pdl_launch_dependents();
+    pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    if (p.only_unaligned && pv.hdr->n_unaligned == 0) return;       // everything was decoded in pass A
     compute_scales(p, pv, s_scale);
     const int n_tiles = pv.hdr->n_tiles;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -241,6 +246,7 @@ __global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p)
                 c.S = s_scale[t];
             }
             if (!c.isL) continue;
+            if (p.only_unaligned && (((c.off_t | p.worker_stride) & 3) == 0)) continue;
             const int64_t wbase = (int64_t)(tile - c.tile_b) * kTile + warp * 512;   // tensor-relative
             const int64_t i = wbase + lane * 16;
             if (i < c.len_t)
@@ -300,7 +306,8 @@ cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s) {
     const int64_t max_tiles = n / kTile + p.T;
     const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
     const int grid = grid_for((max_tiles + kDUnroll - 1) / kDUnroll, 16);
-    decode_kernel<<<grid, kDThreads, smem, s>>>(p);
+    cudaError_t e = launch_kernel(decode_kernel, (unsigned)grid, kDThreads, smem, s, p.pdl != 0, p);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 

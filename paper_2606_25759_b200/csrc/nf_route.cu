@@ -7,6 +7,7 @@
 // tensors are handled in chunks of 1024 with a warp-shuffle block scan carrying three running
 // sums (packed words, tiles, L-tensor count). The same kernel zeroes the accumulating outputs of
 // the fused path so that no separate memset node is needed on the stream.
+#include <stdlib.h>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -60,6 +61,8 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
              uint8_t *__restrict__ route, int64_t *__restrict__ woff, int64_t *__restrict__ summary,
              void *plan, double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
              int64_t zcount, int64_t worker_stride) {
+    pdl_launch_dependents();   // the next kernel may start its prologue
+    pdl_wait();                // the previous call's kernels still read the plan / accumulators
     __shared__ Scan3 s_scan[33];
     PlanLayout L = plan_layout(T);
     char *pb = (char *)plan;
@@ -68,6 +71,8 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     int32_t *lt_index = (int32_t *)(pb + L.lt_index);
     int64_t *lt_woff = (int64_t *)(pb + L.lt_woff);
 
+    int32_t *done = (int32_t *)(pb + L.done);
+    for (int i = threadIdx.x; i < T; i += kRouteThreads) done[i] = 0;
     // zero the accumulating outputs of the fused path (abs_sum, sumsq, nan, inf)
     for (int64_t i = threadIdx.x; i < zcount; i += kRouteThreads) {
         if (z0) z0[i] = 0.0;
@@ -139,6 +144,8 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
         hdr->Wd = carry.words;
         hdr->n_tiles = (status == NF_OK) ? (int32_t)carry.tiles : 0;
         hdr->n_unaligned = s_unal;
+        hdr->tile_cursor = 0;
+        hdr->unit_cursor = 0;
         summary[NF_SUM_WD] = carry.words;
         summary[NF_SUM_NL] = carry.nl;
         summary[NF_SUM_NF] = (int64_t)s_tal[0];
@@ -153,9 +160,10 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
                          nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
                          double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, int64_t worker_stride, cudaStream_t s) {
-    route_kernel<<<1, kRouteThreads, 0, s>>>(off, len, elig, T, n, st, route, woff, summary, plan,
-                                             z0, z1, z2, z3, zcount, worker_stride);
+                         int64_t zcount, int64_t worker_stride, int pdl, cudaStream_t s) {
+    cudaError_t e = launch_kernel(route_kernel, 1, kRouteThreads, 0, s, pdl != 0, off, len, elig, T, n, st, route, woff, summary,
+                                  plan, z0, z1, z2, z3, zcount, worker_stride);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 

@@ -13,6 +13,7 @@
 //  * per-(worker,tensor) abs-sum / sum-of-squares run in FP32 over 8 elements, then FP64 per
 //    thread, one block reduce-scatter + FP64 atomics per tensor change.
 #include <float.h>
+#include <stdlib.h>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -154,6 +155,8 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
     constexpr bool STATS = PACK || HEALTH;
     __shared__ double s_red[kThreads / 32][16];
     __shared__ unsigned int s_nan[8], s_inf[8];
+    pdl_launch_dependents();
+    pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     if (p.skip_fast && pv.hdr->n_unaligned == 0) return;             // nothing left for this kernel
@@ -436,7 +439,8 @@ static cudaError_t launch_stream_t(const StreamParams &p, int64_t n, cudaStream_
     if (max_tiles <= 0) return cudaSuccess;
     int64_t grid = (int64_t)device_sm_count() * per_sm;     // persistent: a multiple of the SM count
     if (grid > max_tiles) grid = max_tiles;
-    stream_kernel<FLAGS><<<(unsigned)grid, kThreads, 0, s>>>(p);
+    cudaError_t e = launch_kernel(stream_kernel<FLAGS>, (unsigned)grid, kThreads, 0, s, p.pdl != 0, p);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
