@@ -199,10 +199,10 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.trace = g_trace;
     p.separate_decode = sep_decode ? 1 : 0;
     p.pdl = use_pdl ? 1 : 0;
-    // W <= 8: full tiles of aligned tensors go through the TMA-ring kernel (nf_fused.cu); the LDG
-    // streaming kernel takes the rest (ragged tails, unaligned tensors) or, for W > 8, everything.
+    // Tensors whose rows are 16-byte aligned go through the TMA-ring kernel (nf_fused.cu), which also
+    // decodes them; the LDG streaming kernel and the decode kernel take the unaligned ones.
     const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);
-    if (W <= 8 && !use_ldg) {
+    if (!use_ldg) {
         e = launch_fused_passA(health, p, n, s);
         if (e != cudaSuccess) return NF_ERR_CUDA;
         p.skip_fast = 1;
@@ -218,7 +218,7 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     r.dirs = (const uint8_t *)workspace; r.plan = plan;
     r.worker_stride = worker_stride;
     r.pdl = use_pdl ? 1 : 0;
-    r.only_unaligned = (W <= 8 && !use_ldg && !sep_decode) ? 1 : 0;      // the TMA-ring kernel decoded the aligned tensors itself
+    r.only_unaligned = (!use_ldg && !sep_decode) ? 1 : 0;      // the TMA-ring kernel decoded the aligned tensors itself
     e = launch_decode(r, n, s);
     prof_mark(3, s);
     if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;

@@ -272,18 +272,19 @@ __device__ __forceinline__ void fast_signs(const float *sb, int nw, float tau, f
 }
 // FP32-route tile: fixed worker order, plain FP32 adds
 template <bool HEALTH, bool FULLW>
-__device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)[8], float (&qf)[8]) {
-    float4 acc = *reinterpret_cast<const float4 *>(sb);
+__device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)[8], float (&qf)[8], float4 acc, bool first) {
 #pragma unroll
     for (int w = 0; w < kGroup; ++w) {
         if (!FULLW && w >= nw) break;
-        const float4 v = (w == 0) ? acc : *reinterpret_cast<const float4 *>(sb + w * kTile);
+        const float4 v = *reinterpret_cast<const float4 *>(sb + w * kTile);
         if (HEALTH) {
             af[w] += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
             qf[w] = fmaf(v.x, v.x, qf[w]); qf[w] = fmaf(v.y, v.y, qf[w]);
             qf[w] = fmaf(v.z, v.z, qf[w]); qf[w] = fmaf(v.w, v.w, qf[w]);
         }
-        if (w > 0) {
+        if (w == 0 && first) {
+            acc = v;
+        } else {
             acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
             acc.z = __fadd_rn(acc.z, v.z); acc.w = __fadd_rn(acc.w, v.w);
         }
@@ -296,7 +297,7 @@ __device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)
 template <bool HEALTH>
 __device__ __forceinline__ void ragged_tile(const float *sb, const float *grow, int64_t worker_stride, int nw, int valid,
                                             bool isL, bool ternary, float tau, float ntau, float (&af)[8],
-                                            float (&qf)[8], uint32_t &posR, uint32_t &negR, float4 &acc) {
+                                            float (&qf)[8], uint32_t &posR, uint32_t &negR, float4 &acc, bool first) {
 #pragma unroll
     for (int w = 0; w < kGroup; ++w) {
         if (w >= nw) break;
@@ -320,7 +321,7 @@ __device__ __forceinline__ void ragged_tile(const float *sb, const float *grow, 
             posR |= ((v.x > tau ? 1u : 0u) | (v.y > tau ? 2u : 0u) | (v.z > tau ? 4u : 0u) | (v.w > tau ? 8u : 0u)) << (4 * w);
             if (ternary)
                 negR |= ((v.x < ntau ? 1u : 0u) | (v.y < ntau ? 2u : 0u) | (v.z < ntau ? 4u : 0u) | (v.w < ntau ? 8u : 0u)) << (4 * w);
-        } else if (w == 0) {
+        } else if (w == 0 && first) {
             acc = v;
         } else {
             acc.x = __fadd_rn(acc.x, v.x); acc.y = __fadd_rn(acc.y, v.y);
@@ -506,16 +507,30 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
     if (trace_me) p.trace[(size_t)blockIdx.x * 8 + 6] = nunits;
 }
 
+// the same vote from byte-packed running counts (W > 8: several worker groups per tile)
+__device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool ternary, int W, int margin) {
+    uint32_t d = 0u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int c_p = (cp >> (8 * j)) & 0xff;
+        const int c_n = ternary ? (int)((cn >> (8 * j)) & 0xff) : W - c_p;
+        const int D = c_p - c_n;
+        if (D > margin) d |= 1u << j;
+        if (D < -margin) d |= 16u << j;
+    }
+    return d;
+}
+
 extern __shared__ __align__(128) unsigned char smem_raw[];
 
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
-template <bool HEALTH>
-__global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ StreamParams p) {
-    constexpr int stages = kStages;
+template <bool HEALTH, bool MULTI>
+__global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ StreamParams p, const int stages_arg) {
+    const int stages = MULTI ? stages_arg : kStages;     // W <= 8: compile-time ring depth
     const FusedSmem sm = carve(smem_raw, stages);
-    const int W = p.W;                          // 1..8: one worker group (launch_fused_passA)
+    const int W = p.W;                          // MULTI: W > 8, several worker groups of 8 per tile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     pdl_launch_dependents();
 
@@ -565,17 +580,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             // whole float4s only (a partial one is read from global memory by its owner thread)
             const uint32_t bytes = rem >= kTile ? (uint32_t)(kTile * 4) : (uint32_t)((rem & ~(int64_t)3) * 4);
             const float *src = p.g + c.off + tile_base;
-            mbar_wait(sm.empty + st, ph ^ 1u);
-            sm.tile_of[st] = tile;
-            if (bytes) {
-                mbar_expect_tx(sm.full + st, (uint32_t)W * bytes);
-                float *dst = sm.ring + (size_t)st * kStageFloats;
-                for (int w = 0; w < W; ++w)
-                    bulk_g2s(dst + w * kTile, src + (size_t)w * p.worker_stride, bytes, sm.full + st, pol);
-            } else {
-                mbar_arrive(sm.full + st);
+            for (int w0 = 0; w0 < W; w0 += kGroup) {              // one stage per (tile, worker group)
+                const int nw = min(kGroup, W - w0);
+                mbar_wait(sm.empty + st, ph ^ 1u);
+                sm.tile_of[st] = tile;
+                if (bytes) {
+                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
+                    float *dst = sm.ring + (size_t)st * kStageFloats;
+                    for (int w = 0; w < nw; ++w)
+                        bulk_g2s(dst + w * kTile, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
+                } else {
+                    mbar_arrive(sm.full + st);
+                }
+                if (++st == stages) { st = 0; ph ^= 1u; }
             }
-            if (++st == stages) { st = 0; ph ^= 1u; }
         }
         return;
     }
@@ -630,7 +648,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     float *pO = nullptr;
 
     auto flush_tensor = [&]() __attribute__((always_inline)) {
-        if (kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
+        if (!MULTI && kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
         consumer_sync();
         for (int j = ctid; j < 2 * W; j += kCThreads) {
             double tot = 0.0;
@@ -675,78 +693,86 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             pD = c.isL ? p.dirs + (size_t)c.woff * 8 + ctid : nullptr;
             pO = p.out + c.off + 4 * ctid;
         }
-        {
-            const int rel = tile - c.tile_b;
+        const int rel = tile - c.tile_b;
+        const int64_t rem_t = c.len - (int64_t)rel * kTile;
+        const bool ragged = rem_t < kTile;                  // last tile of the tensor, need < kTile elements
+        const int need = ragged ? (int)rem_t : kTile;
+        const int valid = min(max(need - 4 * ctid, 0), 4);
+        recent = make_int4(tile, recent.x, recent.y, recent.z);
+        uint32_t posR = 0u, negR = 0u, cp = 0u, cn = 0u;     // cp/cn: byte-packed running counts (MULTI)
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {   // one ring stage per worker group
+            if (MULTI && w0 > 0) mbar_wait(sm.full + st, ph);
+            const int nw = MULTI ? min(kGroup, W - w0) : W;
             const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
             uint64_t *const empty_bar = sm.empty + st;
             if (++st == stages) { st = 0; ph ^= 1u; }
-            const int64_t rem_t = c.len - (int64_t)rel * kTile;
-            if (rem_t < kTile) {
-                // ---- ragged last tile of the tensor ------------------------------------------------
-                const int need = (int)rem_t;
-                const int valid = min(max(need - 4 * ctid, 0), 4);
-                uint32_t posR = 0u, negR = 0u;
-                float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-                ragged_tile<HEALTH>(sb, p.g + c.off + (int64_t)rel * kTile + 4 * ctid, p.worker_stride, W, valid, c.isL,
-                                    ternary, c.tau, -c.tau, af, qf, posR, negR, acc);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar);
-                if (c.isL) {
-                    if (pP) {
-                        const bool stp = ((lane & 7) < W) && (32 * (warp * 4 + (lane >> 3)) < need);
-                        const uint32_t pw = nib_transpose8(posR, tctl);
-                        if (stp) pP[(size_t)rel * (kTile / 32)] = pw;
-                        if (ternary) {
-                            const uint32_t nwd = nib_transpose8(negR, tctl);
-                            if (stp) pN[(size_t)rel * (kTile / 32)] = nwd;
-                        }
-                    }
-                    const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
-                    if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
-                } else {
-                    float *o = pO + (size_t)rel * kTile;
-                    const float r4[4] = {__fmul_rn(p.alpha, acc.x), __fmul_rn(p.alpha, acc.y), __fmul_rn(p.alpha, acc.z),
-                                         __fmul_rn(p.alpha, acc.w)};
-#pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        if (k < valid) o[k] = r4[k];
-                }
+            if (MULTI) { posR = 0u; negR = 0u; }
+            if (ragged) {
+                ragged_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)rel * kTile + 4 * ctid,
+                                    p.worker_stride, nw, valid, c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
+                                    w0 == 0);
             } else if (c.isL) {
-                // ---- full tile, aligned rows, one worker group, data in the ring -----------------
-                uint32_t posR = 0u, negR = 0u;
                 const float tau = c.tau, ntau = -c.tau;
                 if (ternary) {
-                    if (W == kGroup) fast_signs<2, HEALTH, true>(sb, W, tau, ntau, af, qf, posR, negR);
-                    else fast_signs<2, HEALTH, false>(sb, W, tau, ntau, af, qf, posR, negR);
+                    if (nw == kGroup) fast_signs<2, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                    else fast_signs<2, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
                 } else {
-                    if (W == kGroup) fast_signs<1, HEALTH, true>(sb, W, tau, ntau, af, qf, posR, negR);
-                    else fast_signs<1, HEALTH, false>(sb, W, tau, ntau, af, qf, posR, negR);
+                    if (nw == kGroup) fast_signs<1, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                    else fast_signs<1, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar);
+            } else {
+                acc = (nw == kGroup) ? fast_fp32<HEALTH, true>(sb, nw, af, qf, acc, w0 == 0)
+                                     : fast_fp32<HEALTH, false>(sb, nw, af, qf, acc, w0 == 0);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar);              // every lane's reads of the stage are done
+            if (c.isL) {
                 if (pP) {
-                    const bool stp = (lane & 7) < W;
+                    // packed plane words: 8x8 nibble transpose, lane q of an octet stores worker q's word
+                    const bool stp = ((lane & 7) < nw) && (32 * (warp * 4 + (lane >> 3)) < need);
+                    const size_t o = (size_t)rel * (kTile / 32) + (size_t)w0 * p.plane_stride;
                     const uint32_t pw = nib_transpose8(posR, tctl);
-                    if (stp) pP[(size_t)rel * (kTile / 32)] = pw;
+                    if (stp) pP[o] = pw;
                     if (ternary) {
                         const uint32_t nwd = nib_transpose8(negR, tctl);
-                        if (stp) pN[(size_t)rel * (kTile / 32)] = nwd;
+                        if (stp) pN[o] = nwd;
                     }
                 }
-                const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
-                pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
-            } else {
-                float4 r = (W == kGroup) ? fast_fp32<HEALTH, true>(sb, W, af, qf) : fast_fp32<HEALTH, false>(sb, W, af, qf);
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar);
-                r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
-                r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
-                __stcs(reinterpret_cast<float4 *>(pO + (size_t)rel * kTile), r);
+                if (MULTI) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        cp += (uint32_t)__popc(posR & (0x11111111u << j)) << (8 * j);
+                        if (ternary) cn += (uint32_t)__popc(negR & (0x11111111u << j)) << (8 * j);
+                    }
+                }
             }
-            touched = true;
-            ++ntile_acc;
-            recent = make_int4(tile, recent.x, recent.y, recent.z);
-            if (++kcnt == kKTiles) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
+            if (MULTI && (c.isL || HEALTH))
+                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, 1, recent, ctid);
+        }
+        if (c.isL) {
+            // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
+            const uint32_t d = MULTI ? vote4_packed(cp, cn, ternary, W, p.margin)
+                                     : (ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin));
+            if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
+        } else {
+            float *o = pO + (size_t)rel * kTile;
+            float4 r = acc;
+            r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
+            r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
+            if (valid == 4) {
+                __stcs(reinterpret_cast<float4 *>(o), r);
+            } else {
+                if (valid > 0) o[0] = r.x;
+                if (valid > 1) o[1] = r.y;
+                if (valid > 2) o[2] = r.z;
+            }
+        }
+        touched = true;
+        ++ntile_acc;
+        if (!MULTI && ++kcnt == kKTiles) {
+            stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid);
+            kcnt = 0;
         }
     }
     if (ctid == 0) trace_stamp(p, 1);
@@ -759,12 +785,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
-template <bool HEALTH>
+template <bool HEALTH, bool MULTI>
 static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t s) {
-    const size_t smem = fused_smem_bytes(kStages, kGroup);
+    // ring depth: 3 stages unless the per-warp FP64 slots of a very wide fan-in need the room
+    const int stages = (MULTI && p.W > 64) ? 2 : kStages;
+    const size_t smem = fused_smem_bytes(stages, p.W);
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(fused_passA_kernel<HEALTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const size_t a = fused_smem_bytes(kStages, 64), b = fused_smem_bytes(2, 255);
+        cudaError_t e = cudaFuncSetAttribute(fused_passA_kernel<HEALTH, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)(a > b ? a : b));
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -772,16 +802,16 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
     if (work <= 0) return cudaSuccess;
     int64_t grid = device_sm_count();                        // persistent: one CTA per SM
     if (grid > work) grid = work;
-    cudaError_t e = launch_kernel(fused_passA_kernel<HEALTH>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0, p);
+    cudaError_t e = launch_kernel(fused_passA_kernel<HEALTH, MULTI>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0, p, stages);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
-// Full tiles of 16-byte-aligned tensors, W <= 8. The caller runs the LDG streaming kernel with
-// skip_fast = 1 for the tensors whose rows are not 16-byte aligned.
+// Every tensor whose rows are 16-byte aligned, any W. The caller runs the LDG streaming kernel
+// (skip_fast = 1) and the decode kernel (only_unaligned = 1) for the tensors whose rows are not.
 cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s) {
-    if (p.W > kGroup) return cudaErrorInvalidValue;
-    return health ? launch_fused_t<true>(p, n, s) : launch_fused_t<false>(p, n, s);
+    if (p.W > kGroup) return health ? launch_fused_t<true, true>(p, n, s) : launch_fused_t<false, true>(p, n, s);
+    return health ? launch_fused_t<true, false>(p, n, s) : launch_fused_t<false, false>(p, n, s);
 }
 
 }  // namespace nf
