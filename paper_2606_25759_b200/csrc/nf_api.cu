@@ -199,26 +199,29 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.trace = g_trace;
     p.separate_decode = sep_decode ? 1 : 0;
     p.pdl = use_pdl ? 1 : 0;
-    // Tensors whose rows are 16-byte aligned go through the TMA-ring kernel (nf_fused.cu), which also
-    // decodes them; the LDG streaming kernel and the decode kernel take the unaligned ones.
+    // One persistent TMA-ring kernel (nf_fused.cu) does pass A and pass B. NF_PASSA_LDG / NF_DECODE_SEPARATE
+    // select the register-staged streaming kernel / the stand-alone decode kernel for A/B measurements.
     const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);
     if (!use_ldg) {
-        e = launch_fused_passA(health, p, n, s);
+        e = launch_fused_passA(health, p, n, s);                  // pass A + pass B in one kernel
         if (e != cudaSuccess) return NF_ERR_CUDA;
-        p.skip_fast = 1;
+        prof_mark(2, s);
+        if (!sep_decode) {
+            prof_mark(3, s);
+            if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;
+            return NF_OK;
+        }
+    } else {
+        e = launch_stream(flags, p, n, s);
+        if (e != cudaSuccess) return NF_ERR_CUDA;
+        prof_mark(2, s);
     }
-    static const bool skip_ldg = getenv("NF_SKIP_LDG") != nullptr;   // timing aid only (wrong results for unaligned tensors)
-    if (!(skip_ldg && p.skip_fast)) e = launch_stream(flags, p, n, s);
-    if (e != cudaSuccess) return NF_ERR_CUDA;
-    prof_mark(2, s);
-    // pass B: scale x direction for the low-bit positions
+    // pass B as its own kernel (A/B aids only): scale x direction for the low-bit positions
     ReduceParams r{};
     r.W = W; r.T = T; r.off = off; r.len = len; r.route = route; r.woff = woff;
     r.abs_sum = abs_sum; r.out = out; r.scale_out = scale_out;
     r.dirs = (const uint8_t *)workspace; r.plan = plan;
-    r.worker_stride = worker_stride;
     r.pdl = use_pdl ? 1 : 0;
-    r.only_unaligned = (!use_ldg && !sep_decode) ? 1 : 0;      // the TMA-ring kernel decoded the aligned tensors itself
     e = launch_decode(r, n, s);
     prof_mark(3, s);
     if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;

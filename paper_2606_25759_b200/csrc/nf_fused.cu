@@ -28,8 +28,9 @@ constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = o
 constexpr int kDW = 2;                           // decode warps (pass B inside the kernel)
 constexpr int kFThreads = kCThreads + 64 + kDW * 32;   // + producer warp + housekeeping warp + decode warps
 constexpr int kDU = 4;                           // decode: tiles in flight per warp
-constexpr int kStageFloats = kGroup * kTile;     // 8 workers x 2048 elements
-constexpr int kStageBytes = kStageFloats * 4;    // 64 KB
+constexpr int kPitch = kTile + 4;                // ring row: one tile of one worker + room for a misaligned head
+constexpr int kStageFloats = kGroup * kPitch;    // 8 workers
+constexpr int kStageBytes = kStageFloats * 4;    // 64 KB + 128 B
 constexpr int kKTiles = 4;                       // tiles of FP32 partial accumulation
 constexpr int kMaxStages = 4;
 constexpr int kStages = 3;                       // ring depth: 3 x 64 KB
@@ -188,7 +189,7 @@ __device__ __forceinline__ void tensor_lookup(const StreamParams &p, const PlanV
 template <bool HEALTH>
 __device__ __noinline__ double2 exact_redo(const float *__restrict__ g, int64_t worker_stride, int wg,
                                            int64_t off_t, int64_t len_t, int tile_b, int4 recent, int cnt, int ctid,
-                                           unsigned int *s_nan, unsigned int *s_inf, int slot) {
+                                           unsigned int *s_nan, unsigned int *s_inf, int slot, bool aligned) {
     double da = 0.0, dq = 0.0;
     const float *row = g + (size_t)wg * worker_stride + off_t;
     // all loads first (independent, one round trip), then the arithmetic
@@ -200,12 +201,12 @@ __device__ __noinline__ double2 exact_redo(const float *__restrict__ g, int64_t 
 #pragma unroll
         for (int k = 0; k < 4; ++k) x[j][k] = 0.f;
         if (j < cnt) {
-            if (base + 4 <= len_t) {                         // rows of the ring tiles are 16-byte aligned
+            if (aligned && base + 4 <= len_t) {
                 const float4 v = __ldg(reinterpret_cast<const float4 *>(row + base));
                 x[j][0] = v.x; x[j][1] = v.y; x[j][2] = v.z; x[j][3] = v.w;
             } else {
 #pragma unroll
-                for (int k = 0; k < 3; ++k)
+                for (int k = 0; k < 4; ++k)
                     if (base + k < len_t) x[j][k] = __ldg(row + base + k);
             }
         }
@@ -252,7 +253,7 @@ __device__ __forceinline__ void fast_signs(const float *sb, int nw, float tau, f
 #pragma unroll
     for (int w = 0; w < kGroup; ++w) {
         if (!FULLW && w >= nw) break;
-        const float4 v = *reinterpret_cast<const float4 *>(sb + w * kTile);
+        const float4 v = *reinterpret_cast<const float4 *>(sb + w * kPitch);
         af[w] += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
         if (HEALTH) {
             qf[w] = fmaf(v.x, v.x, qf[w]); qf[w] = fmaf(v.y, v.y, qf[w]);
@@ -276,7 +277,7 @@ __device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)
 #pragma unroll
     for (int w = 0; w < kGroup; ++w) {
         if (!FULLW && w >= nw) break;
-        const float4 v = *reinterpret_cast<const float4 *>(sb + w * kTile);
+        const float4 v = *reinterpret_cast<const float4 *>(sb + w * kPitch);
         if (HEALTH) {
             af[w] += (fabsf(v.x) + fabsf(v.y)) + (fabsf(v.z) + fabsf(v.w));
             qf[w] = fmaf(v.x, v.x, qf[w]); qf[w] = fmaf(v.y, v.y, qf[w]);
@@ -291,19 +292,30 @@ __device__ __forceinline__ float4 fast_fp32(const float *sb, int nw, float (&af)
     }
     return acc;
 }
-// Ragged last tile of a tensor (need < kTile elements): the ring holds the whole float4s; the one
-// thread that owns the partial float4 reads its 1..3 elements from global memory; threads past the
-// end see zeros. One instantiation, uniform branches on the tile kind.
+// Slow tiles, one instantiation with uniform branches on the tile kind:
+//  * ragged last tile of an aligned tensor (need < kTile elements): the ring holds the whole float4s;
+//    the one thread that owns the partial float4 reads its 1..3 elements from global memory;
+//  * any tile of a tensor whose rows are NOT 16-byte aligned (unal): the producer copied every row
+//    from the 16-byte boundary below it, so worker w's elements start m_w = (m0 + w*mstep) & 3
+//    floats into its ring row and are read with scalar shared-memory loads.
+// Threads past the end of the tensor see zeros.
 template <bool HEALTH>
-__device__ __forceinline__ void ragged_tile(const float *sb, const float *grow, int64_t worker_stride, int nw, int valid,
+__device__ __forceinline__ void slow_tile(const float *sb, const float *grow, int64_t worker_stride, int nw, int valid,
+                                          bool unal, int m0, int mstep,
                                             bool isL, bool ternary, float tau, float ntau, float (&af)[8],
                                             float (&qf)[8], uint32_t &posR, uint32_t &negR, float4 &acc, bool first) {
 #pragma unroll
     for (int w = 0; w < kGroup; ++w) {
         if (w >= nw) break;
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (valid == 4) {
-            v = *reinterpret_cast<const float4 *>(sb + w * kTile);
+        if (unal) {
+            const float *b = sb + w * kPitch + ((m0 + w * mstep) & 3);
+            if (valid > 0) v.x = b[0];
+            if (valid > 1) v.y = b[1];
+            if (valid > 2) v.z = b[2];
+            if (valid > 3) v.w = b[3];
+        } else if (valid == 4) {
+            v = *reinterpret_cast<const float4 *>(sb + w * kPitch);
         } else if (valid > 0) {
             const float *g = grow + (size_t)w * worker_stride;
             v.x = __ldg(g);
@@ -352,7 +364,7 @@ __device__ __forceinline__ uint32_t vote4(uint32_t posR, uint32_t negR, int W, i
 template <bool HEALTH>
 __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, float (&af)[8], float (&qf)[8],
                                            int64_t off_t, int64_t len_t, int tile_b, int w0, int nw, int cnt,
-                                           int4 recent, int ctid) {
+                                           int4 recent, int ctid, bool aligned) {
     const int lane = ctid & 31, warp = ctid >> 5, W = p.W;
     float v16[16];
 #pragma unroll
@@ -381,7 +393,7 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
                 double2 e = make_double2((double)a_t, (double)q_t);
                 if (!ok_t)
                     e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, recent, cnt, ctid, sm.nan,
-                                           sm.inf, w0 + w);
+                                           sm.inf, w0 + w, aligned);
                 const double ea = warp_sum(e.x), eq = warp_sum(e.y);
                 if (lane == 0) { slot[w * 2] += ea; slot[w * 2 + 1] += eq; }
             } else if ((lane & 1) == 0 && wl == w) {
@@ -442,7 +454,7 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
                 tile_e = __ldg(pv.tile_prefix + t_cur + 1);
                 off_t = __ldg(p.off + t_cur);
                 len_t = __ldg(p.len + t_cur);
-                dec = (__ldg(p.route + t_cur) == NF_ROUTE_L) && (((off_t | p.worker_stride) & 3) == 0);
+                dec = __ldg(p.route + t_cur) == NF_ROUTE_L;
                 if (dec) {
                     woff_t = __ldg(p.woff + t_cur);
                     const int total = tile_e - tile_b;
@@ -493,12 +505,13 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
                     v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
                     v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
                     float *o = p.out + obase[k] + h * 512 + e0;
-                    if (r >= 4) {
+                    if (r >= 4 && (obase[k] & 3) == 0) {
                         __stcs(reinterpret_cast<float4 *>(o), v);
                     } else {
                         o[0] = v.x;
                         if (r > 1) o[1] = v.y;
                         if (r > 2) o[2] = v.z;
+                        if (r > 3) o[3] = v.w;
                     }
                 }
             }
@@ -574,21 +587,33 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 break;
             }
             if (tile >= c.tile_e) tensor_lookup(p, pv, tile, c);
-            if (!c.aligned) continue;                              // LDG kernel + decode kernel
             const int64_t tile_base = (int64_t)(tile - c.tile_b) * kTile;
             const int64_t rem = c.len - tile_base;
-            // whole float4s only (a partial one is read from global memory by its owner thread)
-            const uint32_t bytes = rem >= kTile ? (uint32_t)(kTile * 4) : (uint32_t)((rem & ~(int64_t)3) * 4);
+            const int need = rem >= kTile ? kTile : (int)rem;
+            // aligned rows: whole float4s only (a partial one is read from global memory by its owner
+            // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
+            // (whole 16-byte chunks, each holding at least one element of the row).
+            const uint32_t bytes = (uint32_t)((need & ~3) * 4);
             const float *src = p.g + c.off + tile_base;
             for (int w0 = 0; w0 < W; w0 += kGroup) {              // one stage per (tile, worker group)
                 const int nw = min(kGroup, W - w0);
                 mbar_wait(sm.empty + st, ph ^ 1u);
                 sm.tile_of[st] = tile;
-                if (bytes) {
-                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
-                    float *dst = sm.ring + (size_t)st * kStageFloats;
+                float *dst = sm.ring + (size_t)st * kStageFloats;
+                if (!c.aligned) {
+                    uint32_t tx = 0;
                     for (int w = 0; w < nw; ++w)
-                        bulk_g2s(dst + w * kTile, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
+                        tx += (uint32_t)((((int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
+                    mbar_expect_tx(sm.full + st, tx);
+                    for (int w = 0; w < nw; ++w) {
+                        const int m = (int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
+                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
+                                 (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
+                    }
+                } else if (bytes) {
+                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
+                    for (int w = 0; w < nw; ++w)
+                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
                 } else {
                     mbar_arrive(sm.full + st);
                 }
@@ -604,7 +629,6 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     if (warp == kCW + 1) {
         for (int t = blockIdx.x * 32 + lane; t < p.T; t += (int)gridDim.x * 32) {
             const int64_t off_t = __ldg(p.off + t), len_t = __ldg(p.len + t);
-            if (((off_t | p.worker_stride) & 3) != 0) continue;  // unaligned rows: decode kernel
             const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
             if (isL && len_t > 0) continue;                       // published by the decode
             const float S = isL ? tensor_scale(p.abs_sum, W, p.T, t, len_t) : 0.f;
@@ -648,7 +672,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     float *pO = nullptr;
 
     auto flush_tensor = [&]() __attribute__((always_inline)) {
-        if (!MULTI && kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid); kcnt = 0; }
+        if (!MULTI && kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned); kcnt = 0; }
         consumer_sync();
         for (int j = ctid; j < 2 * W; j += kCThreads) {
             double tot = 0.0;
@@ -708,10 +732,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             uint64_t *const empty_bar = sm.empty + st;
             if (++st == stages) { st = 0; ph ^= 1u; }
             if (MULTI) { posR = 0u; negR = 0u; }
-            if (ragged) {
-                ragged_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)rel * kTile + 4 * ctid,
-                                    p.worker_stride, nw, valid, c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
-                                    w0 == 0);
+            if (ragged || !c.aligned) {
+                slow_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)rel * kTile + 4 * ctid,
+                                  p.worker_stride, nw, valid, !c.aligned, (int)((c.off + (int64_t)w0 * p.worker_stride) & 3),
+                                  (int)(p.worker_stride & 3), c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
+                                  w0 == 0);
             } else if (c.isL) {
                 const float tau = c.tau, ntau = -c.tau;
                 if (ternary) {
@@ -748,7 +773,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 }
             }
             if (MULTI && (c.isL || HEALTH))
-                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, 1, recent, ctid);
+                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, 1, recent, ctid, c.aligned);
         }
         if (c.isL) {
             // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
@@ -760,18 +785,19 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             float4 r = acc;
             r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
             r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
-            if (valid == 4) {
+            if (valid == 4 && c.aligned) {
                 __stcs(reinterpret_cast<float4 *>(o), r);
             } else {
                 if (valid > 0) o[0] = r.x;
                 if (valid > 1) o[1] = r.y;
                 if (valid > 2) o[2] = r.z;
+                if (valid > 3) o[3] = r.w;
             }
         }
         touched = true;
         ++ntile_acc;
         if (!MULTI && ++kcnt == kKTiles) {
-            stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid);
+            stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
             kcnt = 0;
         }
     }
@@ -807,8 +833,7 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
     return cudaGetLastError();
 }
 
-// Every tensor whose rows are 16-byte aligned, any W. The caller runs the LDG streaming kernel
-// (skip_fast = 1) and the decode kernel (only_unaligned = 1) for the tensors whose rows are not.
+// The whole of pass A and pass B for one bucket: any W, any tensor offsets.
 cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s) {
     if (p.W > kGroup) return health ? launch_fused_t<true, true>(p, n, s) : launch_fused_t<false, true>(p, n, s);
     return health ? launch_fused_t<true, false>(p, n, s) : launch_fused_t<false, false>(p, n, s);

@@ -29,7 +29,7 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     int64_t n;
     int64_t Wd;                            // total packed words per worker plane
     int32_t n_tiles;
-    int32_t n_unaligned;                   // non-empty tensors whose rows are not 16-byte aligned
+    int32_t pad0;
     int32_t tile_cursor;                   // fused path: next pass-A tile (dynamic scheduling over the CTAs)
     int32_t unit_cursor;                   // fused path: next pass-B unit (half tile)
     int64_t pad1[2];
@@ -111,7 +111,6 @@ struct StreamParams {
     int separate_decode;       // A/B aid: 1 = no decode inside nf_fused.cu (decode_kernel does everything)
     unsigned long long *trace; // debug: per-CTA globaltimer stamps [grid][8], or NULL
     int pdl;                   // launch with programmatic stream serialization (fused path)
-    int skip_fast;             // LDG kernel: leave the 16-byte-aligned tensors to the TMA-ring kernel
 };
 
 enum : int {
@@ -139,9 +138,7 @@ struct ReduceParams {
     uint8_t *cneg;
     float *scale_out;
     const uint8_t *dirs;       // decode pass of the fused path
-    int64_t worker_stride;     // decode pass: alignment test (with only_unaligned)
     int pdl;                   // launch with programmatic stream serialization (fused path)
-    int only_unaligned;        // decode pass: the aligned tensors were decoded inside nf_fused.cu
     void *plan;
 };
 

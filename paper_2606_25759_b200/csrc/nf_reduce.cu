@@ -107,8 +107,7 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
         float S = 0.f;
         if (p.route[t] == NF_ROUTE_L) S = tensor_scale(p.abs_sum, p.W, p.T, t, p.len[t]);
         s_scale[t] = S;
-        const bool mine = !p.only_unaligned || (((p.off[t] | p.worker_stride) & 3) != 0);
-        if (blockIdx.x == 0 && mine) {
+        if (blockIdx.x == 0) {
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
@@ -221,7 +220,6 @@ __global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p)
     pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    if (p.only_unaligned && pv.hdr->n_unaligned == 0) return;       // everything was decoded in pass A
     compute_scales(p, pv, s_scale);
     const int n_tiles = pv.hdr->n_tiles;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -246,7 +244,6 @@ __global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p)
                 c.S = s_scale[t];
             }
             if (!c.isL) continue;
-            if (p.only_unaligned && (((c.off_t | p.worker_stride) & 3) == 0)) continue;
             const int64_t wbase = (int64_t)(tile - c.tile_b) * kTile + warp * 512;   // tensor-relative
             const int64_t i = wbase + lane * 16;
             if (i < c.len_t)

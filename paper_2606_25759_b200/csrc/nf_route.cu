@@ -83,7 +83,6 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
 
     Scan3 carry{0, 0, 0};
     long long nF = 0, nP = 0, e = 0, tot = 0;   // per-thread partials, reduced at the end
-    int unal = 0;
     int bad = 0;
     for (int base = 0; base < T; base += kRouteThreads) {
         const int t = base + threadIdx.x;
@@ -102,7 +101,6 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
             else if (st.veto || !st.capacity_ok) r = NF_ROUTE_F;
             else r = NF_ROUTE_L;
             v.tiles = (l + kTile - 1) / kTile;
-            if (l > 0 && (((o | worker_stride) & 3) != 0)) ++unal;
             tot += l;
             if (r == NF_ROUTE_L) { v.words = (l + 31) / 32; v.nl = 1; e += l; }
             else if (r == NF_ROUTE_F) ++nF;
@@ -121,15 +119,14 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     }
     // block-reduce the small tallies through shared memory atomics
     __shared__ unsigned long long s_tal[4];
-    __shared__ int s_bad, s_unal;
-    if (threadIdx.x == 0) { s_tal[0] = s_tal[1] = s_tal[2] = s_tal[3] = 0ull; s_bad = 0; s_unal = 0; }
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) { s_tal[0] = s_tal[1] = s_tal[2] = s_tal[3] = 0ull; s_bad = 0; }
     __syncthreads();
     if (nF) atomicAdd(&s_tal[0], (unsigned long long)nF);
     if (nP) atomicAdd(&s_tal[1], (unsigned long long)nP);
     if (e) atomicAdd(&s_tal[2], (unsigned long long)e);
     if (tot) atomicAdd(&s_tal[3], (unsigned long long)tot);
     if (bad) atomicOr(&s_bad, 1);
-    if (unal) atomicAdd(&s_unal, unal);
     __syncthreads();
     if (threadIdx.x == 0) {
         int status = NF_OK;
@@ -143,7 +140,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
         hdr->n = n;
         hdr->Wd = carry.words;
         hdr->n_tiles = (status == NF_OK) ? (int32_t)carry.tiles : 0;
-        hdr->n_unaligned = s_unal;
+        hdr->pad0 = 0;
         hdr->tile_cursor = 0;
         hdr->unit_cursor = 0;
         summary[NF_SUM_WD] = carry.words;

@@ -159,7 +159,6 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
     pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    if (p.skip_fast && pv.hdr->n_unaligned == 0) return;             // nothing left for this kernel
     const int n_tiles = pv.hdr->n_tiles;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 8) { s_nan[tid] = 0u; s_inf[tid] = 0u; }
@@ -197,7 +196,6 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
         }
         const bool do_tile = HEALTH || (isL ? (PACK || COUNT) : FP32);
         if (!do_tile) continue;
-        if (p.skip_fast && aligned) continue;                        // nf_fused.cu takes these
         if (STATS && !multi && acc_t != t) {
             if (acc_t >= 0) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
             acc_t = t;
