@@ -1,0 +1,188 @@
+#!/usr/bin/env python
+"""bench_report.py — the measurement tables of SURVEY.md §8(d) beyond bench.py's single JSON line.
+
+    python bench_report.py [--out gpurun_out/report.md] [--quick]
+
+Table 1: the five BASELINE.json configs (plus the paper's two local-count shapes)
+through the fused call nf_aggregate_bucket: time per step, FP32-gradient GB/s (4*W*n/t),
+elements/s, algorithmic bytes, % of the nominal and of the measured HBM peak.
+Table 2: the reducer-capacity sweep (config 5): for W in {2, 8, 32, 64, 128} on one 25 MB
+all-eligible bucket: (i) nf_sign_count_reduce alone on pre-packed planes, (ii) nf_sign_pack +
+nf_sign_count_reduce, (iii) the fused call, (iv) nf_fp32_reduce on the same W x n — the paper's
+"endpoint service rate vs fan-in" question measured on one B200.
+Timing: median of CUDA-event-timed iterations after 3 warm-ups, inputs resident in HBM. Buckets
+smaller than L2 are rotated over enough copies to exceed 126 MB (stated per row).
+No oracle is used here (parity is the job of tests/); this only times the CUDA path.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L2_BYTES = 126 * 2 ** 20
+NOMINAL = 8000.0
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0
+
+
+def time_fn(fn, iters, warmup=3):
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(iters):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    return statistics.median(ts)
+
+
+def fused_bytes(cfg, planes=True, p=2):
+    tot = 0
+    for b in cfg.buckets:
+        e, n = b.n_eligible, b.n
+        tot += 4 * cfg.W * n + 4 * n + e // 2 + ((p * cfg.W * e) // 8 if planes else 0)
+    return tot
+
+
+def run_config(cfg, iters, dev):
+    """Whole model per iteration through nf_aggregate_bucket; small models are replicated so that
+    one iteration touches more than L2."""
+    import torch
+    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from workloads import gen
+    in_bytes = sum(4 * cfg.W * b.n for b in cfg.buckets)
+    copies = max(1, -(-2 * L2_BYTES // in_bytes)) if in_bytes < 2 * L2_BYTES else 1
+    G, BB = [], []
+    for _ in range(copies):
+        for b in cfg.buckets:
+            G.append(gen.gen_bucket(cfg, b, dev))
+            BB.append(BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, dev, planes=True, health=True))
+
+    def step():
+        for g, bb in zip(G, BB):
+            bb.aggregate(g, g.shape[1], (1, 0, 1), nf.MODE_GTERNARY)
+    ms = time_fn(step, iters) / copies
+    del G, BB
+    torch.cuda.empty_cache()
+    return ms, copies
+
+
+def table_configs(args, dev, peak):
+    from workloads import shapes
+    names = ["tiny", "resnet50", "vit_b16", "gpt2_1p3b"] + [f"sweep_w{w}" for w in shapes.SWEEP_W]
+    rows = []
+    for nme in names:
+        cfg = shapes.get(nme)
+        ms, copies = run_config(cfg, args.iters if cfg.n_params < 5e8 else max(5, args.iters // 4), dev)
+        rows.append((cfg.name, cfg.W, cfg.n_params, len(cfg.buckets), ms, copies, fused_bytes(cfg)))
+    for n in (131_072, 524_288):
+        cfg = shapes.paper_local_count(n)
+        ms, copies = run_config(cfg, args.iters, dev)
+        rows.append((cfg.name + " (PAPER L456 shape)", cfg.W, cfg.n_params, 1, ms, copies, fused_bytes(cfg)))
+    out = ["| config | W | n (elements) | buckets | time / step | FP32-grad GB/s | elements/s | algorithmic bytes | % of 8000 GB/s | "
+           f"% of {peak:.1f} GB/s | note |", "|---|---|---|---|---|---|---|---|---|---|---|"]
+    for name, W, n, nb, ms, copies, ab in rows:
+        t = ms * 1e-3
+        note = f"{copies} rotating copies (input < 2 x L2)" if copies > 1 else "input > L2"
+        out.append(f"| {name} | {W} | {n:,} | {nb} | {ms * 1e3:.1f} us | {4 * W * n / t / 1e9:.1f} | {n / t:.3e} | "
+                   f"{ab / 1e6:.1f} MB | {100 * ab / t / 1e9 / NOMINAL:.1f} | {100 * ab / t / 1e9 / peak:.1f} | {note} |")
+    return "\n".join(out)
+
+
+def table_sweep(args, dev, peak):
+    import torch
+    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from workloads import shapes, gen
+    out = ["| W | planes in (MB) | (i) count-reduce alone | (ii) pack + count-reduce | (iii) fused | (iv) fp32_reduce | "
+           "copies |", "|---|---|---|---|---|---|---|"]
+    for W in shapes.SWEEP_W:
+        cfg = shapes.sweep(W)
+        b = cfg.buckets[0]
+        n = b.n
+        in_bytes = 4 * W * n
+        copies = max(1, -(-2 * L2_BYTES // in_bytes))
+        G = [gen.gen_bucket(cfg, b, dev) for _ in range(copies)]
+        BB = [BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=True) for _ in range(copies)]
+        for g, bb in zip(G, BB):
+            bb.route_bucket((1, 0, 1))
+            bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+        torch.cuda.synchronize()
+        plane_bytes = 2 * W * n // 8
+
+        def reduce_only():
+            for bb in BB:
+                bb.sign_count_reduce(nf.MODE_GTERNARY)
+
+        def pack_reduce():
+            for g, bb in zip(G, BB):
+                bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+                bb.sign_count_reduce(nf.MODE_GTERNARY)
+
+        def fused():
+            for g, bb in zip(G, BB):
+                bb.aggregate(g, g.shape[1], (1, 0, 1), nf.MODE_GTERNARY)
+
+        # (iv): the same bucket with every tensor on the FP32 route
+        FB = [BucketBuffers(b.off, b.length, [0] * len(b.off), n, W, dev, planes=False, health=False) for _ in range(copies)]
+        for fb in FB:
+            fb.route_bucket((1, 0, 1))
+
+        def fp32():
+            for g, fb in zip(G, FB):
+                fb.fp32_reduce(g, g.shape[1])
+        cells = []
+        for fn, own in ((reduce_only, plane_bytes + 4 * n), (pack_reduce, in_bytes + 2 * plane_bytes + 4 * n),
+                        (fused, in_bytes + plane_bytes + n // 2 + 4 * n), (fp32, in_bytes + 4 * n)):
+            t = time_fn(fn, args.iters) / copies * 1e-3
+            cells.append(f"{t * 1e6:.1f} us, {in_bytes / t / 1e9:.0f} GB/s FP32-equiv, {100 * own / t / 1e9 / peak:.0f} % HBM on own bytes")
+        out.append(f"| {W} | {plane_bytes / 1e6:.1f} | " + " | ".join(cells) + f" | {copies} |")
+        del G, BB, FB
+        torch.cuda.empty_cache()
+    return "\n".join(out)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--out", default="")
+    ap.add_argument("--iters", type=int, default=20)
+    ap.add_argument("--skip-configs", action="store_true")
+    args = ap.parse_args()
+    import torch
+    from paper_2606_25759_b200 import build as nf_build
+    nf_build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench_report.py needs a CUDA device (no CPU fallback)")
+    dev = "cuda"
+    peak = measured_peak()
+    parts = [f"GPU: {torch.cuda.get_device_name(0)}; measured HBM copy peak {peak:.1f} GB/s; "
+             f"median of {args.iters} CUDA-event-timed iterations after 3 warm-ups; mode G-Ternary, planes and health on.", ""]
+    if not args.skip_configs:
+        parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
+    parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
+    text = "\n".join(parts)
+    print(text)
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write(text + "\n")
+
+
+if __name__ == "__main__":
+    main()

@@ -132,21 +132,27 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 
 // ---------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic). Everything the hot loop touches sits at a compile-time offset:
-//   [0, 64)      mbarriers full[4], empty[4]
-//   [64, 2112)   NaN / Inf tallies, 256 workers each
-//   [3072, 3088) tile index carried by each ring stage (dynamic tile scheduling)
-//   [4096, 8192) decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
-//   [8192, ...)  ring [stages][8][kTile] floats
-//   after ring   per-warp FP64 totals {abs, sq} per worker: [kCW][2*W] doubles
+//   [0, 64)         mbarriers full[4], empty[4]
+//   [64, 80)        tile index carried by each ring stage (dynamic tile scheduling)
+//   [1024, 3072)    NaN / Inf tallies, 256 workers each
+//   [4096, 8192)    decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
+//   [8192, 17408)   per-tensor metadata of the first kMetaCap tensors (tile prefix, off, len, woff, tau)
+//   [17408, ...)    ring [stages][8][kPitch] floats
+//   after the ring  per-warp FP64 totals {abs, sq} per worker, [kCW][2*W] doubles
 // ---------------------------------------------------------------------------------------------
-constexpr int kSmemHdr = 8192;
+constexpr int kMetaCap = 256;                    // tensors whose metadata is cached in shared memory
+constexpr int kSmemMeta = 8192;
+constexpr int kSmemHdr = kSmemMeta + 9216;       // 4*(cap+1) + 3*8*cap + 4*cap = 8196 bytes, padded
 struct FusedSmem {
     float *ring;
     uint64_t *full, *empty;
-    unsigned int *nan, *inf;
     int *tile_of;                // [kMaxStages] tile held by a stage, -1 = no more tiles
+    unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
-    double *wacc;
+    int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
+    int64_t *m_off, *m_len, *m_woff;   // [kMetaCap]; woff = -1 when the tensor is not low-bit routed
+    float *m_tau;                // [kMetaCap]
+    double *wacc;                // [kCW][2*W]
 };
 __host__ __device__ inline size_t fused_smem_bytes(int stages, int W) {
     return (size_t)kSmemHdr + (size_t)stages * kStageBytes + sizeof(double) * kCW * 2 * (size_t)W;
@@ -155,10 +161,15 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     FusedSmem s;
     s.full = (uint64_t *)base;
     s.empty = s.full + kMaxStages;
-    s.nan = (unsigned int *)(base + 64);
+    s.tile_of = (int *)(base + 64);
+    s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
-    s.tile_of = (int *)(base + 3072);
     s.dtab = (float4 *)(base + 4096);
+    s.m_off = (int64_t *)(base + kSmemMeta);
+    s.m_len = s.m_off + kMetaCap;
+    s.m_woff = s.m_len + kMetaCap;
+    s.m_tau = (float *)(s.m_woff + kMetaCap);
+    s.m_tile = (int32_t *)(s.m_tau + kMetaCap);
     s.ring = (float *)(base + kSmemHdr);
     s.wacc = (double *)(base + kSmemHdr + (size_t)stages * kStageBytes);
     return s;
@@ -171,16 +182,36 @@ struct TensorCur {
     bool isL, aligned;
     float tau;
 };
-__device__ __forceinline__ void tensor_lookup(const StreamParams &p, const PlanView &pv, int tile, TensorCur &c) {
-    const int t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
-    c.t = t;
-    c.tile_b = __ldg(pv.tile_prefix + t);
-    c.tile_e = __ldg(pv.tile_prefix + t + 1);
-    c.off = __ldg(p.off + t);
-    c.len = __ldg(p.len + t);
-    c.isL = __ldg(p.route + t) == NF_ROUTE_L;
-    c.woff = c.isL ? __ldg(p.woff + t) : 0;
-    c.tau = (p.tau && c.isL) ? __ldg(p.tau + t) : 0.f;
+// Tensor of a tile. Buckets of up to kMetaCap tensors are served from the shared-memory copy the
+// CTA made at start (a tensor change then costs a few LDS instead of a chain of L2 round trips).
+__device__ __forceinline__ void tensor_lookup(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int tile,
+                                              TensorCur &c) {
+    if (p.T <= kMetaCap) {
+        int lo = 0, hi = p.T;                    // invariant: m_tile[lo] <= tile < m_tile[hi]
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (sm.m_tile[mid] <= tile) lo = mid; else hi = mid;
+        }
+        c.t = lo;
+        c.tile_b = sm.m_tile[lo];
+        c.tile_e = sm.m_tile[lo + 1];
+        c.off = sm.m_off[lo];
+        c.len = sm.m_len[lo];
+        const int64_t wo = sm.m_woff[lo];
+        c.isL = wo >= 0;
+        c.woff = c.isL ? wo : 0;
+        c.tau = sm.m_tau[lo];
+    } else {
+        const int t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
+        c.t = t;
+        c.tile_b = __ldg(pv.tile_prefix + t);
+        c.tile_e = __ldg(pv.tile_prefix + t + 1);
+        c.off = __ldg(p.off + t);
+        c.len = __ldg(p.len + t);
+        c.isL = __ldg(p.route + t) == NF_ROUTE_L;
+        c.woff = c.isL ? __ldg(p.woff + t) : 0;
+        c.tau = (p.tau && c.isL) ? __ldg(p.tau + t) : 0.f;
+    }
     c.aligned = (((c.off | p.worker_stride) & 3) == 0);
 }
 // Exact FP64 re-read of one thread's elements of worker `wg` over the last `cnt` (<= 4) tiles of the
@@ -422,8 +453,9 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
 // decode warps overlap their stores with the consumers' reads of later tensors; the consumers
 // join when their own tiles are done. Every store instruction writes 512 contiguous bytes.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const float4 *dtab,
+__device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
                                              int n_tiles, int lane) {
+    const float4 *dtab = sm.dtab;
     const int W = p.W;
     const int total_units = n_tiles * 2;
     int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
@@ -449,22 +481,20 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
             if (u >= total_units) continue;
             const int tile = u >> 1;
             if (tile >= tile_e) {
-                t_cur = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
-                tile_b = __ldg(pv.tile_prefix + t_cur);
-                tile_e = __ldg(pv.tile_prefix + t_cur + 1);
-                off_t = __ldg(p.off + t_cur);
-                len_t = __ldg(p.len + t_cur);
-                dec = __ldg(p.route + t_cur) == NF_ROUTE_L;
+TensorCur tc;
+                tensor_lookup(p, pv, sm, tile, tc);
+                t_cur = tc.t; tile_b = tc.tile_b; tile_e = tc.tile_e; off_t = tc.off; len_t = tc.len;
+                dec = tc.isL;
                 if (dec) {
-                    woff_t = __ldg(p.woff + t_cur);
+                    woff_t = tc.woff;
                     const int total = tile_e - tile_b;
                     const int *dp = pv.done + t_cur;
                     int seen;
                     for (unsigned spins = 0;; ++spins) {
                         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(dp) : "memory");
                         if (seen >= total) break;
-                        __nanosleep(4000);
-                        if (spins > (1u << 20)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
+                        __nanosleep(500);
+                        if (spins > (1u << 23)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
                     }
                     S_t = tensor_scale(p.abs_sum, W, p.T, t_cur, len_t);
                     if (trace_me) { trace_stamp(p, first_wait ? 5 : 7); first_wait = false; }
@@ -563,6 +593,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     const int n_tiles = pv.hdr->n_tiles;
+    if (p.T <= kMetaCap) {
+        // per-tensor metadata -> shared memory (one round trip for the whole CTA)
+        for (int t = tid; t <= p.T; t += kFThreads) {
+            sm.m_tile[t] = __ldg(pv.tile_prefix + t);
+            if (t < p.T) {
+                const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
+                sm.m_off[t] = __ldg(p.off + t);
+                sm.m_len[t] = __ldg(p.len + t);
+                sm.m_woff[t] = isL ? __ldg(p.woff + t) : -1;
+                sm.m_tau[t] = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
+            }
+        }
+        __syncthreads();
+    }
 
     // =========================================================================================
     // producer: one elected lane issues the bulk copies of every fast tile
@@ -586,7 +630,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 mbar_arrive(sm.full + st);
                 break;
             }
-            if (tile >= c.tile_e) tensor_lookup(p, pv, tile, c);
+            if (tile >= c.tile_e) tensor_lookup(p, pv, sm, tile, c);
             const int64_t tile_base = (int64_t)(tile - c.tile_b) * kTile;
             const int64_t rem = c.len - tile_base;
             const int need = rem >= kTile ? kTile : (int)rem;
@@ -643,7 +687,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // their own tiles are done.
     // =========================================================================================
     if (warp >= kCW + 2) {
-        if (!p.separate_decode) decode_units(p, pv, sm.dtab, n_tiles, lane);
+        if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
         return;
     }
@@ -709,7 +753,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (tile < 0) break;
         if (tile >= c.tile_e) {
             if (touched) flush_tensor();
-            tensor_lookup(p, pv, tile, c);
+            tensor_lookup(p, pv, sm, tile, c);
             touched = false;
             const size_t pl = (size_t)(lane & 7) * p.plane_stride + c.woff + warp * 4 + (lane >> 3);
             pP = (c.isL && p.P) ? p.P + pl : nullptr;
@@ -804,7 +848,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     if (ctid == 0) trace_stamp(p, 1);
     if (touched) flush_tensor();
     if (ctid == 0) trace_stamp(p, 2);
-    if (!p.separate_decode) decode_units(p, pv, sm.dtab, n_tiles, lane);     // help finish pass B
+    if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane);     // help finish pass B
     if (ctid == 0) trace_stamp(p, 3);
 }
 
