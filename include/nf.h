@@ -137,9 +137,10 @@ int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
 /*
  * Fused path (the one the target is measured on) — same results as
  * nf_route_bucket -> nf_sign_pack -> nf_sign_count_reduce -> nf_fp32_reduce -> nf_health_stats(g),
- * with the W x n gradients read ONCE: pass A routes, packs, counts, votes, sums the FP32 tensors
- * and gathers abs-sums and health statistics from a single read; pass B expands the 2-bit
- * directions by the per-tensor scale. P and N may both be NULL (planes not materialised);
+ * with the W x n gradients read ONCE. Two launches: the route kernel, then one persistent kernel that
+ * packs, counts, votes, sums the FP32 tensors, gathers abs-sums and health statistics from a single read
+ * (pass A) and, tensor by tensor as each completes, expands the 2-bit directions by the per-tensor scale
+ * (pass B). P and N may both be NULL (planes not materialised);
  * sumsq/nan_cnt/inf_cnt may all be NULL (no health statistics); scale_out may be NULL.
  * route/woff/summary/plan are outputs exactly as in nf_route_bucket.
  */
@@ -172,9 +173,9 @@ int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t
 /*
  * Instrumentation (host calls, not part of the data path). nf_prof_enable(k > 0) creates CUDA
  * events for up to k nf_aggregate_bucket calls and makes each such call record four events on
- * its stream (before route, before pass A, after pass A, after pass B); nf_prof_enable(0) frees
+ * its stream (before the route kernel, before the fused kernel, after it, at the end of the call); nf_prof_enable(0) frees
  * them. nf_prof_collect synchronises on the recorded events, writes 3 floats per recorded call
- * (route ms, pass A ms, pass B ms) to the HOST array `ms` (room for 3*max_records floats), resets
+ * (route ms, fused-kernel ms, remainder ms) to the HOST array `ms` (room for 3*max_records floats), resets
  * the record counter and returns the number of calls written (or a negative nf_status).
  */
 int nf_prof_enable(int max_records);

@@ -186,7 +186,7 @@ def nf_prof_enable(max_records: int):
 
 
 def nf_prof_collect(max_records: int):
-    """Returns a list of (route_ms, passA_ms, passB_ms), one per recorded nf_aggregate_bucket call."""
+    """Returns a list of (route_ms, fused_kernel_ms, remainder_ms), one per recorded nf_aggregate_bucket call."""
     buf = (C.c_float * (3 * max(max_records, 1)))()
     k = lib().nf_prof_collect(C.cast(buf, C.c_void_p), int(max_records))
     if k < 0:

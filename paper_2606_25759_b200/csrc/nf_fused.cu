@@ -1,23 +1,25 @@
-// nf_fused.cu — pass A of the fused path (nf_aggregate_bucket): route-aware pack + sign count +
-// majority vote + FP32-route sum + abs-sums + health statistics from ONE read of the W x n
-// gradients. PAPER §5.2, §3.3; SURVEY §8(a) a2/a3/a4a/a4b, §8(d) "fused floor".
+// nf_fused.cu — the fused path of nf_aggregate_bucket after the route kernel: route-aware pack + sign
+// count + majority vote + FP32-route sum + abs-sums + health statistics from ONE read of the W x n
+// gradients (pass A) and the decode out = S_t * d (pass B), in one persistent kernel per bucket.
+// PAPER §5.2, §3.3; SURVEY §8(a) a2/a3/a4a/a4b, §8(d) "fused floor".
 //
-// Blackwell design (HBM-bound streaming, no contraction -> no tensor cores):
-//  * one persistent CTA per SM: 16 consumer warps + 1 producer warp (+ decode warps, see below);
-//  * the producer's elected lane streams tiles (2048 elements x 8 workers = 64 KB) from HBM into a
-//    shared-memory ring with 1-D bulk async copies (cp.async.bulk, the TMA engine) that complete on
-//    an mbarrier, with an L2 evict-first policy (the gradients are read exactly once); the
-//    bytes in flight no longer depend on registers or occupancy;
-//  * consumer warps wait on the stage's "full" mbarrier, pull their 8 float4 (conflict-free
-//    LDS.128), release the stage at once ("empty" mbarrier) and only then compute;
+// Blackwell design (HBM-bound streaming, no contraction -> no tensor cores), DESIGN.md §6:
+//  * one persistent CTA per SM: 16 consumer warps, a producer warp, a housekeeping warp, 2 decode warps;
+//  * the producer's elected lane takes tiles (2048 elements of one tensor) from a device-wide cursor and
+//    streams them, 8 workers at a time (64 KB), from HBM into a 3-stage shared-memory ring with 1-D bulk
+//    async copies (cp.async.bulk, the TMA engine) that complete on an mbarrier, with an L2 evict-first
+//    policy (the gradients are read exactly once);
+//  * consumer warps wait on the stage's "full" mbarrier, read one float4 per worker (conflict-free
+//    LDS.128) and release the stage on its "empty" mbarrier;
 //  * per thread: 4 consecutive elements of up to 8 workers -> one 4-bit nibble per worker in one
 //    register per plane; counts are popcounts under a 0x11111111 mask; packed plane words come
 //    from an 8x8 nibble transpose across 8 lanes;
 //  * abs-sum / sum of squares: FP32 partials over kKTiles tiles (<= 16 elements, pairwise inside a
-//    float4), then FP64 per thread; a failed range check (NaN, Inf, FP32 over/underflow) sends the
-//    thread to an exact FP64 re-read of just those elements.
-// Tiles whose rows cannot be bulk-copied (tensor rows not 16-byte aligned, or a tail that would
-// read past the bucket) take a generic predicated path straight from global memory.
+//    float4), FP32 warp reduce-scatter, FP64 per warp; a failed range check (NaN, Inf, FP32
+//    over/underflow) sends the offending threads to an exact FP64 re-read of just those elements;
+//  * ragged last tiles and tensors whose rows are not 16-byte aligned go through the same ring;
+//  * each CTA publishes its finished tiles per tensor (release); decode warps, and the consumers once
+//    the tiles are exhausted, acquire the per-tensor counter and expand the 2-bit directions.
 #include <float.h>
 #include "nf_internal.cuh"
 
