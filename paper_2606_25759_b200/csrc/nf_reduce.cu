@@ -82,23 +82,44 @@ __device__ __forceinline__ void const_planes(int v, uint32_t (&b)[9]) {
     for (int k = 0; k < 9; ++k) b[k] = ((v >> k) & 1) ? 0xffffffffu : 0u;
 }
 
-// Stream the W words of word position k of one plane into a sliced counter.
-__device__ __forceinline__ void count_words(const uint32_t *__restrict__ base, int64_t stride, int W,
-                                            SlicedCounter &sc) {
-    sc.clear();
-    int w = 0;
-    for (; w + 8 <= W; w += 8) {
-        uint32_t x[8];
+// Stream the W words of word position k of both planes into two sliced counters: 16 workers per round,
+// i.e. up to 32 independent loads in flight per thread (a thread walks W serially, so the depth of
+// each round, not the thread count, is what hides the HBM latency at large fan-in).
+template <bool TERNARY>
+__device__ __forceinline__ void count_words2(const uint32_t *__restrict__ P, const uint32_t *__restrict__ N,
+                                             int64_t stride, int W, SlicedCounter &cp, SlicedCounter &cn) {
+    cp.clear();
+    cn.clear();
+    for (int w = 0; w < W; w += 16) {
+        uint32_t xp[16], xn[16];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = __ldcs(base + (size_t)(w + i) * stride);
-        sc.add8(x);
+        for (int i = 0; i < 16; ++i) {
+            const bool in = w + i < W;
+            xp[i] = in ? __ldcs(P + (size_t)(w + i) * stride) : 0u;
+            xn[i] = (TERNARY && in) ? __ldcs(N + (size_t)(w + i) * stride) : 0u;
+        }
+        cp.add8(reinterpret_cast<const uint32_t(&)[8]>(xp[0]));
+        cp.add8(reinterpret_cast<const uint32_t(&)[8]>(xp[8]));
+        if (TERNARY) {
+            cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[0]));
+            cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[8]));
+        }
     }
-    if (w < W) {
-        uint32_t x[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = (w + i < W) ? __ldcs(base + (size_t)(w + i) * stride) : 0u;
-        sc.add8(x);
+}
+
+// S_t computed by one warp: the per-worker loads and divisions run in parallel across the lanes, the
+// FP64 sum keeps the fixed worker order of tensor_scale() (bit-identical result) through a shuffle chain.
+__device__ __forceinline__ float warp_tensor_scale(const double *__restrict__ abs_sum, int W, int T, int t,
+                                                   int64_t len_t, int lane) {
+    double s = 0.0;
+    const double dl = (double)len_t;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+        const int w = w0 + lane;
+        const float swt = (w < W) ? (float)(__ldcg(abs_sum + (size_t)w * T + t) / dl) : 0.f;
+        const int cnt = min(32, W - w0);
+        for (int j = 0; j < cnt; ++j) s += (double)__shfl_sync(0xffffffffu, swt, j);
     }
+    return (float)(s / (double)W);
 }
 
 // every CTA computes the scales of the L tensors it may touch into shared memory; CTA 0 publishes
@@ -116,16 +137,33 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
 }
 
 template <bool WRITE_COUNTS>
-__global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReduceParams p) {
-    extern __shared__ float s_scale[];
+__global__ void __launch_bounds__(kRThreads, 2) count_reduce_kernel(const ReduceParams p) {
+    __shared__ float4 s_dtab[256];          // byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
+    {
+        const int i = threadIdx.x;          // kRThreads == 256
+        s_dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
+                                (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
+    }
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    compute_scales(p, pv, s_scale);
     const int64_t Wd = pv.hdr->Wd;
     const int nL = pv.hdr->nL;
     const int lane = threadIdx.x & 31;
     const int W = p.W;
     const int64_t n_chunks = (Wd + kRThreads - 1) / kRThreads;
+    __syncthreads();                        // direction table
+    // Scales are computed warp by warp for the tensors a warp's 32 words touch (no CTA-wide serial
+    // prologue: at W = 128 a single thread summing 128 L2 round trips per tensor used to stall every
+    // CTA at a barrier). CTA 0 publishes the scales of the tensors that own no word.
+    if (blockIdx.x == 0) {
+        for (int t = threadIdx.x; t < p.T; t += kRThreads) {
+            const bool isL = p.route[t] == NF_ROUTE_L;
+            if (isL && p.len[t] > 0) continue;
+            const float S0 = isL ? tensor_scale(p.abs_sum, W, p.T, t, p.len[t]) : 0.f;
+            pv.scale[t] = S0;
+            if (p.scale_out) p.scale_out[t] = S0;
+        }
+    }
 
     for (int64_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
         const int64_t k = chunk * kRThreads + threadIdx.x;      // global word position
@@ -133,6 +171,7 @@ __global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReducePar
         int nvalid = 0;
         int64_t obase = 0;
         float S = 0.f;
+        int my_li = -1;
         SlicedCounter cpv, cnv;
         cpv.clear(); cnv.clear();
         if (k < Wd) {
@@ -142,10 +181,10 @@ __global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReducePar
             const int64_t rem = __ldg(p.len + t) - i0;
             nvalid = rem >= 32 ? 32 : (int)rem;
             obase = __ldg(p.off + t) + i0;
-            S = s_scale[t];
-            count_words(p.P + k, p.plane_stride, W, cpv);
+            my_li = li;
+            if (p.ternary) count_words2<true>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
+            else count_words2<false>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
             if (p.ternary) {
-                count_words(p.N + k, p.plane_stride, W, cnv);
                 // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
                 uint32_t b[9];
                 sliced_add_const(cnv.c, p.margin, b);
@@ -170,7 +209,51 @@ __global__ void __launch_bounds__(kRThreads) count_reduce_kernel(const ReducePar
             dpos &= vmask;
             dneg &= vmask;
         }
-        // warp-cooperative, coalesced write-back: iteration j handles the word of lane j
+        {
+            // one cooperative scale per distinct tensor among the warp's words (usually one)
+            const int li_lo = __shfl_sync(0xffffffffu, my_li, 0);
+            int li_hi = my_li;
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) li_hi = max(li_hi, __shfl_xor_sync(0xffffffffu, li_hi, d));
+            for (int li = li_lo; li >= 0 && li <= li_hi; ++li) {
+                const int t = __ldg(pv.lt_index + li);
+                const float St = warp_tensor_scale(p.abs_sum, W, p.T, t, __ldg(p.len + t), lane);
+                if (my_li == li) S = St;
+                const int64_t kfirst = __ldg(pv.lt_woff + li);
+                if (lane == 0 && kfirst >= k && kfirst < k + 32) {      // this warp holds the tensor's first word
+                    pv.scale[t] = St;
+                    if (p.scale_out) p.scale_out[t] = St;
+                }
+            }
+        }
+        // Fast write-back: the warp's 32 words are 1024 consecutive, 16-byte-aligned elements of ONE tensor.
+        // Each thread turns its two masks into 8 direction bytes (low nibble +, high nibble -); a byte
+        // indexes a shared-memory table of float4 directions, and every store writes 512 contiguous bytes.
+        const int64_t ob0 = __shfl_sync(0xffffffffu, obase, 0);
+        const bool fast = !WRITE_COUNTS && __all_sync(0xffffffffu, nvalid == 32 && obase == ob0 + 32 * lane) &&
+                          ((ob0 & 3) == 0);
+        if (fast) {
+            auto spread = [](uint32_t x) {           // 4 nibbles of a 16-bit value -> low nibbles of 4 bytes
+                x = (x | (x << 8)) & 0x00ff00ffu;
+                return (x | (x << 4)) & 0x0f0f0f0fu;
+            };
+            const uint32_t lo = spread(dpos & 0xffffu) | (spread(dneg & 0xffffu) << 4);
+            const uint32_t hi = spread(dpos >> 16) | (spread(dneg >> 16) << 4);
+            const float S0 = __shfl_sync(0xffffffffu, S, 0);
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                // store j covers elements j*128 + lane*4 .. +3 = byte (lane & 7) of thread j*4 + (lane >> 3)
+                const int src = j * 4 + (lane >> 3);
+                const uint32_t wl = __shfl_sync(0xffffffffu, lo, src), wh = __shfl_sync(0xffffffffu, hi, src);
+                const uint32_t d = (((lane & 4) ? wh : wl) >> (8 * (lane & 3))) & 0xffu;
+                float4 v = s_dtab[d];
+                v.x = __fmul_rn(S0, v.x); v.y = __fmul_rn(S0, v.y);
+                v.z = __fmul_rn(S0, v.z); v.w = __fmul_rn(S0, v.w);
+                __stcs(reinterpret_cast<float4 *>(p.out + ob0 + j * 128 + lane * 4), v);
+            }
+            continue;
+        }
+        // general write-back (tensor boundaries, ragged words, count outputs): iteration j handles the word of lane j
 #pragma unroll 4
         for (int j = 0; j < 32; ++j) {
             const int nv = __shfl_sync(0xffffffffu, nvalid, j);

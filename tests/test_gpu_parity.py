@@ -131,3 +131,22 @@ def test_gpu_invariants_without_oracle():
     bb.sign_count_reduce(nf.MODE_GTERNARY)
     torch.cuda.synchronize()
     assert torch.equal(cp0, bb.cpos)
+
+
+@pytest.mark.parametrize("name", ["tiny", "sweep_w8", "sweep_w32", "resnet50"])
+@pytest.mark.parametrize("mode", [O.MODE_GBINARY, O.MODE_GTERNARY])
+def test_count_reduce_without_count_outputs(name, mode):
+    """nf_sign_count_reduce with cpos/cneg == NULL takes its own write-back path (1024-element runs of one
+    tensor through the direction table); the count-output variant is covered by run_both."""
+    cfg = shapes.get(name, small=(name != "tiny"))
+    for b in cfg.buckets:
+        g = gen.gen_bucket(cfg, b, DEV)
+        ref = O.aggregate_bucket(np.ascontiguousarray(_np(g)[:, :b.n]), b.off, b.length, b.elig, (1, 0, 1), mode)
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=True, counts=False, health=True)
+        bb.out.fill_(-77.0)
+        bb.route_bucket((1, 0, 1))
+        bb.sign_pack(g, g.shape[1], mode)
+        bb.sign_count_reduce(mode)
+        bb.fp32_reduce(g, g.shape[1])
+        bb.health_stats(g, g.shape[1])
+        compare(bb, ref, cfg.W, mode, check_counts=False, what=f"{cfg.name} bucket {b.index} 5-call, no counts")
