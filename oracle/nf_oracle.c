@@ -23,6 +23,8 @@
  *   O3 decode : W identical workers => mean|g|*sign(g) (textbook scaled signSGD); W=1; sign flip
  *   O4a fp32  : numpy float32 ordered add; integer-valued exactness; W=1 identity
  *   O4b health: constant closed form; injected NaN/Inf counts; numpy.linalg.norm on finite part
+ *   NEXT-1    : hand-worked 2 x 2 split of the same bucket; hierarchical == flat O3 (all splits);
+ *               one worker per group => partial planes == packed planes; plane count closed form
  * Readings #3-#9 and #11 (what G-Ternary gating is, tie rule, scale granularity, scale
  * combination, NaN handling) are NOT fixed by the paper: "parity unpinned by the paper" for
  * those choices — they are pinned only by DESIGN.md and sit behind named parameters.
@@ -270,6 +272,84 @@ int nfo_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
             sumsq[(int64_t)r * T + t] = Q;
             nan_cnt[(int64_t)r * T + t] = cn;
             inf_cnt[(int64_t)r * T + t] = ci;
+        }
+    }
+    return NFO_OK;
+}
+
+/*
+ * NEXT-1 — two-level hierarchical sign count. PAPER L243: the reducer "aggregates
+ * compact worker updates through node-local counting and inter-node partial-count exchange before
+ * returning a synchronized aggregate direction"; L267: "performs node-local sign counting,
+ * exchanges partial counts, and returns the aggregate direction".
+ *
+ * Level 1, node-local counting of one group ("node") of Wg workers: for every packed word k and
+ * bit j, c = sum_{w < Wg} bit_j(plane_w[k]); the partial count is stored bit-sliced, plane b of
+ * word k holding bit b of c at bit position j (the partial-count payload a node sends): B planes,
+ * B >= number of bits of Wg (reading: smallest B with 2^B > Wg, nfo_count_planes).
+ */
+int nfo_count_planes(int Wg) {
+    int B = 0;
+    while ((1 << B) <= Wg) ++B;
+    return B;
+}
+
+int nfo_partial_count(const uint32_t *planes, int64_t plane_stride, int Wg, int64_t Wd, int B,
+                      uint32_t *cnt, int64_t count_stride) {
+    if (Wg < 1 || Wg > 255 || B < 1 || B > 8 || (1 << B) <= Wg) return NFO_ERR_RANGE;
+    for (int b = 0; b < B; ++b)
+        for (int64_t k = 0; k < Wd; ++k) cnt[(int64_t)b * count_stride + k] = 0u;
+    for (int64_t k = 0; k < Wd; ++k)
+        for (int j = 0; j < 32; ++j) {
+            int c = 0;
+            for (int w = 0; w < Wg; ++w) c += (int)((planes[(int64_t)w * plane_stride + k] >> j) & 1u);
+            for (int b = 0; b < B; ++b)
+                cnt[(int64_t)b * count_stride + k] |= (uint32_t)((c >> b) & 1) << j;
+        }
+    return NFO_OK;
+}
+
+/*
+ * Level 2, partial-count merge + decode: cpos = sum over the G groups of their partial counts
+ * (read back from the bit-sliced planes), likewise cneg (G-Binary: cneg = W - cpos), then the vote,
+ * the scale and the output exactly as in nfo_sign_count_reduce (O3), W = total number of workers,
+ * abs_sum[W][T] in global worker order. Layout: cnt[(g*B + b)*count_stride + k].
+ */
+int nfo_partial_count_merge(const uint32_t *cnt_pos, const uint32_t *cnt_neg, int64_t count_stride, int G,
+                            int B, int W, int64_t n, const int64_t *off, const int64_t *len,
+                            const uint8_t *route, const int64_t *woff, int T, int mode, int margin,
+                            const double *abs_sum, float *out, uint8_t *cpos, uint8_t *cneg,
+                            float *scale_out) {
+    if (W < 1 || W > 255 || G < 1 || G > W || B < 1 || B > 8 || margin < 0 || margin > 255) return NFO_ERR_RANGE;
+    if (mode != NFO_MODE_GBINARY && mode != NFO_MODE_GTERNARY) return NFO_ERR_ARG;
+    if (nfo_check_layout(off, len, T, n) != NFO_OK) return NFO_ERR_ARG;
+    for (int t = 0; t < T; ++t) {
+        if (scale_out) scale_out[t] = 0.0f;
+        if (route[t] != NFO_ROUTE_L) continue;
+        double ssum = 0.0;
+        for (int w = 0; w < W; ++w) {
+            float s_wt = (float)(abs_sum[(int64_t)w * T + t] / (double)len[t]);
+            ssum += (double)s_wt;
+        }
+        float S = (float)(ssum / (double)W);
+        if (scale_out) scale_out[t] = S;
+        for (int64_t i = 0; i < len[t]; ++i) {
+            int64_t k = woff[t] + i / 32;
+            int j = (int)(i % 32);
+            int cp = 0, cn = 0;
+            for (int g = 0; g < G; ++g)
+                for (int b = 0; b < B; ++b) {
+                    cp += (int)((cnt_pos[((int64_t)g * B + b) * count_stride + k] >> j) & 1u) << b;
+                    if (mode == NFO_MODE_GTERNARY)
+                        cn += (int)((cnt_neg[((int64_t)g * B + b) * count_stride + k] >> j) & 1u) << b;
+                }
+            if (cp > W || cn > W) return NFO_ERR_RANGE;
+            if (mode == NFO_MODE_GBINARY) cn = W - cp;
+            int D = cp - cn;
+            int d = (D > margin) - (D < -margin);
+            out[off[t] + i] = S * (float)d;
+            if (cpos) cpos[off[t] + i] = (uint8_t)cp;
+            if (cneg) cneg[off[t] + i] = (uint8_t)cn;
         }
     }
     return NFO_OK;

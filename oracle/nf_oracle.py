@@ -24,7 +24,8 @@ def lib() -> C.CDLL:
     if _lib is None:
         _lib = C.CDLL(_build.build())
         for name in ("nfo_route_bucket", "nfo_sign_pack", "nfo_sign_count_reference",
-                     "nfo_sign_count_reduce", "nfo_fp32_reduce", "nfo_health_stats"):
+                     "nfo_sign_count_reduce", "nfo_fp32_reduce", "nfo_health_stats", "nfo_count_planes",
+                     "nfo_partial_count", "nfo_partial_count_merge"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -141,6 +142,52 @@ def sign_count_reduce(P, N, W, n, off, length, route, woff, mode, margin, abs_su
                                      _p(out, C.c_float), _p(cpos, C.c_uint8), _p(cneg, C.c_uint8),
                                      _p(scale, C.c_float))
     _check(rc, "nfo_sign_count_reduce")
+    return out, cpos, cneg, scale
+
+
+def count_planes(Wg: int) -> int:
+    """NEXT-1: bit-planes of a partial count of Wg workers (smallest B with 2^B > Wg)."""
+    return int(lib().nfo_count_planes(C.c_int(int(Wg))))
+
+
+def partial_count(planes, B=None):
+    """NEXT-1 level 1 (PAPER L243/L267 node-local counting): planes [Wg][Wd] uint32 of one group ->
+    bit-sliced partial counts [B][Wd] uint32."""
+    planes = np.ascontiguousarray(planes, dtype=np.uint32)
+    Wg, Wd = planes.shape
+    B = count_planes(Wg) if B is None else int(B)
+    cnt = np.zeros((B, max(Wd, 1)), np.uint32)
+    rc = lib().nfo_partial_count(_p(planes, C.c_uint32), C.c_int64(planes.shape[1]), C.c_int(Wg), C.c_int64(Wd),
+                                 C.c_int(B), _p(cnt, C.c_uint32), C.c_int64(cnt.shape[1]))
+    _check(rc, "nfo_partial_count")
+    return cnt[:, :Wd]
+
+
+def partial_count_merge(cnt_pos, cnt_neg, W, n, off, length, route, woff, mode, margin, abs_sum, out=None):
+    """NEXT-1 level 2: cnt_pos/cnt_neg [G][B][Wd] uint32 (cnt_neg None for G-Binary) -> (out, cpos, cneg, scale)
+    exactly as sign_count_reduce."""
+    cnt_pos = np.ascontiguousarray(cnt_pos, dtype=np.uint32)
+    G, B, cs = cnt_pos.shape
+    if cnt_neg is not None:
+        cnt_neg = np.ascontiguousarray(cnt_neg, dtype=np.uint32)
+        assert cnt_neg.shape == cnt_pos.shape
+    off, length, woff = _i64(off), _i64(length), _i64(woff)
+    route = np.ascontiguousarray(route, dtype=np.uint8)
+    T = len(off)
+    A = np.ascontiguousarray(abs_sum, dtype=np.float64)
+    assert A.shape == (W, T)
+    if out is None:
+        out = np.zeros(n, np.float32)
+    cpos = np.zeros(n, np.uint8)
+    cneg = np.zeros(n, np.uint8)
+    scale = np.zeros(T, np.float32)
+    rc = lib().nfo_partial_count_merge(_p(cnt_pos, C.c_uint32), _p(cnt_neg, C.c_uint32), C.c_int64(cs), C.c_int(G),
+                                       C.c_int(B), C.c_int(W), C.c_int64(n), _p(off, C.c_int64),
+                                       _p(length, C.c_int64), _p(route, C.c_uint8), _p(woff, C.c_int64),
+                                       C.c_int(T), C.c_int(mode), C.c_int(margin), _p(A, C.c_double),
+                                       _p(out, C.c_float), _p(cpos, C.c_uint8), _p(cneg, C.c_uint8),
+                                       _p(scale, C.c_float))
+    _check(rc, "nfo_partial_count_merge")
     return out, cpos, cneg, scale
 
 
