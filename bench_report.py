@@ -159,6 +159,49 @@ def table_sweep(args, dev, peak):
     return "\n".join(out)
 
 
+def table_hier(args, dev, peak):
+    """NEXT-1: node-local counting per group of W/G workers (level 1), merge of the G
+    partial-count sets + decode (level 2), against the flat count-reduce over all W."""
+    import torch
+    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from workloads import shapes, gen
+    out = ["| W | G (nodes) | workers/node | B planes | payload per node: packed signs -> partial counts | level 1 (one node) | "
+           "level 2 merge + decode | flat count-reduce |", "|---|---|---|---|---|---|---|---|"]
+    for W, G in ((32, 4), (32, 8), (128, 4), (128, 8), (128, 16)):
+        cfg = shapes.sweep(W)
+        b = cfg.buckets[0]
+        n = b.n
+        g = gen.gen_bucket(cfg, b, dev)
+        bb = BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=False)
+        bb.route_bucket((1, 0, 1))
+        bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+        torch.cuda.synchronize()
+        Wd = int(bb.summary[nf.SUM_WD])
+        Wg = W // G
+        B = nf.nf_count_planes(Wg)
+        cs = (Wd + 3) // 4 * 4
+        cp = torch.zeros((G, B, cs), dtype=torch.int32, device=dev)
+        cn = torch.zeros((G, B, cs), dtype=torch.int32, device=dev)
+        for gi in range(G):
+            nf.nf_partial_count(bb.P[gi * Wg:], bb.N[gi * Wg:], bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[gi], cn[gi], cs)
+
+        def level1():
+            nf.nf_partial_count(bb.P, bb.N, bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[0], cn[0], cs)
+
+        def level2():
+            nf.nf_partial_count_merge(cp, cn, cs, G, B, W, n, bb.off, bb.len, bb.route, bb.woff, bb.T, nf.MODE_GTERNARY, 0,
+                                      bb.abs_sum, bb.out, None, None, bb.scale, bb.plan)
+
+        def flat():
+            bb.sign_count_reduce(nf.MODE_GTERNARY)
+        t1, t2, t3 = (time_fn(f, args.iters) * 1e3 for f in (level1, level2, flat))
+        packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
+        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us |")
+        del g, bb, cp, cn
+        torch.cuda.empty_cache()
+    return "\n".join(out)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default="")
@@ -177,6 +220,8 @@ def main():
     if not args.skip_configs:
         parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
     parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
+    parts += ["### NEXT-1: two-level hierarchical sign count on the same bucket (G-Ternary; results identical to the flat reduce)", "",
+              table_hier(args, dev, peak), ""]
     text = "\n".join(parts)
     print(text)
     if args.out:

@@ -117,6 +117,35 @@ int nf_sign_count_reduce(const uint32_t *P, const uint32_t *N, int64_t plane_str
                          void *plan, nf_stream stream);
 
 /*
+ * NEXT-1: two-level hierarchical sign count — PAPER L243 ("node-local counting and
+ * inter-node partial-count exchange before returning a synchronized aggregate direction"), L267
+ * ("performs node-local sign counting, exchanges partial counts, and returns the aggregate
+ * direction"). Results are identical to nf_sign_count_reduce over all W workers.
+ *
+ * nf_count_planes (host): bit-planes of a partial count of Wg workers = smallest B with 2^B > Wg
+ * (1..8), or NF_ERR_RANGE.
+ *
+ * nf_partial_count — level 1, one group ("node") of Wg workers: for every packed word k < Wd and
+ * bit j, c = number of the group's workers whose bit j of word k is set; stored bit-sliced:
+ * cnt_pos[b*count_stride + k] bit j = bit b of c, b < B (2^B > Wg required). cnt_neg likewise
+ * from N (G-Ternary only; N and cnt_neg may be NULL for G-Binary). P/N are the group's planes
+ * [Wg][plane_stride]. The B x Wd words per sign are the partial-count payload a node sends.
+ *
+ * nf_partial_count_merge — level 2: adds the G groups' partial counts, cnt[(g*B + b)*count_stride
+ * + k], into cpos/cneg (G-Binary: cneg = W - cpos, W = total workers), then votes, scales and
+ * writes exactly as nf_sign_count_reduce: abs_sum[W][T] in global worker order, same plan, same
+ * optional outputs. Groups may hold different numbers of workers as long as each count fits B planes.
+ */
+int nf_count_planes(int Wg);
+int nf_partial_count(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int Wg, int64_t Wd, int mode,
+                     int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride, nf_stream stream);
+int nf_partial_count_merge(const uint32_t *cnt_pos, const uint32_t *cnt_neg, int64_t count_stride, int G, int B,
+                           int W, int64_t n, const int64_t *off, const int64_t *len, const uint8_t *route,
+                           const int64_t *woff, int T, int mode, int margin, const double *abs_sum,
+                           float *out, uint8_t *cpos, uint8_t *cneg, float *scale_out, void *plan,
+                           nf_stream stream);
+
+/*
  * a4a FP32 route — PAPER L50, L66, L144 (oracle O4a). For every P/F tensor:
  * out[i] = alpha * (((g_0[i] + g_1[i]) + g_2[i]) + ... + g_{W-1}[i]) in FP32, fixed worker order.
  */

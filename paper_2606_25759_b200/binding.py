@@ -23,7 +23,8 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
-           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect")
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect",
+           "nf_count_planes", "nf_partial_count", "nf_partial_count_merge")
 
 
 class NfState(C.Structure):
@@ -75,6 +76,13 @@ def lib() -> C.CDLL:
     L.nf_aggregate_bucket_host.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32,
                                            f32, vp, vp, vp, vp, vp, vp, vp, vp, vp,
                                            vp, sz, vp, sz, vp]
+    L.nf_count_planes.restype = i32
+    L.nf_count_planes.argtypes = [i32]
+    L.nf_partial_count.restype = i32
+    L.nf_partial_count.argtypes = [vp, vp, i64, i32, i64, i32, i32, vp, vp, i64, vp]
+    L.nf_partial_count_merge.restype = i32
+    L.nf_partial_count_merge.argtypes = [vp, vp, i64, i32, i32, i32, i64, vp, vp, vp, vp, i32, i32, i32, vp,
+                                         vp, vp, vp, vp, vp, vp]
     L.nf_prof_enable.restype = i32
     L.nf_prof_enable.argtypes = [i32]
     L.nf_prof_collect.restype = i32
@@ -179,6 +187,27 @@ def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, el
         _ptr(route), _ptr(woff), _ptr(summary), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt), _ptr(inf_cnt),
         _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_count_planes(Wg: int) -> int:
+    B = lib().nf_count_planes(int(Wg))
+    if B < 0:
+        raise NfError("nf_count_planes", B)
+    return B
+
+
+def nf_partial_count(P, N, plane_stride, Wg, Wd, mode, B, cnt_pos, cnt_neg, count_stride, stream=None):
+    _check("nf_partial_count", lib().nf_partial_count(
+        _ptr(P), _ptr(N), int(plane_stride), int(Wg), int(Wd), int(mode), int(B), _ptr(cnt_pos), _ptr(cnt_neg),
+        int(count_stride), _stream(stream)))
+
+
+def nf_partial_count_merge(cnt_pos, cnt_neg, count_stride, G, B, W, n, off, length, route, woff, T, mode, margin,
+                           abs_sum, out, cpos, cneg, scale_out, plan, stream=None):
+    _check("nf_partial_count_merge", lib().nf_partial_count_merge(
+        _ptr(cnt_pos), _ptr(cnt_neg), int(count_stride), int(G), int(B), int(W), int(n), _ptr(off), _ptr(length),
+        _ptr(route), _ptr(woff), int(T), int(mode), int(margin), _ptr(abs_sum), _ptr(out), _ptr(cpos),
+        _ptr(cneg), _ptr(scale_out), _ptr(plan), _stream(stream)))
 
 
 def nf_prof_enable(max_records: int):

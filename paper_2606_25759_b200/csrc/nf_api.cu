@@ -111,6 +111,48 @@ int nf_sign_count_reduce(const uint32_t *P, const uint32_t *N, int64_t plane_str
     return cuda_rc(launch_count_reduce(p, n, (cudaStream_t)stream));
 }
 
+int nf_count_planes(int Wg) {
+    if (Wg < 1 || Wg > 255) return NF_ERR_RANGE;
+    int B = 0;
+    while ((1 << B) <= Wg) ++B;
+    return B;
+}
+
+int nf_partial_count(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int Wg, int64_t Wd, int mode,
+                     int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride, nf_stream stream) {
+    if (Wg < 1 || Wg > 255 || B < 1 || B > 8 || (1 << B) <= Wg) return NF_ERR_RANGE;
+    if (Wd < 0 || Wd > ((int64_t)1 << 35)) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (plane_stride < Wd || count_stride < Wd) return NF_ERR_ARG;
+    if (Wd > 0 && (!P || !cnt_pos)) return NF_ERR_ARG;
+    if (mode == NF_MODE_GTERNARY && Wd > 0 && (!N || !cnt_neg)) return NF_ERR_ARG;
+    if (misaligned16(P) || misaligned16(N) || misaligned16(cnt_pos) || misaligned16(cnt_neg)) return NF_ERR_ALIGN;
+    return cuda_rc(launch_partial_count(P, N, plane_stride, Wg, Wd, mode == NF_MODE_GTERNARY, B, cnt_pos, cnt_neg,
+                                        count_stride, (cudaStream_t)stream));
+}
+
+int nf_partial_count_merge(const uint32_t *cnt_pos, const uint32_t *cnt_neg, int64_t count_stride, int G, int B,
+                           int W, int64_t n, const int64_t *off, const int64_t *len, const uint8_t *route,
+                           const int64_t *woff, int T, int mode, int margin, const double *abs_sum,
+                           float *out, uint8_t *cpos, uint8_t *cneg, float *scale_out, void *plan,
+                           nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (margin < 0 || margin > 255 || G < 1 || G > W || B < 1 || B > 8) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!plan || count_stride < 0) return NF_ERR_ARG;
+    if (T > 0 && (!cnt_pos || !off || !len || !route || !woff || !abs_sum || !out)) return NF_ERR_ARG;
+    if (mode == NF_MODE_GTERNARY && T > 0 && !cnt_neg) return NF_ERR_ARG;
+    if (misaligned16(cnt_pos) || misaligned16(cnt_neg) || misaligned16(out) || misaligned16(plan)) return NF_ERR_ALIGN;
+    if (T == 0) return NF_OK;
+    ReduceParams p{};
+    p.cnt_pos = cnt_pos; p.cnt_neg = cnt_neg; p.count_stride = count_stride; p.G = G; p.B = B;
+    p.W = W; p.T = T; p.off = off; p.len = len; p.route = route; p.woff = woff;
+    p.ternary = (mode == NF_MODE_GTERNARY); p.margin = margin; p.abs_sum = abs_sum;
+    p.out = out; p.cpos = cpos; p.cneg = cneg; p.scale_out = scale_out; p.plan = plan;
+    return cuda_rc(launch_count_reduce(p, n, (cudaStream_t)stream));
+}
+
 int nf_fp32_reduce(const float *g, int64_t worker_stride, int W, int64_t n,
                    const int64_t *off, const int64_t *len, const uint8_t *route, int T,
                    float alpha, float *out, void *plan, nf_stream stream) {

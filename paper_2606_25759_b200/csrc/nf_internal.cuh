@@ -138,6 +138,10 @@ struct ReduceParams {
     uint8_t *cneg;
     float *scale_out;
     const uint8_t *dirs;       // decode pass of the fused path
+    const uint32_t *cnt_pos;   // NEXT-1 merge: bit-sliced partial counts [(g*B + b)*count_stride + k], else NULL
+    const uint32_t *cnt_neg;
+    int64_t count_stride;
+    int G, B;
     int pdl;                   // launch with programmatic stream serialization (fused path)
     void *plan;
 };
@@ -151,6 +155,9 @@ cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStrea
 cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s);
+cudaError_t launch_partial_count(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int Wg, int64_t Wd,
+                                 int ternary, int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride,
+                                 cudaStream_t s);
 int device_sm_count();
 
 

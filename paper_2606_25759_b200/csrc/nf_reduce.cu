@@ -54,6 +54,17 @@ struct SlicedCounter {
     }
 };
 
+// c += x where x is a bit-sliced number of up to 8 planes (NEXT-1: adding a group's partial count)
+__device__ __forceinline__ void sliced_add(SlicedCounter &sc, const uint32_t (&x)[8]) {
+    uint32_t carry = 0u;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const uint32_t a = sc.c[b];
+        sc.c[b] = a ^ x[b] ^ carry;
+        carry = (a & x[b]) | (a & carry) | (x[b] & carry);
+    }
+}
+
 // gt = (a > b) bitwise over 32 lanes; a has 8 planes, b has 9 planes (b may exceed 255)
 __device__ __forceinline__ uint32_t sliced_gt(const uint32_t (&a)[8], const uint32_t (&b)[9]) {
     uint32_t gt = 0u, eq = ~b[8];            // a's plane 8 is zero: if b[8] is set, a < b
@@ -136,7 +147,7 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
     __syncthreads();
 }
 
-template <bool WRITE_COUNTS>
+template <bool WRITE_COUNTS, bool MERGE>
 __global__ void __launch_bounds__(kRThreads, 2) count_reduce_kernel(const ReduceParams p) {
     __shared__ float4 s_dtab[256];          // byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
     {
@@ -182,8 +193,24 @@ __global__ void __launch_bounds__(kRThreads, 2) count_reduce_kernel(const Reduce
             nvalid = rem >= 32 ? 32 : (int)rem;
             obase = __ldg(p.off + t) + i0;
             my_li = li;
-            if (p.ternary) count_words2<true>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
-            else count_words2<false>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
+            if (MERGE) {
+                // NEXT-1 level 2: sum of the G groups' bit-sliced partial counts
+                for (int g = 0; g < p.G; ++g) {
+                    uint32_t xp[8], xn[8];
+#pragma unroll
+                    for (int b = 0; b < 8; ++b) {
+                        const size_t o = ((size_t)g * p.B + b) * p.count_stride + k;
+                        xp[b] = (b < p.B) ? __ldcs(p.cnt_pos + o) : 0u;
+                        xn[b] = (b < p.B && p.ternary) ? __ldcs(p.cnt_neg + o) : 0u;
+                    }
+                    sliced_add(cpv, xp);
+                    if (p.ternary) sliced_add(cnv, xn);
+                }
+            } else if (p.ternary) {
+                count_words2<true>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
+            } else {
+                count_words2<false>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
+            }
             if (p.ternary) {
                 // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
                 uint32_t b[9];
@@ -366,6 +393,25 @@ __global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p)
     }
 }
 
+// NEXT-1 level 1 ("node-local counting", L267): the bit-sliced per-position counts of one
+// group of Wg workers' packed planes, B planes per sign = the partial-count payload a node sends.
+__global__ void __launch_bounds__(kRThreads, 2)
+partial_count_kernel(const uint32_t *__restrict__ P, const uint32_t *__restrict__ N, int64_t plane_stride, int Wg,
+                     int64_t Wd, int ternary, int B, uint32_t *__restrict__ cnt_pos, uint32_t *__restrict__ cnt_neg,
+                     int64_t count_stride) {
+    for (int64_t k = (int64_t)blockIdx.x * kRThreads + threadIdx.x; k < Wd; k += (int64_t)gridDim.x * kRThreads) {
+        SlicedCounter cp, cn;
+        if (ternary) count_words2<true>(P + k, N + k, plane_stride, Wg, cp, cn);
+        else count_words2<false>(P + k, N, plane_stride, Wg, cp, cn);
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            if (b >= B) break;
+            cnt_pos[(size_t)b * count_stride + k] = cp.c[b];
+            if (ternary) cnt_neg[(size_t)b * count_stride + k] = cn.c[b];
+        }
+    }
+}
+
 static int grid_for(int64_t units, int per_sm) {
     int64_t g = (int64_t)device_sm_count() * per_sm;
     if (g > units) g = units;
@@ -375,10 +421,24 @@ static int grid_for(int64_t units, int per_sm) {
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s) {
     const int64_t max_words = n / 32 + p.T;
     const int64_t chunks = (max_words + kRThreads - 1) / kRThreads;
-    const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
     const int grid = grid_for(chunks, 8);
-    if (p.cpos || p.cneg) count_reduce_kernel<true><<<grid, kRThreads, smem, s>>>(p);
-    else count_reduce_kernel<false><<<grid, kRThreads, smem, s>>>(p);
+    const bool counts = p.cpos || p.cneg;
+    if (p.cnt_pos) {
+        if (counts) count_reduce_kernel<true, true><<<grid, kRThreads, 0, s>>>(p);
+        else count_reduce_kernel<false, true><<<grid, kRThreads, 0, s>>>(p);
+    } else {
+        if (counts) count_reduce_kernel<true, false><<<grid, kRThreads, 0, s>>>(p);
+        else count_reduce_kernel<false, false><<<grid, kRThreads, 0, s>>>(p);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t launch_partial_count(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int Wg, int64_t Wd,
+                                 int ternary, int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride,
+                                 cudaStream_t s) {
+    if (Wd <= 0) return cudaSuccess;
+    const int grid = grid_for((Wd + kRThreads - 1) / kRThreads, 8);
+    partial_count_kernel<<<grid, kRThreads, 0, s>>>(P, N, plane_stride, Wg, Wd, ternary, B, cnt_pos, cnt_neg, count_stride);
     return cudaGetLastError();
 }
 
