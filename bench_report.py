@@ -166,7 +166,8 @@ def table_hier(args, dev, peak):
     from paper_2606_25759_b200 import BucketBuffers, binding as nf
     from workloads import shapes, gen
     out = ["| W | G (nodes) | workers/node | B planes | payload per node: packed signs -> partial counts | level 1 (one node) | "
-           "level 2 merge + decode | flat count-reduce |", "|---|---|---|---|---|---|---|---|"]
+           "level 2 merge + decode | flat count-reduce | NEXT-2: stock packed-sign, W replicated counts | hierarchical, all nodes "
+           "(G x level 1 + level 2) |", "|---|---|---|---|---|---|---|---|---|---|"]
     for W, G in ((32, 4), (32, 8), (128, 4), (128, 8), (128, 16)):
         cfg = shapes.sweep(W)
         b = cfg.buckets[0]
@@ -194,9 +195,18 @@ def table_hier(args, dev, peak):
 
         def flat():
             bb.sign_count_reduce(nf.MODE_GTERNARY)
-        t1, t2, t3 = (time_fn(f, args.iters) * 1e3 for f in (level1, level2, flat))
+        def stock():      # NEXT-2: every worker receives all W sign streams and counts them itself
+            for _ in range(W):
+                bb.sign_count_reduce(nf.MODE_GTERNARY)
+
+        def hier_all():   # all G nodes count locally, one merge + decode
+            for gi in range(G):
+                nf.nf_partial_count(bb.P[gi * Wg:], bb.N[gi * Wg:], bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[gi], cn[gi], cs)
+            level2()
+        t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5)) * 1e3
+                              for f in (level1, level2, flat, stock, hier_all))
         packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
-        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us |")
+        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us |")
         del g, bb, cp, cn
         torch.cuda.empty_cache()
     return "\n".join(out)
@@ -220,7 +230,8 @@ def main():
     if not args.skip_configs:
         parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
     parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
-    parts += ["### NEXT-1: two-level hierarchical sign count on the same bucket (G-Ternary; results identical to the flat reduce)", "",
+    parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
+              "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange)", "",
               table_hier(args, dev, peak), ""]
     text = "\n".join(parts)
     print(text)

@@ -200,6 +200,35 @@ int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t
                              nf_stream stream);
 
 /*
+ * NEXT-4: Supervisor recovery controller (HOST functions, no device work) — PAPER L158
+ * ("slack is the tolerated per-step increase in the smoothed training-health signal before degradation
+ * evidence accumulates, and the threshold is the accumulated excess that triggers fallback to FP32"),
+ * L177-179 (smoothed signal + CUSUM; fallback, cooldown, guarded readmission), Table 2. It produces the
+ * nf_state flags nf_route_bucket / nf_aggregate_bucket read. Per step (readings #15-#19):
+ *   m_0 = x_0, m_k = beta*m_{k-1} + (1-beta)*x_k;  y_k = m_k - m_{k-1};
+ *   S_k = max(0, S_{k-1} + y_k - slack) while low-bit is admitted;  alarm iff S_k > threshold, or any
+ *   NaN/Inf tally (nf_health_stats) / non-finite signal in the step;
+ *   WARMUP (admitted = 0, warmup_steps) -> ADMITTED -> alarm -> COOLDOWN (veto = 1, cooldown_steps) ->
+ *   GUARD (guard_steps; an alarm here re-enters COOLDOWN with twice the length) -> ADMITTED.
+ * nf_supervisor_step consumes the signal of the step just finished and writes the flags for the next
+ * route decisions; capacity_ok is passed through. The struct is plain caller-owned host memory.
+ */
+typedef struct nf_supervisor_cfg {
+    int32_t warmup_steps, cooldown_steps, guard_steps, reserved;
+    double ema_beta, slack, threshold;
+} nf_supervisor_cfg;
+typedef struct nf_supervisor {
+    nf_supervisor_cfg cfg;
+    int32_t phase;      /* 0 warm-up, 1 admitted, 2 cooldown, 3 guard */
+    int32_t remaining;  /* steps left in the current timed phase */
+    int64_t step, detections;
+    double ema, cusum;
+} nf_supervisor;
+int nf_supervisor_init(nf_supervisor *s /*host*/, const nf_supervisor_cfg *cfg /*host*/);
+int nf_supervisor_step(nf_supervisor *s /*host*/, double signal, uint64_t nan_count, uint64_t inf_count,
+                       int capacity_ok, nf_state *out /*host*/);
+
+/*
  * Instrumentation (host calls, not part of the data path). nf_prof_enable(k > 0) creates CUDA
  * events for up to k nf_aggregate_bucket calls and makes each such call record four events on
  * its stream (before the route kernel, before the fused kernel, after it, at the end of the call); nf_prof_enable(0) frees

@@ -24,11 +24,22 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
            "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect",
-           "nf_count_planes", "nf_partial_count", "nf_partial_count_merge")
+           "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
+           "nf_supervisor_step")
 
 
 class NfState(C.Structure):
     _fields_ = [("admitted", C.c_int32), ("veto", C.c_int32), ("capacity_ok", C.c_int32)]
+
+
+class NfSupervisorCfg(C.Structure):
+    _fields_ = [("warmup_steps", C.c_int32), ("cooldown_steps", C.c_int32), ("guard_steps", C.c_int32),
+                ("reserved", C.c_int32), ("ema_beta", C.c_double), ("slack", C.c_double), ("threshold", C.c_double)]
+
+
+class NfSupervisor(C.Structure):
+    _fields_ = [("cfg", NfSupervisorCfg), ("phase", C.c_int32), ("remaining", C.c_int32), ("step", C.c_int64),
+                ("detections", C.c_int64), ("ema", C.c_double), ("cusum", C.c_double)]
 
 
 class NfError(RuntimeError):
@@ -83,6 +94,10 @@ def lib() -> C.CDLL:
     L.nf_partial_count_merge.restype = i32
     L.nf_partial_count_merge.argtypes = [vp, vp, i64, i32, i32, i32, i64, vp, vp, vp, vp, i32, i32, i32, vp,
                                          vp, vp, vp, vp, vp, vp]
+    L.nf_supervisor_init.restype = i32
+    L.nf_supervisor_init.argtypes = [C.POINTER(NfSupervisor), C.POINTER(NfSupervisorCfg)]
+    L.nf_supervisor_step.restype = i32
+    L.nf_supervisor_step.argtypes = [C.POINTER(NfSupervisor), C.c_double, C.c_uint64, C.c_uint64, i32, C.POINTER(NfState)]
     L.nf_prof_enable.restype = i32
     L.nf_prof_enable.argtypes = [i32]
     L.nf_prof_collect.restype = i32
@@ -208,6 +223,27 @@ def nf_partial_count_merge(cnt_pos, cnt_neg, count_stride, G, B, W, n, off, leng
         _ptr(cnt_pos), _ptr(cnt_neg), int(count_stride), int(G), int(B), int(W), int(n), _ptr(off), _ptr(length),
         _ptr(route), _ptr(woff), int(T), int(mode), int(margin), _ptr(abs_sum), _ptr(out), _ptr(cpos),
         _ptr(cneg), _ptr(scale_out), _ptr(plan), _stream(stream)))
+
+
+class Supervisor:
+    """Marshalling for nf_supervisor_init / nf_supervisor_step (host functions of libnf.so)."""
+
+    def __init__(self, warmup_steps, ema_beta, slack, threshold, cooldown_steps, guard_steps):
+        self._s = NfSupervisor()
+        cfg = NfSupervisorCfg(int(warmup_steps), int(cooldown_steps), int(guard_steps), 0, float(ema_beta),
+                              float(slack), float(threshold))
+        _check("nf_supervisor_init", lib().nf_supervisor_init(C.byref(self._s), C.byref(cfg)))
+
+    def step(self, signal, nan_count=0, inf_count=0, capacity_ok=1):
+        st = NfState()
+        _check("nf_supervisor_step", lib().nf_supervisor_step(C.byref(self._s), float(signal), int(nan_count),
+                                                               int(inf_count), int(capacity_ok), C.byref(st)))
+        return st.admitted, st.veto, st.capacity_ok
+
+    phase = property(lambda self: self._s.phase)
+    detections = property(lambda self: self._s.detections)
+    cusum = property(lambda self: self._s.cusum)
+    ema = property(lambda self: self._s.ema)
 
 
 def nf_prof_enable(max_records: int):
