@@ -17,6 +17,7 @@ LIB = os.path.join(HERE, "libnf.so")
 SOURCES = ["nf_route.cu", "nf_stream.cu", "nf_fused.cu", "nf_reduce.cu", "nf_api.cu", "nf_supervisor.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # no --use_fast_math; the FP32 route uses explicit __fadd_rn/__fmul_rn so contraction cannot touch it
+EXTRA = os.environ.get("NF_EXTRA_NVCC", "").split()   # tuning aid, e.g. NF_EXTRA_NVCC="-DNF_KDW=3"
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 
@@ -35,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def cc(src):
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        subprocess.check_call([NVCC, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj])
+        subprocess.check_call([NVCC, *NVCC_FLAGS, *EXTRA, *extra, "-c", os.path.join(CSRC, src), "-o", obj])
         return obj
 
     with ThreadPoolExecutor(max_workers=6) as ex:

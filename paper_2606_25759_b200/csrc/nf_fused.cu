@@ -27,13 +27,22 @@ namespace nf {
 
 constexpr int kCW = 16;                          // consumer warps
 constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = one tile
-constexpr int kDW = 2;                           // decode warps (pass B inside the kernel)
+#ifndef NF_KDW
+#define NF_KDW 2
+#endif
+#ifndef NF_KDU
+#define NF_KDU 2
+#endif
+#ifndef NF_KKT
+#define NF_KKT 4
+#endif
+constexpr int kDW = NF_KDW;                      // decode warps (pass B inside the kernel)
 constexpr int kFThreads = kCThreads + 64 + kDW * 32;   // + producer warp + housekeeping warp + decode warps
-constexpr int kDU = 4;                           // decode: tiles in flight per warp
+constexpr int kDU = NF_KDU;                      // decode: units in flight per warp
 constexpr int kPitch = kTile + 4;                // ring row: one tile of one worker + room for a misaligned head
 constexpr int kStageFloats = kGroup * kPitch;    // 8 workers
 constexpr int kStageBytes = kStageFloats * 4;    // 64 KB + 128 B
-constexpr int kKTiles = 4;                       // tiles of FP32 partial accumulation
+constexpr int kKTiles = NF_KKT;                  // tiles of FP32 partial accumulation (<= 4: exact_redo's list)
 constexpr int kMaxStages = 4;
 constexpr int kStages = 3;                       // ring depth: 3 x 64 KB
 static_assert(kTile == kCThreads * 4, "one float4 per consumer thread per worker and tile");
