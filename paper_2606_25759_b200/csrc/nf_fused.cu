@@ -748,8 +748,8 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
         }
         // publish: every consumer's direction bytes / plane words / atomics of this tensor are ordered
-        // before the counter the decode warps (of any CTA) acquire
-        __threadfence();
+        // before the counter the decode warps (of any CTA) acquire (FP32-route tensors have no decode)
+        if (c.isL) __threadfence();
         consumer_sync();
         if (ctid == 0 && c.isL) {
             __threadfence();
