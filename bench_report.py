@@ -167,7 +167,8 @@ def table_hier(args, dev, peak):
     from workloads import shapes, gen
     out = ["| W | G (nodes) | workers/node | B planes | payload per node: packed signs -> partial counts | level 1 (one node) | "
            "level 2 merge + decode | flat count-reduce | NEXT-2: stock packed-sign, W replicated counts | hierarchical, all nodes "
-           "(G x level 1 + level 2) |", "|---|---|---|---|---|---|---|---|---|---|"]
+           "(G x level 1 + level 2) | NEXT-3: measured endpoint service rate | guard verdict at 12.5 / 50 / 400 GB/s per node |",
+           "|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for W, G in ((32, 4), (32, 8), (128, 4), (128, 8), (128, 16)):
         cfg = shapes.sweep(W)
         b = cfg.buckets[0]
@@ -206,7 +207,10 @@ def table_hier(args, dev, peak):
         t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5)) * 1e3
                               for f in (level1, level2, flat, stock, hier_all))
         packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
-        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us |")
+        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us | "
+                   f"{packed / (t1 * 1e-6) / 1e9:.0f} GB/s | "
+                   + " / ".join("admit" if nf.nf_capacity_guard(n, G, Wg, packed / (t1 * 1e-6), bw, 2)[0] else "FP32"
+                                for bw in (12.5e9, 50e9, 400e9)) + " |")
         del g, bb, cp, cn
         torch.cuda.empty_cache()
     return "\n".join(out)

@@ -200,6 +200,25 @@ int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t
                              nf_stream stream);
 
 /*
+ * NEXT-3, HOST functions. nf_mgtr — PAPER L110-114: modeled gradient-communication traffic
+ * ratio of a route log, MGTR = sum_e bytes(route_e) / sum_e bytes(FP32_e). Event e = (numel[e], route[e]
+ * (nf_route), mode[e] (nf_mode, read for L events only)): an L event counts numel*bits/8 + scale_bytes with
+ * bits = bits_binary or bits_ternary (reading #14: 1 and log2(3)), F and P events count 4*numel;
+ * the denominator counts 4*numel for every event. No events -> 1.
+ *
+ * nf_capacity_guard — PAPER L273-275: admit a candidate low-bit bucket only when the estimated
+ * hierarchical-reducer time is lower than the matched FP32 time. Time model (reading #20, not the
+ * paper's): t_fp32 = 2(N-1)/N * 4n / net_bw; t_hier = F * (p*n/8) / service_rate + 2(N-1)/N * (p*B*n/8) /
+ * net_bw with N = nodes, F = local_fan_in, p = planes (1 G-Binary, 2 G-Ternary), B = nf_count_planes(N*F),
+ * rates in bytes/s. Returns 1 (admit: capacity_ok), 0 (stay on FP32) or a negative nf_status; the two times
+ * are written when the pointers are not NULL.
+ */
+int nf_mgtr(const int64_t *numel /*host*/, const uint8_t *route /*host*/, const uint8_t *mode /*host*/,
+            int64_t n_events, double bits_binary, double bits_ternary, int scale_bytes, double *mgtr /*host*/);
+int nf_capacity_guard(int64_t n, int nodes, int local_fan_in, double service_rate, double net_bw, int planes,
+                      double *t_hier /*host*/, double *t_fp32 /*host*/);
+
+/*
  * NEXT-4: Supervisor recovery controller (HOST functions, no device work) — PAPER L158
  * ("slack is the tolerated per-step increase in the smoothed training-health signal before degradation
  * evidence accumulates, and the threshold is the accumulated excess that triggers fallback to FP32"),

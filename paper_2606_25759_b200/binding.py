@@ -25,7 +25,7 @@ EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_byte
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
            "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
-           "nf_supervisor_step")
+           "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard")
 
 
 class NfState(C.Structure):
@@ -98,6 +98,11 @@ def lib() -> C.CDLL:
     L.nf_supervisor_init.argtypes = [C.POINTER(NfSupervisor), C.POINTER(NfSupervisorCfg)]
     L.nf_supervisor_step.restype = i32
     L.nf_supervisor_step.argtypes = [C.POINTER(NfSupervisor), C.c_double, C.c_uint64, C.c_uint64, i32, C.POINTER(NfState)]
+    L.nf_mgtr.restype = i32
+    L.nf_mgtr.argtypes = [vp, vp, vp, i64, C.c_double, C.c_double, i32, C.POINTER(C.c_double)]
+    L.nf_capacity_guard.restype = i32
+    L.nf_capacity_guard.argtypes = [i64, i32, i32, C.c_double, C.c_double, i32, C.POINTER(C.c_double),
+                                    C.POINTER(C.c_double)]
     L.nf_prof_enable.restype = i32
     L.nf_prof_enable.argtypes = [i32]
     L.nf_prof_collect.restype = i32
@@ -223,6 +228,28 @@ def nf_partial_count_merge(cnt_pos, cnt_neg, count_stride, G, B, W, n, off, leng
         _ptr(cnt_pos), _ptr(cnt_neg), int(count_stride), int(G), int(B), int(W), int(n), _ptr(off), _ptr(length),
         _ptr(route), _ptr(woff), int(T), int(mode), int(margin), _ptr(abs_sum), _ptr(out), _ptr(cpos),
         _ptr(cneg), _ptr(scale_out), _ptr(plan), _stream(stream)))
+
+
+def nf_mgtr(numel, route, mode, bits_binary=1.0, bits_ternary=1.584962500721156, scale_bytes=4) -> float:
+    """Host call: MGTR of a route log."""
+    import numpy as np
+    a = np.ascontiguousarray(numel, dtype=np.int64)
+    r = np.ascontiguousarray(route, dtype=np.uint8)
+    m = np.ascontiguousarray(mode, dtype=np.uint8)
+    out = C.c_double(0.0)
+    _check("nf_mgtr", lib().nf_mgtr(a.ctypes.data, r.ctypes.data, m.ctypes.data, int(a.size), float(bits_binary),
+                                    float(bits_ternary), int(scale_bytes), C.byref(out)))
+    return out.value
+
+
+def nf_capacity_guard(n, nodes, local_fan_in, service_rate, net_bw, planes):
+    """Host call: (admit, t_hier, t_fp32) of the endpoint-capacity guard."""
+    th, tf = C.c_double(0.0), C.c_double(0.0)
+    rc = lib().nf_capacity_guard(int(n), int(nodes), int(local_fan_in), float(service_rate), float(net_bw),
+                                 int(planes), C.byref(th), C.byref(tf))
+    if rc < 0:
+        raise NfError("nf_capacity_guard", rc)
+    return rc, th.value, tf.value
 
 
 class Supervisor:
