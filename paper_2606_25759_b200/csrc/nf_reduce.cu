@@ -95,25 +95,26 @@ __device__ __forceinline__ void const_planes(int v, uint32_t (&b)[9]) {
 
 // Stream the W words of word position k of both planes into two sliced counters: 16 workers per round,
 // i.e. up to 32 independent loads in flight per thread (a thread walks W serially, so the depth of
-// each round, not the thread count, is what hides the HBM latency at large fan-in).
-template <bool TERNARY>
+// each round, not the thread count, is what hides the HBM latency at large fan-in). Small fan-in (W <= 16)
+// uses 8 per round: fewer registers, twice the resident CTAs, fewer waves of the latency-bound prologue.
+template <bool TERNARY, int ROUND>
 __device__ __forceinline__ void count_words2(const uint32_t *__restrict__ P, const uint32_t *__restrict__ N,
                                              int64_t stride, int W, SlicedCounter &cp, SlicedCounter &cn) {
+    static_assert(ROUND == 8 || ROUND == 16, "workers per round");
     cp.clear();
     cn.clear();
-    for (int w = 0; w < W; w += 16) {
-        uint32_t xp[16], xn[16];
+    for (int w = 0; w < W; w += ROUND) {
+        uint32_t xp[ROUND], xn[ROUND];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
+        for (int i = 0; i < ROUND; ++i) {
             const bool in = w + i < W;
             xp[i] = in ? __ldcs(P + (size_t)(w + i) * stride) : 0u;
             xn[i] = (TERNARY && in) ? __ldcs(N + (size_t)(w + i) * stride) : 0u;
         }
-        cp.add8(reinterpret_cast<const uint32_t(&)[8]>(xp[0]));
-        cp.add8(reinterpret_cast<const uint32_t(&)[8]>(xp[8]));
-        if (TERNARY) {
-            cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[0]));
-            cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[8]));
+#pragma unroll
+        for (int h = 0; h < ROUND; h += 8) {
+            cp.add8(reinterpret_cast<const uint32_t(&)[8]>(xp[h]));
+            if (TERNARY) cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[h]));
         }
     }
 }
@@ -147,8 +148,8 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
     __syncthreads();
 }
 
-template <bool WRITE_COUNTS, bool MERGE>
-__global__ void __launch_bounds__(kRThreads, 2) count_reduce_kernel(const ReduceParams p) {
+template <bool WRITE_COUNTS, bool MERGE, int ROUND>
+__global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : 2) count_reduce_kernel(const ReduceParams p) {
     __shared__ float4 s_dtab[256];          // byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
     {
         const int i = threadIdx.x;          // kRThreads == 256
@@ -207,9 +208,9 @@ __global__ void __launch_bounds__(kRThreads, 2) count_reduce_kernel(const Reduce
                     if (p.ternary) sliced_add(cnv, xn);
                 }
             } else if (p.ternary) {
-                count_words2<true>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
+                count_words2<true, ROUND>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
             } else {
-                count_words2<false>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
+                count_words2<false, ROUND>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
             }
             if (p.ternary) {
                 // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
@@ -401,8 +402,8 @@ partial_count_kernel(const uint32_t *__restrict__ P, const uint32_t *__restrict_
                      int64_t count_stride) {
     for (int64_t k = (int64_t)blockIdx.x * kRThreads + threadIdx.x; k < Wd; k += (int64_t)gridDim.x * kRThreads) {
         SlicedCounter cp, cn;
-        if (ternary) count_words2<true>(P + k, N + k, plane_stride, Wg, cp, cn);
-        else count_words2<false>(P + k, N, plane_stride, Wg, cp, cn);
+        if (ternary) count_words2<true, 16>(P + k, N + k, plane_stride, Wg, cp, cn);
+        else count_words2<false, 16>(P + k, N, plane_stride, Wg, cp, cn);
 #pragma unroll
         for (int b = 0; b < 8; ++b) {
             if (b >= B) break;
@@ -423,12 +424,16 @@ cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s
     const int64_t chunks = (max_words + kRThreads - 1) / kRThreads;
     const int grid = grid_for(chunks, 8);
     const bool counts = p.cpos || p.cneg;
+    const bool small = !p.cnt_pos && p.W <= 16;              // shallow rounds, 4 CTAs per SM
     if (p.cnt_pos) {
-        if (counts) count_reduce_kernel<true, true><<<grid, kRThreads, 0, s>>>(p);
-        else count_reduce_kernel<false, true><<<grid, kRThreads, 0, s>>>(p);
+        if (counts) count_reduce_kernel<true, true, 16><<<grid, kRThreads, 0, s>>>(p);
+        else count_reduce_kernel<false, true, 16><<<grid, kRThreads, 0, s>>>(p);
+    } else if (small) {
+        if (counts) count_reduce_kernel<true, false, 8><<<grid, kRThreads, 0, s>>>(p);
+        else count_reduce_kernel<false, false, 8><<<grid, kRThreads, 0, s>>>(p);
     } else {
-        if (counts) count_reduce_kernel<true, false><<<grid, kRThreads, 0, s>>>(p);
-        else count_reduce_kernel<false, false><<<grid, kRThreads, 0, s>>>(p);
+        if (counts) count_reduce_kernel<true, false, 16><<<grid, kRThreads, 0, s>>>(p);
+        else count_reduce_kernel<false, false, 16><<<grid, kRThreads, 0, s>>>(p);
     }
     return cudaGetLastError();
 }
