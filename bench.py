@@ -287,7 +287,7 @@ def run_nf(args):
                 "input_elements_per_s": round(world * n_total * W / (ms_per_step * 1e-3), 1),
                 "pct_hbm_peak_measured": round(100 * all_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 2),
                 "pct_hbm_peak_nominal_8TBs": round(100 * all_bytes / (ms_per_step * 1e-3) / 1e9 / HBM_NOMINAL_GBS, 2),
-                "gpu_launches": args.steps * nb * 2,
+                "gpu_launches": args.steps * sum(1 if len(b.tensors) <= 256 else 2 for b in cfg.buckets),
                 "roofline": roofline, "clocks": clocks, "e2e": e2e, "cpu_baseline": cpu,
                 "setup_s": round(gen_s, 1)}
         print(json.dumps(line))

@@ -166,8 +166,8 @@ int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
 /*
  * Fused path (the one the target is measured on) — same results as
  * nf_route_bucket -> nf_sign_pack -> nf_sign_count_reduce -> nf_fp32_reduce -> nf_health_stats(g),
- * with the W x n gradients read ONCE. Two launches: the route kernel, then one persistent kernel that
- * packs, counts, votes, sums the FP32 tensors, gathers abs-sums and health statistics from a single read
+ * with the W x n gradients read ONCE. One launch for buckets of up to 256 tensors (the persistent kernel
+ * routes the bucket itself; larger T: the route kernel first): it packs, counts, votes, sums the FP32 tensors, gathers abs-sums and health statistics from a single read
  * (pass A) and, tensor by tensor as each completes, expands the 2-bit directions by the per-tensor scale
  * (pass B). P and N may both be NULL (planes not materialised);
  * sumsq/nan_cnt/inf_cnt may all be NULL (no health statistics); scale_out may be NULL.

@@ -221,12 +221,18 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     static const bool sep_decode = getenv("NF_DECODE_SEPARATE") != nullptr;   // A/B aid: pass B as its own kernel
     cudaStream_t s = (cudaStream_t)stream;
     prof_mark(0, s);
-    // a1 (+ zeroing of the accumulators, so no memset nodes sit on the stream)
-    cudaError_t e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
-                                 abs_sum, sumsq, (unsigned long long *)nan_cnt,
-                                 (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, use_pdl ? 1 : 0, s);
-    if (e != cudaSuccess) return NF_ERR_CUDA;
-    if (T == 0 || n == 0) return NF_OK;
+    // a1: inside the fused kernel for buckets of up to kMetaCap tensors (one launch per bucket), else
+    // (or with NF_ROUTE_KERNEL set, an A/B aid) by the route kernel, which also zeroes the accumulators
+    static const bool route_kernel_forced = getenv("NF_ROUTE_KERNEL") != nullptr;
+    const bool inkernel = T > 0 && n > 0 && T <= kMetaCap && !use_ldg && !sep_decode && !route_kernel_forced;
+    cudaError_t e = cudaSuccess;
+    if (!inkernel) {
+        e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
+                         abs_sum, sumsq, (unsigned long long *)nan_cnt,
+                         (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, use_pdl ? 1 : 0, s);
+        if (e != cudaSuccess) return NF_ERR_CUDA;
+        if (T == 0 || n == 0) return NF_OK;
+    }
     prof_mark(1, s);
     // pass A: one read of the W x n gradients
     StreamParams p{};
@@ -241,6 +247,8 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.trace = g_trace;
     p.separate_decode = sep_decode ? 1 : 0;
     p.pdl = use_pdl ? 1 : 0;
+    p.inkernel_route = inkernel ? 1 : 0;
+    p.elig = elig; p.st = state; p.n = n; p.route_w = route; p.woff_w = woff; p.summary = summary;
     // One persistent TMA-ring kernel (nf_fused.cu) does pass A and pass B. NF_PASSA_LDG / NF_DECODE_SEPARATE
     // select the register-staged streaming kernel / the stand-alone decode kernel for A/B measurements.
     const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);

@@ -20,6 +20,7 @@
 //  * ragged last tiles and tensors whose rows are not 16-byte aligned go through the same ring;
 //  * each CTA publishes its finished tiles per tensor (release); decode warps, and the consumers once
 //    the tiles are exhausted, acquire the per-tensor counter and expand the 2-bit directions.
+#include <cooperative_groups.h>
 #include <float.h>
 #include "nf_internal.cuh"
 
@@ -151,7 +152,6 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [17408, ...)    ring [stages][8][kPitch] floats
 //   after the ring  per-warp FP64 totals {abs, sq} per worker, [kCW][2*W] doubles
 // ---------------------------------------------------------------------------------------------
-constexpr int kMetaCap = 256;                    // tensors whose metadata is cached in shared memory
 constexpr int kSmemMeta = 8192;
 constexpr int kSmemHdr = kSmemMeta + 9216;       // 4*(cap+1) + 3*8*cap + 4*cap = 8196 bytes, padded
 struct FusedSmem {
@@ -602,21 +602,135 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // and the zeroed accumulators are visible after this point
     pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
-    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    const int n_tiles = pv.hdr->n_tiles;
-    if (p.T <= kMetaCap) {
-        // per-tensor metadata -> shared memory (one round trip for the whole CTA)
-        for (int t = tid; t <= p.T; t += kFThreads) {
-            sm.m_tile[t] = __ldg(pv.tile_prefix + t);
-            if (t < p.T) {
-                const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
-                sm.m_off[t] = __ldg(p.off + t);
-                sm.m_len[t] = __ldg(p.len + t);
-                sm.m_woff[t] = isL ? __ldg(p.woff + t) : -1;
-                sm.m_tau[t] = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
+    int n_tiles;
+    if (p.inkernel_route) {
+        // ---- step a1 inside this kernel (T <= kMetaCap) --------
+        // Every CTA derives the routing of the bucket into its shared-memory metadata (redundant O(T)
+        // work, no dependence on another kernel); CTA 0 also writes the a1 outputs and the plan; all
+        // CTAs zero a slice of the accumulators; one grid-wide barrier (cooperative launch) orders the
+        // zeroing before anybody's atomics.
+        const int T = p.T;
+        long long l = 0, o = 0, v_tiles = 0, v_words = 0, v_nl = 0;
+        int r = NF_ROUTE_P;
+        int bad = 0;
+        if (tid < T) {
+            o = __ldg(p.off + tid);
+            l = __ldg(p.len + tid);
+            const long long prev_end = tid == 0 ? 0 : __ldg(p.off + tid - 1) + __ldg(p.len + tid - 1);
+            if (l < 0 || o < prev_end || o + l > p.n) bad = 1;
+            if (l < 0) l = 0;
+            if (!p.st.admitted) r = NF_ROUTE_P;
+            else if (__ldg(p.elig + tid) == 0) r = NF_ROUTE_P;
+            else if (p.st.veto || !p.st.capacity_ok) r = NF_ROUTE_F;
+            else r = NF_ROUTE_L;
+            v_tiles = (l + kTile - 1) / kTile;
+            if (r == NF_ROUTE_L) { v_words = (l + 31) / 32; v_nl = 1; }
+        }
+        // exclusive scan of (tiles, words, nl) over the first kMetaCap threads (8 warps)
+        long long i_tiles = v_tiles, i_words = v_words, i_nl = v_nl;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const long long a = __shfl_up_sync(0xffffffffu, i_tiles, d), b = __shfl_up_sync(0xffffffffu, i_words, d),
+                            c = __shfl_up_sync(0xffffffffu, i_nl, d);
+            if (lane >= d) { i_tiles += a; i_words += b; i_nl += c; }
+        }
+        long long *s_scan = reinterpret_cast<long long *>(smem_raw + 128);        // [3][8] warp totals, [24..27] tallies
+        if (tid < 32) s_scan[tid] = 0;
+        __syncthreads();
+        if (warp < kMetaCap / 32 && lane == 31) { s_scan[warp] = i_tiles; s_scan[8 + warp] = i_words; s_scan[16 + warp] = i_nl; }
+        if (tid < T) {
+            unsigned long long *tal = reinterpret_cast<unsigned long long *>(s_scan + 24);
+            if (r == NF_ROUTE_F) atomicAdd(tal + 0, 1ull);
+            else if (r == NF_ROUTE_P) atomicAdd(tal + 1, 1ull);
+            else atomicAdd(tal + 2, (unsigned long long)l);
+            atomicAdd(tal + 3, (unsigned long long)l);
+        }
+        const int any_bad = __syncthreads_or(bad);
+        long long b_tiles = 0, b_words = 0, b_nl = 0, t_tiles = 0, t_words = 0, t_nl = 0;
+#pragma unroll
+        for (int k = 0; k < kMetaCap / 32; ++k) {
+            if (k < warp) { b_tiles += s_scan[k]; b_words += s_scan[8 + k]; b_nl += s_scan[16 + k]; }
+            t_tiles += s_scan[k]; t_words += s_scan[8 + k]; t_nl += s_scan[16 + k];
+        }
+        const long long ex_tiles = b_tiles + i_tiles - v_tiles, ex_words = b_words + i_words - v_words,
+                        ex_nl = b_nl + i_nl - v_nl;
+        const int status = (any_bad || t_tiles > 0x7fffffffLL) ? NF_ERR_ARG : NF_OK;
+        if (tid < T) {
+            sm.m_tile[tid] = (int32_t)ex_tiles;
+            sm.m_off[tid] = o;
+            sm.m_len[tid] = l;
+            sm.m_woff[tid] = r == NF_ROUTE_L ? ex_words : -1;
+            sm.m_tau[tid] = (p.tau && r == NF_ROUTE_L) ? __ldg(p.tau + tid) : 0.f;
+        }
+        if (tid == 0) sm.m_tile[T] = (int32_t)t_tiles;
+        PlanLayout PL = plan_layout(T);
+        char *pb = (char *)p.plan;
+        if (blockIdx.x == 0) {
+            int32_t *tile_prefix = (int32_t *)(pb + PL.tile_prefix);
+            int32_t *lt_index = (int32_t *)(pb + PL.lt_index);
+            int64_t *lt_woff = (int64_t *)(pb + PL.lt_woff);
+            if (tid < T) {
+                p.route_w[tid] = (uint8_t)r;
+                p.woff_w[tid] = r == NF_ROUTE_L ? ex_words : -1;
+                tile_prefix[tid] = (int32_t)ex_tiles;
+                if (r == NF_ROUTE_L) { lt_index[ex_nl] = tid; lt_woff[ex_nl] = ex_words; }
+            }
+            if (tid == 0) {
+                const unsigned long long *tal = reinterpret_cast<const unsigned long long *>(s_scan + 24);
+                PlanHeader *hdr = (PlanHeader *)pb;
+                tile_prefix[T] = (int32_t)t_tiles;
+                lt_woff[t_nl] = t_words;
+                hdr->magic = kPlanMagic;
+                hdr->status = status;
+                hdr->T = T;
+                hdr->nL = (int32_t)t_nl;
+                hdr->n = p.n;
+                hdr->Wd = t_words;
+                hdr->n_tiles = status == NF_OK ? (int32_t)t_tiles : 0;
+                hdr->pad0 = 0;
+                hdr->tile_cursor = 0;
+                hdr->unit_cursor = 0;
+                p.summary[NF_SUM_WD] = t_words;
+                p.summary[NF_SUM_NL] = t_nl;
+                p.summary[NF_SUM_NF] = (int64_t)tal[0];
+                p.summary[NF_SUM_NP] = (int64_t)tal[1];
+                p.summary[NF_SUM_E] = (int64_t)tal[2];
+                p.summary[NF_SUM_F] = (int64_t)(tal[3] - tal[2]);
+                p.summary[NF_SUM_TILES] = t_tiles;
+                p.summary[NF_SUM_STATUS] = status;
             }
         }
-        __syncthreads();
+        // zero the accumulating outputs and the per-tensor completion counters, one slice per CTA
+        {
+            int32_t *done = (int32_t *)(pb + PL.done);
+            const int64_t zc = (int64_t)W * T;
+            for (int64_t i = (int64_t)blockIdx.x * kFThreads + tid; i < zc; i += (int64_t)gridDim.x * kFThreads) {
+                p.abs_sum[i] = 0.0;
+                if (HEALTH) { p.sumsq[i] = 0.0; p.nan_cnt[i] = 0ull; p.inf_cnt[i] = 0ull; }
+                if (i < T) done[i] = 0;
+            }
+        }
+        __threadfence();
+        cooperative_groups::this_grid().sync();
+        if (status != NF_OK) return;
+        n_tiles = (int)t_tiles;
+    } else {
+        if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+        n_tiles = pv.hdr->n_tiles;
+        if (p.T <= kMetaCap) {
+            // per-tensor metadata -> shared memory (one round trip for the whole CTA)
+            for (int t = tid; t <= p.T; t += kFThreads) {
+                sm.m_tile[t] = __ldg(pv.tile_prefix + t);
+                if (t < p.T) {
+                    const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
+                    sm.m_off[t] = __ldg(p.off + t);
+                    sm.m_len[t] = __ldg(p.len + t);
+                    sm.m_woff[t] = isL ? __ldg(p.woff + t) : -1;
+                    sm.m_tau[t] = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
+                }
+            }
+            __syncthreads();
+        }
     }
 
     // =========================================================================================
@@ -683,8 +797,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // =========================================================================================
     if (warp == kCW + 1) {
         for (int t = blockIdx.x * 32 + lane; t < p.T; t += (int)gridDim.x * 32) {
-            const int64_t off_t = __ldg(p.off + t), len_t = __ldg(p.len + t);
-            const bool isL = __ldg(p.route + t) == NF_ROUTE_L;
+            int64_t len_t;
+            bool isL;
+            if (p.T <= kMetaCap) { len_t = sm.m_len[t]; isL = sm.m_woff[t] >= 0; }
+            else { len_t = __ldg(p.len + t); isL = __ldg(p.route + t) == NF_ROUTE_L; }
             if (isL && len_t > 0) continue;                       // published by the decode
             const float S = isL ? tensor_scale(p.abs_sum, W, p.T, t, len_t) : 0.f;
             pv.scale[t] = S;
@@ -883,7 +999,8 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
     if (work <= 0) return cudaSuccess;
     int64_t grid = device_sm_count();                        // persistent: one CTA per SM
     if (grid > work) grid = work;
-    cudaError_t e = launch_kernel(fused_passA_kernel<HEALTH, MULTI>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0, p, stages);
+    cudaError_t e = launch_kernel_ex(fused_passA_kernel<HEALTH, MULTI>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0,
+                                     p.inkernel_route != 0, p, stages);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

@@ -20,6 +20,7 @@ constexpr int kRowElems = kThreads * 4;    // 1024 elements per row
 constexpr int kTile = kRows * kRowElems;   // 2048 elements per tile
 constexpr int kGroup = 8;                  // workers per register group (8 x 4-bit nibbles = 32 bits)
 constexpr uint32_t kPlanMagic = 0x4e46504cu;  // "NFPL"
+constexpr int kMetaCap = 256;              // fused kernel: tensors whose metadata lives in shared memory
 
 struct PlanHeader {                        // 64 bytes, at plan + 0
     uint32_t magic;
@@ -111,6 +112,14 @@ struct StreamParams {
     int separate_decode;       // A/B aid: 1 = no decode inside nf_fused.cu (decode_kernel does everything)
     unsigned long long *trace; // debug: per-CTA globaltimer stamps [grid][8], or NULL
     int pdl;                   // launch with programmatic stream serialization (fused path)
+    // in-kernel routing (fused path, T <= kMetaCap): step a1 is computed by the fused kernel itself
+    int inkernel_route;
+    const uint8_t *elig;       // [T]
+    nf_state st;
+    int64_t n;
+    uint8_t *route_w;          // [T] out
+    int64_t *woff_w;           // [T] out
+    int64_t *summary;          // [NF_SUM_LEN] out
 };
 
 enum : int {
@@ -172,19 +181,33 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 template <typename... KArgs, typename... Args>
-inline cudaError_t launch_kernel(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s,
-                                 bool pdl, Args... args) {
+inline cudaError_t launch_kernel_ex(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s,
+                                    bool pdl, bool cooperative, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid, 1, 1);
     cfg.blockDim = dim3(block, 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if (pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (cooperative) {                       // grid-wide barrier inside the kernel: all CTAs co-resident
+        attr[na].id = cudaLaunchAttributeCooperative;
+        attr[na].val.cooperative = 1;
+        ++na;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1 : 0;
+    cfg.numAttrs = na;
     return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s,
+                                 bool pdl, Args... args) {
+    return launch_kernel_ex(kernel, grid, block, smem, s, pdl, false, args...);
 }
 #endif
 
