@@ -150,3 +150,19 @@ def test_count_reduce_without_count_outputs(name, mode):
         bb.fp32_reduce(g, g.shape[1])
         bb.health_stats(g, g.shape[1])
         compare(bb, ref, cfg.W, mode, check_counts=False, what=f"{cfg.name} bucket {b.index} 5-call, no counts")
+
+
+@pytest.mark.parametrize("T", [256, 257, 700])
+def test_many_tensor_buckets(T):
+    """Buckets around and above the fused kernel's shared-memory metadata capacity (256 tensors): T <= 256 routes
+    inside the fused kernel, larger T goes through the route kernel and global-memory lookups."""
+    rng = np.random.default_rng(T)
+    lens = [int(x) for x in rng.integers(1, 3000, T)]
+    lens[5] = 2048 * 3            # a few multi-tile tensors
+    lens[T // 2] = 2048 * 2 + 17
+    off, ln, n = layout(lens)
+    elig = [int(x) for x in rng.integers(0, 2, T)]
+    W = 5
+    g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
+    g[rng.random((W, n)) < 0.05] = 0.0
+    run_both(_dev(g), off, ln, elig, what=f"T={T}")
