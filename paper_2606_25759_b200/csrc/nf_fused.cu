@@ -285,7 +285,7 @@ __device__ __forceinline__ unsigned warp_sum(unsigned v) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// fast path: a full tile of a 16-byte-aligned tensor, one worker group (W <= 8), data in the ring
+// full tiles of a 16-byte-aligned tensor, one worker group of up to 8 workers, data in the ring
 // ---------------------------------------------------------------------------------------------
 // L tile: sign indicators of this thread's 4 elements of every worker (nibble w of posR / negR) and
 // the FP32 abs / square partials. KIND 1 = G-Binary, 2 = G-Ternary.
@@ -448,6 +448,8 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
     __syncwarp();
 }
 
+// debug aid (nf_debug_trace): globaltimer stamps per CTA: 0 consumers start, 1 tiles exhausted, 2 last flush,
+// 3 consumers' decode done, 4 decode warp done
 __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
     if (p.trace) {
         unsigned long long t;
@@ -474,9 +476,6 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
     int64_t off_t = 0, len_t = 0, woff_t = 0;
     bool dec = false;
     float S_t = 0.f;
-    const bool trace_me = p.trace && threadIdx.x == 0;
-    bool first_wait = true;
-    unsigned long long nunits = 0;
     for (;;) {
         int u0 = 0;
         if (lane == 0) u0 = atomicAdd(cursor, kDU);
@@ -508,11 +507,9 @@ TensorCur tc;
                         if (spins > (1u << 23)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
                     }
                     S_t = tensor_scale(p.abs_sum, W, p.T, t_cur, len_t);
-                    if (trace_me) { trace_stamp(p, first_wait ? 5 : 7); first_wait = false; }
                 }
             }
             if (!dec) continue;
-            ++nunits;
             if (tile == tile_b && (u & 1) == 0 && lane == 0) {
                 pv.scale[t_cur] = S_t;
                 if (p.scale_out) p.scale_out[t_cur] = S_t;
@@ -558,7 +555,6 @@ TensorCur tc;
             }
         }
     }
-    if (trace_me) p.trace[(size_t)blockIdx.x * 8 + 6] = nunits;
 }
 
 // the same vote from byte-packed running counts (W > 8: several worker groups per tile)
@@ -734,7 +730,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
 
     // =========================================================================================
-    // producer: one elected lane issues the bulk copies of every fast tile
+    // producer: one elected lane issues the bulk copies of every (tile, worker group)
     // =========================================================================================
     if (warp == kCW) {
         if (lane != 0) return;
