@@ -37,6 +37,9 @@ constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = o
 #ifndef NF_KKT
 #define NF_KKT 4
 #endif
+#ifndef NF_KCHUNK
+#define NF_KCHUNK 4                      // longest run of consecutive tiles one CTA takes at a time
+#endif
 constexpr int kDW = NF_KDW;                      // decode warps (pass B inside the kernel)
 constexpr int kFThreads = kCThreads + 64 + kDW * 32;   // + producer warp + housekeeping warp + decode warps
 constexpr int kDU = NF_KDU;                      // decode: units in flight per warp
@@ -742,9 +745,19 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // Dynamic tile scheduling: tiles are handed out by a device-wide cursor, so a CTA that runs
         // ahead (SM position, co-running decode warps) simply takes more. Every tile of an aligned
         // tensor enters the ring; the stage carries its tile index to the consumers.
+        // Tiles are taken in runs of consecutive tiles (guided self-scheduling: up to NF_KCHUNK early, single
+        // tiles near the end), so that a CTA stays inside one tensor for a while — a tensor change costs a
+        // CTA-wide flush — without giving up the balance at the tail.
         int32_t *cursor = const_cast<int32_t *>(&pv.hdr->tile_cursor);
+        int next = 0, run_end = 0;
         for (;;) {
-            const int tile = atomicAdd(cursor, 1);
+            if (next >= run_end) {
+                int want = (n_tiles - run_end) / (4 * (int)gridDim.x);     // run_end: last position seen
+                want = want < 1 ? 1 : (want > NF_KCHUNK ? NF_KCHUNK : want);
+                next = atomicAdd(cursor, want);
+                run_end = next + want;
+            }
+            const int tile = next++;
             if (tile >= n_tiles) {
                 mbar_wait(sm.empty + st, ph ^ 1u);
                 sm.tile_of[st] = -1;                               // sentinel: the consumers stop
