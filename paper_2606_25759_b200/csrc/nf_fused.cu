@@ -451,8 +451,9 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
     __syncwarp();
 }
 
-// debug aid (nf_debug_trace): globaltimer stamps per CTA: 0 consumers start, 1 tiles exhausted, 2 last flush,
-// 3 consumers' decode done, 4 decode warp done
+// debug aid (nf_debug_trace): globaltimer stamps per CTA: 5 kernel entry, 6 after griddepcontrol.wait, 7 after the
+// grid barrier of the in-kernel routing, 0 consumers start, 1 tiles exhausted, 2 last flush, 3 consumers' decode
+// done, 4 decode warp done
 __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
     if (p.trace) {
         unsigned long long t;
@@ -586,6 +587,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     const int W = p.W;                          // MULTI: W > 8, several worker groups of 8 per tile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     pdl_launch_dependents();
+    if (tid == 0) trace_stamp(p, 5);
 
     if (tid == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(sm.full + s, 1); mbar_init(sm.empty + s, kCW); }
@@ -600,6 +602,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // everything above touched shared memory only and overlapped the route kernel (PDL); the plan
     // and the zeroed accumulators are visible after this point
     pdl_wait();
+    if (tid == 0) trace_stamp(p, 6);
     const PlanView pv = plan_view(p.plan, p.T);
     int n_tiles;
     if (p.inkernel_route) {
@@ -711,6 +714,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
         __threadfence();
         cooperative_groups::this_grid().sync();
+        if (tid == 0) trace_stamp(p, 7);
         if (status != NF_OK) return;
         n_tiles = (int)t_tiles;
     } else {
