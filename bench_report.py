@@ -38,7 +38,9 @@ def measured_peak():
         return 6650.0
 
 
-def time_fn(fn, iters, warmup=3):
+def time_fn(fn, iters, warmup=3, reps=1):
+    """Median over `iters` samples of the time of `reps` back-to-back calls, per call (ms). reps > 1 keeps the
+    launch latency of a short call from being counted as its duration."""
     import torch
     for _ in range(warmup):
         fn()
@@ -47,10 +49,11 @@ def time_fn(fn, iters, warmup=3):
     for _ in range(iters):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        fn()
+        for _ in range(reps):
+            fn()
         e1.record()
         e1.synchronize()
-        ts.append(e0.elapsed_time(e1))
+        ts.append(e0.elapsed_time(e1) / reps)
     return statistics.median(ts)
 
 
@@ -216,6 +219,39 @@ def table_hier(args, dev, peak):
     return "\n".join(out)
 
 
+def table_five_calls(args, dev, peak):
+    """The five stand-alone calls of include/nf.h and the fused call on one GPT-2-1.3B-shaped bucket (bucket 0:
+    33,568,768 elements, W = 8, all low-bit) and on its 401 MB FP32-route bucket: time and % of the measured HBM
+    peak on each call's own algorithmic bytes; 8 back-to-back calls per sample."""
+    import torch
+    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from workloads import shapes, gen
+    cfg = shapes.gpt2_1p3b()
+    out = ["| bucket | call | time | own algorithmic bytes | % of measured HBM peak |", "|---|---|---|---|---|"]
+    for bi in (0, 36):
+        b = cfg.buckets[bi]
+        W, n, e = cfg.W, b.n, b.n_eligible
+        f = n - e
+        g = gen.gen_bucket(cfg, b, dev)
+        bb = BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=True)
+        bb.aggregate(g, g.shape[1])
+        torch.cuda.synchronize()
+        planes = 2 * W * e // 8
+        calls = [("nf_route_bucket (a1)", lambda: bb.route_bucket((1, 0, 1)), 0),
+                 ("nf_sign_pack (a2)", lambda: bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY), 4 * W * e + planes),
+                 ("nf_sign_count_reduce (a3)", lambda: bb.sign_count_reduce(nf.MODE_GTERNARY), planes + 4 * e),
+                 ("nf_fp32_reduce (a4a)", lambda: bb.fp32_reduce(g, g.shape[1]), 4 * W * f + 4 * f),
+                 ("nf_health_stats (a4b)", lambda: bb.health_stats(g, g.shape[1]), 4 * W * n),
+                 ("nf_aggregate_bucket (fused)", lambda: bb.aggregate(g, g.shape[1]), 4 * W * n + planes + e // 2 + 4 * n)]
+        for name, fn, own in calls:
+            t = time_fn(fn, args.iters, reps=8) * 1e-3
+            pct = f"{100 * own / t / 1e9 / peak:.0f}" if own > 1e6 else "- (O(T) latency)"
+            out.append(f"| {bi} (n = {n:,}, {100 * e / n:.0f} % low-bit) | {name} | {t * 1e6:.1f} us | {own / 1e6:.1f} MB | {pct} |")
+        del g, bb
+        torch.cuda.empty_cache()
+    return "\n".join(out)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default="")
@@ -233,6 +269,8 @@ def main():
              f"median of {args.iters} CUDA-event-timed iterations after 3 warm-ups; mode G-Ternary, planes and health on.", ""]
     if not args.skip_configs:
         parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
+    parts += ["### The five stand-alone calls and the fused call on GPT buckets 0 (all low-bit) and 36 (all FP32 route)", "",
+              table_five_calls(args, dev, peak), ""]
     parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
     parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
               "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange)", "",
