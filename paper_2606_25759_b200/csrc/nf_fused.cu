@@ -37,6 +37,9 @@ constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = o
 #ifndef NF_KKT
 #define NF_KKT 4
 #endif
+#ifndef NF_KGRAB
+#define NF_KGRAB 4                       // decode units a consumer warp takes per trip to the cursor at the end
+#endif
 #ifndef NF_KCHUNK
 #define NF_KCHUNK 4                      // longest run of consecutive tiles one CTA takes at a time
 #endif
@@ -471,7 +474,7 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
 // join when their own tiles are done. Every store instruction writes 512 contiguous bytes.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
-                                             int n_tiles, int lane) {
+                                             int n_tiles, int lane, int grab) {
     const float4 *dtab = sm.dtab;
     const int W = p.W;
     const int total_units = n_tiles * 2;
@@ -480,10 +483,19 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
     int64_t off_t = 0, len_t = 0, woff_t = 0;
     bool dec = false;
     float S_t = 0.f;
+    // `grab` units per trip to the device-wide cursor, processed kDU at a time: the dedicated decode warps
+    // take few (they run beside the consumers for the whole kernel), the consumers that join at the end take
+    // more, so that a few thousand warps arriving together do not serialise on one atomic.
+    int u_next = 0, u_end = 0;
     for (;;) {
-        int u0 = 0;
-        if (lane == 0) u0 = atomicAdd(cursor, kDU);
-        u0 = __shfl_sync(0xffffffffu, u0, 0);
+        if (u_next >= u_end) {
+            int ub = 0;
+            if (lane == 0) ub = atomicAdd(cursor, grab);
+            u_next = __shfl_sync(0xffffffffu, ub, 0);
+            u_end = u_next + grab;
+        }
+        const int u0 = u_next;
+        u_next += kDU;
         if (u0 >= total_units) break;
         uint32_t dv[kDU][2];
         int64_t obase[kDU], rem[kDU];
@@ -827,7 +839,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // their own tiles are done.
     // =========================================================================================
     if (warp >= kCW + 2) {
-        if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane);
+        if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane, kDU);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
         return;
     }
@@ -988,7 +1000,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     if (ctid == 0) trace_stamp(p, 1);
     if (touched) flush_tensor();
     if (ctid == 0) trace_stamp(p, 2);
-    if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane);     // help finish pass B
+    if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane, NF_KGRAB);     // help finish pass B
     if (ctid == 0) trace_stamp(p, 3);
 }
 
