@@ -38,7 +38,7 @@ constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = o
 #define NF_KKT 4
 #endif
 #ifndef NF_KGRAB
-#define NF_KGRAB 4                       // decode units a consumer warp takes per trip to the cursor at the end
+#define NF_KGRAB 2                       // decode units a consumer warp takes per trip to the cursor at the end
 #endif
 #ifndef NF_KCHUNK
 #define NF_KCHUNK 4                      // longest run of consecutive tiles one CTA takes at a time
