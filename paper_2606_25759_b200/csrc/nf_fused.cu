@@ -22,6 +22,7 @@
 //    the tiles are exhausted, acquire the per-tensor counter and expand the 2-bit directions.
 #include <cooperative_groups.h>
 #include <float.h>
+#include <utility>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -624,6 +625,28 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // CTAs zero a slice of the accumulators; one grid-wide barrier (cooperative launch) orders the
         // zeroing before anybody's atomics.
         const int T = p.T;
+        PlanLayout PL = plan_layout(T);
+        char *pb = (char *)p.plan;
+        // zero a slice of the accumulating outputs and of the per-tensor completion counters (CTA 0: the two
+        // cursors as well), then ARRIVE at the grid barrier; the routing below needs none of it and runs while
+        // the other CTAs arrive
+        {
+            int32_t *done = (int32_t *)(pb + PL.done);
+            const int64_t zc = (int64_t)W * T;
+            for (int64_t i = (int64_t)blockIdx.x * kFThreads + tid; i < zc; i += (int64_t)gridDim.x * kFThreads) {
+                p.abs_sum[i] = 0.0;
+                if (HEALTH) { p.sumsq[i] = 0.0; p.nan_cnt[i] = 0ull; p.inf_cnt[i] = 0ull; }
+                if (i < T) done[i] = 0;
+            }
+            if (blockIdx.x == 0 && tid == 0) {
+                PlanHeader *hdr = (PlanHeader *)pb;
+                hdr->tile_cursor = 0;
+                hdr->unit_cursor = 0;
+            }
+        }
+        __threadfence();
+        cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+        auto zeroed = grid.barrier_arrive();
         long long l = 0, o = 0, v_tiles = 0, v_words = 0, v_nl = 0;
         int r = NF_ROUTE_P;
         int bad = 0;
@@ -677,8 +700,6 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             sm.m_tau[tid] = (p.tau && r == NF_ROUTE_L) ? __ldg(p.tau + tid) : 0.f;
         }
         if (tid == 0) sm.m_tile[T] = (int32_t)t_tiles;
-        PlanLayout PL = plan_layout(T);
-        char *pb = (char *)p.plan;
         if (blockIdx.x == 0) {
             int32_t *tile_prefix = (int32_t *)(pb + PL.tile_prefix);
             int32_t *lt_index = (int32_t *)(pb + PL.lt_index);
@@ -701,9 +722,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 hdr->n = p.n;
                 hdr->Wd = t_words;
                 hdr->n_tiles = status == NF_OK ? (int32_t)t_tiles : 0;
-                hdr->pad0 = 0;
-                hdr->tile_cursor = 0;
-                hdr->unit_cursor = 0;
+                hdr->pad0 = 0;                           // (the cursors were zeroed before the barrier)
                 p.summary[NF_SUM_WD] = t_words;
                 p.summary[NF_SUM_NL] = t_nl;
                 p.summary[NF_SUM_NF] = (int64_t)tal[0];
@@ -714,18 +733,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 p.summary[NF_SUM_STATUS] = status;
             }
         }
-        // zero the accumulating outputs and the per-tensor completion counters, one slice per CTA
-        {
-            int32_t *done = (int32_t *)(pb + PL.done);
-            const int64_t zc = (int64_t)W * T;
-            for (int64_t i = (int64_t)blockIdx.x * kFThreads + tid; i < zc; i += (int64_t)gridDim.x * kFThreads) {
-                p.abs_sum[i] = 0.0;
-                if (HEALTH) { p.sumsq[i] = 0.0; p.nan_cnt[i] = 0ull; p.inf_cnt[i] = 0ull; }
-                if (i < T) done[i] = 0;
-            }
-        }
-        __threadfence();
-        cooperative_groups::this_grid().sync();
+        grid.barrier_wait(std::move(zeroed));               // everybody's slice is zero, the cursors too
         if (tid == 0) trace_stamp(p, 7);
         if (status != NF_OK) return;
         n_tiles = (int)t_tiles;
