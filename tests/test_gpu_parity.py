@@ -166,3 +166,25 @@ def test_many_tensor_buckets(T):
     g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
     g[rng.random((W, n)) < 0.05] = 0.0
     run_both(_dev(g), off, ln, elig, what=f"T={T}")
+
+
+def test_host_buffer_entry_point_matches_oracle():
+    """nf_aggregate_bucket_host (the call bench.py's e2e leg times): pinned host gradients in, aggregated bucket
+    back in pinned host memory, same values as the oracle."""
+    cfg = shapes.tiny()
+    b = cfg.buckets[0]
+    g_dev_src = gen.gen_bucket(cfg, b, DEV)
+    stride = g_dev_src.shape[1]
+    g_host = torch.empty((cfg.W, stride), dtype=torch.float32, pin_memory=True)
+    g_host.copy_(g_dev_src)
+    ref = O.aggregate_bucket(np.ascontiguousarray(g_host.numpy()[:, :b.n]), b.off, b.length, b.elig)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=False, health=True)
+    staging = torch.zeros((cfg.W, stride), dtype=torch.float32, device=DEV)
+    out_host = torch.full((b.n,), -3.0, dtype=torch.float32).pin_memory()
+    nf.nf_aggregate_bucket_host(g_host, staging, stride, cfg.W, b.n, bb.off, bb.len, bb.elig, bb.T, (1, 0, 1),
+                                nf.MODE_GTERNARY, None, 0, 1.0, bb.route, bb.woff, bb.summary, bb.abs_sum, bb.sumsq,
+                                bb.nan_cnt, bb.inf_cnt, bb.out, out_host, bb.plan, bb.workspace)
+    torch.cuda.synchronize()
+    compare(bb, ref, cfg.W, O.MODE_GTERNARY, check_planes=False, check_scale=False,      # the host call has no scale_out
+            what="host entry point")
+    assert np.array_equal(out_host.numpy(), _np(bb.out)[:b.n])
