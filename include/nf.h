@@ -257,6 +257,11 @@ int nf_supervisor_step(nf_supervisor *s /*host*/, double signal, uint64_t nan_co
  */
 int nf_prof_enable(int max_records);
 int nf_prof_collect(float *ms /*host*/, int max_records);
+/* Debug aid: nf_debug_trace(1, NULL) allocates a device buffer of 256 x 8 globaltimer stamps that every CTA of
+ * the fused kernel fills from then on (kernel entry, after the dependency wait, after the routing barrier,
+ * consumers start, tiles exhausted, last flush, decode done); with `out` != NULL (room for 2048 uint64, HOST) the
+ * stamps are copied out (synchronises the device); nf_debug_trace(0, ...) frees the buffer. */
+int nf_debug_trace(int on, unsigned long long *out /*host*/);
 
 #ifdef __cplusplus
 }

@@ -25,7 +25,7 @@ EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_byte
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
            "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
-           "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard")
+           "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace")
 
 
 class NfState(C.Structure):

@@ -278,7 +278,7 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     return cuda_rc(e);
 }
 
-// debug, not in nf.h: enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;
+// debug aid (nf.h): enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;
 // with `out` != NULL the stamps are copied to the host (synchronises).
 int nf_debug_trace(int on, unsigned long long *out) {
     if (on && !g_trace) { if (cudaMalloc(&g_trace, 256 * 8 * 8) != cudaSuccess) return NF_ERR_CUDA; cudaMemset(g_trace, 0, 256 * 8 * 8); }
