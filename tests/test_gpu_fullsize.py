@@ -77,3 +77,9 @@ def test_paper_local_count_shapes(n):
     """8 x 131K and 8 x 524K logical buckets, zero mismatches."""
     cfg = shapes.paper_local_count(n)
     _check_bucket(cfg, cfg.buckets[0], five_call=True)
+
+
+def test_gpt2_bucket_binary_mode_full_size():
+    """G-Binary (one plane, cneg = W - cpos) on a full 33.6 M-element GPT bucket through the fused call."""
+    cfg = shapes.gpt2_1p3b()
+    _check_bucket(cfg, cfg.buckets[2], mode=O.MODE_GBINARY)

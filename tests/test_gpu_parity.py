@@ -188,3 +188,46 @@ def test_host_buffer_entry_point_matches_oracle():
     compare(bb, ref, cfg.W, O.MODE_GTERNARY, check_planes=False, check_scale=False,      # the host call has no scale_out
             what="host entry point")
     assert np.array_equal(out_host.numpy(), _np(bb.out)[:b.n])
+
+
+@pytest.mark.parametrize("seed", range(24))
+def test_random_layouts(seed):
+    """Seeded random buckets: tensor counts, lengths (from 1 element to several tiles), gaps, unaligned offsets
+    and strides, W (one or several worker groups), mode, tau, margin, alpha, state — fused call and five calls
+    against the oracle."""
+    rng = np.random.default_rng(9000 + seed)
+    T = int(rng.integers(1, 40))
+    lens = []
+    for _ in range(T):
+        kind = rng.integers(0, 4)
+        lens.append(int({0: rng.integers(1, 40), 1: rng.integers(40, 2100), 2: rng.integers(2100, 9000),
+                         3: 2048 * int(rng.integers(1, 4))}[int(kind)]))
+    align = bool(rng.integers(0, 2))
+    off, o = [], 0 if align else int(rng.integers(0, 4))
+    for l in lens:
+        off.append(o)
+        o += l
+        if rng.random() < 0.2:
+            o += int(rng.integers(1, 9))                      # gap
+        if align:
+            o = (o + 3) // 4 * 4
+    n = o + int(rng.integers(0, 3))
+    W = int(rng.choice([1, 2, 3, 5, 8, 9, 16, 23, 40]))
+    elig = [int(x) for x in rng.integers(0, 2, T)]
+    mode = O.MODE_GTERNARY if rng.random() < 0.6 else O.MODE_GBINARY
+    g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-5, 1, (1, n))).astype(np.float32)
+    g[rng.random((W, n)) < 0.08] = 0.0
+    if rng.random() < 0.3:
+        g[rng.integers(0, W), rng.integers(0, n)] = np.nan
+    if rng.random() < 0.3:
+        g[rng.integers(0, W), rng.integers(0, n)] = np.inf
+    tau = (rng.random(T) * 1e-3).astype(np.float32) if rng.random() < 0.5 else None
+    margin = int(rng.integers(0, 3))
+    alpha = 1.0 if rng.random() < 0.5 else 1.0 / W
+    state = (1, 0, 1) if rng.random() < 0.8 else (1, 1, 1)
+    pad = rng.random() < 0.5                                   # worker stride a multiple of 4 or exactly n
+    gd = _dev(g, pad_to4=pad)
+    if gd.shape[1] < n:                                        # _dev pads tiny buckets to 4 columns
+        pytest.skip("degenerate")
+    run_both(gd, np.array(off, np.int64), np.array(lens, np.int64), elig, state=state, mode=mode, tau=tau,
+             margin=margin, alpha=alpha, what=f"random layout seed {seed}")
