@@ -21,6 +21,12 @@
  *    (gap positions are never read or written). len[t] >= 0.
  *  - Alignment: g, out, P, N must be 16-byte aligned (else NF_ERR_ALIGN). Tensor offsets and
  *    strides may be arbitrary; tensors whose rows are not 16-byte aligned take a scalar path.
+ *    The fused call moves gradients with 16-byte bulk copies: for such unaligned rows it reads the
+ *    whole 16-byte chunks that contain the row's first and last element, i.e. up to 12 bytes before
+ *    / after the row inside the chunk (never a chunk without an element of the row; nothing is written).
+ *  - "gap positions are never read" holds up to that chunk granularity for unaligned rows.
+ *  - nf_aggregate_bucket uses a cooperative launch (grid = one CTA per SM) when T <= 256; calls on
+ *    different streams are serialised by the device, not rejected.
  *  - Packed planes (reading #10): uint32 words, LSB = lowest element index, each L tensor starts
  *    at word woff[t] and is padded with 0 bits to a word boundary; worker w's plane starts at
  *    P + w*plane_stride (plane_stride >= Wd words).
