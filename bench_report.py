@@ -116,7 +116,7 @@ def table_sweep(args, dev, peak):
     from workloads import shapes, gen
     out = ["| W | planes in (MB) | (i) count-reduce alone | (ii) pack + count-reduce | (iii) fused | (iv) fp32_reduce | "
            "copies |", "|---|---|---|---|---|---|---|"]
-    for W in shapes.SWEEP_W:
+    for W in ([args.sweep_w] if args.sweep_w else shapes.SWEEP_W):
         cfg = shapes.sweep(W)
         b = cfg.buckets[0]
         n = b.n
@@ -257,6 +257,9 @@ def main():
     ap.add_argument("--out", default="")
     ap.add_argument("--iters", type=int, default=20)
     ap.add_argument("--skip-configs", action="store_true")
+    ap.add_argument("--only", default="", choices=["", "configs", "five", "sweep", "hier"],
+                    help="print one table only (short runs under ncu: see profiles/)")
+    ap.add_argument("--sweep-w", type=int, default=0, help="restrict the sweep table to one worker count")
     args = ap.parse_args()
     import torch
     from paper_2606_25759_b200 import build as nf_build
@@ -267,14 +270,18 @@ def main():
     peak = measured_peak()
     parts = [f"GPU: {torch.cuda.get_device_name(0)}; measured HBM copy peak {peak:.1f} GB/s; "
              f"median of {args.iters} CUDA-event-timed iterations after 3 warm-ups; mode G-Ternary, planes and health on.", ""]
-    if not args.skip_configs:
+    want = lambda name: args.only in ("", name)
+    if want("configs") and not args.skip_configs:
         parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
-    parts += ["### The five stand-alone calls and the fused call on GPT buckets 0 (all low-bit) and 36 (all FP32 route)", "",
-              table_five_calls(args, dev, peak), ""]
-    parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
-    parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
-              "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange)", "",
-              table_hier(args, dev, peak), ""]
+    if want("five"):
+        parts += ["### The five stand-alone calls and the fused call on GPT buckets 0 (all low-bit) and 36 (all FP32 route)", "",
+                  table_five_calls(args, dev, peak), ""]
+    if want("sweep"):
+        parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
+    if want("hier"):
+        parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
+                  "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange)", "",
+                  table_hier(args, dev, peak), ""]
     text = "\n".join(parts)
     print(text)
     if args.out:

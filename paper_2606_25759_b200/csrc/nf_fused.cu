@@ -51,6 +51,11 @@ constexpr int kPitch = kTile + 4;                // ring row: one tile of one wo
 constexpr int kStageFloats = kGroup * kPitch;    // 8 workers
 constexpr int kStageBytes = kStageFloats * 4;    // 64 KB + 128 B
 constexpr int kKTiles = NF_KKT;                  // tiles of FP32 partial accumulation (<= 4: exact_redo's list)
+#ifndef NF_MRUN
+#define NF_MRUN 4
+#endif
+constexpr int kMRun = NF_MRUN;                   // MULTI: tiles per group-major run (1 = tile-major order), <= kKTiles
+static_assert(kMRun >= 1 && kMRun <= kKTiles && kMRun <= 4, "a run is flushed once: exact_redo lists <= 4 tiles");
 constexpr int kMaxStages = 4;
 constexpr int kStages = 3;                       // ring depth: 3 x 64 KB
 static_assert(kTile == kCThreads * 4, "one float4 per consumer thread per worker and tile");
@@ -165,6 +170,7 @@ struct FusedSmem {
     float *ring;
     uint64_t *full, *empty;
     int *tile_of;                // [kMaxStages] tile held by a stage, -1 = no more tiles
+    int *run_of;                 // [kMaxStages] MULTI: length R of the run of tiles the stage belongs to
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -180,6 +186,7 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.full = (uint64_t *)base;
     s.empty = s.full + kMaxStages;
     s.tile_of = (int *)(base + 64);
+    s.run_of = (int *)(base + 80);
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -508,7 +515,7 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
             if (u >= total_units) continue;
             const int tile = u >> 1;
             if (tile >= tile_e) {
-TensorCur tc;
+                TensorCur tc;
                 tensor_lookup(p, pv, sm, tile, tc);
                 t_cur = tc.t; tile_b = tc.tile_b; tile_e = tc.tile_e; off_t = tc.off; len_t = tc.len;
                 dec = tc.isL;
@@ -523,7 +530,7 @@ TensorCur tc;
                         __nanosleep(500);
                         if (spins > (1u << 23)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
                     }
-                    S_t = tensor_scale(p.abs_sum, W, p.T, t_cur, len_t);
+                    S_t = warp_tensor_scale(p.abs_sum, W, p.T, t_cur, len_t, lane);   // warp-uniform branch
                 }
             }
             if (!dec) continue;
@@ -675,12 +682,26 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (tid < 32) s_scan[tid] = 0;
         __syncthreads();
         if (warp < kMetaCap / 32 && lane == 31) { s_scan[warp] = i_tiles; s_scan[8 + warp] = i_words; s_scan[16 + warp] = i_nl; }
-        if (tid < T) {
+        if (blockIdx.x == 0 && warp < kMetaCap / 32) {
+            // summary tallies (CTA 0 publishes them): warp sums by shuffle, one shared-memory add per warp
+            // (64-bit shared-memory atomics are compare-and-swap loops: one per tensor cost 5 us at T = 96)
             unsigned long long *tal = reinterpret_cast<unsigned long long *>(s_scan + 24);
-            if (r == NF_ROUTE_F) atomicAdd(tal + 0, 1ull);
-            else if (r == NF_ROUTE_P) atomicAdd(tal + 1, 1ull);
-            else atomicAdd(tal + 2, (unsigned long long)l);
-            atomicAdd(tal + 3, (unsigned long long)l);
+            const bool in = tid < T;
+            unsigned q_f = (in && r == NF_ROUTE_F) ? 1u : 0u, q_p = (in && r == NF_ROUTE_P) ? 1u : 0u;
+            long long e_l = (in && r == NF_ROUTE_L) ? l : 0, e_all = in ? l : 0;
+            q_f = warp_sum(q_f);
+            q_p = warp_sum(q_p);
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) {
+                e_l += __shfl_xor_sync(0xffffffffu, e_l, d);
+                e_all += __shfl_xor_sync(0xffffffffu, e_all, d);
+            }
+            if (lane == 0) {
+                atomicAdd(tal + 0, (unsigned long long)q_f);
+                atomicAdd(tal + 1, (unsigned long long)q_p);
+                atomicAdd(tal + 2, (unsigned long long)e_l);
+                atomicAdd(tal + 3, (unsigned long long)e_all);
+            }
         }
         const int any_bad = __syncthreads_or(bad);
         long long b_tiles = 0, b_words = 0, b_nl = 0, t_tiles = 0, t_words = 0, t_nl = 0;
@@ -781,7 +802,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 next = atomicAdd(cursor, want);
                 run_end = next + want;
             }
-            const int tile = next++;
+            const int tile = next;
             if (tile >= n_tiles) {
                 mbar_wait(sm.empty + st, ph ^ 1u);
                 sm.tile_of[st] = -1;                               // sentinel: the consumers stop
@@ -789,37 +810,46 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 break;
             }
             if (tile >= c.tile_e) tensor_lookup(p, pv, sm, tile, c);
-            const int64_t tile_base = (int64_t)(tile - c.tile_b) * kTile;
-            const int64_t rem = c.len - tile_base;
-            const int need = rem >= kTile ? kTile : (int)rem;
-            // aligned rows: whole float4s only (a partial one is read from global memory by its owner
-            // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
-            // (whole 16-byte chunks, each holding at least one element of the row).
-            const uint32_t bytes = (uint32_t)((need & ~3) * 4);
-            const float *src = p.g + c.off + tile_base;
+            // Several worker groups (MULTI), low-bit tensor: the stages of a run of R <= kKTiles consecutive
+            // tiles of one tensor go group-major (group 0 of tiles 0..R-1, then group 1, ...), so that the
+            // consumers flush their FP32 partials of a group once per run instead of once per stage.
+            int R = 1;
+            if (MULTI && c.isL) R = min(min(min(run_end, n_tiles), c.tile_e) - tile, kMRun);
+            next += R;
             for (int w0 = 0; w0 < W; w0 += kGroup) {              // one stage per (tile, worker group)
                 const int nw = min(kGroup, W - w0);
-                mbar_wait(sm.empty + st, ph ^ 1u);
-                sm.tile_of[st] = tile;
-                float *dst = sm.ring + (size_t)st * kStageFloats;
-                if (!c.aligned) {
-                    uint32_t tx = 0;
-                    for (int w = 0; w < nw; ++w)
-                        tx += (uint32_t)((((int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
-                    mbar_expect_tx(sm.full + st, tx);
-                    for (int w = 0; w < nw; ++w) {
-                        const int m = (int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
-                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
-                                 (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
+                for (int r = 0; r < R; ++r) {
+                    const int64_t tile_base = (int64_t)(tile + r - c.tile_b) * kTile;
+                    const int64_t rem = c.len - tile_base;
+                    const int need = rem >= kTile ? kTile : (int)rem;
+                    // aligned rows: whole float4s only (a partial one is read from global memory by its owner
+                    // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
+                    // (whole 16-byte chunks, each holding at least one element of the row).
+                    const uint32_t bytes = (uint32_t)((need & ~3) * 4);
+                    const float *src = p.g + c.off + tile_base;
+                    mbar_wait(sm.empty + st, ph ^ 1u);
+                    sm.tile_of[st] = tile + r;
+                    if (MULTI) sm.run_of[st] = R;
+                    float *dst = sm.ring + (size_t)st * kStageFloats;
+                    if (!c.aligned) {
+                        uint32_t tx = 0;
+                        for (int w = 0; w < nw; ++w)
+                            tx += (uint32_t)((((int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
+                        mbar_expect_tx(sm.full + st, tx);
+                        for (int w = 0; w < nw; ++w) {
+                            const int m = (int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
+                            bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
+                                     (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
+                        }
+                    } else if (bytes) {
+                        mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
+                        for (int w = 0; w < nw; ++w)
+                            bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
+                    } else {
+                        mbar_arrive(sm.full + st);
                     }
-                } else if (bytes) {
-                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
-                    for (int w = 0; w < nw; ++w)
-                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
-                } else {
-                    mbar_arrive(sm.full + st);
+                    if (++st == stages) { st = 0; ph ^= 1u; }
                 }
-                if (++st == stages) { st = 0; ph ^= 1u; }
             }
         }
         return;
@@ -922,68 +952,89 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             pO = p.out + c.off + 4 * ctid;
         }
         const int rel = tile - c.tile_b;
-        const int64_t rem_t = c.len - (int64_t)rel * kTile;
-        const bool ragged = rem_t < kTile;                  // last tile of the tensor, need < kTile elements
-        const int need = ragged ? (int)rem_t : kTile;
-        const int valid = min(max(need - 4 * ctid, 0), 4);
-        recent = make_int4(tile, recent.x, recent.y, recent.z);
-        uint32_t posR = 0u, negR = 0u, cp = 0u, cn = 0u;     // cp/cn: byte-packed running counts (MULTI)
+        // MULTI, low-bit tensor: the producer sends a run of R consecutive tiles group-major (see there)
+        const int R = MULTI ? sm.run_of[st] : 1;
+        if (MULTI) recent = make_int4(tile + R - 1, tile + R - 2, tile + R - 3, tile + R - 4);
+        else recent = make_int4(tile, recent.x, recent.y, recent.z);
+        uint32_t posR = 0u, negR = 0u;
+        uint32_t cp0 = 0u, cp1 = 0u, cp2 = 0u, cp3 = 0u;     // byte-packed running counts of the run's tiles (MULTI)
+        uint32_t cn0 = 0u, cn1 = 0u, cn2 = 0u, cn3 = 0u;
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {   // one ring stage per worker group
-            if (MULTI && w0 > 0) mbar_wait(sm.full + st, ph);
+        int valid = 0;
+        for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {   // one ring stage per (tile, worker group)
             const int nw = MULTI ? min(kGroup, W - w0) : W;
-            const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
-            uint64_t *const empty_bar = sm.empty + st;
-            if (++st == stages) { st = 0; ph ^= 1u; }
-            if (MULTI) { posR = 0u; negR = 0u; }
-            if (ragged || !c.aligned) {
-                slow_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)rel * kTile + 4 * ctid,
-                                  p.worker_stride, nw, valid, !c.aligned, (int)((c.off + (int64_t)w0 * p.worker_stride) & 3),
-                                  (int)(p.worker_stride & 3), c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
-                                  w0 == 0);
-            } else if (c.isL) {
-                const float tau = c.tau, ntau = -c.tau;
-                if (ternary) {
-                    if (nw == kGroup) fast_signs<2, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
-                    else fast_signs<2, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
-                } else {
-                    if (nw == kGroup) fast_signs<1, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
-                    else fast_signs<1, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
-                }
-            } else {
-                acc = (nw == kGroup) ? fast_fp32<HEALTH, true>(sb, nw, af, qf, acc, w0 == 0)
-                                     : fast_fp32<HEALTH, false>(sb, nw, af, qf, acc, w0 == 0);
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_bar);              // every lane's reads of the stage are done
-            if (c.isL) {
-                if (pP) {
-                    // packed plane words: 8x8 nibble transpose, lane q of an octet stores worker q's word
-                    const bool stp = ((lane & 7) < nw) && (32 * (warp * 4 + (lane >> 3)) < need);
-                    const size_t o = (size_t)rel * (kTile / 32) + (size_t)w0 * p.plane_stride;
-                    const uint32_t pw = nib_transpose8(posR, tctl);
-                    if (stp) pP[o] = pw;
+            for (int r = 0; r < R; ++r) {
+                if (MULTI && (w0 > 0 || r > 0)) mbar_wait(sm.full + st, ph);
+                const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
+                uint64_t *const empty_bar = sm.empty + st;
+                if (++st == stages) { st = 0; ph ^= 1u; }
+                const int64_t rem_t = c.len - (int64_t)(rel + r) * kTile;
+                const bool ragged = rem_t < kTile;              // last tile of the tensor, need < kTile elements
+                const int need = ragged ? (int)rem_t : kTile;
+                valid = min(max(need - 4 * ctid, 0), 4);
+                if (MULTI) { posR = 0u; negR = 0u; }
+                if (ragged || !c.aligned) {
+                    slow_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)(rel + r) * kTile + 4 * ctid,
+                                      p.worker_stride, nw, valid, !c.aligned, (int)((c.off + (int64_t)w0 * p.worker_stride) & 3),
+                                      (int)(p.worker_stride & 3), c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
+                                      w0 == 0);
+                } else if (c.isL) {
+                    const float tau = c.tau, ntau = -c.tau;
                     if (ternary) {
-                        const uint32_t nwd = nib_transpose8(negR, tctl);
-                        if (stp) pN[o] = nwd;
+                        if (nw == kGroup) fast_signs<2, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                        else fast_signs<2, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
+                    } else {
+                        if (nw == kGroup) fast_signs<1, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                        else fast_signs<1, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
                     }
+                } else {
+                    acc = (nw == kGroup) ? fast_fp32<HEALTH, true>(sb, nw, af, qf, acc, w0 == 0)
+                                         : fast_fp32<HEALTH, false>(sb, nw, af, qf, acc, w0 == 0);
                 }
-                if (MULTI) {
+                __syncwarp();
+                if (lane == 0) mbar_arrive(empty_bar);          // every lane's reads of the stage are done
+                if (c.isL) {
+                    if (pP) {
+                        // packed plane words: 8x8 nibble transpose, lane q of an octet stores worker q's word
+                        const bool stp = ((lane & 7) < nw) && (32 * (warp * 4 + (lane >> 3)) < need);
+                        const size_t o = (size_t)(rel + r) * (kTile / 32) + (size_t)w0 * p.plane_stride;
+                        const uint32_t pw = nib_transpose8(posR, tctl);
+                        if (stp) pP[o] = pw;
+                        if (ternary) {
+                            const uint32_t nwd = nib_transpose8(negR, tctl);
+                            if (stp) pN[o] = nwd;
+                        }
+                    }
+                    if (MULTI) {
+                        uint32_t dp = 0u, dn = 0u;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        cp += (uint32_t)__popc(posR & (0x11111111u << j)) << (8 * j);
-                        if (ternary) cn += (uint32_t)__popc(negR & (0x11111111u << j)) << (8 * j);
+                        for (int j = 0; j < 4; ++j) {
+                            dp += (uint32_t)__popc(posR & (0x11111111u << j)) << (8 * j);
+                            if (ternary) dn += (uint32_t)__popc(negR & (0x11111111u << j)) << (8 * j);
+                        }
+                        cp0 += r == 0 ? dp : 0u; cp1 += r == 1 ? dp : 0u; cp2 += r == 2 ? dp : 0u; cp3 += r == 3 ? dp : 0u;
+                        cn0 += r == 0 ? dn : 0u; cn1 += r == 1 ? dn : 0u; cn2 += r == 2 ? dn : 0u; cn3 += r == 3 ? dn : 0u;
                     }
                 }
             }
             if (MULTI && (c.isL || HEALTH))
-                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, 1, recent, ctid, c.aligned);
+                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
         }
         if (c.isL) {
             // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
-            const uint32_t d = MULTI ? vote4_packed(cp, cn, ternary, W, p.margin)
-                                     : (ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin));
-            if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
+            if (!MULTI) {
+                const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
+                if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
+            } else {
+#pragma unroll
+                for (int r = 0; r < kKTiles; ++r) {
+                    if (r < R) {
+                        const uint32_t d = vote4_packed(r == 0 ? cp0 : (r == 1 ? cp1 : (r == 2 ? cp2 : cp3)),
+                                                        r == 0 ? cn0 : (r == 1 ? cn1 : (r == 2 ? cn2 : cn3)), ternary, W, p.margin);
+                        if (c.len - (int64_t)(rel + r) * kTile > 4 * ctid) pD[(size_t)(rel + r) * (kTile / 4)] = (uint8_t)d;
+                    }
+                }
+            }
         } else {
             float *o = pO + (size_t)rel * kTile;
             float4 r = acc;
@@ -999,7 +1050,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
         }
         touched = true;
-        ++ntile_acc;
+        ntile_acc += R;
         if (!MULTI && ++kcnt == kKTiles) {
             stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
             kcnt = 0;

@@ -238,6 +238,21 @@ __device__ __forceinline__ float tensor_scale(const double *__restrict__ abs_sum
     }
     return (float)(s / (double)W);
 }
+// The same value computed by a whole (converged) warp: the W loads of a round of 32 workers are in
+// flight together (one L2 round trip per 32 workers instead of one per worker) and the FP64 adds
+// run in the same fixed worker order through a shuffle chain, so the result is bit-identical.
+__device__ __forceinline__ float warp_tensor_scale(const double *__restrict__ abs_sum, int W, int T, int t,
+                                                   int64_t len_t, int lane) {
+    double s = 0.0;
+    const double dl = (double)len_t;
+    for (int w0 = 0; w0 < W; w0 += 32) {
+        const int w = w0 + lane;
+        const float swt = (w < W) ? (float)(__ldcg(abs_sum + (size_t)w * T + t) / dl) : 0.f;
+        const int cnt = min(32, W - w0);
+        for (int j = 0; j < cnt; ++j) s += (double)__shfl_sync(0xffffffffu, swt, j);
+    }
+    return (float)(s / (double)W);
+}
 #endif
 
 }  // namespace nf

@@ -119,21 +119,6 @@ __device__ __forceinline__ void count_words2(const uint32_t *__restrict__ P, con
     }
 }
 
-// S_t computed by one warp: the per-worker loads and divisions run in parallel across the lanes, the
-// FP64 sum keeps the fixed worker order of tensor_scale() (bit-identical result) through a shuffle chain.
-__device__ __forceinline__ float warp_tensor_scale(const double *__restrict__ abs_sum, int W, int T, int t,
-                                                   int64_t len_t, int lane) {
-    double s = 0.0;
-    const double dl = (double)len_t;
-    for (int w0 = 0; w0 < W; w0 += 32) {
-        const int w = w0 + lane;
-        const float swt = (w < W) ? (float)(__ldcg(abs_sum + (size_t)w * T + t) / dl) : 0.f;
-        const int cnt = min(32, W - w0);
-        for (int j = 0; j < cnt; ++j) s += (double)__shfl_sync(0xffffffffu, swt, j);
-    }
-    return (float)(s / (double)W);
-}
-
 // every CTA computes the scales of the L tensors it may touch into shared memory; CTA 0 publishes
 __device__ __forceinline__ void compute_scales(const ReduceParams &p, const PlanView &pv, float *s_scale) {
     for (int t = threadIdx.x; t < p.T; t += blockDim.x) {

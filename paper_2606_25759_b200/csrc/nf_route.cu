@@ -122,10 +122,17 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     __shared__ int s_bad;
     if (threadIdx.x == 0) { s_tal[0] = s_tal[1] = s_tal[2] = s_tal[3] = 0ull; s_bad = 0; }
     __syncthreads();
-    if (nF) atomicAdd(&s_tal[0], (unsigned long long)nF);
-    if (nP) atomicAdd(&s_tal[1], (unsigned long long)nP);
-    if (e) atomicAdd(&s_tal[2], (unsigned long long)e);
-    if (tot) atomicAdd(&s_tal[3], (unsigned long long)tot);
+    // warp sums first: 64-bit shared-memory atomics are compare-and-swap loops, one per thread serialises
+    {
+        unsigned long long q[4] = {(unsigned long long)nF, (unsigned long long)nP, (unsigned long long)e,
+                                   (unsigned long long)tot};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) q[k] += __shfl_xor_sync(0xffffffffu, q[k], d);
+            if ((threadIdx.x & 31) == 0 && q[k]) atomicAdd(&s_tal[k], q[k]);
+        }
+    }
     if (bad) atomicOr(&s_bad, 1);
     __syncthreads();
     if (threadIdx.x == 0) {
