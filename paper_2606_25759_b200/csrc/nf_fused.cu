@@ -624,7 +624,105 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     pdl_wait();
     if (tid == 0) trace_stamp(p, 6);
     const PlanView pv = plan_view(p.plan, p.T);
-    int n_tiles;
+    int n_tiles = 0;
+
+    // -----------------------------------------------------------------------------------------
+    // producer (one elected lane of warp kCW): issues the bulk copies of every (tile, worker group).
+    // Dynamic tile scheduling: tiles are handed out by a device-wide cursor, so a CTA that runs ahead
+    // (SM position, co-running decode warps) simply takes more. Every tile enters the ring; the stage
+    // carries its tile index to the consumers. Tiles are taken in runs of consecutive tiles (guided
+    // self-scheduling: up to NF_KCHUNK early, single tiles near the end), so that a CTA stays inside one
+    // tensor for a while — a tensor change costs a CTA-wide flush — without giving up the balance at the
+    // tail. The FIRST run of every CTA is static (CTA b: tiles [b*want0, (b+1)*want0), the cursor counts
+    // from gridDim.x*want0), so it needs nothing another CTA wrote: with the in-kernel routing the
+    // producer fills the ring with it while the grid barrier is still pending (prefetch = true: never
+    // blocks, never touches the cursor).
+    // -----------------------------------------------------------------------------------------
+    int pr_st = 0, pr_next = 0, pr_end = 0, pr_tile = 0, pr_R = 1, pr_w0 = 0, pr_r = 0;
+    uint32_t pr_ph = 0;
+    bool pr_have = false, pr_first = true;
+    TensorCur pc{};
+    pc.tile_e = 0;
+    auto produce = [&](int max_stages, bool prefetch) __attribute__((always_inline)) {
+        const uint64_t pol = policy_evict_first();
+        int32_t *cursor = const_cast<int32_t *>(&pv.hdr->tile_cursor);
+        int want0 = n_tiles / (4 * (int)gridDim.x);
+        want0 = want0 < 1 ? 1 : (want0 > NF_KCHUNK ? NF_KCHUNK : want0);
+        const int dyn0 = (int)gridDim.x * want0;                       // first dynamically assigned tile
+        for (int issued = 0; issued < max_stages; ++issued) {
+            if (!pr_have) {
+                if (pr_first) {
+                    pr_first = false;
+                    pr_next = (int)blockIdx.x * want0;
+                    pr_end = pr_next + want0;
+                } else if (pr_next >= pr_end) {
+                    if (prefetch) return;
+                    int want = (n_tiles - pr_end) / (4 * (int)gridDim.x);     // pr_end: last position seen
+                    want = want < 1 ? 1 : (want > NF_KCHUNK ? NF_KCHUNK : want);
+                    pr_next = dyn0 + atomicAdd(cursor, want);
+                    pr_end = pr_next + want;
+                }
+                pr_tile = pr_next;
+                if (pr_tile >= n_tiles) {
+                    if (prefetch) return;
+                    mbar_wait(sm.empty + pr_st, pr_ph ^ 1u);
+                    sm.tile_of[pr_st] = -1;                            // sentinel: the consumers stop
+                    mbar_arrive(sm.full + pr_st);
+                    return;
+                }
+                if (pr_tile >= pc.tile_e) tensor_lookup(p, pv, sm, pr_tile, pc);
+                // Several worker groups (MULTI), low-bit tensor: the stages of a run of R <= kMRun consecutive
+                // tiles of one tensor go group-major (group 0 of tiles 0..R-1, then group 1, ...), so that the
+                // consumers flush their FP32 partials of a group once per run instead of once per stage.
+                pr_R = 1;
+                if (MULTI && pc.isL) pr_R = min(min(min(pr_end, n_tiles), pc.tile_e) - pr_tile, kMRun);
+                pr_next += pr_R;
+                pr_w0 = 0;
+                pr_r = 0;
+                pr_have = true;
+            }
+            {
+                const int w0 = pr_w0, nw = min(kGroup, W - w0);
+                const int64_t tile_base = (int64_t)(pr_tile + pr_r - pc.tile_b) * kTile;
+                const int64_t rem = pc.len - tile_base;
+                const int need = rem >= kTile ? kTile : (int)rem;
+                // aligned rows: whole float4s only (a partial one is read from global memory by its owner
+                // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
+                // (whole 16-byte chunks, each holding at least one element of the row).
+                const uint32_t bytes = (uint32_t)((need & ~3) * 4);
+                const float *src = p.g + pc.off + tile_base;
+                const int st = pr_st;
+                mbar_wait(sm.empty + st, pr_ph ^ 1u);                  // first lap: passes at once
+                sm.tile_of[st] = pr_tile + pr_r;
+                if (MULTI) sm.run_of[st] = pr_R;
+                float *dst = sm.ring + (size_t)st * kStageFloats;
+                if (!pc.aligned) {
+                    uint32_t tx = 0;
+                    for (int w = 0; w < nw; ++w)
+                        tx += (uint32_t)((((int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
+                    mbar_expect_tx(sm.full + st, tx);
+                    for (int w = 0; w < nw; ++w) {
+                        const int m = (int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
+                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
+                                 (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
+                    }
+                } else if (bytes) {
+                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
+                    for (int w = 0; w < nw; ++w)
+                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
+                } else {
+                    mbar_arrive(sm.full + st);
+                }
+                if (++pr_st == stages) { pr_st = 0; pr_ph ^= 1u; }
+                if (++pr_r == pr_R) {
+                    pr_r = 0;
+                    pr_w0 += kGroup;
+                    if (pr_w0 >= W) pr_have = false;
+                }
+            }
+        }
+    };
+
     if (p.inkernel_route) {
         // ---- step a1 inside this kernel (T <= kMetaCap) --------
         // Every CTA derives the routing of the bucket into its shared-memory metadata (redundant O(T)
@@ -651,7 +749,8 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 hdr->unit_cursor = 0;
             }
         }
-        __threadfence();
+        // (no fence of our own: barrier_arrive is a CTA barrier followed by the master's release at GPU scope,
+        // which is cumulative over the zeroing stores of the whole CTA)
         cooperative_groups::grid_group grid = cooperative_groups::this_grid();
         auto zeroed = grid.barrier_arrive();
         long long l = 0, o = 0, v_tiles = 0, v_words = 0, v_nl = 0;
@@ -754,6 +853,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 p.summary[NF_SUM_STATUS] = status;
             }
         }
+        // the ring is filled with this CTA's static first run while the barrier is pending (the shared-memory
+        // metadata it needs was written just above)
+        n_tiles = status == NF_OK ? (int)t_tiles : 0;
+        __syncthreads();
+        if (warp == kCW && lane == 0 && status == NF_OK) produce(stages, true);
         grid.barrier_wait(std::move(zeroed));               // everybody's slice is zero, the cursors too
         if (tid == 0) trace_stamp(p, 7);
         if (status != NF_OK) return;
@@ -778,80 +882,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
 
     // =========================================================================================
-    // producer: one elected lane issues the bulk copies of every (tile, worker group)
+    // producer: one elected lane issues the bulk copies of every (tile, worker group): produce() above
     // =========================================================================================
     if (warp == kCW) {
-        if (lane != 0) return;
-        const uint64_t pol = policy_evict_first();
-        int st = 0;
-        uint32_t ph = 0;
-        TensorCur c{};
-        c.tile_e = 0;
-        // Dynamic tile scheduling: tiles are handed out by a device-wide cursor, so a CTA that runs
-        // ahead (SM position, co-running decode warps) simply takes more. Every tile of an aligned
-        // tensor enters the ring; the stage carries its tile index to the consumers.
-        // Tiles are taken in runs of consecutive tiles (guided self-scheduling: up to NF_KCHUNK early, single
-        // tiles near the end), so that a CTA stays inside one tensor for a while — a tensor change costs a
-        // CTA-wide flush — without giving up the balance at the tail.
-        int32_t *cursor = const_cast<int32_t *>(&pv.hdr->tile_cursor);
-        int next = 0, run_end = 0;
-        for (;;) {
-            if (next >= run_end) {
-                int want = (n_tiles - run_end) / (4 * (int)gridDim.x);     // run_end: last position seen
-                want = want < 1 ? 1 : (want > NF_KCHUNK ? NF_KCHUNK : want);
-                next = atomicAdd(cursor, want);
-                run_end = next + want;
-            }
-            const int tile = next;
-            if (tile >= n_tiles) {
-                mbar_wait(sm.empty + st, ph ^ 1u);
-                sm.tile_of[st] = -1;                               // sentinel: the consumers stop
-                mbar_arrive(sm.full + st);
-                break;
-            }
-            if (tile >= c.tile_e) tensor_lookup(p, pv, sm, tile, c);
-            // Several worker groups (MULTI), low-bit tensor: the stages of a run of R <= kKTiles consecutive
-            // tiles of one tensor go group-major (group 0 of tiles 0..R-1, then group 1, ...), so that the
-            // consumers flush their FP32 partials of a group once per run instead of once per stage.
-            int R = 1;
-            if (MULTI && c.isL) R = min(min(min(run_end, n_tiles), c.tile_e) - tile, kMRun);
-            next += R;
-            for (int w0 = 0; w0 < W; w0 += kGroup) {              // one stage per (tile, worker group)
-                const int nw = min(kGroup, W - w0);
-                for (int r = 0; r < R; ++r) {
-                    const int64_t tile_base = (int64_t)(tile + r - c.tile_b) * kTile;
-                    const int64_t rem = c.len - tile_base;
-                    const int need = rem >= kTile ? kTile : (int)rem;
-                    // aligned rows: whole float4s only (a partial one is read from global memory by its owner
-                    // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
-                    // (whole 16-byte chunks, each holding at least one element of the row).
-                    const uint32_t bytes = (uint32_t)((need & ~3) * 4);
-                    const float *src = p.g + c.off + tile_base;
-                    mbar_wait(sm.empty + st, ph ^ 1u);
-                    sm.tile_of[st] = tile + r;
-                    if (MULTI) sm.run_of[st] = R;
-                    float *dst = sm.ring + (size_t)st * kStageFloats;
-                    if (!c.aligned) {
-                        uint32_t tx = 0;
-                        for (int w = 0; w < nw; ++w)
-                            tx += (uint32_t)((((int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
-                        mbar_expect_tx(sm.full + st, tx);
-                        for (int w = 0; w < nw; ++w) {
-                            const int m = (int)((c.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
-                            bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
-                                     (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
-                        }
-                    } else if (bytes) {
-                        mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
-                        for (int w = 0; w < nw; ++w)
-                            bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
-                    } else {
-                        mbar_arrive(sm.full + st);
-                    }
-                    if (++st == stages) { st = 0; ph ^= 1u; }
-                }
-            }
-        }
+        if (lane == 0) produce(0x7fffffff, false);
         return;
     }
     // =========================================================================================
