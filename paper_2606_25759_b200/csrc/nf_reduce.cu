@@ -133,19 +133,199 @@ __device__ __forceinline__ void compute_scales(const ReduceParams &p, const Plan
     __syncthreads();
 }
 
+// ---------------------------------------------------------------------------------------------
+// The three pieces every a3 kernel shares: where a word position lives, the vote, the write-back.
+// ---------------------------------------------------------------------------------------------
+struct WordMeta {
+    int nvalid;        // elements of the word that exist (0: no such word), 32 except in a tensor's last word
+    int li;            // index of the word's tensor in the plan's list of L tensors, -1: no such word
+    int64_t obase;     // bucket position of the word's first element
+};
+
+__device__ __forceinline__ WordMeta word_meta(const ReduceParams &p, const PlanView &pv, int nL, int64_t Wd, int64_t k) {
+    WordMeta m{0, -1, 0};
+    if (k < Wd) {
+        const int li = upper_tensor<int64_t>(pv.lt_woff, nL, k);
+        const int t = __ldg(pv.lt_index + li);
+        const int64_t i0 = (k - __ldg(pv.lt_woff + li)) * 32;  // tensor-relative first element
+        const int64_t rem = __ldg(p.len + t) - i0;
+        m.nvalid = rem >= 32 ? 32 : (int)rem;
+        m.obase = __ldg(p.off + t) + i0;
+        m.li = li;
+    }
+    return m;
+}
+
+// The tensor a warp's previous 32 words fell into, kept in registers: consecutive units of a warp mostly
+// stay inside one tensor (the low-bit tensors are the big ones), and then neither the lookups above nor the
+// per-tensor scale (each a chain of dependent L2 round trips) are repeated.
+struct TensorCache {
+    int li;                    // -1: empty
+    int64_t kfirst, kend;      // word range [kfirst, kend) of the tensor
+    int64_t len, off;
+    float S;
+};
+
+// true (warp-uniform) iff the 32 words k - lane .. k - lane + 31 all belong to the cached tensor
+__device__ __forceinline__ bool cached_meta(const TensorCache &c, int64_t k, int lane, WordMeta &m) {
+    const int64_t k0 = k - lane;
+    if (c.li < 0 || k0 < c.kfirst || k0 + 32 > c.kend) return false;
+    const int64_t i0 = (k - c.kfirst) * 32;
+    const int64_t rem = c.len - i0;
+    m.nvalid = rem >= 32 ? 32 : (int)rem;
+    m.obase = c.off + i0;
+    m.li = c.li;
+    return true;
+}
+
+// majority vote with margin on 32 bit-sliced counts: masks of the elements that decode to +S_t and -S_t
+__device__ __forceinline__ void vote_masks(const ReduceParams &p, int W, const SlicedCounter &cpv, const SlicedCounter &cnv,
+                                           int nvalid, uint32_t &dpos, uint32_t &dneg) {
+    if (p.ternary) {
+        // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
+        uint32_t b[9];
+        sliced_add_const(cnv.c, p.margin, b);
+        dpos = sliced_gt(cpv.c, b);
+        sliced_add_const(cpv.c, p.margin, b);
+        dneg = sliced_gt(cnv.c, b);
+    } else {
+        // G-Binary: cneg = W - cpos; D = 2 cpos - W.  d+ : cpos > floor((W+m)/2);
+        // d- : cpos < ceil((W-m)/2)  (never if W <= m)
+        uint32_t b[9], a9[9];
+        const_planes((W + p.margin) >> 1, b);
+        dpos = sliced_gt(cpv.c, b);
+        const int k2 = (W > p.margin) ? (W - p.margin + 1) >> 1 : 0;
+        // k2 > cpos  <=>  const(k2) > cpos : compare with roles swapped
+        uint32_t ka[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { ka[q] = ((k2 >> q) & 1) ? 0xffffffffu : 0u; a9[q] = cpv.c[q]; }
+        a9[8] = 0u;
+        dneg = sliced_gt(ka, a9);
+    }
+    const uint32_t vmask = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
+    dpos &= vmask;
+    dneg &= vmask;
+}
+
+// A (converged) warp holding 32 consecutive word positions k0 .. k0+31 (lane = word) computes the scales of
+// the tensors those words touch and writes out = S_t * d (and the counts, when asked for).
+template <bool WRITE_COUNTS>
+__device__ __forceinline__ void write_back(const ReduceParams &p, const PlanView &pv, int W, int lane, int64_t k,
+                                           const WordMeta &m, bool hit, TensorCache &tc, uint32_t dpos, uint32_t dneg,
+                                           const SlicedCounter &cpv, const SlicedCounter &cnv, const float4 *s_dtab) {
+    float S = tc.S;
+    if (!hit) {
+        S = 0.f;
+        // one cooperative scale per distinct tensor among the warp's words (usually one)
+        const int li_lo = __shfl_sync(0xffffffffu, m.li, 0);
+        int li_hi = m.li;
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) li_hi = max(li_hi, __shfl_xor_sync(0xffffffffu, li_hi, d));
+        for (int li = li_lo; li >= 0 && li <= li_hi; ++li) {
+            const int t = __ldg(pv.lt_index + li);
+            const float St = warp_tensor_scale(p.abs_sum, W, p.T, t, __ldg(p.len + t), lane);
+            if (m.li == li) S = St;
+            const int64_t kfirst = __ldg(pv.lt_woff + li);
+            if (lane == 0 && kfirst >= k && kfirst < k + 32) {      // this warp holds the tensor's first word
+                pv.scale[t] = St;
+                if (p.scale_out) p.scale_out[t] = St;
+            }
+            if (li == li_hi) {                                      // remember the last tensor seen (warp-uniform)
+                tc.li = li;
+                tc.kfirst = kfirst;
+                tc.kend = __ldg(pv.lt_woff + li + 1);
+                tc.len = __ldg(p.len + t);
+                tc.off = __ldg(p.off + t);
+                tc.S = St;
+            }
+        }
+    }
+    // Fast write-back: the warp's 32 words are 1024 consecutive, 16-byte-aligned elements of ONE tensor.
+    // Each thread turns its two masks into 8 direction bytes (low nibble +, high nibble -); a byte
+    // indexes a shared-memory table of float4 directions, and every store writes 512 contiguous bytes.
+    const int64_t ob0 = __shfl_sync(0xffffffffu, m.obase, 0);
+    const bool fast = !WRITE_COUNTS && __all_sync(0xffffffffu, m.nvalid == 32 && m.obase == ob0 + 32 * lane) &&
+                      ((ob0 & 3) == 0);
+    if (fast) {
+        auto spread = [](uint32_t x) {           // 4 nibbles of a 16-bit value -> low nibbles of 4 bytes
+            x = (x | (x << 8)) & 0x00ff00ffu;
+            return (x | (x << 4)) & 0x0f0f0f0fu;
+        };
+        const uint32_t lo = spread(dpos & 0xffffu) | (spread(dneg & 0xffffu) << 4);
+        const uint32_t hi = spread(dpos >> 16) | (spread(dneg >> 16) << 4);
+        const float S0 = __shfl_sync(0xffffffffu, S, 0);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            // store j covers elements j*128 + lane*4 .. +3 = byte (lane & 7) of thread j*4 + (lane >> 3)
+            const int src = j * 4 + (lane >> 3);
+            const uint32_t wl = __shfl_sync(0xffffffffu, lo, src), wh = __shfl_sync(0xffffffffu, hi, src);
+            const uint32_t d = (((lane & 4) ? wh : wl) >> (8 * (lane & 3))) & 0xffu;
+            float4 v = s_dtab[d];
+            v.x = __fmul_rn(S0, v.x); v.y = __fmul_rn(S0, v.y);
+            v.z = __fmul_rn(S0, v.z); v.w = __fmul_rn(S0, v.w);
+            __stcs(reinterpret_cast<float4 *>(p.out + ob0 + j * 128 + lane * 4), v);
+        }
+        return;
+    }
+    // general write-back (tensor boundaries, ragged words, count outputs): iteration j handles the word of lane j
+#pragma unroll 4
+    for (int j = 0; j < 32; ++j) {
+        const int nv = __shfl_sync(0xffffffffu, m.nvalid, j);
+        if (nv == 0) continue;                               // warp-uniform
+        const uint32_t dp = __shfl_sync(0xffffffffu, dpos, j);
+        const uint32_t dn = __shfl_sync(0xffffffffu, dneg, j);
+        const int64_t ob = __shfl_sync(0xffffffffu, m.obase, j);
+        const float Sj = __shfl_sync(0xffffffffu, S, j);
+        const int d = (int)((dp >> lane) & 1u) - (int)((dn >> lane) & 1u);
+        if (lane < nv) p.out[ob + lane] = __fmul_rn(Sj, (float)d);
+        if (WRITE_COUNTS) {
+            uint32_t c1 = 0u, c2 = 0u;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                c1 |= ((__shfl_sync(0xffffffffu, cpv.c[b], j) >> lane) & 1u) << b;
+                c2 |= ((__shfl_sync(0xffffffffu, cnv.c[b], j) >> lane) & 1u) << b;
+            }
+            if (!p.ternary) c2 = (uint32_t)W - c1;
+            if (lane < nv) {
+                if (p.cpos) p.cpos[ob + lane] = (uint8_t)c1;
+                if (p.cneg) p.cneg[ob + lane] = (uint8_t)c2;
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ void fill_direction_table(float4 *s_dtab, int i) {   // i in [0, 256)
+    s_dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
+                            (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
+}
+
+// CTA 0 publishes the scales of the tensors that own no word (the others are published by the warp that
+// holds the tensor's first word)
+__device__ __forceinline__ void publish_wordless_scales(const ReduceParams &p, const PlanView &pv, int W, int nthreads) {
+    if (blockIdx.x != 0) return;
+    for (int t = threadIdx.x; t < p.T; t += nthreads) {
+        const bool isL = p.route[t] == NF_ROUTE_L;
+        if (isL && p.len[t] > 0) continue;
+        const float S0 = isL ? tensor_scale(p.abs_sum, W, p.T, t, p.len[t]) : 0.f;
+        pv.scale[t] = S0;
+        if (p.scale_out) p.scale_out[t] = S0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3, register-staged variant: one thread walks the W words of its word position with plain loads.
+// Used for the level-2 merge of NEXT-1 (MERGE), for planes the bulk-copy engine cannot take (rows not
+// 16-byte aligned) and as the A/B comparator of the ring kernel below (NF_CR_LDG=1).
 // resident CTAs per SM of the deep-round variant: 3 (80 registers, no spills) measured 20-25 % faster than 2
 // at W >= 32 (a thread walks W serially, so the bytes in flight per SM come from occupancy)
+// ---------------------------------------------------------------------------------------------
 #ifndef NF_CR_MINB
 #define NF_CR_MINB 3
 #endif
 template <bool WRITE_COUNTS, bool MERGE, int ROUND>
 __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_reduce_kernel(const ReduceParams p) {
     __shared__ float4 s_dtab[256];          // byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
-    {
-        const int i = threadIdx.x;          // kRThreads == 256
-        s_dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
-                                (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
-    }
+    fill_direction_table(s_dtab, threadIdx.x);      // kRThreads == 256
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     const int64_t Wd = pv.hdr->Wd;
@@ -156,34 +336,19 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
     __syncthreads();                        // direction table
     // Scales are computed warp by warp for the tensors a warp's 32 words touch (no CTA-wide serial
     // prologue: at W = 128 a single thread summing 128 L2 round trips per tensor used to stall every
-    // CTA at a barrier). CTA 0 publishes the scales of the tensors that own no word.
-    if (blockIdx.x == 0) {
-        for (int t = threadIdx.x; t < p.T; t += kRThreads) {
-            const bool isL = p.route[t] == NF_ROUTE_L;
-            if (isL && p.len[t] > 0) continue;
-            const float S0 = isL ? tensor_scale(p.abs_sum, W, p.T, t, p.len[t]) : 0.f;
-            pv.scale[t] = S0;
-            if (p.scale_out) p.scale_out[t] = S0;
-        }
-    }
+    // CTA at a barrier).
+    publish_wordless_scales(p, pv, W, kRThreads);
+    TensorCache tc{-1, 0, 0, 0, 0, 0.f};
 
     for (int64_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
         const int64_t k = chunk * kRThreads + threadIdx.x;      // global word position
         uint32_t dpos = 0u, dneg = 0u;
-        int nvalid = 0;
-        int64_t obase = 0;
-        float S = 0.f;
-        int my_li = -1;
         SlicedCounter cpv, cnv;
         cpv.clear(); cnv.clear();
+        WordMeta m{0, -1, 0};
+        const bool hit = cached_meta(tc, k, lane, m);
+        if (!hit) m = word_meta(p, pv, nL, Wd, k);
         if (k < Wd) {
-            const int li = upper_tensor<int64_t>(pv.lt_woff, nL, k);
-            const int t = __ldg(pv.lt_index + li);
-            const int64_t i0 = (k - __ldg(pv.lt_woff + li)) * 32;  // tensor-relative first element
-            const int64_t rem = __ldg(p.len + t) - i0;
-            nvalid = rem >= 32 ? 32 : (int)rem;
-            obase = __ldg(p.off + t) + i0;
-            my_li = li;
             if (MERGE) {
                 // NEXT-1 level 2: sum of the G groups' bit-sliced partial counts
                 for (int g = 0; g < p.G; ++g) {
@@ -202,100 +367,132 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
             } else {
                 count_words2<false, ROUND>(p.P + k, p.N, p.plane_stride, W, cpv, cnv);
             }
-            if (p.ternary) {
-                // d+ = cpos > cneg + m ; d- = cneg > cpos + m      (D = cpos - cneg vs margin)
-                uint32_t b[9];
-                sliced_add_const(cnv.c, p.margin, b);
-                dpos = sliced_gt(cpv.c, b);
-                sliced_add_const(cpv.c, p.margin, b);
-                dneg = sliced_gt(cnv.c, b);
-            } else {
-                // G-Binary: cneg = W - cpos; D = 2 cpos - W.  d+ : cpos > floor((W+m)/2);
-                // d- : cpos < ceil((W-m)/2)  (never if W <= m)
-                uint32_t b[9], a9[9];
-                const_planes((W + p.margin) >> 1, b);
-                dpos = sliced_gt(cpv.c, b);
-                const int k2 = (W > p.margin) ? (W - p.margin + 1) >> 1 : 0;
-                // k2 > cpos  <=>  const(k2) > cpos : compare with roles swapped
-                uint32_t ka[8];
-#pragma unroll
-                for (int q = 0; q < 8; ++q) { ka[q] = ((k2 >> q) & 1) ? 0xffffffffu : 0u; a9[q] = cpv.c[q]; }
-                a9[8] = 0u;
-                dneg = sliced_gt(ka, a9);
-            }
-            const uint32_t vmask = nvalid >= 32 ? 0xffffffffu : ((1u << nvalid) - 1u);
-            dpos &= vmask;
-            dneg &= vmask;
+            vote_masks(p, W, cpv, cnv, m.nvalid, dpos, dneg);
         }
-        {
-            // one cooperative scale per distinct tensor among the warp's words (usually one)
-            const int li_lo = __shfl_sync(0xffffffffu, my_li, 0);
-            int li_hi = my_li;
-#pragma unroll
-            for (int d = 16; d >= 1; d >>= 1) li_hi = max(li_hi, __shfl_xor_sync(0xffffffffu, li_hi, d));
-            for (int li = li_lo; li >= 0 && li <= li_hi; ++li) {
-                const int t = __ldg(pv.lt_index + li);
-                const float St = warp_tensor_scale(p.abs_sum, W, p.T, t, __ldg(p.len + t), lane);
-                if (my_li == li) S = St;
-                const int64_t kfirst = __ldg(pv.lt_woff + li);
-                if (lane == 0 && kfirst >= k && kfirst < k + 32) {      // this warp holds the tensor's first word
-                    pv.scale[t] = St;
-                    if (p.scale_out) p.scale_out[t] = St;
+        write_back<WRITE_COUNTS>(p, pv, W, lane, k, m, hit, tc, dpos, dneg, cpv, cnv, s_dtab);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3, ring variant (the default). The endpoint's service rate under fan-in W is an
+// HBM-streaming problem: p*W rows of packed words per word position. A thread that walks its W words
+// with plain loads has the bytes in flight capped by its registers; here a producer lane issues
+// one-dimensional bulk async copies (cp.async.bulk, the TMA engine; 1 KB = 256 words of one worker's
+// plane per copy, L2 evict-first: the planes are read once) into a ring of stages of 16 rows that
+// complete on the stage's "full" mbarrier, and 8 consumer warps (thread = word position) add each
+// stage into their bit-sliced counters (conflict-free LDS.32), release it on the "empty" mbarrier
+// and, once the W workers are in, vote and write back exactly as above. A stage holds 8 workers'
+// P rows and N rows (G-Ternary) or 16 workers' P rows (G-Binary). The bytes in flight per SM
+// (NF_CRQ_MINB CTAs x NF_CRQ_STAGES x 16 KB) do not depend on registers or on W; the write-back of
+// unit u overlaps the copies of units u+1 ...
+// ---------------------------------------------------------------------------------------------
+#ifndef NF_CRQ_STAGES
+#define NF_CRQ_STAGES 4
+#endif
+#ifndef NF_CRQ_MINB
+#define NF_CRQ_MINB 3
+#endif
+constexpr int kQWords = 256;                       // word positions per unit = consumer threads
+constexpr int kQRows = 16;                         // rows (worker, plane) per stage
+constexpr int kQStageWords = kQRows * kQWords;     // 16 KB
+constexpr int kQStages = NF_CRQ_STAGES;
+constexpr int kQThreads = kQWords + 32;            // + producer warp
+constexpr int kQHdr = 256 + 4096;                  // mbarriers, direction table
+constexpr size_t kQSmem = kQHdr + (size_t)kQStages * kQStageWords * 4;
+static_assert(2 * kQStages * 8 <= 256, "mbarriers fit the header");
+
+template <bool WRITE_COUNTS>
+__global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kernel(const __grid_constant__ ReduceParams p) {
+    extern __shared__ __align__(128) unsigned char q_smem[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(q_smem);
+    uint64_t *empty = full + kQStages;
+    float4 *s_dtab = reinterpret_cast<float4 *>(q_smem + 256);
+    uint32_t *ring = reinterpret_cast<uint32_t *>(q_smem + kQHdr);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+        for (int s = 0; s < kQStages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kQWords / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (tid < 256) fill_direction_table(s_dtab, tid);
+    __syncthreads();
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    const int64_t Wd = pv.hdr->Wd;
+    const int nL = pv.hdr->nL;
+    const int W = p.W;
+    const bool ternary = p.ternary != 0;
+    const int64_t n_units = (Wd + kQWords - 1) / kQWords;
+    const int wadv = ternary ? 8 : 16;             // workers per stage
+    const int n_stg = (W + wadv - 1) / wadv;       // stages per unit
+
+    if (warp == kQWords / 32) {
+        // ---- producer ----
+        if (lane != 0) return;
+        const uint64_t pol = policy_evict_first();
+        int st = 0;
+        uint32_t ph = 0;
+        for (int64_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+            const int64_t k0 = unit * kQWords;
+            const int64_t left = Wd - k0;
+            // whole 16-byte chunks (plane_stride is a multiple of 4 words: the last chunk stays inside the row)
+            const uint32_t bytes = (uint32_t)(((left >= kQWords ? kQWords : (int)left) + 3) & ~3) * 4u;
+            for (int g = 0; g < n_stg; ++g) {
+                const int w0 = g * wadv;
+                const int nw = min(wadv, W - w0);
+                mbar_wait(empty + st, ph ^ 1u);                        // first lap: passes at once
+                uint32_t *dst = ring + (size_t)st * kQStageWords;
+                if (ternary) {
+                    mbar_expect_tx(full + st, 2u * (uint32_t)nw * bytes);
+                    for (int w = 0; w < nw; ++w) {
+                        const size_t o = (size_t)(w0 + w) * p.plane_stride + k0;
+                        bulk_g2s(dst + w * kQWords, p.P + o, bytes, full + st, pol);
+                        bulk_g2s(dst + (8 + w) * kQWords, p.N + o, bytes, full + st, pol);
+                    }
+                } else {
+                    mbar_expect_tx(full + st, (uint32_t)nw * bytes);
+                    for (int w = 0; w < nw; ++w)
+                        bulk_g2s(dst + w * kQWords, p.P + (size_t)(w0 + w) * p.plane_stride + k0, bytes, full + st, pol);
                 }
+                if (++st == kQStages) { st = 0; ph ^= 1u; }
             }
         }
-        // Fast write-back: the warp's 32 words are 1024 consecutive, 16-byte-aligned elements of ONE tensor.
-        // Each thread turns its two masks into 8 direction bytes (low nibble +, high nibble -); a byte
-        // indexes a shared-memory table of float4 directions, and every store writes 512 contiguous bytes.
-        const int64_t ob0 = __shfl_sync(0xffffffffu, obase, 0);
-        const bool fast = !WRITE_COUNTS && __all_sync(0xffffffffu, nvalid == 32 && obase == ob0 + 32 * lane) &&
-                          ((ob0 & 3) == 0);
-        if (fast) {
-            auto spread = [](uint32_t x) {           // 4 nibbles of a 16-bit value -> low nibbles of 4 bytes
-                x = (x | (x << 8)) & 0x00ff00ffu;
-                return (x | (x << 4)) & 0x0f0f0f0fu;
-            };
-            const uint32_t lo = spread(dpos & 0xffffu) | (spread(dneg & 0xffffu) << 4);
-            const uint32_t hi = spread(dpos >> 16) | (spread(dneg >> 16) << 4);
-            const float S0 = __shfl_sync(0xffffffffu, S, 0);
+        return;
+    }
+
+    // ---- consumers: thread = word position ----
+    publish_wordless_scales(p, pv, W, kQWords);
+    int st = 0;
+    uint32_t ph = 0;
+    TensorCache tc{-1, 0, 0, 0, 0, 0.f};
+    for (int64_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
+        const int64_t k = unit * kQWords + tid;
+        WordMeta m{0, -1, 0};
+        const bool hit = cached_meta(tc, k, lane, m);
+        if (!hit) m = word_meta(p, pv, nL, Wd, k);                     // overlaps the copies in flight
+        SlicedCounter cpv, cnv;
+        cpv.clear(); cnv.clear();
+        for (int g = 0; g < n_stg; ++g) {
+            const int left = W - g * wadv;                             // workers from this stage on
+            const int na = min(8, left);                               // rows 0..7 in use
+            const int nb = ternary ? na : min(8, left - 8);            // rows 8..15 in use (may be <= 0)
+            mbar_wait(full + st, ph);
+            const uint32_t *src = ring + (size_t)st * kQStageWords + tid;
+            uint32_t xa[8], xb[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                // store j covers elements j*128 + lane*4 .. +3 = byte (lane & 7) of thread j*4 + (lane >> 3)
-                const int src = j * 4 + (lane >> 3);
-                const uint32_t wl = __shfl_sync(0xffffffffu, lo, src), wh = __shfl_sync(0xffffffffu, hi, src);
-                const uint32_t d = (((lane & 4) ? wh : wl) >> (8 * (lane & 3))) & 0xffu;
-                float4 v = s_dtab[d];
-                v.x = __fmul_rn(S0, v.x); v.y = __fmul_rn(S0, v.y);
-                v.z = __fmul_rn(S0, v.z); v.w = __fmul_rn(S0, v.w);
-                __stcs(reinterpret_cast<float4 *>(p.out + ob0 + j * 128 + lane * 4), v);
+            for (int i = 0; i < 8; ++i) {
+                xa[i] = i < na ? src[i * kQWords] : 0u;
+                xb[i] = i < nb ? src[(8 + i) * kQWords] : 0u;
             }
-            continue;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + st);                    // every lane's reads of the stage are done
+            cpv.add8(xa);
+            if (ternary) cnv.add8(xb);
+            else if (nb > 0) cpv.add8(xb);
+            if (++st == kQStages) { st = 0; ph ^= 1u; }
         }
-        // general write-back (tensor boundaries, ragged words, count outputs): iteration j handles the word of lane j
-#pragma unroll 4
-        for (int j = 0; j < 32; ++j) {
-            const int nv = __shfl_sync(0xffffffffu, nvalid, j);
-            if (nv == 0) continue;                               // warp-uniform
-            const uint32_t dp = __shfl_sync(0xffffffffu, dpos, j);
-            const uint32_t dn = __shfl_sync(0xffffffffu, dneg, j);
-            const int64_t ob = __shfl_sync(0xffffffffu, obase, j);
-            const float Sj = __shfl_sync(0xffffffffu, S, j);
-            const int d = (int)((dp >> lane) & 1u) - (int)((dn >> lane) & 1u);
-            if (lane < nv) p.out[ob + lane] = __fmul_rn(Sj, (float)d);
-            if (WRITE_COUNTS) {
-                uint32_t c1 = 0u, c2 = 0u;
-#pragma unroll
-                for (int b = 0; b < 8; ++b) {
-                    c1 |= ((__shfl_sync(0xffffffffu, cpv.c[b], j) >> lane) & 1u) << b;
-                    c2 |= ((__shfl_sync(0xffffffffu, cnv.c[b], j) >> lane) & 1u) << b;
-                }
-                if (!p.ternary) c2 = (uint32_t)W - c1;
-                if (lane < nv) {
-                    if (p.cpos) p.cpos[ob + lane] = (uint8_t)c1;
-                    if (p.cneg) p.cneg[ob + lane] = (uint8_t)c2;
-                }
-            }
-        }
+        uint32_t dpos = 0u, dneg = 0u;
+        if (k < Wd) vote_masks(p, W, cpv, cnv, m.nvalid, dpos, dneg);
+        write_back<WRITE_COUNTS>(p, pv, W, lane, k, m, hit, tc, dpos, dneg, cpv, cnv, s_dtab);
     }
 }
 
@@ -409,12 +606,31 @@ static int grid_for(int64_t units, int per_sm) {
     return (int)(g < 1 ? 1 : g);
 }
 
+template <bool WRITE_COUNTS>
+static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_t s) {
+    static bool attr_set = false;                    // per template instance
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(count_reduce_ring_kernel<WRITE_COUNTS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kQSmem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int grid = grid_for(units, NF_CRQ_MINB);
+    count_reduce_ring_kernel<WRITE_COUNTS><<<grid, kQThreads, kQSmem, s>>>(p);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s) {
     const int64_t max_words = n / 32 + p.T;
     const int64_t chunks = (max_words + kRThreads - 1) / kRThreads;
     const int grid = grid_for(chunks, 8);
     const bool counts = p.cpos || p.cneg;
     const bool small = !p.cnt_pos && p.W <= 16;              // shallow rounds, 4 CTAs per SM
+    static const bool force_ldg = getenv("NF_CR_LDG") != nullptr;       // A/B aid: register-staged kernel
+    // the bulk copies need 16-byte-aligned rows: P, N are (nf_sign_count_reduce checks), so plane_stride % 4 == 0
+    if (!p.cnt_pos && !force_ldg && (p.plane_stride & 3) == 0)
+        return counts ? launch_ring<true>(p, (max_words + kQWords - 1) / kQWords, s)
+                      : launch_ring<false>(p, (max_words + kQWords - 1) / kQWords, s);
     if (p.cnt_pos) {
         if (counts) count_reduce_kernel<true, true, 16><<<grid, kRThreads, 0, s>>>(p);
         else count_reduce_kernel<false, true, 16><<<grid, kRThreads, 0, s>>>(p);
