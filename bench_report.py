@@ -11,7 +11,9 @@ all-eligible bucket: (i) nf_sign_count_reduce alone on pre-packed planes, (ii) n
 nf_sign_count_reduce, (iii) the fused call, (iv) nf_fp32_reduce on the same W x n — the paper's
 "endpoint service rate vs fan-in" question measured on one B200.
 Timing: median of CUDA-event-timed iterations after 3 warm-ups, inputs resident in HBM. Buckets
-smaller than L2 are rotated over enough copies to exceed 126 MB (stated per row).
+smaller than L2 are rotated over enough copies to exceed 126 MB (stated per row). Tables 2-4 time the
+calls replayed from a CUDA graph (a call shorter than the ~15 us Python/ctypes needs to issue it is
+otherwise host-bound); table 1 gives both the eager and the graph-replay time.
 No oracle is used here (parity is the job of tests/); this only times the CUDA path.
 """
 from __future__ import annotations
@@ -38,19 +40,37 @@ def measured_peak():
         return 6650.0
 
 
-def time_fn(fn, iters, warmup=3, reps=1):
+def time_fn(fn, iters, warmup=3, reps=1, graph=False):
     """Median over `iters` samples of the time of `reps` back-to-back calls, per call (ms). reps > 1 keeps the
-    launch latency of a short call from being counted as its duration."""
+    launch latency of a short call from being counted as its duration. graph=True captures the `reps` calls into
+    a CUDA graph and times its replay: the calls then follow each other on the device without waiting for the
+    host, which otherwise bounds calls shorter than the ~15 us Python/ctypes takes to issue one."""
     import torch
     for _ in range(warmup):
         fn()
     torch.cuda.synchronize()
+    run = None
+    if graph:
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):          # the library's lazy one-time setup must not happen under capture
+            fn()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for _ in range(reps):
+                fn()
+        g.replay()
+        torch.cuda.synchronize()
+        run = g.replay
     ts = []
     for _ in range(iters):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(reps):
-            fn()
+        if run is not None:
+            run()
+        else:
+            for _ in range(reps):
+                fn()
         e1.record()
         e1.synchronize()
         ts.append(e0.elapsed_time(e1) / reps)
@@ -83,9 +103,10 @@ def run_config(cfg, iters, dev):
         for g, bb in zip(G, BB):
             bb.aggregate(g, g.shape[1], (1, 0, 1), nf.MODE_GTERNARY)
     ms = time_fn(step, iters) / copies
+    ms_graph = time_fn(step, iters, graph=True) / copies
     del G, BB
     torch.cuda.empty_cache()
-    return ms, copies
+    return ms, ms_graph, copies
 
 
 def table_configs(args, dev, peak):
@@ -94,19 +115,20 @@ def table_configs(args, dev, peak):
     rows = []
     for nme in names:
         cfg = shapes.get(nme)
-        ms, copies = run_config(cfg, args.iters if cfg.n_params < 5e8 else max(5, args.iters // 4), dev)
-        rows.append((cfg.name, cfg.W, cfg.n_params, len(cfg.buckets), ms, copies, fused_bytes(cfg)))
+        ms, msg, copies = run_config(cfg, args.iters if cfg.n_params < 5e8 else max(5, args.iters // 4), dev)
+        rows.append((cfg.name, cfg.W, cfg.n_params, len(cfg.buckets), ms, msg, copies, fused_bytes(cfg)))
     for n in (131_072, 524_288):
         cfg = shapes.paper_local_count(n)
-        ms, copies = run_config(cfg, args.iters, dev)
-        rows.append((cfg.name + " (PAPER L456 shape)", cfg.W, cfg.n_params, 1, ms, copies, fused_bytes(cfg)))
+        ms, msg, copies = run_config(cfg, args.iters, dev)
+        rows.append((cfg.name + " (PAPER L456 shape)", cfg.W, cfg.n_params, 1, ms, msg, copies, fused_bytes(cfg)))
     out = ["| config | W | n (elements) | buckets | time / step | FP32-grad GB/s | elements/s | algorithmic bytes | % of 8000 GB/s | "
-           f"% of {peak:.1f} GB/s | note |", "|---|---|---|---|---|---|---|---|---|---|---|"]
-    for name, W, n, nb, ms, copies, ab in rows:
+           f"% of {peak:.1f} GB/s | same calls replayed from a CUDA graph | note |", "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    for name, W, n, nb, ms, msg, copies, ab in rows:
         t = ms * 1e-3
         note = f"{copies} rotating copies (input < 2 x L2)" if copies > 1 else "input > L2"
         out.append(f"| {name} | {W} | {n:,} | {nb} | {ms * 1e3:.1f} us | {4 * W * n / t / 1e9:.1f} | {n / t:.3e} | "
-                   f"{ab / 1e6:.1f} MB | {100 * ab / t / 1e9 / NOMINAL:.1f} | {100 * ab / t / 1e9 / peak:.1f} | {note} |")
+                   f"{ab / 1e6:.1f} MB | {100 * ab / t / 1e9 / NOMINAL:.1f} | {100 * ab / t / 1e9 / peak:.1f} | "
+                   f"{msg * 1e3:.1f} us, {100 * ab / (msg * 1e-3) / 1e9 / peak:.1f} % | {note} |")
     return "\n".join(out)
 
 
@@ -115,7 +137,7 @@ def table_sweep(args, dev, peak):
     from paper_2606_25759_b200 import BucketBuffers, binding as nf
     from workloads import shapes, gen
     out = ["| W | planes in (MB) | (i) count-reduce alone | (ii) pack + count-reduce | (iii) fused | (iv) fp32_reduce | "
-           "copies |", "|---|---|---|---|---|---|---|"]
+           "rotating copies (i) / (ii)-(iv) |", "|---|---|---|---|---|---|---|"]
     for W in ([args.sweep_w] if args.sweep_w else shapes.SWEEP_W):
         cfg = shapes.sweep(W)
         b = cfg.buckets[0]
@@ -127,12 +149,19 @@ def table_sweep(args, dev, peak):
         for g, bb in zip(G, BB):
             bb.route_bucket((1, 0, 1))
             bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
-        torch.cuda.synchronize()
         plane_bytes = 2 * W * n // 8
+        # (i) reads only the planes: its own rotating set, sized on the bytes a3 touches (planes + output)
+        rcopies = max(1, -(-2 * L2_BYTES // (plane_bytes + 4 * n)))
+        RB = BB[:rcopies] + [BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=False)
+                             for _ in range(max(0, rcopies - copies))]
+        for rb in RB[copies:]:
+            rb.route_bucket((1, 0, 1))
+            rb.sign_pack(G[0], G[0].shape[1], nf.MODE_GTERNARY)
+        torch.cuda.synchronize()
 
         def reduce_only():
-            for bb in BB:
-                bb.sign_count_reduce(nf.MODE_GTERNARY)
+            for rb in RB:
+                rb.sign_count_reduce(nf.MODE_GTERNARY)
 
         def pack_reduce():
             for g, bb in zip(G, BB):
@@ -154,10 +183,11 @@ def table_sweep(args, dev, peak):
         cells = []
         for fn, own in ((reduce_only, plane_bytes + 4 * n), (pack_reduce, in_bytes + 2 * plane_bytes + 4 * n),
                         (fused, in_bytes + plane_bytes + n // 2 + 4 * n), (fp32, in_bytes + 4 * n)):
-            t = time_fn(fn, args.iters) / copies * 1e-3
+            ncp = rcopies if fn is reduce_only else copies
+            t = time_fn(fn, args.iters, reps=max(1, 8 // ncp), graph=True) / ncp * 1e-3
             cells.append(f"{t * 1e6:.1f} us, {in_bytes / t / 1e9:.0f} GB/s FP32-equiv, {100 * own / t / 1e9 / peak:.0f} % HBM on own bytes")
-        out.append(f"| {W} | {plane_bytes / 1e6:.1f} | " + " | ".join(cells) + f" | {copies} |")
-        del G, BB, FB
+        out.append(f"| {W} | {plane_bytes / 1e6:.1f} | " + " | ".join(cells) + f" | {rcopies} / {copies} |")
+        del G, BB, FB, RB
         torch.cuda.empty_cache()
     return "\n".join(out)
 
@@ -207,7 +237,7 @@ def table_hier(args, dev, peak):
             for gi in range(G):
                 nf.nf_partial_count(bb.P[gi * Wg:], bb.N[gi * Wg:], bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[gi], cn[gi], cs)
             level2()
-        t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5)) * 1e3
+        t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5), reps=1 if f is stock else 4, graph=True) * 1e3
                               for f in (level1, level2, flat, stock, hier_all))
         packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
         out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us | "
@@ -244,7 +274,7 @@ def table_five_calls(args, dev, peak):
                  ("nf_health_stats (a4b)", lambda: bb.health_stats(g, g.shape[1]), 4 * W * n),
                  ("nf_aggregate_bucket (fused)", lambda: bb.aggregate(g, g.shape[1]), 4 * W * n + planes + e // 2 + 4 * n)]
         for name, fn, own in calls:
-            t = time_fn(fn, args.iters, reps=8) * 1e-3
+            t = time_fn(fn, args.iters, reps=8, graph=True) * 1e-3
             pct = f"{100 * own / t / 1e9 / peak:.0f}" if own > 1e6 else "- (O(T) latency)"
             out.append(f"| {bi} (n = {n:,}, {100 * e / n:.0f} % low-bit) | {name} | {t * 1e6:.1f} us | {own / 1e6:.1f} MB | {pct} |")
         del g, bb
@@ -269,7 +299,10 @@ def main():
     dev = "cuda"
     peak = measured_peak()
     parts = [f"GPU: {torch.cuda.get_device_name(0)}; measured HBM copy peak {peak:.1f} GB/s; "
-             f"median of {args.iters} CUDA-event-timed iterations after 3 warm-ups; mode G-Ternary, planes and health on.", ""]
+             f"median of {args.iters} CUDA-event-timed iterations after 3 warm-ups; mode G-Ternary, planes and health on. "
+             "The stand-alone calls, the sweep and the hierarchical table are timed as replays of a CUDA graph holding the "
+             "calls back to back (issued one by one from Python, a call shorter than ~15 us is host-bound); the config "
+             "table gives both.", ""]
     want = lambda name: args.only in ("", name)
     if want("configs") and not args.skip_configs:
         parts += ["### Configs through nf_aggregate_bucket (route + fused kernel per bucket)", "", table_configs(args, dev, peak), ""]
@@ -280,7 +313,7 @@ def main():
         parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
     if want("hier"):
         parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
-                  "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange)", "",
+                  "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange; the level-1 and level-2 inputs of W = 32 and one node's planes at W = 128 are smaller than L2 and stay resident across replays, so those cells are L2-bandwidth figures)", "",
                   table_hier(args, dev, peak), ""]
     text = "\n".join(parts)
     print(text)

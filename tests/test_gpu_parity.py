@@ -152,6 +152,32 @@ def test_count_reduce_without_count_outputs(name, mode):
         compare(bb, ref, cfg.W, mode, check_counts=False, what=f"{cfg.name} bucket {b.index} 5-call, no counts")
 
 
+@pytest.mark.parametrize("stride_pad", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("counts", [False, True])
+@pytest.mark.parametrize("name,mode", [("tiny", O.MODE_GTERNARY), ("sweep_w32", O.MODE_GBINARY), ("vit_b16", O.MODE_GTERNARY)])
+def test_count_reduce_both_kernels(name, mode, counts, stride_pad):
+    """nf_sign_count_reduce has two kernels: the bulk-copy ring (plane rows 16-byte aligned, i.e. plane_stride a
+    multiple of 4 words) and the register-staged one (any plane_stride). Both must give the oracle's result, with
+    and without count outputs; the ring's last unit copies whole 16-byte chunks up to the row's end."""
+    cfg = shapes.get(name, small=(name != "tiny"))
+    for b in cfg.buckets:
+        g = gen.gen_bucket(cfg, b, DEV)
+        ref = O.aggregate_bucket(np.ascontiguousarray(_np(g)[:, :b.n]), b.off, b.length, b.elig, (1, 0, 1), mode)
+        Wd = sum((int(l) + 31) // 32 for l, e in zip(b.length, b.elig) if e)
+        ps = (Wd + 3) // 4 * 4 + stride_pad
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=True, counts=counts, health=True,
+                           plane_stride=ps)
+        assert bb.plane_stride == max(ps, 4)
+        bb.out.fill_(-77.0)
+        bb.route_bucket((1, 0, 1))
+        bb.sign_pack(g, g.shape[1], mode)
+        bb.sign_count_reduce(mode)
+        bb.fp32_reduce(g, g.shape[1])
+        bb.health_stats(g, g.shape[1])
+        compare(bb, ref, cfg.W, mode, check_counts=counts,
+                what=f"{cfg.name} bucket {b.index} plane_stride {bb.plane_stride} counts {counts}")
+
+
 @pytest.mark.parametrize("T", [256, 257, 700])
 def test_many_tensor_buckets(T):
     """Buckets around and above the fused kernel's shared-memory metadata capacity (256 tensors): T <= 256 routes
