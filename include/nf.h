@@ -115,6 +115,10 @@ int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
  * s_wt = (float)(abs_sum[w*T+t]/len_t); S_t = (float)(sum_w (double)s_wt / W);
  * out[off_t+i] = S_t * (float)d. Optional: cpos/cneg [n] uint8 at bucket positions (L positions
  * only are written), scale_out[T] (0 for non-L tensors).
+ * Plane rows that are 16-byte aligned (plane_stride a multiple of 4 words) are read with bulk async
+ * copies of whole 16-byte chunks, i.e. up to 3 words past Wd inside the row; any other plane_stride
+ * takes a register-staged kernel with the same results. The call writes the per-tensor scales into
+ * the plan's scratch: calls given the same plan must be ordered on one stream.
  */
 int nf_sign_count_reduce(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int W, int64_t n,
                          const int64_t *off, const int64_t *len, const uint8_t *route,

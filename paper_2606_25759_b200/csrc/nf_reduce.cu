@@ -392,7 +392,10 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
 #ifndef NF_CRQ_MINB
 #define NF_CRQ_MINB 3
 #endif
-constexpr int kQWords = 256;                       // word positions per unit = consumer threads
+#ifndef NF_CRQ_WORDS
+#define NF_CRQ_WORDS 256
+#endif
+constexpr int kQWords = NF_CRQ_WORDS;              // word positions per unit = consumer threads
 constexpr int kQRows = 16;                         // rows (worker, plane) per stage
 constexpr int kQStageWords = kQRows * kQWords;     // 16 KB
 constexpr int kQStages = NF_CRQ_STAGES;
@@ -409,12 +412,14 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     float4 *s_dtab = reinterpret_cast<float4 *>(q_smem + 256);
     uint32_t *ring = reinterpret_cast<uint32_t *>(q_smem + kQHdr);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_launch_dependents();                 // the next kernel's launch and prologue may overlap this kernel
     if (tid == 0) {
         for (int s = 0; s < kQStages; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, kQWords / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (tid < 256) fill_direction_table(s_dtab, tid);
+    for (int i = tid; i < 256; i += kQThreads) fill_direction_table(s_dtab, i);
     __syncthreads();
+    pdl_wait();                              // everything above touched shared memory only
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     const int64_t Wd = pv.hdr->Wd;
@@ -616,8 +621,11 @@ static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_
         attr_set = true;
     }
     const int grid = grid_for(units, NF_CRQ_MINB);
-    count_reduce_ring_kernel<WRITE_COUNTS><<<grid, kQThreads, kQSmem, s>>>(p);
-    return cudaGetLastError();
+    // programmatic stream serialization: the kernel waits (griddepcontrol.wait) for its predecessor on the stream
+    // before it touches global memory; only its launch latency and shared-memory prologue overlap (NF_NO_PDL=1: off)
+    static const bool use_pdl = getenv("NF_NO_PDL") == nullptr;
+    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS>, (unsigned)grid, kQThreads, kQSmem, s, use_pdl, p);
+    return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s) {
