@@ -207,44 +207,62 @@ def table_hier(args, dev, peak):
         b = cfg.buckets[0]
         n = b.n
         g = gen.gen_bucket(cfg, b, dev)
-        bb = BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=False)
-        bb.route_bucket((1, 0, 1))
-        bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
-        torch.cuda.synchronize()
-        Wd = int(bb.summary[nf.SUM_WD])
         Wg = W // G
         B = nf.nf_count_planes(Wg)
+        Wd = (n + 31) // 32
         cs = (Wd + 3) // 4 * 4
-        cp = torch.zeros((G, B, cs), dtype=torch.int32, device=dev)
-        cn = torch.zeros((G, B, cs), dtype=torch.int32, device=dev)
-        for gi in range(G):
-            nf.nf_partial_count(bb.P[gi * Wg:], bb.N[gi * Wg:], bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[gi], cn[gi], cs)
+        # rotating sets of (planes, partial counts, output) so that every timed function streams from HBM, not L2
+        per_copy = 2 * W * Wd * 4 + 2 * G * B * cs * 4 + 4 * n
+        rc = max(1, -(-2 * L2_BYTES // per_copy))
+        BBs, CPs, CNs = [], [], []
+        for _ in range(rc):
+            bb = BucketBuffers(b.off, b.length, b.elig, n, W, dev, planes=True, health=False)
+            bb.route_bucket((1, 0, 1))
+            bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+            BBs.append(bb)
+            CPs.append(torch.zeros((G, B, cs), dtype=torch.int32, device=dev))
+            CNs.append(torch.zeros((G, B, cs), dtype=torch.int32, device=dev))
+        torch.cuda.synchronize()
+        assert int(BBs[0].summary[nf.SUM_WD]) == Wd
 
-        def level1():
-            nf.nf_partial_count(bb.P, bb.N, bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[0], cn[0], cs)
-
-        def level2():
-            nf.nf_partial_count_merge(cp, cn, cs, G, B, W, n, bb.off, bb.len, bb.route, bb.woff, bb.T, nf.MODE_GTERNARY, 0,
-                                      bb.abs_sum, bb.out, None, None, bb.scale, bb.plan)
-
-        def flat():
-            bb.sign_count_reduce(nf.MODE_GTERNARY)
-        def stock():      # NEXT-2 (PAPER L267): every worker receives all W sign streams and counts them itself
-            for _ in range(W):
-                bb.sign_count_reduce(nf.MODE_GTERNARY)
-
-        def hier_all():   # all G nodes count locally, one merge + decode
+        def node_counts(bb, cp, cn):      # level 1 of every node of one copy
             for gi in range(G):
                 nf.nf_partial_count(bb.P[gi * Wg:], bb.N[gi * Wg:], bb.plane_stride, Wg, Wd, nf.MODE_GTERNARY, B, cp[gi], cn[gi], cs)
-            level2()
-        t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5), reps=1 if f is stock else 4, graph=True) * 1e3
-                              for f in (level1, level2, flat, stock, hier_all))
+
+        def merge(bb, cp, cn):
+            nf.nf_partial_count_merge(cp, cn, cs, G, B, W, n, bb.off, bb.len, bb.route, bb.woff, bb.T, nf.MODE_GTERNARY, 0,
+                                      bb.abs_sum, bb.out, None, None, bb.scale, bb.plan)
+        for bb, cp, cn in zip(BBs, CPs, CNs):
+            node_counts(bb, cp, cn)
+
+        def level1():     # rc x G node-local counts
+            for bb, cp, cn in zip(BBs, CPs, CNs):
+                node_counts(bb, cp, cn)
+
+        def level2():
+            for bb, cp, cn in zip(BBs, CPs, CNs):
+                merge(bb, cp, cn)
+
+        def flat():
+            for bb in BBs:
+                bb.sign_count_reduce(nf.MODE_GTERNARY)
+
+        def stock():      # NEXT-2 (PAPER L267): every worker receives all W sign streams and counts them itself
+            for i in range(W):
+                BBs[i % rc].sign_count_reduce(nf.MODE_GTERNARY)
+
+        def hier_all():   # all G nodes count locally, one merge + decode
+            for bb, cp, cn in zip(BBs, CPs, CNs):
+                node_counts(bb, cp, cn)
+                merge(bb, cp, cn)
+        t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5), reps=1, graph=True) * 1e3 / div
+                              for f, div in ((level1, rc * G), (level2, rc), (flat, rc), (stock, 1), (hier_all, rc)))
         packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
         out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us | "
                    f"{packed / (t1 * 1e-6) / 1e9:.0f} GB/s | "
                    + " / ".join("admit" if nf.nf_capacity_guard(n, G, Wg, packed / (t1 * 1e-6), bw, 2)[0] else "FP32"
                                 for bw in (12.5e9, 50e9, 400e9)) + " |")
-        del g, bb, cp, cn
+        del g, bb, cp, cn, BBs, CPs, CNs
         torch.cuda.empty_cache()
     return "\n".join(out)
 
@@ -313,7 +331,7 @@ def main():
         parts += ["### Reducer-capacity sweep (config 5: one 25 MB all-eligible bucket, n = 6,553,600)", "", table_sweep(args, dev, peak), ""]
     if want("hier"):
         parts += ["### NEXT-1 / NEXT-2: two-level hierarchical sign count vs replicated counting of stock packed-sign transport, same bucket "
-                  "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange; the level-1 and level-2 inputs of W = 32 and one node's planes at W = 128 are smaller than L2 and stay resident across replays, so those cells are L2-bandwidth figures)", "",
+                  "(G-Ternary; results identical to the flat reduce; all work of all nodes / workers emulated on ONE GPU, no exchange; every cell rotates over enough copies of the planes, partial counts and output to stream from HBM)", "",
                   table_hier(args, dev, peak), ""]
     text = "\n".join(parts)
     print(text)

@@ -351,16 +351,23 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
         if (k < Wd) {
             if (MERGE) {
                 // NEXT-1 level 2: sum of the G groups' bit-sliced partial counts
-                for (int g = 0; g < p.G; ++g) {
-                    uint32_t xp[8], xn[8];
+                // (two groups' planes in flight per round: up to 32 independent loads per thread)
+                for (int g = 0; g < p.G; g += 2) {
+                    uint32_t xp[2][8], xn[2][8];
 #pragma unroll
-                    for (int b = 0; b < 8; ++b) {
-                        const size_t o = ((size_t)g * p.B + b) * p.count_stride + k;
-                        xp[b] = (b < p.B) ? __ldcs(p.cnt_pos + o) : 0u;
-                        xn[b] = (b < p.B && p.ternary) ? __ldcs(p.cnt_neg + o) : 0u;
+                    for (int u = 0; u < 2; ++u)
+#pragma unroll
+                        for (int b = 0; b < 8; ++b) {
+                            const bool in = b < p.B && g + u < p.G;
+                            const size_t o = ((size_t)(g + u) * p.B + b) * p.count_stride + k;
+                            xp[u][b] = in ? __ldcs(p.cnt_pos + o) : 0u;
+                            xn[u][b] = (in && p.ternary) ? __ldcs(p.cnt_neg + o) : 0u;
+                        }
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        sliced_add(cpv, xp[u]);
+                        if (p.ternary) sliced_add(cnv, xn[u]);
                     }
-                    sliced_add(cpv, xp);
-                    if (p.ternary) sliced_add(cnv, xn);
                 }
             } else if (p.ternary) {
                 count_words2<true, ROUND>(p.P + k, p.N + k, p.plane_stride, W, cpv, cnv);
@@ -404,7 +411,7 @@ constexpr int kQHdr = 256 + 4096;                  // mbarriers, direction table
 constexpr size_t kQSmem = kQHdr + (size_t)kQStages * kQStageWords * 4;
 static_assert(2 * kQStages * 8 <= 256, "mbarriers fit the header");
 
-template <bool WRITE_COUNTS>
+template <bool WRITE_COUNTS, bool MERGE>
 __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kernel(const __grid_constant__ ReduceParams p) {
     extern __shared__ __align__(128) unsigned char q_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(q_smem);
@@ -428,7 +435,9 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     const bool ternary = p.ternary != 0;
     const int64_t n_units = (Wd + kQWords - 1) / kQWords;
     const int wadv = ternary ? 8 : 16;             // workers per stage
-    const int n_stg = (W + wadv - 1) / wadv;       // stages per unit
+    // stages per unit. MERGE (NEXT-1 level 2, PAPER L243 / L267): one stage per group, rows 0..B-1 = the B bit-planes
+    // of the group's partial pos-count, rows 8..8+B-1 = of its neg-count
+    const int n_stg = MERGE ? p.G : (W + wadv - 1) / wadv;
 
     if (warp == kQWords / 32) {
         // ---- producer ----
@@ -446,7 +455,14 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
                 const int nw = min(wadv, W - w0);
                 mbar_wait(empty + st, ph ^ 1u);                        // first lap: passes at once
                 uint32_t *dst = ring + (size_t)st * kQStageWords;
-                if (ternary) {
+                if (MERGE) {
+                    mbar_expect_tx(full + st, (ternary ? 2u : 1u) * (uint32_t)p.B * bytes);
+                    for (int b = 0; b < p.B; ++b) {
+                        const size_t o = ((size_t)g * p.B + b) * p.count_stride + k0;
+                        bulk_g2s(dst + b * kQWords, p.cnt_pos + o, bytes, full + st, pol);
+                        if (ternary) bulk_g2s(dst + (8 + b) * kQWords, p.cnt_neg + o, bytes, full + st, pol);
+                    }
+                } else if (ternary) {
                     mbar_expect_tx(full + st, 2u * (uint32_t)nw * bytes);
                     for (int w = 0; w < nw; ++w) {
                         const size_t o = (size_t)(w0 + w) * p.plane_stride + k0;
@@ -478,8 +494,9 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
         cpv.clear(); cnv.clear();
         for (int g = 0; g < n_stg; ++g) {
             const int left = W - g * wadv;                             // workers from this stage on
-            const int na = min(8, left);                               // rows 0..7 in use
-            const int nb = ternary ? na : min(8, left - 8);            // rows 8..15 in use (may be <= 0)
+            const int na = MERGE ? p.B : min(8, left);                 // rows 0..7 in use
+            const int nb = MERGE ? (ternary ? p.B : 0)
+                                 : (ternary ? na : min(8, left - 8));  // rows 8..15 in use (may be <= 0)
             mbar_wait(full + st, ph);
             const uint32_t *src = ring + (size_t)st * kQStageWords + tid;
             uint32_t xa[8], xb[8];
@@ -490,9 +507,14 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(empty + st);                    // every lane's reads of the stage are done
-            cpv.add8(xa);
-            if (ternary) cnv.add8(xb);
-            else if (nb > 0) cpv.add8(xb);
+            if (MERGE) {
+                sliced_add(cpv, xa);                                   // + the group's bit-sliced partial count
+                if (ternary) sliced_add(cnv, xb);
+            } else {
+                cpv.add8(xa);
+                if (ternary) cnv.add8(xb);
+                else if (nb > 0) cpv.add8(xb);
+            }
             if (++st == kQStages) { st = 0; ph ^= 1u; }
         }
         uint32_t dpos = 0u, dneg = 0u;
@@ -611,11 +633,11 @@ static int grid_for(int64_t units, int per_sm) {
     return (int)(g < 1 ? 1 : g);
 }
 
-template <bool WRITE_COUNTS>
+template <bool WRITE_COUNTS, bool MERGE>
 static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_t s) {
     static bool attr_set = false;                    // per template instance
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(count_reduce_ring_kernel<WRITE_COUNTS>,
+        cudaError_t e = cudaFuncSetAttribute(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kQSmem);
         if (e != cudaSuccess) return e;
         attr_set = true;
@@ -624,7 +646,7 @@ static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_
     // programmatic stream serialization: the kernel waits (griddepcontrol.wait) for its predecessor on the stream
     // before it touches global memory; only its launch latency and shared-memory prologue overlap (NF_NO_PDL=1: off)
     static const bool use_pdl = getenv("NF_NO_PDL") == nullptr;
-    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS>, (unsigned)grid, kQThreads, kQSmem, s, use_pdl, p);
+    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>, (unsigned)grid, kQThreads, kQSmem, s, use_pdl, p);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -636,9 +658,13 @@ cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s
     const bool small = !p.cnt_pos && p.W <= 16;              // shallow rounds, 4 CTAs per SM
     static const bool force_ldg = getenv("NF_CR_LDG") != nullptr;       // A/B aid: register-staged kernel
     // the bulk copies need 16-byte-aligned rows: P, N are (nf_sign_count_reduce checks), so plane_stride % 4 == 0
+    const int64_t units = (max_words + kQWords - 1) / kQWords;
     if (!p.cnt_pos && !force_ldg && (p.plane_stride & 3) == 0)
-        return counts ? launch_ring<true>(p, (max_words + kQWords - 1) / kQWords, s)
-                      : launch_ring<false>(p, (max_words + kQWords - 1) / kQWords, s);
+        return counts ? launch_ring<true, false>(p, units, s) : launch_ring<false, false>(p, units, s);
+    // level-2 merge: rows of partial-count planes, same alignment rule
+    if (p.cnt_pos && !force_ldg && (p.count_stride & 3) == 0 && ((uintptr_t)p.cnt_pos & 15) == 0 &&
+        (!p.ternary || ((uintptr_t)p.cnt_neg & 15) == 0))
+        return counts ? launch_ring<true, true>(p, units, s) : launch_ring<false, true>(p, units, s);
     if (p.cnt_pos) {
         if (counts) count_reduce_kernel<true, true, 16><<<grid, kRThreads, 0, s>>>(p);
         else count_reduce_kernel<false, true, 16><<<grid, kRThreads, 0, s>>>(p);

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 DEV = "cuda"
 
 
-def _hier(cfg, b, groups, mode, margin=0):
+def _hier(cfg, b, groups, mode, margin=0, cs_pad=0):
     W = cfg.W
     assert sum(groups) == W
     g = gen.gen_bucket(cfg, b, DEV)
@@ -30,7 +30,10 @@ def _hier(cfg, b, groups, mode, margin=0):
     ternary = mode == nf.MODE_GTERNARY
     G = len(groups)
     B = max(nf.nf_count_planes(x) for x in groups)
+    # count_stride a multiple of 4 words: bulk-copy ring kernel; anything else: register-staged merge kernel
     cs = (max(Wd, 1) + 3) // 4 * 4
+    if cs_pad and (G == 1 or (B * (cs + cs_pad)) % 4 == 0):     # every group's planes must stay 16-byte aligned
+        cs += cs_pad
     cnt_pos = torch.zeros((G, B, cs), dtype=torch.int32, device=DEV)
     cnt_neg = torch.zeros((G, B, cs), dtype=torch.int32, device=DEV) if ternary else None
     w0 = 0
@@ -79,6 +82,7 @@ def test_tiny_hierarchical(groups, mode):
     cfg = shapes.tiny()
     _hier(cfg, cfg.buckets[0], groups, mode)
     _hier(cfg, cfg.buckets[0], groups, mode, margin=1)
+    _hier(cfg, cfg.buckets[0], groups, mode, cs_pad=2)
 
 
 @pytest.mark.parametrize("name,groups", [("resnet50", [4, 4]), ("vit_b16", [8, 8]), ("vit_b16", [4, 4, 4, 4]),
@@ -87,6 +91,7 @@ def test_configs_hierarchical_small(name, groups):
     cfg = shapes.get(name, small=True)
     for b in cfg.buckets[:3]:
         _hier(cfg, b, groups, nf.MODE_GTERNARY)
+    _hier(cfg, cfg.buckets[0], groups, nf.MODE_GBINARY, cs_pad=2)
 
 
 def test_sweep_full_size_hierarchical():
