@@ -208,11 +208,10 @@ __device__ __forceinline__ void vote_masks(const ReduceParams &p, int W, const S
 }
 
 // A (converged) warp holding 32 consecutive word positions k0 .. k0+31 (lane = word) computes the scales of
-// the tensors those words touch and writes out = S_t * d (and the counts, when asked for).
-template <bool WRITE_COUNTS>
-__device__ __forceinline__ void write_back(const ReduceParams &p, const PlanView &pv, int W, int lane, int64_t k,
-                                           const WordMeta &m, bool hit, TensorCache &tc, uint32_t dpos, uint32_t dneg,
-                                           const SlicedCounter &cpv, const SlicedCounter &cnv, const float4 *s_dtab) {
+// the tensors those words touch (none when the warp is still inside the cached tensor), publishes the scale of a
+// tensor whose first word it holds, and returns the scale of this lane's word.
+__device__ __forceinline__ float warp_scales(const ReduceParams &p, const PlanView &pv, int W, int lane, int64_t k,
+                                             const WordMeta &m, bool hit, TensorCache &tc) {
     float S = tc.S;
     if (!hit) {
         S = 0.f;
@@ -240,6 +239,14 @@ __device__ __forceinline__ void write_back(const ReduceParams &p, const PlanView
             }
         }
     }
+    return S;
+}
+
+// The warp writes out = S_t * d for its 32 words (and the counts, when asked for).
+template <bool WRITE_COUNTS>
+__device__ __forceinline__ void write_back(const ReduceParams &p, int W, int lane, const WordMeta &m, float S,
+                                           uint32_t dpos, uint32_t dneg, const SlicedCounter &cpv,
+                                           const SlicedCounter &cnv, const float4 *s_dtab) {
     // Fast write-back: the warp's 32 words are 1024 consecutive, 16-byte-aligned elements of ONE tensor.
     // Each thread turns its two masks into 8 direction bytes (low nibble +, high nibble -); a byte
     // indexes a shared-memory table of float4 directions, and every store writes 512 contiguous bytes.
@@ -376,7 +383,8 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
             }
             vote_masks(p, W, cpv, cnv, m.nvalid, dpos, dneg);
         }
-        write_back<WRITE_COUNTS>(p, pv, W, lane, k, m, hit, tc, dpos, dneg, cpv, cnv, s_dtab);
+        const float S = warp_scales(p, pv, W, lane, k, m, hit, tc);
+        write_back<WRITE_COUNTS>(p, W, lane, m, S, dpos, dneg, cpv, cnv, s_dtab);
     }
 }
 
@@ -489,7 +497,8 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
         const int64_t k = unit * kQWords + tid;
         WordMeta m{0, -1, 0};
         const bool hit = cached_meta(tc, k, lane, m);
-        if (!hit) m = word_meta(p, pv, nL, Wd, k);                     // overlaps the copies in flight
+        if (!hit) m = word_meta(p, pv, nL, Wd, k);                     // overlaps the copies in flight,
+        const float S = warp_scales(p, pv, W, lane, k, m, hit, tc);    // and so does the chain of W abs-sums
         SlicedCounter cpv, cnv;
         cpv.clear(); cnv.clear();
         for (int g = 0; g < n_stg; ++g) {
@@ -519,7 +528,7 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
         }
         uint32_t dpos = 0u, dneg = 0u;
         if (k < Wd) vote_masks(p, W, cpv, cnv, m.nvalid, dpos, dneg);
-        write_back<WRITE_COUNTS>(p, pv, W, lane, k, m, hit, tc, dpos, dneg, cpv, cnv, s_dtab);
+        write_back<WRITE_COUNTS>(p, W, lane, m, S, dpos, dneg, cpv, cnv, s_dtab);
     }
 }
 
