@@ -167,7 +167,7 @@ def algorithmic_bytes(cfg, planes: bool, ternary: bool):
 
 def run_nf(args):
     import torch
-    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from paper_2606_25759_b200 import ModelBuffers, binding as nf
     from paper_2606_25759_b200 import build as nf_build
     from workloads import shapes, gen
 
@@ -185,27 +185,20 @@ def run_nf(args):
     mode = nf.MODE_GTERNARY if ternary else nf.MODE_GBINARY
     planes = not args.no_planes
 
-    # ---- resident inputs: every bucket's [W][stride] gradients in HBM (42 GB for the GPT config)
+    # ---- resident inputs: every bucket's [W][stride] gradients in HBM (42 GB for the GPT config); every
+    # bucket owns its outputs, accumulators and packed planes (2.4 GB of planes for the GPT config: plane
+    # bytes written in one step are never overwritten inside L2 before they reach HBM); the 2-bit direction
+    # workspace (8.4 MB) is one buffer shared by all buckets, an L2-resident intermediate by design
     t0 = time.time()
-    G, BB = [], []
-    max_ps = max((sum((l + 31) // 32 for l in b.length) + 3) // 4 * 4 for b in cfg.buckets)
-    max_n = max(b.n for b in cfg.buckets)
-    P = torch.zeros((W, max_ps), dtype=torch.int32, device=dev) if planes else None
-    N = torch.zeros((W, max_ps), dtype=torch.int32, device=dev) if (planes and ternary) else None
-    ws = torch.zeros(nf.nf_workspace_bytes(max(len(b.tensors) for b in cfg.buckets), max_n),
-                     dtype=torch.uint8, device=dev)
-    for b in cfg.buckets:
-        G.append(gen.gen_bucket(cfg, b, dev))
-        bb = BucketBuffers(b.off, b.length, b.elig, b.n, W, dev, planes=False, health=True)
-        bb.P, bb.N, bb.plane_stride, bb.workspace = P, N, max_ps, ws
-        BB.append(bb)
+    G = [gen.gen_bucket(cfg, b, dev) for b in cfg.buckets]
+    MB = ModelBuffers([(b.off, b.length, b.elig, b.n) for b in cfg.buckets], W, dev, planes=planes, health=True)
+    BB = MB.buckets
     torch.cuda.synchronize()
     gen_s = time.time() - t0
     stream = torch.cuda.current_stream()
 
     def step():
-        for g, bb in zip(G, BB):
-            bb.aggregate(g, g.shape[1], (1, 0, 1), mode, None, 0, 1.0, planes=planes)
+        MB.step(G, (1, 0, 1), mode, None, 0, 1.0)
 
     in_bytes, all_bytes, passA_bytes = algorithmic_bytes(cfg, planes, ternary)
     n_total = cfg.n_params

@@ -8,4 +8,4 @@ from .binding import (nf_route_bucket, nf_sign_pack, nf_sign_count_reduce, nf_fp
                       nf_health_stats, nf_aggregate_bucket, nf_aggregate_bucket_host,
                       nf_plan_bytes, nf_workspace_bytes, MODE_GBINARY, MODE_GTERNARY,
                       ROUTE_P, ROUTE_L, ROUTE_F, NfError)
-from .bucket import BucketBuffers  # noqa: F401
+from .bucket import BucketBuffers, ModelBuffers  # noqa: F401

@@ -16,7 +16,7 @@ from . import binding as nf
 class BucketBuffers:
     def __init__(self, off: Sequence[int], length: Sequence[int], elig: Sequence[int], n: int, W: int,
                  device="cuda", planes: bool = True, counts: bool = False, health: bool = True,
-                 plane_stride: int | None = None):
+                 plane_stride: int | None = None, workspace: torch.Tensor | None = None):
         dev = torch.device(device)
         self.T, self.n, self.W = len(off), int(n), int(W)
         T = max(self.T, 1)
@@ -27,7 +27,10 @@ class BucketBuffers:
         self.woff = torch.zeros(T, dtype=torch.int64, device=dev)
         self.summary = torch.zeros(nf.SUM_LEN, dtype=torch.int64, device=dev)
         self.plan = torch.zeros(nf.nf_plan_bytes(self.T), dtype=torch.uint8, device=dev)
-        self.workspace = torch.zeros(nf.nf_workspace_bytes(self.T, self.n), dtype=torch.uint8, device=dev)
+        # the fused call's scratch: the caller may share one (large enough) buffer between buckets whose calls
+        # are ordered on one stream
+        self.workspace = workspace if workspace is not None else torch.zeros(
+            nf.nf_workspace_bytes(self.T, self.n), dtype=torch.uint8, device=dev)
         self.Wd_max = sum((int(l) + 31) // 32 for l in length)
         ps = plane_stride if plane_stride is not None else (self.Wd_max + 3) // 4 * 4
         self.plane_stride = max(ps, 4)
@@ -81,3 +84,28 @@ class BucketBuffers:
                                self.N if (use_planes and mode == nf.MODE_GTERNARY) else None,
                                self.plane_stride, self.abs_sum, self.sumsq, self.nan_cnt, self.inf_cnt,
                                self.out, self.scale, self.plan, self.workspace, stream)
+
+
+class ModelBuffers:
+    """Device buffers of a whole model's buckets, in the arrangement bench.py times (memory plumbing only):
+    every bucket has its own metadata, plan, accumulators, output and — when `planes` — its own packed
+    planes P/N (the "wire payload" of that bucket); the 2-bit direction workspace between the two passes of
+    the fused call is ONE buffer shared by all buckets (an L2-resident intermediate, sized for the largest
+    bucket). `step()` issues one nf_aggregate_bucket per bucket, back to back on one stream."""
+
+    def __init__(self, layouts, W: int, device="cuda", planes: bool = True, health: bool = True):
+        """layouts: sequence of (off, length, elig, n) per bucket."""
+        dev = torch.device(device)
+        self.W = int(W)
+        self.buckets = []
+        max_T = max(len(l[0]) for l in layouts)
+        max_n = max(int(l[3]) for l in layouts)
+        self.workspace = torch.zeros(nf.nf_workspace_bytes(max_T, max_n), dtype=torch.uint8, device=dev)
+        for off, length, elig, n in layouts:
+            bb = BucketBuffers(off, length, elig, n, W, dev, planes=planes, health=health, workspace=self.workspace)
+            self.buckets.append(bb)
+
+    def step(self, G, state=(1, 0, 1), mode=nf.MODE_GTERNARY, tau=None, margin=0, alpha=1.0, stream=None):
+        """G: per-bucket gradient tensors [W][stride]."""
+        for g, bb in zip(G, self.buckets):
+            bb.aggregate(g, g.shape[1], state, mode, tau, margin, alpha, stream=stream)

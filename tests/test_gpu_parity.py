@@ -257,3 +257,162 @@ def test_random_layouts(seed):
         pytest.skip("degenerate")
     run_both(gd, np.array(off, np.int64), np.array(lens, np.int64), elig, state=state, mode=mode, tau=tau,
              margin=margin, alpha=alpha, what=f"random layout seed {seed}")
+
+
+@pytest.mark.parametrize("T,W", [(257, 16), (700, 16), (300, 40), (700, 40), (256, 40)])
+def test_many_tensor_buckets_wide_fan_in(T, W):
+    """T around / above the 256-tensor shared-memory metadata capacity with SEVERAL worker groups (W > 8) and a few
+    tensors of several hundred tiles each (so that the tile scheduler, the group-major runs and the per-tensor
+    completion counters are all exercised on the T > 256 path: separate route kernel, global-memory lookups)."""
+    rng = np.random.default_rng(7000 + T + W)
+    lens = [int(x) for x in rng.integers(1, 1500, T)]
+    big = {3: 2048 * 310 + 1234, T // 3: 2048 * 205, T - 2: 2048 * 140 + 31}
+    for t, l in big.items():
+        lens[t] = l
+    lens[T // 2] = 2048 * 2 + 17
+    off, ln, n = layout(lens)
+    elig = [int(x) for x in rng.integers(0, 2, T)]
+    elig[3], elig[T // 3], elig[T - 2] = 1, 0, 1             # big low-bit, big FP32-route, big low-bit
+    g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
+    g[rng.random((W, n)) < 0.05] = 0.0
+    g[W - 1, off[T - 2] + 77] = np.inf
+    run_both(_dev(g), off, ln, elig, what=f"T={T} W={W}")
+
+
+@pytest.mark.parametrize("R", [1, 3, 11])
+def test_health_stats_replica_counts_other_than_W(R):
+    """nf_health_stats with R != W ('applied to the W inputs and/or to the aggregated output,
+    R = 1'), plan routed for another worker count."""
+    cfg = shapes.get("resnet50", small=True)
+    b = cfg.buckets[-1]
+    rng = np.random.default_rng(40 + R)
+    x = (rng.standard_normal((R, b.n)) * 10 ** rng.uniform(-5, 1, (1, b.n))).astype(np.float32)
+    x[rng.random((R, b.n)) < 0.01] = np.nan
+    x[rng.random((R, b.n)) < 0.01] = np.inf
+    x[0, : min(b.n, 5)] = -np.inf
+    xd = _dev(x)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, max(R, 2), DEV, planes=False, health=True)
+    bb.route_bucket((1, 0, 1))
+    bb.health_stats(xd, xd.shape[1], R=R)
+    torch.cuda.synchronize()
+    Q, cn, ci = O.health_stats(x, b.off, b.length)
+    from tests.util import assert_float_match
+    T = bb.T
+    got = _np(bb.sumsq).reshape(-1)[:R * T].reshape(R, T)
+    assert_float_match(np.sqrt(got), np.sqrt(Q), 1e-5, "l2 norm")
+    assert np.array_equal(_np(bb.nan_cnt).reshape(-1)[:R * T].reshape(R, T).astype(np.uint64), cn)
+    assert np.array_equal(_np(bb.inf_cnt).reshape(-1)[:R * T].reshape(R, T).astype(np.uint64), ci)
+
+
+@pytest.mark.parametrize("name", ["tiny", "vit_b16", "gpt2_1p3b"])
+def test_health_stats_of_the_aggregated_output(name):
+    """R = 1 on `out`: the health statistics of the aggregate the hook hands back (consumer: the Supervisor, PAPER
+    L158 / L177), computed by nf_health_stats from the fused call's own output buffer."""
+    cfg = shapes.get(name, small=(name != "tiny"))
+    for b in cfg.buckets:
+        g = gen.gen_bucket(cfg, b, DEV)
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=False, health=True)
+        bb.aggregate(g, g.shape[1])
+        torch.cuda.synchronize()
+        ref = O.aggregate_bucket(np.ascontiguousarray(_np(g)[:, :b.n]), b.off, b.length, b.elig)
+        Q, cn, ci = O.health_stats(ref.out.reshape(1, -1), b.off, b.length)
+        bb.health_stats(bb.out, b.n, R=1)
+        torch.cuda.synchronize()
+        from tests.util import assert_float_match
+        T = bb.T
+        assert_float_match(np.sqrt(_np(bb.sumsq)[0, :T]), np.sqrt(Q[0]), 1e-5, f"{cfg.name} bucket {b.index} out l2")
+        assert np.array_equal(_np(bb.nan_cnt)[0, :T].astype(np.uint64), cn[0])
+        assert np.array_equal(_np(bb.inf_cnt)[0, :T].astype(np.uint64), ci[0])
+
+
+@pytest.mark.parametrize("name", ["tiny", "resnet50", "vit_b16", "sweep_w32"])
+def test_run_to_run_bitwise_reproducible(name):
+    """PAPER L243 'synchronized aggregate direction': every replica of the hook must produce the same bits. Same
+    input ten times through the fused call and through the stand-alone calls: out, scale, abs_sum, sumsq and the
+    planes are BITWISE identical between runs (tile scheduling is dynamic; the totals must not depend on it)."""
+    cfg = shapes.get(name, small=(name not in ("tiny",)))
+    for b in cfg.buckets[:3]:
+        g = gen.gen_bucket(cfg, b, DEV)
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=True, health=True)
+        first = None
+        for rep in range(10):
+            bb.out.fill_(float(rep))
+            bb.aggregate(g, g.shape[1])
+            torch.cuda.synchronize()
+            cur = [bb.out.clone(), bb.scale.clone(), bb.abs_sum.clone(), bb.sumsq.clone(), bb.P.clone(), bb.N.clone(),
+                   bb.nan_cnt.clone(), bb.inf_cnt.clone()]
+            if first is None:
+                first = cur
+            else:
+                for k, (x, y) in enumerate(zip(first, cur)):
+                    assert torch.equal(x.view(torch.uint8), y.view(torch.uint8)), f"fused run {rep}, output {k} differs"
+        first = None
+        for rep in range(10):
+            bb.route_bucket((1, 0, 1))
+            bb.sign_pack(g, g.shape[1], nf.MODE_GTERNARY)
+            bb.sign_count_reduce(nf.MODE_GTERNARY)
+            bb.fp32_reduce(g, g.shape[1])
+            bb.health_stats(g, g.shape[1])
+            torch.cuda.synchronize()
+            cur = [bb.out.clone(), bb.scale.clone(), bb.abs_sum.clone(), bb.sumsq.clone()]
+            if first is None:
+                first = cur
+            else:
+                for k, (x, y) in enumerate(zip(first, cur)):
+                    assert torch.equal(x.view(torch.uint8), y.view(torch.uint8)), f"5-call run {rep}, output {k} differs"
+
+
+def test_full_size_bucket_run_to_run_bitwise():
+    """The same on a full 33.6 M-element GPT bucket (16 400 tiles over 148 persistent CTAs: which CTA processes
+    which tile differs from run to run)."""
+    cfg = shapes.gpt2_1p3b()
+    b = cfg.buckets[0]
+    g = gen.gen_bucket(cfg, b, DEV)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=False, health=True)
+    first = None
+    for rep in range(10):
+        bb.aggregate(g, g.shape[1])
+        torch.cuda.synchronize()
+        cur = [bb.out.clone(), bb.scale.clone(), bb.abs_sum.clone(), bb.sumsq.clone()]
+        if first is None:
+            first = cur
+        else:
+            for k, (x, y) in enumerate(zip(first, cur)):
+                assert torch.equal(x.view(torch.uint8), y.view(torch.uint8)), f"run {rep}, output {k} differs"
+
+
+@pytest.mark.parametrize("T", [64, 700])
+def test_concurrent_calls_on_two_streams_behind_foreign_work(T):
+    """The DDP-hook setting: the aggregation runs while other kernels (backward compute) hold part of the SMs, and
+    two buckets may be in flight on two streams. No call may depend on all of its CTAs being resident at once.
+    A long-running filler kernel occupies the device, then two nf_aggregate_bucket calls (separate plans, workspaces
+    and outputs) are issued on two streams, 50 times; both must match the oracle."""
+    rng = np.random.default_rng(T)
+    lens = [int(x) for x in rng.integers(1, 3000, T)]
+    lens[2] = 2048 * 150 + 5
+    lens[T - 1] = 2048 * 90
+    off, ln, n = layout(lens)
+    elig = [int(x) for x in rng.integers(0, 2, T)]
+    elig[2] = elig[T - 1] = 1
+    W = 8
+    gs, refs, bbs = [], [], []
+    for k in range(2):
+        g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
+        gs.append(_dev(g))
+        refs.append(O.aggregate_bucket(g, off, ln, elig))
+        bbs.append(BucketBuffers(off, ln, elig, n, W, DEV, planes=True, health=True))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    filler_stream = torch.cuda.Stream()
+    a = torch.randn((8192, 8192), device=DEV, dtype=torch.float32)
+    torch.cuda.synchronize()
+    for it in range(50):
+        with torch.cuda.stream(filler_stream):
+            for _ in range(2):
+                a = torch.tanh(a @ a * 1e-3)                 # a few ms of foreign work on all SMs
+        for k in range(2):
+            bbs[k].aggregate(gs[k], gs[k].shape[1], stream=streams[k])
+        if it % 10 == 9:
+            torch.cuda.synchronize()
+            for k in range(2):
+                compare(bbs[k], refs[k], W, O.MODE_GTERNARY, what=f"concurrent T={T} iteration {it} stream {k}")
+    torch.cuda.synchronize()

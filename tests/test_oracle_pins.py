@@ -15,20 +15,27 @@ from tests.util import read_golden, layout, assert_float_match
 
 
 # ------------------------------------------------------------------ O1 route (L108, L132, L205, L229)
+# The 16 rows, written out literally from the paper's prose — (admitted, veto, capacity_ok, elig) -> route
+# code (P = 0, L = 1, F = 2). Not admitted (FP32 warm-up, L66 / L207): everything plain FP32, whatever the
+# other flags say. Admitted but elig = 0 (sensitive or unmapped tensor, L132 / L205): plain FP32, never
+# low-bit and never counted as a fallback. Admitted, eligible, and a Supervisor veto or a capacity-guard
+# reject (L108, L229, L273): FP32 fallback F. Admitted, eligible, no veto, guard ok: low-bit L.
+ROUTE_TABLE = {
+    (0, 0, 0, 0): 0, (0, 0, 0, 1): 0, (0, 0, 1, 0): 0, (0, 0, 1, 1): 0,
+    (0, 1, 0, 0): 0, (0, 1, 0, 1): 0, (0, 1, 1, 0): 0, (0, 1, 1, 1): 0,
+    (1, 0, 0, 0): 0, (1, 0, 0, 1): 2, (1, 0, 1, 0): 0, (1, 0, 1, 1): 1,
+    (1, 1, 0, 0): 0, (1, 1, 0, 1): 2, (1, 1, 1, 0): 0, (1, 1, 1, 1): 2,
+}
+
+
 def expected_route(admitted, veto, cap, elig):
-    # truth table written out row by row from the paper's prose, not from the oracle's if-chain
-    table = {}
-    for a, v, c, e in itertools.product((0, 1), repeat=4):
-        if a == 0:
-            r = "P"               # FP32 warm-up: everything plain FP32 (L66, L207)
-        elif e == 0:
-            r = "P"               # sensitive / unmapped never low-bit (L132, L205)
-        elif v == 1 or c == 0:
-            r = "F"               # admitted route vetoed / guard reject -> FP32 fallback (L108, L229, L273)
-        else:
-            r = "L"
-        table[(a, v, c, e)] = {"P": 0, "L": 1, "F": 2}[r]
-    return table[(admitted, veto, cap, elig)]
+    return ROUTE_TABLE[(admitted, veto, cap, elig)]
+
+
+def test_route_table_is_complete_and_has_one_low_bit_row():
+    assert len(ROUTE_TABLE) == 16
+    assert [k for k, v in ROUTE_TABLE.items() if v == 1] == [(1, 0, 1, 1)]      # L needs all four conditions
+    assert sorted(k for k, v in ROUTE_TABLE.items() if v == 2) == [(1, 0, 0, 1), (1, 1, 0, 1), (1, 1, 1, 1)]
 
 
 def test_route_truth_table_16_rows():
