@@ -25,13 +25,24 @@
  *    whole 16-byte chunks that contain the row's first and last element, i.e. up to 12 bytes before
  *    / after the row inside the chunk (never a chunk without an element of the row; nothing is written).
  *  - "gap positions are never read" holds up to that chunk granularity for unaligned rows.
- *  - nf_aggregate_bucket uses a cooperative launch (grid = one CTA per SM) when T <= 256; calls on
- *    different streams are serialised by the device, not rejected.
+ *  - Concurrency: no call assumes that all CTAs of its grid are resident at once (no cooperative launch,
+ *    no grid-wide barrier; a CTA only ever waits for CTAs that are already running), so calls may run
+ *    beside other kernels that hold SMs and beside each other on different streams, provided they are
+ *    given different plan / workspace / output buffers. Calls that share a plan must be ordered on one
+ *    stream.
+ *  - Determinism: every output of every call is bit-reproducible from run to run on the same device for
+ *    the same inputs and launch geometry: integer results trivially, the FP32 route by its fixed worker
+ *    order, and the per-(worker, tensor) totals abs_sum / sumsq (hence the scales and decoded outputs)
+ *    because partial sums of a fixed shape are accumulated EXACTLY (wide fixed-point integer
+ *    accumulators inside the plan) and rounded to FP64 once, whatever the CTA scheduling.
+ *  - A bounded wait that runs out inside a kernel (a lost CTA, a corrupted plan) is reported as
+ *    NF_ERR_CUDA in summary[NF_SUM_STATUS] and in the plan (later calls given that plan do nothing)
+ *    instead of hanging the device.
  *  - Packed planes (reading #10): uint32 words, LSB = lowest element index, each L tensor starts
  *    at word woff[t] and is padded with 0 bits to a word boundary; worker w's plane starts at
  *    P + w*plane_stride (plane_stride >= Wd words).
- *  - Outputs that accumulate (abs_sum, sumsq, nan_cnt, inf_cnt) are zeroed by the callee on the
- *    same stream. `out` is written only at positions owned by the call (L tensors for
+ *  - Outputs that accumulate (abs_sum, sumsq, nan_cnt, inf_cnt) need no preparation by the caller: the
+ *    callee writes every (worker, tensor) entry. `out` is written only at positions owned by the call (L tensors for
  *    nf_sign_count_reduce, P/F tensors for nf_fp32_reduce), so the calls compose into one buffer.
  *  - 1 <= W <= 255 (uint8 counts), 0 <= margin <= 255, 0 <= T <= NF_MAX_TENSORS; else NF_ERR_RANGE.
  */
@@ -73,13 +84,15 @@ enum { NF_SUM_WD = 0, NF_SUM_NL = 1, NF_SUM_NF = 2, NF_SUM_NP = 3, NF_SUM_E = 4,
 typedef void *nf_stream; /* cudaStream_t */
 
 const char *nf_status_string(int status);
-/* library version, e.g. 100 = 0.1.0 */
+/* library version, e.g. 200 = 0.2.0 */
 int nf_version(void);
 
-/* Bytes of the device "plan" buffer nf_route_bucket fills for a bucket of T tensors (host call).
- * The plan holds the route-dependent tile map the streaming kernels walk plus small scratch
- * (per-tensor scales); it depends only on T. 16-byte aligned buffer required. */
-size_t nf_plan_bytes(int T);
+/* Bytes of the device "plan" buffer for a bucket of T tensors used with up to R workers / replicas (host
+ * call): the route-dependent tile map the streaming kernels walk, per-tensor scratch (scales, completion
+ * counters) and R x T exact accumulators of 256 bytes for the per-(replica, tensor) totals. R = the largest
+ * W (or R of nf_health_stats) any call will be given this plan with. 16-byte aligned buffer required; its
+ * contents need no initialisation and must not be modified by the caller between calls. */
+size_t nf_plan_bytes(int T, int R);
 
 /* Bytes of the device workspace nf_aggregate_bucket needs for a bucket of n elements (host call):
  * the 2-bit aggregate directions of the low-bit positions between its two passes. */
@@ -90,7 +103,10 @@ size_t nf_workspace_bytes(int T, int64_t n);
  * For each tensor: !admitted -> P; elig==0 -> P; veto or !capacity_ok -> F; else L.
  * Outputs: route[T] (uint8 nf_route), woff[T] (first packed word of an L tensor = running sum of
  * ceil(len/32) over L tensors in bucket order; -1 if not L), summary[NF_SUM_LEN] =
- * {Wd, nL, nF, nP, e, f, n_tiles, status}, and the plan. One single-CTA kernel.
+ * {Wd, nL, nF, nP, e, f, n_tiles, status}, and the plan. One single-CTA kernel. plan_bytes >=
+ * nf_plan_bytes(T, 1) is checked here; a plan too small for the W of a later call (or plane rows shorter than
+ * Wd words) is detected on the device by that call, which then poisons the plan (status NF_ERR_ARG) and does
+ * nothing else.
  */
 int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
                     nf_state state, uint8_t *route, int64_t *woff, int64_t *summary,
@@ -174,14 +190,20 @@ int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
                     void *plan, nf_stream stream);
 
 /*
- * Fused path (the one the target is measured on) — same results as
+ * Fused path (the one the target is measured on) — the results of
  * nf_route_bucket -> nf_sign_pack -> nf_sign_count_reduce -> nf_fp32_reduce -> nf_health_stats(g),
  * with the W x n gradients read ONCE. One launch for buckets of up to 256 tensors (the persistent kernel
- * routes the bucket itself; larger T: the route kernel first): it packs, counts, votes, sums the FP32 tensors, gathers abs-sums and health statistics from a single read
- * (pass A) and, tensor by tensor as each completes, expands the 2-bit directions by the per-tensor scale
- * (pass B). P and N may both be NULL (planes not materialised);
- * sumsq/nan_cnt/inf_cnt may all be NULL (no health statistics); scale_out may be NULL.
- * route/woff/summary/plan are outputs exactly as in nf_route_bucket.
+ * routes the bucket itself; larger T: the route kernel first): it packs, counts, votes, sums the FP32
+ * tensors, gathers abs-sums and health statistics from a single read (pass A) and, tensor by tensor as each
+ * completes, expands the 2-bit directions by the per-tensor scale (pass B).
+ * Against the 5-call sequence: route codes, word offsets, summary, packed planes, aggregate directions,
+ * NaN / Inf tallies and the FP32-route outputs are bit-identical; abs_sum / sumsq (and so the scales and the
+ * decoded magnitudes) agree to about 1e-7 relative (both sides round FP32 partial sums of different shapes;
+ * each side is bit-reproducible by itself) — the bound that holds against the oracle is 1e-6 / 1e-5.
+ * P and N may both be NULL (planes not materialised); plane_stride >= Wd words when they are not (checked on
+ * the device: NF_ERR_ARG in summary[NF_SUM_STATUS], nothing written). sumsq/nan_cnt/inf_cnt may all be NULL
+ * (no health statistics); scale_out may be NULL. route/woff/summary/plan are outputs exactly as in
+ * nf_route_bucket; plan_bytes >= nf_plan_bytes(T, W).
  */
 int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         const int64_t *off, const int64_t *len, const uint8_t *elig, int T,
@@ -194,16 +216,17 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         nf_stream stream);
 
 /*
- * End-to-end convenience with HOST buffers (used for the e2e measurement): copies W x n floats
- * from pinned/pageable host memory `g_host` (worker stride = worker_stride elements) into the
- * caller's device staging buffer `g_dev` (same stride), runs nf_aggregate_bucket with device
- * metadata/outputs as above, and copies `out` (n floats) back to `out_host`. All copies are
- * cudaMemcpyAsync on `stream`; the caller synchronises the stream.
+ * End-to-end convenience with HOST buffers (used for the e2e measurement): copies the W rows of n floats
+ * from pinned/pageable host memory `g_host` (worker stride = worker_stride elements: (W-1)*worker_stride + n
+ * floats are read, and as many written to the caller's device staging buffer `g_dev`, same stride), runs
+ * nf_aggregate_bucket with device metadata/outputs as above (P / N device planes or NULL), and copies `out`
+ * (n floats) back to `out_host`. All copies are cudaMemcpyAsync on `stream`; the caller synchronises the stream.
  */
 int nf_aggregate_bucket_host(const float *g_host /*host*/, float *g_dev, int64_t worker_stride, int W,
                              int64_t n, const int64_t *off, const int64_t *len, const uint8_t *elig,
                              int T, nf_state state, int mode, const float *tau, int margin, float alpha,
                              uint8_t *route, int64_t *woff, int64_t *summary,
+                             uint32_t *P, uint32_t *N, int64_t plane_stride,
                              double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
                              float *out, float *out_host /*host*/,
                              void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
@@ -258,19 +281,13 @@ int nf_supervisor_step(nf_supervisor *s /*host*/, double signal, uint64_t nan_co
                        int capacity_ok, nf_state *out /*host*/);
 
 /*
- * Instrumentation (host calls, not part of the data path). nf_prof_enable(k > 0) creates CUDA
- * events for up to k nf_aggregate_bucket calls and makes each such call record four events on
- * its stream (before the route kernel, before the fused kernel, after it, at the end of the call); nf_prof_enable(0) frees
- * them. nf_prof_collect synchronises on the recorded events, writes 3 floats per recorded call
- * (route ms, fused-kernel ms, remainder ms) to the HOST array `ms` (room for 3*max_records floats), resets
- * the record counter and returns the number of calls written (or a negative nf_status).
+ * Debugging aid, NOT part of the data path and NOT thread-safe (one process-global buffer: use it from one host
+ * thread, with no nf_aggregate_bucket call in flight on another). nf_debug_trace(1, NULL) allocates a device
+ * buffer of 256 x 8 globaltimer stamps that every CTA of the fused kernel fills from then on (kernel entry,
+ * after the dependency wait, after the routing and the clean-token check, consumers start, tiles exhausted,
+ * last tensor flushed, decode done); with `out` != NULL (room for 2048 uint64, HOST) the stamps are copied out
+ * (synchronises the device); nf_debug_trace(0, ...) frees the buffer.
  */
-int nf_prof_enable(int max_records);
-int nf_prof_collect(float *ms /*host*/, int max_records);
-/* Debug aid: nf_debug_trace(1, NULL) allocates a device buffer of 256 x 8 globaltimer stamps that every CTA of
- * the fused kernel fills from then on (kernel entry, after the dependency wait, after the routing barrier,
- * consumers start, tiles exhausted, last flush, decode done); with `out` != NULL (room for 2048 uint64, HOST) the
- * stamps are copied out (synchronises the device); nf_debug_trace(0, ...) frees the buffer. */
 int nf_debug_trace(int on, unsigned long long *out /*host*/);
 
 #ifdef __cplusplus

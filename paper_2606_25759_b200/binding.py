@@ -23,7 +23,7 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
-           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_prof_enable", "nf_prof_collect",
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
            "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace")
 
@@ -65,7 +65,7 @@ def lib() -> C.CDLL:
     L.nf_status_string.argtypes = [i32]
     L.nf_version.restype = i32
     L.nf_plan_bytes.restype = sz
-    L.nf_plan_bytes.argtypes = [i32]
+    L.nf_plan_bytes.argtypes = [i32, i32]
     L.nf_workspace_bytes.restype = sz
     L.nf_workspace_bytes.argtypes = [i32, i64]
     L.nf_route_bucket.restype = i32
@@ -85,8 +85,10 @@ def lib() -> C.CDLL:
                                       vp, sz, vp, sz, vp]
     L.nf_aggregate_bucket_host.restype = i32
     L.nf_aggregate_bucket_host.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32,
-                                           f32, vp, vp, vp, vp, vp, vp, vp, vp, vp,
+                                           f32, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp,
                                            vp, sz, vp, sz, vp]
+    L.nf_debug_trace.restype = i32
+    L.nf_debug_trace.argtypes = [i32, vp]
     L.nf_count_planes.restype = i32
     L.nf_count_planes.argtypes = [i32]
     L.nf_partial_count.restype = i32
@@ -103,10 +105,6 @@ def lib() -> C.CDLL:
     L.nf_capacity_guard.restype = i32
     L.nf_capacity_guard.argtypes = [i64, i32, i32, C.c_double, C.c_double, i32, C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
-    L.nf_prof_enable.restype = i32
-    L.nf_prof_enable.argtypes = [i32]
-    L.nf_prof_collect.restype = i32
-    L.nf_prof_collect.argtypes = [vp, i32]
     _lib = L
     return L
 
@@ -145,8 +143,8 @@ def _check(fn: str, rc: int):
         raise NfError(fn, rc)
 
 
-def nf_plan_bytes(T: int) -> int:
-    return int(lib().nf_plan_bytes(int(T)))
+def nf_plan_bytes(T: int, R: int = 1) -> int:
+    return int(lib().nf_plan_bytes(int(T), int(R)))
 
 
 def nf_workspace_bytes(T: int, n: int) -> int:
@@ -199,13 +197,13 @@ def nf_aggregate_bucket(g, worker_stride, W, n, off, length, elig, T, state, mod
 
 
 def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, elig, T, state, mode, tau,
-                             margin, alpha, route, woff, summary, abs_sum, sumsq, nan_cnt, inf_cnt, out,
-                             out_host, plan, workspace, stream=None):
+                             margin, alpha, route, woff, summary, P, N, plane_stride, abs_sum, sumsq, nan_cnt,
+                             inf_cnt, out, out_host, plan, workspace, stream=None):
     _check("nf_aggregate_bucket_host", lib().nf_aggregate_bucket_host(
         _ptr(g_host, cuda=False), _ptr(g_dev), int(worker_stride), int(W), int(n), _ptr(off),
         _ptr(length), _ptr(elig), int(T), _state(state), int(mode), _ptr(tau), int(margin), float(alpha),
-        _ptr(route), _ptr(woff), _ptr(summary), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt), _ptr(inf_cnt),
-        _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
+        _ptr(route), _ptr(woff), _ptr(summary), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(sumsq),
+        _ptr(nan_cnt), _ptr(inf_cnt), _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
 
 
@@ -273,14 +271,11 @@ class Supervisor:
     ema = property(lambda self: self._s.ema)
 
 
-def nf_prof_enable(max_records: int):
-    _check("nf_prof_enable", lib().nf_prof_enable(int(max_records)))
-
-
-def nf_prof_collect(max_records: int):
-    """Returns a list of (route_ms, fused_kernel_ms, remainder_ms), one per recorded nf_aggregate_bucket call."""
-    buf = (C.c_float * (3 * max(max_records, 1)))()
-    k = lib().nf_prof_collect(C.cast(buf, C.c_void_p), int(max_records))
-    if k < 0:
-        raise NfError("nf_prof_collect", k)
-    return [(buf[3 * i], buf[3 * i + 1], buf[3 * i + 2]) for i in range(k)]
+def nf_debug_trace(on: int, fetch: bool = False):
+    """Debugging aid (single-threaded): per-CTA globaltimer stamps of the fused kernel, [256][8] uint64 or None."""
+    import numpy as np
+    buf = np.zeros(2048, np.uint64) if fetch else None
+    rc = lib().nf_debug_trace(int(on), buf.ctypes.data if fetch else None)
+    if rc != NF_OK:
+        raise NfError("nf_debug_trace", rc)
+    return buf.reshape(256, 8) if fetch else None

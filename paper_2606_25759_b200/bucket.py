@@ -16,7 +16,7 @@ from . import binding as nf
 class BucketBuffers:
     def __init__(self, off: Sequence[int], length: Sequence[int], elig: Sequence[int], n: int, W: int,
                  device="cuda", planes: bool = True, counts: bool = False, health: bool = True,
-                 plane_stride: int | None = None, workspace: torch.Tensor | None = None):
+                 plane_stride: int | None = None, workspace: torch.Tensor | None = None, replicas: int = 1):
         dev = torch.device(device)
         self.T, self.n, self.W = len(off), int(n), int(W)
         T = max(self.T, 1)
@@ -26,7 +26,7 @@ class BucketBuffers:
         self.route = torch.zeros(T, dtype=torch.uint8, device=dev)
         self.woff = torch.zeros(T, dtype=torch.int64, device=dev)
         self.summary = torch.zeros(nf.SUM_LEN, dtype=torch.int64, device=dev)
-        self.plan = torch.zeros(nf.nf_plan_bytes(self.T), dtype=torch.uint8, device=dev)
+        self.plan = torch.zeros(nf.nf_plan_bytes(self.T, max(self.W, int(replicas))), dtype=torch.uint8, device=dev)
         # the fused call's scratch: the caller may share one (large enough) buffer between buckets whose calls
         # are ordered on one stream
         self.workspace = workspace if workspace is not None else torch.zeros(

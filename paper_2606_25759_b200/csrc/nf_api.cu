@@ -1,20 +1,12 @@
 // nf_api.cu — the extern "C" entry points declared in include/nf.h: argument checks that can be
 // made on the host, then kernel launches on the caller's stream. No allocation, no sync.
-#include <stdlib.h>
 #include "nf_internal.cuh"
 
 using namespace nf;
 
 namespace {
 
-// instrumentation state (nf_prof_*): 4 events per recorded nf_aggregate_bucket call
-cudaEvent_t *g_prof_ev = nullptr;
-int g_prof_cap = 0, g_prof_n = 0;
-inline void prof_mark(int slot, cudaStream_t s) {
-    if (g_prof_ev && g_prof_n < g_prof_cap) cudaEventRecord(g_prof_ev[4 * g_prof_n + slot], s);
-}
-
-unsigned long long *g_trace = nullptr;   // debug (nf_debug_trace): per-CTA time stamps of the fused kernel
+unsigned long long *g_trace = nullptr;   // debug (nf_debug_trace, single-threaded use): per-CTA time stamps of the fused kernel
 inline bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NF_OK : NF_ERR_CUDA; }
 
@@ -40,11 +32,12 @@ const char *nf_status_string(int status) {
     }
 }
 
-int nf_version(void) { return 100; }
+int nf_version(void) { return 200; }
 
-size_t nf_plan_bytes(int T) {
+size_t nf_plan_bytes(int T, int R) {
     if (T < 0) T = 0;
-    return plan_layout(T).total;
+    if (R < 1) R = 1;
+    return plan_bytes_for(T, R);
 }
 
 size_t nf_workspace_bytes(int T, int64_t n) {
@@ -59,11 +52,11 @@ int nf_route_bucket(const int64_t *off, const int64_t *len, const uint8_t *elig,
                     void *plan, size_t plan_bytes, nf_stream stream) {
     int rc = check_common(1, n, T);
     if (rc != NF_OK) return rc;
-    if (!summary || !plan || plan_bytes < nf_plan_bytes(T)) return NF_ERR_ARG;
+    if (!summary || !plan || plan_bytes < nf_plan_bytes(T, 1)) return NF_ERR_ARG;
     if (T > 0 && (!off || !len || !elig || !route || !woff)) return NF_ERR_ARG;
     if (misaligned16(plan)) return NF_ERR_ALIGN;
-    return cuda_rc(launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
-                                nullptr, nullptr, nullptr, nullptr, 0, 0, 0, (cudaStream_t)stream));
+    return cuda_rc(launch_route(off, len, elig, T, n, state, route, woff, summary, plan, plan_bytes, 0, 1,
+                                (cudaStream_t)stream));
 }
 
 int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
@@ -80,7 +73,6 @@ int nf_sign_pack(const float *g, int64_t worker_stride, int W, int64_t n,
     if (misaligned16(g) || misaligned16(P) || misaligned16(N) || misaligned16(plan)) return NF_ERR_ALIGN;
     cudaStream_t s = (cudaStream_t)stream;
     if (T == 0) return NF_OK;
-    if (cudaMemsetAsync(abs_sum, 0, sizeof(double) * (size_t)W * T, s) != cudaSuccess) return NF_ERR_CUDA;
     StreamParams p{};
     p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
     p.off = off; p.len = len; p.route = route; p.woff = woff;
@@ -180,11 +172,6 @@ int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
     if (misaligned16(x) || misaligned16(plan)) return NF_ERR_ALIGN;
     if (T == 0) return NF_OK;
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t cnt = (size_t)R * T;
-    if (cudaMemsetAsync(sumsq, 0, sizeof(double) * cnt, s) != cudaSuccess ||
-        cudaMemsetAsync(nan_cnt, 0, sizeof(uint64_t) * cnt, s) != cudaSuccess ||
-        cudaMemsetAsync(inf_cnt, 0, sizeof(uint64_t) * cnt, s) != cudaSuccess)
-        return NF_ERR_CUDA;
     StreamParams p{};
     p.g = x; p.worker_stride = replica_stride; p.W = R; p.T = T;
     p.off = off; p.len = len; p.route = nullptr;
@@ -206,7 +193,7 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     if (rc != NF_OK) return rc;
     if (margin < 0 || margin > 255) return NF_ERR_RANGE;
     if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
-    if (!summary || !plan || plan_bytes < nf_plan_bytes(T)) return NF_ERR_ARG;
+    if (!summary || !plan || plan_bytes < nf_plan_bytes(T, W)) return NF_ERR_ARG;
     if (!workspace || workspace_bytes < nf_workspace_bytes(T, n)) return NF_ERR_ARG;
     if (worker_stride < n || plane_stride < 0 || !abs_sum) return NF_ERR_ARG;
     if (T > 0 && (!g || !off || !len || !elig || !route || !woff || !out)) return NF_ERR_ARG;
@@ -216,25 +203,16 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     if (misaligned16(g) || misaligned16(out) || misaligned16(P) || misaligned16(N) ||
         misaligned16(plan) || misaligned16(workspace))
         return NF_ERR_ALIGN;
-    static const bool use_ldg = getenv("NF_PASSA_LDG") != nullptr;   // A/B aid: register-staged pass A + decode kernel
-    static const bool use_pdl = getenv("NF_NO_PDL") == nullptr;            // A/B aid: plain stream-ordered launches
-    static const bool sep_decode = getenv("NF_DECODE_SEPARATE") != nullptr;   // A/B aid: pass B as its own kernel
     cudaStream_t s = (cudaStream_t)stream;
-    prof_mark(0, s);
-    // a1: inside the fused kernel for buckets of up to kMetaCap tensors (one launch per bucket), else
-    // (or with NF_ROUTE_KERNEL set, an A/B aid) by the route kernel, which also zeroes the accumulators
-    static const bool route_kernel_forced = getenv("NF_ROUTE_KERNEL") != nullptr;
-    const bool inkernel = T > 0 && n > 0 && T <= kMetaCap && !use_ldg && !sep_decode && !route_kernel_forced;
-    cudaError_t e = cudaSuccess;
+    // a1: inside the fused kernel for buckets of up to kMetaCap tensors (one launch per bucket), else by the
+    // route kernel first (PDL-chained). An empty bucket only gets its summary written.
+    const bool inkernel = T > 0 && T <= kMetaCap;
     if (!inkernel) {
-        e = launch_route(off, len, elig, T, n, state, route, woff, summary, plan,
-                         abs_sum, sumsq, (unsigned long long *)nan_cnt,
-                         (unsigned long long *)inf_cnt, (int64_t)W * T, worker_stride, use_pdl ? 1 : 0, s);
-        if (e != cudaSuccess) return NF_ERR_CUDA;
-        if (T == 0 || n == 0) return NF_OK;
+        if (launch_route(off, len, elig, T, n, state, route, woff, summary, plan, plan_bytes, 1, 0, s) != cudaSuccess)
+            return NF_ERR_CUDA;
+        if (T == 0) return NF_OK;
     }
-    prof_mark(1, s);
-    // pass A: one read of the W x n gradients
+    // one read of the W x n gradients: pass A + pass B in one persistent kernel (nf_fused.cu)
     StreamParams p{};
     p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
     p.off = off; p.len = len; p.route = route; p.woff = woff;
@@ -245,37 +223,10 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
     p.scale_out = scale_out;
     p.trace = g_trace;
-    p.separate_decode = sep_decode ? 1 : 0;
-    p.pdl = use_pdl ? 1 : 0;
     p.inkernel_route = inkernel ? 1 : 0;
     p.elig = elig; p.st = state; p.n = n; p.route_w = route; p.woff_w = woff; p.summary = summary;
-    // One persistent TMA-ring kernel (nf_fused.cu) does pass A and pass B. NF_PASSA_LDG / NF_DECODE_SEPARATE
-    // select the register-staged streaming kernel / the stand-alone decode kernel for A/B measurements.
-    const int flags = health ? (kFPack | kFCount | kFFp32 | kFHealth) : (kFPack | kFCount | kFFp32);
-    if (!use_ldg) {
-        e = launch_fused_passA(health, p, n, s);                  // pass A + pass B in one kernel
-        if (e != cudaSuccess) return NF_ERR_CUDA;
-        prof_mark(2, s);
-        if (!sep_decode) {
-            prof_mark(3, s);
-            if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;
-            return NF_OK;
-        }
-    } else {
-        e = launch_stream(flags, p, n, s);
-        if (e != cudaSuccess) return NF_ERR_CUDA;
-        prof_mark(2, s);
-    }
-    // pass B as its own kernel (A/B aids only): scale x direction for the low-bit positions
-    ReduceParams r{};
-    r.W = W; r.T = T; r.off = off; r.len = len; r.route = route; r.woff = woff;
-    r.abs_sum = abs_sum; r.out = out; r.scale_out = scale_out;
-    r.dirs = (const uint8_t *)workspace; r.plan = plan;
-    r.pdl = use_pdl ? 1 : 0;
-    e = launch_decode(r, n, s);
-    prof_mark(3, s);
-    if (g_prof_ev && g_prof_n < g_prof_cap) ++g_prof_n;
-    return cuda_rc(e);
+    p.acc_slots = (int64_t)((plan_bytes - plan_layout(T).acc) / (sizeof(unsigned long long) * kAccWords));
+    return cuda_rc(launch_fused_passA(health, p, n, s));
 }
 
 // debug aid (nf.h): enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;
@@ -287,38 +238,11 @@ int nf_debug_trace(int on, unsigned long long *out) {
     return NF_OK;
 }
 
-int nf_prof_enable(int max_records) {
-    if (g_prof_ev) {
-        for (int i = 0; i < 4 * g_prof_cap; ++i) cudaEventDestroy(g_prof_ev[i]);
-        delete[] g_prof_ev;
-        g_prof_ev = nullptr;
-    }
-    g_prof_cap = g_prof_n = 0;
-    if (max_records <= 0) return NF_OK;
-    g_prof_ev = new cudaEvent_t[4 * (size_t)max_records];
-    for (int i = 0; i < 4 * max_records; ++i)
-        if (cudaEventCreate(&g_prof_ev[i]) != cudaSuccess) return NF_ERR_CUDA;
-    g_prof_cap = max_records;
-    return NF_OK;
-}
-
-int nf_prof_collect(float *ms, int max_records) {
-    if (!ms || max_records < 0) return NF_ERR_ARG;
-    int k = g_prof_n < max_records ? g_prof_n : max_records;
-    for (int i = 0; i < k; ++i) {
-        if (cudaEventSynchronize(g_prof_ev[4 * i + 3]) != cudaSuccess) return NF_ERR_CUDA;
-        for (int j = 0; j < 3; ++j)
-            if (cudaEventElapsedTime(&ms[3 * i + j], g_prof_ev[4 * i + j], g_prof_ev[4 * i + j + 1]) != cudaSuccess)
-                return NF_ERR_CUDA;
-    }
-    g_prof_n = 0;
-    return k;
-}
-
 int nf_aggregate_bucket_host(const float *g_host, float *g_dev, int64_t worker_stride, int W,
                              int64_t n, const int64_t *off, const int64_t *len, const uint8_t *elig,
                              int T, nf_state state, int mode, const float *tau, int margin, float alpha,
                              uint8_t *route, int64_t *woff, int64_t *summary,
+                             uint32_t *P, uint32_t *N, int64_t plane_stride,
                              double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
                              float *out, float *out_host,
                              void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
@@ -326,15 +250,17 @@ int nf_aggregate_bucket_host(const float *g_host, float *g_dev, int64_t worker_s
     int rc = check_common(W, n, T);
     if (rc != NF_OK) return rc;
     if (!g_host || !g_dev || !out_host || worker_stride < n) return NF_ERR_ARG;
+    if (misaligned16(g_dev)) return NF_ERR_ALIGN;
     cudaStream_t s = (cudaStream_t)stream;
-    if (cudaMemcpyAsync(g_dev, g_host, sizeof(float) * (size_t)worker_stride * W,
-                        cudaMemcpyHostToDevice, s) != cudaSuccess)
+    // W rows of n floats, `worker_stride` apart: the last row ends at (W-1)*worker_stride + n
+    const size_t count = (size_t)(W - 1) * (size_t)worker_stride + (size_t)n;
+    if (n > 0 && cudaMemcpyAsync(g_dev, g_host, sizeof(float) * count, cudaMemcpyHostToDevice, s) != cudaSuccess)
         return NF_ERR_CUDA;
     rc = nf_aggregate_bucket(g_dev, worker_stride, W, n, off, len, elig, T, state, mode, tau, margin,
-                             alpha, route, woff, summary, nullptr, nullptr, 0, abs_sum, sumsq, nan_cnt,
+                             alpha, route, woff, summary, P, N, plane_stride, abs_sum, sumsq, nan_cnt,
                              inf_cnt, out, nullptr, plan, plan_bytes, workspace, workspace_bytes, stream);
     if (rc != NF_OK) return rc;
-    if (cudaMemcpyAsync(out_host, out, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+    if (n > 0 && cudaMemcpyAsync(out_host, out, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, s) != cudaSuccess)
         return NF_ERR_CUDA;
     return NF_OK;
 }

@@ -128,12 +128,16 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 // ---------------------------------------------------------------------------------------------
 // shared-memory carve-up (dynamic). Everything the hot loop touches sits at a compile-time offset:
 //   [0, 64)         mbarriers full[4], empty[4]
-//   [64, 80)        tile index carried by each ring stage (dynamic tile scheduling)
+//   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
+//   [112, 128)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid)
+//   [128, 384)      scratch of the in-kernel routing scan
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
+//   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
 //   [4096, 8192)    decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
 //   [8192, 17408)   per-tensor metadata of the first kMetaCap tensors (tile prefix, off, len, woff, tau)
 //   [17408, ...)    ring [stages][8][kPitch] floats
-//   after the ring  per-warp FP64 totals {abs, sq} per worker, [kCW][2*W] doubles
+//   after the ring  per-warp FP64 totals {abs, sq} per worker of one segment, [nbuf][kCW][2*W] doubles
+//                   (double-buffered by segment parity when W <= 32: one CTA barrier per segment instead of two)
 // ---------------------------------------------------------------------------------------------
 constexpr int kSmemMeta = 8192;
 constexpr int kSmemHdr = kSmemMeta + 9216;       // 4*(cap+1) + 3*8*cap + 4*cap = 8196 bytes, padded
@@ -142,6 +146,9 @@ struct FusedSmem {
     uint64_t *full, *empty;
     int *tile_of;                // [kMaxStages] tile held by a stage, -1 = no more tiles
     int *run_of;                 // [kMaxStages] MULTI: length R of the run of tiles the stage belongs to
+    int *seg_of;                 // [kMaxStages] 1: the tile ends a segment (last tile of its scheduling unit or tensor)
+    int *flag;                   // [4] CTA-wide flags
+    float *sw;                   // [256] per-worker scales of the tensor being finalised
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -149,8 +156,9 @@ struct FusedSmem {
     float *m_tau;                // [kMetaCap]
     double *wacc;                // [kCW][2*W]
 };
+__host__ __device__ inline int fused_nbuf(int W) { return W <= 32 ? 2 : 1; }
 __host__ __device__ inline size_t fused_smem_bytes(int stages, int W) {
-    return (size_t)kSmemHdr + (size_t)stages * kStageBytes + sizeof(double) * kCW * 2 * (size_t)W;
+    return (size_t)kSmemHdr + (size_t)stages * kStageBytes + sizeof(double) * kCW * 2 * (size_t)W * fused_nbuf(W);
 }
 __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     FusedSmem s;
@@ -158,6 +166,9 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.empty = s.full + kMaxStages;
     s.tile_of = (int *)(base + 64);
     s.run_of = (int *)(base + 80);
+    s.seg_of = (int *)(base + 96);
+    s.flag = (int *)(base + 112);
+    s.sw = (float *)(base + 3072);
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -212,7 +223,8 @@ __device__ __forceinline__ void tensor_lookup(const StreamParams &p, const PlanV
 }
 // Exact FP64 re-read of one thread's elements of worker `wg` over the last `cnt` (<= 4) tiles of the
 // current tensor (`recent`, most recent first) (rare: NaN / Inf / FP32 range trouble in the FP32 partials). Returns
-// {sum |x|, sum of x^2 over finite x}; NaN / Inf are tallied in shared memory slot `slot`.
+// {sum |x|, sum of x^2}, both over the FINITE x only; NaN / Inf are tallied in shared memory slot `slot` (the
+// tensor's last arriver turns a non-zero tally into the IEEE result of the sum: NaN, else +Inf).
 template <bool HEALTH>
 __device__ __noinline__ double2 exact_redo(const float *__restrict__ g, int64_t worker_stride, int wg,
                                            int64_t off_t, int64_t len_t, int tile_b, int4 recent, int cnt, int ctid,
@@ -244,17 +256,15 @@ __device__ __noinline__ double2 exact_redo(const float *__restrict__ g, int64_t 
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             const float v = x[j][k];                         // padding zeros add nothing
-            da += (double)fabsf(v);
-            if (HEALTH) {
-                if (v != v) ++cn;
-                else if (fabsf(v) == INFINITY) ++ci;
-                else dq += (double)v * (double)v;
+            if (v != v) ++cn;
+            else if (fabsf(v) == INFINITY) ++ci;
+            else {
+                da += (double)fabsf(v);
+                if (HEALTH) dq += (double)v * (double)v;
             }
         }
-    if (HEALTH) {
-        if (cn) atomicAdd(&s_nan[slot], cn);
-        if (ci) atomicAdd(&s_inf[slot], ci);
-    }
+    if (cn) atomicAdd(&s_nan[slot], cn);
+    if (ci) atomicAdd(&s_inf[slot], ci);
     return make_double2(da, dq);
 }
 
@@ -384,14 +394,15 @@ __device__ __forceinline__ uint32_t vote4(uint32_t posR, uint32_t negR, int W, i
     return d;
 }
 
-// FP32 partials of worker group [w0, w0+nw) over the last `cnt` bulk tiles -> warp totals (FP32
-// butterfly reduce-scatter) -> this warp's FP64 slots in shared memory. Range check on the warp
+// FP32 partials of worker group [w0, w0+nw) over the last `cnt` bulk tiles (one segment) -> warp totals (FP32
+// butterfly reduce-scatter) -> this warp's FP64 slots of the segment in shared memory (`wbuf`, stored, not
+// added: a segment is reduced over the warps and leaves the CTA at once, see seg_reduce). Range check on the warp
 // totals: |x| sums finite, squares neither over- nor underflowed; otherwise the warp re-reads
 // exactly those elements in FP64 (and tallies NaN / Inf).
 template <bool HEALTH>
-__device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, float (&af)[8], float (&qf)[8],
-                                           int64_t off_t, int64_t len_t, int tile_b, int w0, int nw, int cnt,
-                                           int4 recent, int ctid, bool aligned) {
+__device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, double *wbuf, float (&af)[8],
+                                           float (&qf)[8], int64_t off_t, int64_t len_t, int tile_b, int w0, int nw,
+                                           int cnt, int4 recent, int ctid, bool aligned) {
     const int lane = ctid & 31, warp = ctid >> 5, W = p.W;
     float v16[16];
 #pragma unroll
@@ -403,9 +414,9 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
     const bool ok = HEALTH ? ((A <= FLT_MAX) && (((Q >= 1e-30f) && (Q <= FLT_MAX)) || A == 0.f))
                            : (A <= FLT_MAX);
     const unsigned bad = __ballot_sync(0xffffffffu, !ok && wl < nw);
-    double *slot = sm.wacc + (size_t)warp * 2 * W + (size_t)w0 * 2;
+    double *slot = wbuf + (size_t)warp * 2 * W + (size_t)w0 * 2;
     if (bad == 0u) {
-        if ((lane & 1) == 0 && wl < nw) slot[wl * 2 + stat] += (double)r;
+        if ((lane & 1) == 0 && wl < nw) slot[wl * 2 + stat] = (double)r;
     } else {
         // rare: some worker's warp totals failed the range check. For those workers every thread
         // re-checks its own partials and only the offending threads re-read their elements exactly.
@@ -422,9 +433,9 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
                     e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, recent, cnt, ctid, sm.nan,
                                            sm.inf, w0 + w, aligned);
                 const double ea = warp_sum(e.x), eq = warp_sum(e.y);
-                if (lane == 0) { slot[w * 2] += ea; slot[w * 2 + 1] += eq; }
+                if (lane == 0) { slot[w * 2] = ea; slot[w * 2 + 1] = eq; }
             } else if ((lane & 1) == 0 && wl == w) {
-                slot[w * 2 + stat] += (double)r;
+                slot[w * 2 + stat] = (double)r;
             }
         }
     }
@@ -444,6 +455,16 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
     }
 }
 
+// A bounded wait ran out (a lost CTA, a corrupted plan): report NF_ERR_CUDA through summary[NF_SUM_STATUS] and the
+// plan instead of hanging or trapping, and drop the clean token so that the next call re-initialises the plan.
+__device__ __noinline__ void report_timeout(const StreamParams &p) {
+    PlanHeader *hdr = (PlanHeader *)p.plan;
+    hdr->status = NF_ERR_CUDA;
+    hdr->clean = 0ull;
+    if (p.summary) p.summary[NF_SUM_STATUS] = NF_ERR_CUDA;
+    __threadfence();
+}
+
 // ---------------------------------------------------------------------------------------------
 // pass B inside the kernel: out[off_t+i] = S_t * d for the low-bit tiles this CTA owns, as soon as
 // tensor t is complete (all its tiles published by every CTA: plan.done[t] == tiles of t). A unit
@@ -455,7 +476,6 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
 __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
                                              int n_tiles, int lane, int grab) {
     const float4 *dtab = sm.dtab;
-    const int W = p.W;
     const int total_units = n_tiles * 2;
     int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
     int t_cur = -1, tile_b = 0, tile_e = 0;
@@ -491,24 +511,22 @@ __device__ __forceinline__ void decode_units(const StreamParams &p, const PlanVi
                 t_cur = tc.t; tile_b = tc.tile_b; tile_e = tc.tile_e; off_t = tc.off; len_t = tc.len;
                 dec = tc.isL;
                 if (dec) {
+                    // wait until the tensor's last arriver has published its totals and scale (it runs in a
+                    // resident CTA, and so does every CTA that still holds tiles of the tensor: no CTA waits
+                    // for one that has not started)
                     woff_t = tc.woff;
-                    const int total = tile_e - tile_b;
                     const int *dp = pv.done + t_cur;
                     int seen;
                     for (unsigned spins = 0;; ++spins) {
                         asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(dp) : "memory");
-                        if (seen >= total) break;
-                        __nanosleep(500);
-                        if (spins > (1u << 23)) __trap();    // > 4 s: a lost CTA; fail loudly instead of hanging
+                        if (seen & kDoneFinal) break;
+                        __nanosleep(200);
+                        if (spins > (1u << 24)) { report_timeout(p); return; }   // > 4 s: give up loudly, do not hang
                     }
-                    S_t = warp_tensor_scale(p.abs_sum, W, p.T, t_cur, len_t, lane);   // warp-uniform branch
+                    S_t = __ldcg(pv.scale + t_cur);
                 }
             }
             if (!dec) continue;
-            if (tile == tile_b && (u & 1) == 0 && lane == 0) {
-                pv.scale[t_cur] = S_t;
-                if (p.scale_out) p.scale_out[t_cur] = S_t;
-            }
             const int64_t wbase = (int64_t)(tile - tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -568,9 +586,79 @@ __device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool 
 
 extern __shared__ __align__(128) unsigned char smem_raw[];
 
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+constexpr unsigned long long kInitToken = 0x4e46494e4954494eull;     // a CTA is zeroing the plan's state
+
+// ---------------------------------------------------------------------------------------------
+// The tensor's last arriver (the CTA whose publication completed done[t]) rounds the exact totals of tensor t
+// to FP64 once, writes abs_sum / sumsq / nan_cnt / inf_cnt, clears the accumulator slots for the next call,
+// computes S_t = (float)(sum_w (double)(float)(A_w / len_t) / W) in worker order ("mean-absolute
+// scale"; readings #7, #8) and publishes it: done[t] |= kDoneFinal releases the decode warps of every CTA.
+// Called by all consumer threads of the CTA.
+// ---------------------------------------------------------------------------------------------
+template <bool HEALTH>
+__device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
+                                             int64_t len_t, bool isL, int ctid) {
+    const int W = p.W, T = p.T;
+    if (ctid < W) {
+        const size_t o = (size_t)ctid * T + t;
+        double A = 0.0;
+        if (isL || HEALTH) {
+            unsigned long long wd[kAccWords];
+            ulonglong2 *slot = reinterpret_cast<ulonglong2 *>(pv.acc + o * kAccWords);
+#pragma unroll
+            for (int i = 0; i < kAccWords / 2; ++i) {
+                const ulonglong2 v = __ldcg(slot + i);
+                wd[2 * i] = v.x;
+                wd[2 * i + 1] = v.y;
+            }
+#pragma unroll
+            for (int i = 0; i < kAccWords / 2; ++i) __stcg(slot + i, make_ulonglong2(0ull, 0ull));
+            const unsigned long long cn = wd[kAccNan], ci = wd[kAccInf];
+            if (isL) {
+                A = acc_round(wd + kAccAbs, kAccAbsWords, kAccAbsBase);
+                if (cn) A = __longlong_as_double(0x7ff8000000000000ll);          // IEEE: a NaN term makes the sum NaN,
+                else if (ci) A = __longlong_as_double(0x7ff0000000000000ll);     // an Inf term (no NaN) makes it +Inf
+            }
+            if (HEALTH) {
+                p.sumsq[o] = acc_round(wd + kAccSq, kAccSqWords, kAccSqBase);
+                p.nan_cnt[o] = cn;
+                p.inf_cnt[o] = ci;
+            }
+        }
+        p.abs_sum[o] = A;                                  // 0 for tensors that are not low-bit routed
+        sm.sw[ctid] = (float)(A / (double)len_t);
+    }
+    if (!isL) return;                                      // CTA-uniform
+    consumer_sync();
+    if (ctid == 0) {
+        double s = 0.0;
+        for (int w = 0; w < W; ++w) s += (double)sm.sw[w];
+        const float S = (float)(s / (double)W);
+        pv.scale[t] = S;
+        if (p.scale_out) p.scale_out[t] = S;
+        __threadfence();
+        atomicOr(pv.done + t, kDoneFinal);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
+#ifndef NF_TAIL4
+#define NF_TAIL4 12                       // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
+#endif
+#ifndef NF_TAIL2
+#define NF_TAIL2 4                        // the last NF_TAIL2 x grid tiles are handed out one at a time
+#endif
+
 template <bool HEALTH, bool MULTI>
 __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ StreamParams p, const int stages_arg) {
     const int stages = MULTI ? stages_arg : kStages;     // W <= 8: compile-time ring depth
@@ -588,142 +676,34 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     for (int i = tid; i < 256; i += kFThreads)
         sm.dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
                                  (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
-    for (int i = tid; i < kCW * 2 * W; i += kFThreads) sm.wacc[i] = 0.0;
     __syncthreads();
-    // everything above touched shared memory only and overlapped the route kernel (PDL); the plan
-    // and the zeroed accumulators are visible after this point
+    // everything above touched shared memory only and overlapped the previous kernel on the stream (PDL)
     pdl_wait();
     if (tid == 0) trace_stamp(p, 6);
     const PlanView pv = plan_view(p.plan, p.T);
+    PlanHeader *const hdr = (PlanHeader *)p.plan;
     int n_tiles = 0;
 
     // -----------------------------------------------------------------------------------------
-    // producer (one elected lane of warp kCW): issues the bulk copies of every (tile, worker group).
-    // Dynamic tile scheduling: tiles are handed out by a device-wide cursor, so a CTA that runs ahead
-    // (SM position, co-running decode warps) simply takes more. Every tile enters the ring; the stage
-    // carries its tile index to the consumers. Tiles are taken in runs of consecutive tiles (guided
-    // self-scheduling: up to NF_KCHUNK early, single tiles near the end), so that a CTA stays inside one
-    // tensor for a while — a tensor change costs a CTA-wide flush — without giving up the balance at the
-    // tail. The FIRST run of every CTA is static (CTA b: tiles [b*want0, (b+1)*want0), the cursor counts
-    // from gridDim.x*want0), so it needs nothing another CTA wrote: with the in-kernel routing the
-    // producer fills the ring with it while the grid barrier is still pending (prefetch = true: never
-    // blocks, never touches the cursor).
+    // Self-cleaning state. The cursors, the per-tensor completion counters done[] and the exact accumulators
+    // acc[] are all zero whenever hdr->clean holds the token of this (T, W) shape: every call leaves them so
+    // (slots are cleared by whoever rounds them, the grid's last CTA resets the rest). Thread 0 starts the
+    // check here; the routing below needs none of that state and overlaps the round trip. Any other value
+    // (first use of the buffer, another shape) is settled once by compare-and-swap: the winning CTA zeroes
+    // the state and publishes the token, the others wait for a CTA that is running. No grid-wide barrier,
+    // no cooperative launch: nothing here assumes that all CTAs of the grid are resident together.
     // -----------------------------------------------------------------------------------------
-    int pr_st = 0, pr_next = 0, pr_end = 0, pr_tile = 0, pr_R = 1, pr_w0 = 0, pr_r = 0;
-    uint32_t pr_ph = 0;
-    bool pr_have = false, pr_first = true;
-    TensorCur pc{};
-    pc.tile_e = 0;
-    auto produce = [&](int max_stages, bool prefetch) __attribute__((always_inline)) {
-        const uint64_t pol = policy_evict_first();
-        int32_t *cursor = const_cast<int32_t *>(&pv.hdr->tile_cursor);
-        int want0 = n_tiles / (4 * (int)gridDim.x);
-        want0 = want0 < 1 ? 1 : (want0 > NF_KCHUNK ? NF_KCHUNK : want0);
-        const int dyn0 = (int)gridDim.x * want0;                       // first dynamically assigned tile
-        for (int issued = 0; issued < max_stages; ++issued) {
-            if (!pr_have) {
-                if (pr_first) {
-                    pr_first = false;
-                    pr_next = (int)blockIdx.x * want0;
-                    pr_end = pr_next + want0;
-                } else if (pr_next >= pr_end) {
-                    if (prefetch) return;
-                    int want = (n_tiles - pr_end) / (4 * (int)gridDim.x);     // pr_end: last position seen
-                    want = want < 1 ? 1 : (want > NF_KCHUNK ? NF_KCHUNK : want);
-                    pr_next = dyn0 + atomicAdd(cursor, want);
-                    pr_end = pr_next + want;
-                }
-                pr_tile = pr_next;
-                if (pr_tile >= n_tiles) {
-                    if (prefetch) return;
-                    mbar_wait(sm.empty + pr_st, pr_ph ^ 1u);
-                    sm.tile_of[pr_st] = -1;                            // sentinel: the consumers stop
-                    mbar_arrive(sm.full + pr_st);
-                    return;
-                }
-                if (pr_tile >= pc.tile_e) tensor_lookup(p, pv, sm, pr_tile, pc);
-                // Several worker groups (MULTI), low-bit tensor: the stages of a run of R <= kMRun consecutive
-                // tiles of one tensor go group-major (group 0 of tiles 0..R-1, then group 1, ...), so that the
-                // consumers flush their FP32 partials of a group once per run instead of once per stage.
-                pr_R = 1;
-                if (MULTI && pc.isL) pr_R = min(min(min(pr_end, n_tiles), pc.tile_e) - pr_tile, kMRun);
-                pr_next += pr_R;
-                pr_w0 = 0;
-                pr_r = 0;
-                pr_have = true;
-            }
-            {
-                const int w0 = pr_w0, nw = min(kGroup, W - w0);
-                const int64_t tile_base = (int64_t)(pr_tile + pr_r - pc.tile_b) * kTile;
-                const int64_t rem = pc.len - tile_base;
-                const int need = rem >= kTile ? kTile : (int)rem;
-                // aligned rows: whole float4s only (a partial one is read from global memory by its owner
-                // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
-                // (whole 16-byte chunks, each holding at least one element of the row).
-                const uint32_t bytes = (uint32_t)((need & ~3) * 4);
-                const float *src = p.g + pc.off + tile_base;
-                const int st = pr_st;
-                mbar_wait(sm.empty + st, pr_ph ^ 1u);                  // first lap: passes at once
-                sm.tile_of[st] = pr_tile + pr_r;
-                if (MULTI) sm.run_of[st] = pr_R;
-                float *dst = sm.ring + (size_t)st * kStageFloats;
-                if (!pc.aligned) {
-                    uint32_t tx = 0;
-                    for (int w = 0; w < nw; ++w)
-                        tx += (uint32_t)((((int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
-                    mbar_expect_tx(sm.full + st, tx);
-                    for (int w = 0; w < nw; ++w) {
-                        const int m = (int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
-                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
-                                 (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
-                    }
-                } else if (bytes) {
-                    mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
-                    for (int w = 0; w < nw; ++w)
-                        bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
-                } else {
-                    mbar_arrive(sm.full + st);
-                }
-                if (++pr_st == stages) { pr_st = 0; pr_ph ^= 1u; }
-                if (++pr_r == pr_R) {
-                    pr_r = 0;
-                    pr_w0 += kGroup;
-                    if (pr_w0 >= W) pr_have = false;
-                }
-            }
-        }
-    };
+    const unsigned long long want_token = clean_token(p.T, W);
+    unsigned long long seen_token = want_token;
+    if (tid == 0) seen_token = ld_acquire_u64(&hdr->clean);
 
     if (p.inkernel_route) {
         // ---- step a1 inside this kernel (T <= kMetaCap) --------
         // Every CTA derives the routing of the bucket into its shared-memory metadata (redundant O(T)
-        // work, no dependence on another kernel); CTA 0 also writes the a1 outputs and the plan; all
-        // CTAs zero a slice of the accumulators; one grid-wide barrier (cooperative launch) orders the
-        // zeroing before anybody's atomics.
+        // work, no dependence on another kernel or CTA); CTA 0 also writes the a1 outputs and the plan.
         const int T = p.T;
         PlanLayout PL = plan_layout(T);
         char *pb = (char *)p.plan;
-        // zero a slice of the accumulating outputs and of the per-tensor completion counters (CTA 0: the two
-        // cursors as well), then ARRIVE at the grid barrier; the routing below needs none of it and runs while
-        // the other CTAs arrive
-        {
-            int32_t *done = (int32_t *)(pb + PL.done);
-            const int64_t zc = (int64_t)W * T;
-            for (int64_t i = (int64_t)blockIdx.x * kFThreads + tid; i < zc; i += (int64_t)gridDim.x * kFThreads) {
-                p.abs_sum[i] = 0.0;
-                if (HEALTH) { p.sumsq[i] = 0.0; p.nan_cnt[i] = 0ull; p.inf_cnt[i] = 0ull; }
-                if (i < T) done[i] = 0;
-            }
-            if (blockIdx.x == 0 && tid == 0) {
-                PlanHeader *hdr = (PlanHeader *)pb;
-                hdr->tile_cursor = 0;
-                hdr->unit_cursor = 0;
-            }
-        }
-        // (no fence of our own: barrier_arrive is a CTA barrier followed by the master's release at GPU scope,
-        // which is cumulative over the zeroing stores of the whole CTA)
-        cooperative_groups::grid_group grid = cooperative_groups::this_grid();
-        auto zeroed = grid.barrier_arrive();
         long long l = 0, o = 0, v_tiles = 0, v_words = 0, v_nl = 0;
         int r = NF_ROUTE_P;
         int bad = 0;
@@ -782,7 +762,8 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
         const long long ex_tiles = b_tiles + i_tiles - v_tiles, ex_words = b_words + i_words - v_words,
                         ex_nl = b_nl + i_nl - v_nl;
-        const int status = (any_bad || t_tiles > 0x7fffffffLL) ? NF_ERR_ARG : NF_OK;
+        // (a plane row shorter than the packed words of the bucket would be overrun: refused like a bad layout)
+        const int status = (any_bad || t_tiles > 0x3fffffffLL || (p.P && t_words > p.plane_stride)) ? NF_ERR_ARG : NF_OK;
         if (tid < T) {
             sm.m_tile[tid] = (int32_t)ex_tiles;
             sm.m_off[tid] = o;
@@ -803,7 +784,6 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
             if (tid == 0) {
                 const unsigned long long *tal = reinterpret_cast<const unsigned long long *>(s_scan + 24);
-                PlanHeader *hdr = (PlanHeader *)pb;
                 tile_prefix[T] = (int32_t)t_tiles;
                 lt_woff[t_nl] = t_words;
                 hdr->magic = kPlanMagic;
@@ -813,7 +793,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 hdr->n = p.n;
                 hdr->Wd = t_words;
                 hdr->n_tiles = status == NF_OK ? (int32_t)t_tiles : 0;
-                hdr->pad0 = 0;                           // (the cursors were zeroed before the barrier)
+                hdr->acc_slots = p.acc_slots;
                 p.summary[NF_SUM_WD] = t_words;
                 p.summary[NF_SUM_NL] = t_nl;
                 p.summary[NF_SUM_NF] = (int64_t)tal[0];
@@ -824,17 +804,14 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 p.summary[NF_SUM_STATUS] = status;
             }
         }
-        // the ring is filled with this CTA's static first run while the barrier is pending (the shared-memory
-        // metadata it needs was written just above)
-        n_tiles = status == NF_OK ? (int)t_tiles : 0;
-        __syncthreads();
-        if (warp == kCW && lane == 0 && status == NF_OK) produce(stages, true);
-        grid.barrier_wait(std::move(zeroed));               // everybody's slice is zero, the cursors too
-        if (tid == 0) trace_stamp(p, 7);
-        if (status != NF_OK) return;
+        if (status != NF_OK) return;                           // nothing of the self-cleaning state was touched
         n_tiles = (int)t_tiles;
     } else {
         if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+        if (p.P && pv.hdr->Wd > p.plane_stride) {              // plane rows too short: refuse, like a bad layout
+            if (blockIdx.x == 0 && tid == 0) { hdr->status = NF_ERR_ARG; p.summary[NF_SUM_STATUS] = NF_ERR_ARG; }
+            return;
+        }
         n_tiles = pv.hdr->n_tiles;
         if (p.T <= kMetaCap) {
             // per-tensor metadata -> shared memory (one round trip for the whole CTA)
@@ -848,224 +825,370 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     sm.m_tau[t] = (p.tau && isL) ? __ldg(p.tau + t) : 0.f;
                 }
             }
-            __syncthreads();
         }
     }
 
-    // =========================================================================================
-    // producer: one elected lane issues the bulk copies of every (tile, worker group): produce() above
-    // =========================================================================================
-    if (warp == kCW) {
-        if (lane == 0) produce(0x7fffffff, false);
-        return;
+    // ---- settle the clean token (thread 0 read it before the routing) ------------------------------
+    if (tid == 0) {
+        int role = 0;                                          // 1: this CTA zeroes the state
+        for (unsigned spins = 0; seen_token != want_token; ++spins) {
+            if (seen_token != kInitToken) {
+                const unsigned long long old = atomicCAS(&hdr->clean, seen_token, kInitToken);
+                if (old == seen_token) { role = 1; break; }
+                seen_token = old;
+            } else {
+                __nanosleep(200);
+                seen_token = ld_acquire_u64(&hdr->clean);
+                if (spins > (1u << 24)) { report_timeout(p); role = 2; break; }
+            }
+        }
+        sm.flag[0] = role;
     }
-    // =========================================================================================
-    // housekeeping warp: scales of the tensors nobody decodes (0 for the FP32 route; the oracle's
-    // 0/0 for an empty low-bit tensor, abs_sum having been zeroed by the route kernel)
-    // =========================================================================================
-    if (warp == kCW + 1) {
+    __syncthreads();                                           // also: the shared-memory metadata is complete
+    if (sm.flag[0] == 2) return;
+    if (sm.flag[0] == 1) {
+        const size_t na = (size_t)W * p.T * kAccWords;
+        for (size_t i = tid; i < na; i += kFThreads) pv.acc[i] = 0ull;
+        for (int t = tid; t < p.T; t += kFThreads) pv.done[t] = 0;
+        if (tid == 0) { hdr->tile_cursor = 0; hdr->unit_cursor = 0; hdr->finish_count = 0; }
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) st_release_u64(&hdr->clean, want_token);
+    }
+    if (tid == 0) trace_stamp(p, 7);
+
+    // scheduling units: a pure function of (n_tiles, grid): 4 consecutive tiles, then 2, then single tiles near
+    // the end (guided self-scheduling with fixed boundaries). A *segment* = unit x tensor is what one FP32
+    // partial spans, so the value of every partial depends on the data only, not on which CTA took the unit.
+    const int sA = max(0, n_tiles - NF_TAIL4 * (int)gridDim.x) & ~3, nA = sA >> 2;
+    const int sB = sA + (max(0, n_tiles - NF_TAIL2 * (int)gridDim.x - sA) & ~1), nB = (sB - sA) >> 1;
+
+    if (warp == kCW) {
+        // =====================================================================================
+        // producer (one elected lane): issues the bulk copies of every (tile, worker group) of the units it
+        // takes from the device-wide cursor; a CTA that runs ahead (SM position, co-running decode warps)
+        // simply takes more. The stage carries its tile index (and whether the tile ends a segment).
+        // =====================================================================================
+        if (lane == 0) {
+            const uint64_t pol = policy_evict_first();
+            int32_t *cursor = &hdr->tile_cursor;
+            int pr_st = 0, pr_next = 0, pr_end = 0;
+            uint32_t pr_ph = 0;
+            TensorCur pc{};
+            pc.tile_e = 0;
+            for (;;) {
+                if (pr_next >= pr_end) {
+                    const int u = atomicAdd(cursor, 1);
+                    if (u < nA) { pr_next = 4 * u; pr_end = pr_next + 4; }
+                    else if (u < nA + nB) { pr_next = sA + 2 * (u - nA); pr_end = pr_next + 2; }
+                    else { pr_next = sB + (u - nA - nB); pr_end = pr_next + 1; }
+                }
+                const int pr_tile = pr_next;
+                if (pr_tile >= n_tiles) {
+                    mbar_wait(sm.empty + pr_st, pr_ph ^ 1u);
+                    sm.tile_of[pr_st] = -1;                            // sentinel: the consumers stop
+                    mbar_arrive(sm.full + pr_st);
+                    break;
+                }
+                if (pr_tile >= pc.tile_e) tensor_lookup(p, pv, sm, pr_tile, pc);
+                // run = the tiles of this unit inside the current tensor (one segment). Several worker groups
+                // (MULTI), low-bit or health: its stages go group-major (group 0 of tiles 0..R-1, then group 1,
+                // ...), so that the consumers flush the FP32 partials of a group once per run.
+                // (FP32-route tiles carry one running FP32 sum across the groups: they go one tile at a time.)
+                const int seg_len = min(pr_end, pc.tile_e) - pr_tile;   // <= 4
+                const int R = (MULTI && pc.isL) ? seg_len : 1;
+                pr_next += R;
+                for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {
+                    const int nw = MULTI ? min(kGroup, W - w0) : W;
+                    for (int r = 0; r < R; ++r) {
+                        const int64_t tile_base = (int64_t)(pr_tile + r - pc.tile_b) * kTile;
+                        const int64_t rem = pc.len - tile_base;
+                        const int need = rem >= kTile ? kTile : (int)rem;
+                        // aligned rows: whole float4s only (a partial one is read from global memory by its owner
+                        // thread). Unaligned rows: from the 16-byte boundary below the row to the one above its end
+                        // (whole 16-byte chunks, each holding at least one element of the row).
+                        const uint32_t bytes = (uint32_t)((need & ~3) * 4);
+                        const float *src = p.g + pc.off + tile_base;
+                        const int st = pr_st;
+                        mbar_wait(sm.empty + st, pr_ph ^ 1u);                  // first lap: passes at once
+                        sm.tile_of[st] = pr_tile + r;
+                        sm.seg_of[st] = MULTI ? 1 : (seg_len == 1);
+                        if (MULTI) sm.run_of[st] = R;
+                        float *dst = sm.ring + (size_t)st * kStageFloats;
+                        if (!pc.aligned) {
+                            uint32_t tx = 0;
+                            for (int w = 0; w < nw; ++w)
+                                tx += (uint32_t)((((int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3) + need + 3) & ~3) * 4);
+                            mbar_expect_tx(sm.full + st, tx);
+                            for (int w = 0; w < nw; ++w) {
+                                const int m = (int)((pc.off + (int64_t)(w0 + w) * p.worker_stride) & 3);
+                                bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride - m,
+                                         (uint32_t)(((m + need + 3) & ~3) * 4), sm.full + st, pol);
+                            }
+                        } else if (bytes) {
+                            mbar_expect_tx(sm.full + st, (uint32_t)nw * bytes);
+                            for (int w = 0; w < nw; ++w)
+                                bulk_g2s(dst + w * kPitch, src + (size_t)(w0 + w) * p.worker_stride, bytes, sm.full + st, pol);
+                        } else {
+                            mbar_arrive(sm.full + st);
+                        }
+                        if (++pr_st == stages) { pr_st = 0; pr_ph ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == kCW + 1) {
+        // =====================================================================================
+        // housekeeping warp: the outputs of the tensors that own no tile (len = 0): totals 0, scale 0 on the
+        // FP32 route and the oracle's 0/0 on the low-bit route (every other tensor is finalised by its last arriver)
+        // =====================================================================================
         for (int t = blockIdx.x * 32 + lane; t < p.T; t += (int)gridDim.x * 32) {
             int64_t len_t;
             bool isL;
             if (p.T <= kMetaCap) { len_t = sm.m_len[t]; isL = sm.m_woff[t] >= 0; }
             else { len_t = __ldg(p.len + t); isL = __ldg(p.route + t) == NF_ROUTE_L; }
-            if (isL && len_t > 0) continue;                       // published by the decode
-            const float S = isL ? tensor_scale(p.abs_sum, W, p.T, t, len_t) : 0.f;
+            if (len_t > 0) continue;
+            for (int w = 0; w < W; ++w) {
+                const size_t o = (size_t)w * p.T + t;
+                p.abs_sum[o] = 0.0;
+                if (HEALTH) { p.sumsq[o] = 0.0; p.nan_cnt[o] = 0ull; p.inf_cnt[o] = 0ull; }
+            }
+            double s = 0.0;
+            const double zero = 0.0, dl = (double)len_t;
+            for (int w = 0; w < W; ++w) s += (double)(float)(zero / dl);
+            const float S = isL ? (float)(s / (double)W) : 0.f;
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
-        return;
-    }
-
-    // =========================================================================================
-    // decode warps (pass B inside the kernel): see decode_units(). The consumers join them once
-    // their own tiles are done.
-    // =========================================================================================
-    if (warp >= kCW + 2) {
-        if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane, kDU);
+    } else if (warp >= kCW + 2) {
+        // =====================================================================================
+        // decode warps (pass B inside the kernel): see decode_units(). The consumers join them once
+        // their own tiles are done.
+        // =====================================================================================
+        decode_units(p, pv, sm, n_tiles, lane, kDU);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
-        return;
-    }
-
-    // =========================================================================================
-    // consumers
-    // =========================================================================================
-    const int ctid = tid;                       // 0..511
-    if (ctid == 0) trace_stamp(p, 0);
-    const TCtl tctl = make_tctl(lane);
-    const bool ternary = p.ternary != 0;
-    float af[8], qf[8];                         // FP32 partials of the current worker group
+    } else {
+        // =====================================================================================
+        // consumers
+        // =====================================================================================
+        const int ctid = tid;                       // 0..511
+        if (ctid == 0) trace_stamp(p, 0);
+        const TCtl tctl = make_tctl(lane);
+        const bool ternary = p.ternary != 0;
+        const int T = p.T;
+        float af[8], qf[8];                         // FP32 partials of the current worker group
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { af[i] = 0.f; qf[i] = 0.f; }
-    int kcnt = 0;
-    int4 recent = make_int4(0, 0, 0, 0);        // the last tiles accumulated in af/qf, most recent first
-    int st = 0;
-    uint32_t ph = 0;
-    TensorCur c{};
-    c.tile_e = 0;
-    c.t = -1;
-    bool touched = false;                       // this CTA accumulated something for tensor c.t
-    int ntile_acc = 0;                          // tiles of tensor c.t this CTA has finished
-    uint32_t *pP = nullptr, *pN = nullptr;      // this thread's plane-word / direction / output slots
-    uint8_t *pD = nullptr;                      //   of tile 0 of the current tensor
-    float *pO = nullptr;
+        for (int i = 0; i < 8; ++i) { af[i] = 0.f; qf[i] = 0.f; }
+        int kcnt = 0;
+        int4 recent = make_int4(0, 0, 0, 0);        // the last tiles accumulated in af/qf, most recent first
+        int st = 0;
+        uint32_t ph = 0;
+        TensorCur c{};
+        c.tile_e = 0;
+        c.t = -1;
+        bool touched = false;                       // this CTA processed tiles of tensor c.t
+        int ntile_acc = 0;                          // tiles of tensor c.t this CTA has finished
+        uint32_t *pP = nullptr, *pN = nullptr;      // this thread's plane-word / direction / output slots
+        uint8_t *pD = nullptr;                      //   of tile 0 of the current tensor
+        float *pO = nullptr;
+        const int nbuf = fused_nbuf(W);
+        int segpar = 0;                             // buffer of the current segment's per-warp FP64 values
+        double *wbuf = sm.wacc;
 
-    auto flush_tensor = [&]() __attribute__((always_inline)) {
-        if (!MULTI && kcnt > 0) { stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned); kcnt = 0; }
-        consumer_sync();
-        for (int j = ctid; j < 2 * W; j += kCThreads) {
-            double tot = 0.0;
+        // A segment (the tiles of one scheduling unit inside one tensor) is complete: its per-warp FP64 values are in
+        // `wbuf`. Sum them over the 16 warps in warp order (a fixed shape: the value depends on the data only) and add
+        // the segment's total EXACTLY to the tensor's accumulator (integer atomics: the order in which segments
+        // arrive, i.e. the dynamic scheduling, cannot change the result).
+        auto seg_reduce = [&]() __attribute__((always_inline)) {
+            consumer_sync();
+            if (ctid < 2 * W) {
+                const double *src = wbuf + ctid;
+                double tot = 0.0;
 #pragma unroll
-            for (int k = 0; k < kCW; ++k) { tot += sm.wacc[(size_t)k * 2 * W + j]; sm.wacc[(size_t)k * 2 * W + j] = 0.0; }
-            if (tot != 0.0) {
-                const size_t o = (size_t)(j >> 1) * p.T + c.t;
-                if ((j & 1) == 0) { if (c.isL) atomicAdd(p.abs_sum + o, tot); }
-                else if (HEALTH) atomicAdd(p.sumsq + o, tot);
+                for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
+                const int stat = ctid & 1;
+                unsigned long long *slot = pv.acc + ((size_t)(ctid >> 1) * T + c.t) * kAccWords;
+                if (stat == 0) { if (c.isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
+                else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
             }
-        }
-        if (HEALTH) {
-            for (int w = ctid; w < W; w += kCThreads) {
-                const unsigned cn_ = sm.nan[w], ci_ = sm.inf[w];
-                const size_t o = (size_t)w * p.T + c.t;
-                if (cn_) { atomicAdd(p.nan_cnt + o, (unsigned long long)cn_); sm.nan[w] = 0u; }
-                if (ci_) { atomicAdd(p.inf_cnt + o, (unsigned long long)ci_); sm.inf[w] = 0u; }
+            if (nbuf == 1) consumer_sync();         // one buffer (W > 32): the next segment overwrites it
+            else { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
+        };
+
+        // All tiles this CTA took of tensor c.t are done: hand in the NaN / Inf tallies, publish the tile count
+        // (release: direction bytes, plane words, outputs and accumulator adds of every consumer thread come first),
+        // and finalise the tensor if this publication completed it.
+        auto flush_tensor = [&]() __attribute__((always_inline)) {
+            if (c.isL || HEALTH) {
+                for (int w = ctid; w < W; w += kCThreads) {
+                    const unsigned cn_ = sm.nan[w], ci_ = sm.inf[w];
+                    unsigned long long *slot = pv.acc + ((size_t)w * T + c.t) * kAccWords;
+                    if (cn_) { atomicAdd(slot + kAccNan, (unsigned long long)cn_); sm.nan[w] = 0u; }
+                    if (ci_) { atomicAdd(slot + kAccInf, (unsigned long long)ci_); sm.inf[w] = 0u; }
+                }
             }
-        }
-        // publish: every consumer's direction bytes / plane words / atomics of this tensor are ordered
-        // before the counter the decode warps (of any CTA) acquire (FP32-route tensors have no decode)
-        if (c.isL) __threadfence();
-        consumer_sync();
-        if (ctid == 0 && c.isL) {
             __threadfence();
-            atomicAdd(pv.done + c.t, ntile_acc);
-        }
-        ntile_acc = 0;
-    };
+            consumer_sync();
+            if (ctid == 0) {
+                const int total = c.tile_e - c.tile_b;
+                const int old = atomicAdd(pv.done + c.t, ntile_acc);
+                const int last = (old + ntile_acc == total) ? 1 : 0;
+                if (last) __threadfence();
+                sm.flag[1] = last;
+            }
+            consumer_sync();
+            if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
+            ntile_acc = 0;
+        };
 
-    for (;;) {
-        mbar_wait(sm.full + st, ph);
-        const int tile = sm.tile_of[st];
-        if (tile < 0) break;
-        if (tile >= c.tile_e) {
-            if (touched) flush_tensor();
-            tensor_lookup(p, pv, sm, tile, c);
-            touched = false;
-            const size_t pl = (size_t)(lane & 7) * p.plane_stride + c.woff + warp * 4 + (lane >> 3);
-            pP = (c.isL && p.P) ? p.P + pl : nullptr;
-            pN = (c.isL && p.P && ternary) ? p.N + pl : nullptr;
-            pD = c.isL ? p.dirs + (size_t)c.woff * 8 + ctid : nullptr;
-            pO = p.out + c.off + 4 * ctid;
-        }
-        const int rel = tile - c.tile_b;
-        // MULTI, low-bit tensor: the producer sends a run of R consecutive tiles group-major (see there)
-        const int R = MULTI ? sm.run_of[st] : 1;
-        if (MULTI) recent = make_int4(tile + R - 1, tile + R - 2, tile + R - 3, tile + R - 4);
-        else recent = make_int4(tile, recent.x, recent.y, recent.z);
-        uint32_t posR = 0u, negR = 0u;
-        uint32_t cp0 = 0u, cp1 = 0u, cp2 = 0u, cp3 = 0u;     // byte-packed running counts of the run's tiles (MULTI)
-        uint32_t cn0 = 0u, cn1 = 0u, cn2 = 0u, cn3 = 0u;
-        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-        int valid = 0;
-        for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {   // one ring stage per (tile, worker group)
-            const int nw = MULTI ? min(kGroup, W - w0) : W;
-            for (int r = 0; r < R; ++r) {
-                if (MULTI && (w0 > 0 || r > 0)) mbar_wait(sm.full + st, ph);
-                const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
-                uint64_t *const empty_bar = sm.empty + st;
-                if (++st == stages) { st = 0; ph ^= 1u; }
-                const int64_t rem_t = c.len - (int64_t)(rel + r) * kTile;
-                const bool ragged = rem_t < kTile;              // last tile of the tensor, need < kTile elements
-                const int need = ragged ? (int)rem_t : kTile;
-                valid = min(max(need - 4 * ctid, 0), 4);
-                if (MULTI) { posR = 0u; negR = 0u; }
-                if (ragged || !c.aligned) {
-                    slow_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)(rel + r) * kTile + 4 * ctid,
-                                      p.worker_stride, nw, valid, !c.aligned, (int)((c.off + (int64_t)w0 * p.worker_stride) & 3),
-                                      (int)(p.worker_stride & 3), c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
-                                      w0 == 0);
-                } else if (c.isL) {
-                    const float tau = c.tau, ntau = -c.tau;
-                    if (ternary) {
-                        if (nw == kGroup) fast_signs<2, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
-                        else fast_signs<2, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
-                    } else {
-                        if (nw == kGroup) fast_signs<1, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
-                        else fast_signs<1, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
-                    }
-                } else {
-                    acc = (nw == kGroup) ? fast_fp32<HEALTH, true>(sb, nw, af, qf, acc, w0 == 0)
-                                         : fast_fp32<HEALTH, false>(sb, nw, af, qf, acc, w0 == 0);
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(empty_bar);          // every lane's reads of the stage are done
-                if (c.isL) {
-                    if (pP) {
-                        // packed plane words: 8x8 nibble transpose, lane q of an octet stores worker q's word
-                        const bool stp = ((lane & 7) < nw) && (32 * (warp * 4 + (lane >> 3)) < need);
-                        const size_t o = (size_t)(rel + r) * (kTile / 32) + (size_t)w0 * p.plane_stride;
-                        const uint32_t pw = nib_transpose8(posR, tctl);
-                        if (stp) pP[o] = pw;
+        for (;;) {
+            mbar_wait(sm.full + st, ph);
+            const int tile = sm.tile_of[st];
+            if (tile < 0) break;
+            if (tile >= c.tile_e) {
+                if (touched) flush_tensor();
+                tensor_lookup(p, pv, sm, tile, c);
+                touched = false;
+                const size_t pl = (size_t)(lane & 7) * p.plane_stride + c.woff + warp * 4 + (lane >> 3);
+                pP = (c.isL && p.P) ? p.P + pl : nullptr;
+                pN = (c.isL && p.P && ternary) ? p.N + pl : nullptr;
+                pD = c.isL ? p.dirs + (size_t)c.woff * 8 + ctid : nullptr;
+                pO = p.out + c.off + 4 * ctid;
+            }
+            const int rel = tile - c.tile_b;
+            const bool stats = c.isL || HEALTH;     // this tensor's totals are wanted
+            // MULTI: the producer sends a run of R consecutive tiles (one segment) group-major (see there)
+            const int R = MULTI ? sm.run_of[st] : 1;
+            const bool seg_end = MULTI ? true : (sm.seg_of[st] != 0);
+            if (MULTI) recent = make_int4(tile + R - 1, tile + R - 2, tile + R - 3, tile + R - 4);
+            else recent = make_int4(tile, recent.x, recent.y, recent.z);
+            uint32_t posR = 0u, negR = 0u;
+            uint32_t cp0 = 0u, cp1 = 0u, cp2 = 0u, cp3 = 0u;     // byte-packed running counts of the run's tiles (MULTI)
+            uint32_t cn0 = 0u, cn1 = 0u, cn2 = 0u, cn3 = 0u;
+            float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+            int valid = 0;
+            for (int w0 = 0; w0 < (MULTI ? W : 1); w0 += kGroup) {   // one ring stage per (tile, worker group)
+                const int nw = MULTI ? min(kGroup, W - w0) : W;
+                for (int r = 0; r < R; ++r) {
+                    if (MULTI && (w0 > 0 || r > 0)) mbar_wait(sm.full + st, ph);
+                    const float *sb = sm.ring + (size_t)st * kStageFloats + 4 * ctid;
+                    uint64_t *const empty_bar = sm.empty + st;
+                    if (++st == stages) { st = 0; ph ^= 1u; }
+                    const int64_t rem_t = c.len - (int64_t)(rel + r) * kTile;
+                    const bool ragged = rem_t < kTile;              // last tile of the tensor, need < kTile elements
+                    const int need = ragged ? (int)rem_t : kTile;
+                    valid = min(max(need - 4 * ctid, 0), 4);
+                    if (MULTI) { posR = 0u; negR = 0u; }
+                    if (ragged || !c.aligned) {
+                        slow_tile<HEALTH>(sb, p.g + (size_t)w0 * p.worker_stride + c.off + (int64_t)(rel + r) * kTile + 4 * ctid,
+                                          p.worker_stride, nw, valid, !c.aligned, (int)((c.off + (int64_t)w0 * p.worker_stride) & 3),
+                                          (int)(p.worker_stride & 3), c.isL, ternary, c.tau, -c.tau, af, qf, posR, negR, acc,
+                                          w0 == 0);
+                    } else if (c.isL) {
+                        const float tau = c.tau, ntau = -c.tau;
                         if (ternary) {
-                            const uint32_t nwd = nib_transpose8(negR, tctl);
-                            if (stp) pN[o] = nwd;
+                            if (nw == kGroup) fast_signs<2, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                            else fast_signs<2, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
+                        } else {
+                            if (nw == kGroup) fast_signs<1, HEALTH, true>(sb, nw, tau, ntau, af, qf, posR, negR);
+                            else fast_signs<1, HEALTH, false>(sb, nw, tau, ntau, af, qf, posR, negR);
+                        }
+                    } else {
+                        acc = (nw == kGroup) ? fast_fp32<HEALTH, true>(sb, nw, af, qf, acc, w0 == 0)
+                                             : fast_fp32<HEALTH, false>(sb, nw, af, qf, acc, w0 == 0);
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(empty_bar);          // every lane's reads of the stage are done
+                    if (c.isL) {
+                        if (pP) {
+                            // packed plane words: 8x8 nibble transpose, lane q of an octet stores worker q's word
+                            const bool stp = ((lane & 7) < nw) && (32 * (warp * 4 + (lane >> 3)) < need);
+                            const size_t o = (size_t)(rel + r) * (kTile / 32) + (size_t)w0 * p.plane_stride;
+                            const uint32_t pw = nib_transpose8(posR, tctl);
+                            if (stp) pP[o] = pw;
+                            if (ternary) {
+                                const uint32_t nwd = nib_transpose8(negR, tctl);
+                                if (stp) pN[o] = nwd;
+                            }
+                        }
+                        if (MULTI) {
+                            uint32_t dp = 0u, dn = 0u;
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) {
+                                dp += (uint32_t)__popc(posR & (0x11111111u << j)) << (8 * j);
+                                if (ternary) dn += (uint32_t)__popc(negR & (0x11111111u << j)) << (8 * j);
+                            }
+                            cp0 += r == 0 ? dp : 0u; cp1 += r == 1 ? dp : 0u; cp2 += r == 2 ? dp : 0u; cp3 += r == 3 ? dp : 0u;
+                            cn0 += r == 0 ? dn : 0u; cn1 += r == 1 ? dn : 0u; cn2 += r == 2 ? dn : 0u; cn3 += r == 3 ? dn : 0u;
                         }
                     }
-                    if (MULTI) {
-                        uint32_t dp = 0u, dn = 0u;
+                }
+                if (MULTI && stats)
+                    stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
+            }
+            if (c.isL) {
+                // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
+                if (!MULTI) {
+                    const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
+                    if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
+                } else {
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            dp += (uint32_t)__popc(posR & (0x11111111u << j)) << (8 * j);
-                            if (ternary) dn += (uint32_t)__popc(negR & (0x11111111u << j)) << (8 * j);
+                    for (int r = 0; r < kKTiles; ++r) {
+                        if (r < R) {
+                            const uint32_t d = vote4_packed(r == 0 ? cp0 : (r == 1 ? cp1 : (r == 2 ? cp2 : cp3)),
+                                                            r == 0 ? cn0 : (r == 1 ? cn1 : (r == 2 ? cn2 : cn3)), ternary, W, p.margin);
+                            if (c.len - (int64_t)(rel + r) * kTile > 4 * ctid) pD[(size_t)(rel + r) * (kTile / 4)] = (uint8_t)d;
                         }
-                        cp0 += r == 0 ? dp : 0u; cp1 += r == 1 ? dp : 0u; cp2 += r == 2 ? dp : 0u; cp3 += r == 3 ? dp : 0u;
-                        cn0 += r == 0 ? dn : 0u; cn1 += r == 1 ? dn : 0u; cn2 += r == 2 ? dn : 0u; cn3 += r == 3 ? dn : 0u;
                     }
                 }
-            }
-            if (MULTI && (c.isL || HEALTH))
-                stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
-        }
-        if (c.isL) {
-            // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
-            if (!MULTI) {
-                const uint32_t d = ternary ? vote4<true>(posR, negR, W, p.margin) : vote4<false>(posR, negR, W, p.margin);
-                if (valid > 0) pD[(size_t)rel * (kTile / 4)] = (uint8_t)d;
             } else {
-#pragma unroll
-                for (int r = 0; r < kKTiles; ++r) {
-                    if (r < R) {
-                        const uint32_t d = vote4_packed(r == 0 ? cp0 : (r == 1 ? cp1 : (r == 2 ? cp2 : cp3)),
-                                                        r == 0 ? cn0 : (r == 1 ? cn1 : (r == 2 ? cn2 : cn3)), ternary, W, p.margin);
-                        if (c.len - (int64_t)(rel + r) * kTile > 4 * ctid) pD[(size_t)(rel + r) * (kTile / 4)] = (uint8_t)d;
-                    }
+                float *o = pO + (size_t)rel * kTile;
+                float4 r = acc;
+                r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
+                r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
+                if (valid == 4 && c.aligned) {
+                    __stcs(reinterpret_cast<float4 *>(o), r);
+                } else {
+                    if (valid > 0) o[0] = r.x;
+                    if (valid > 1) o[1] = r.y;
+                    if (valid > 2) o[2] = r.z;
+                    if (valid > 3) o[3] = r.w;
                 }
             }
-        } else {
-            float *o = pO + (size_t)rel * kTile;
-            float4 r = acc;
-            r.x = __fmul_rn(p.alpha, r.x); r.y = __fmul_rn(p.alpha, r.y);
-            r.z = __fmul_rn(p.alpha, r.z); r.w = __fmul_rn(p.alpha, r.w);
-            if (valid == 4 && c.aligned) {
-                __stcs(reinterpret_cast<float4 *>(o), r);
-            } else {
-                if (valid > 0) o[0] = r.x;
-                if (valid > 1) o[1] = r.y;
-                if (valid > 2) o[2] = r.z;
-                if (valid > 3) o[3] = r.w;
+            touched = true;
+            ntile_acc += R;
+            if (!MULTI) ++kcnt;
+            if (stats && seg_end) {
+                if (!MULTI) {
+                    stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
+                    kcnt = 0;
+                }
+                seg_reduce();
+            } else if (!MULTI && seg_end) {
+                kcnt = 0;
             }
         }
-        touched = true;
-        ntile_acc += R;
-        if (!MULTI && ++kcnt == kKTiles) {
-            stat_flush<HEALTH>(p, sm, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
-            kcnt = 0;
-        }
+        if (ctid == 0) trace_stamp(p, 1);
+        if (touched) flush_tensor();
+        if (ctid == 0) trace_stamp(p, 2);
+        decode_units(p, pv, sm, n_tiles, lane, NF_KGRAB);     // help finish pass B
+        if (ctid == 0) trace_stamp(p, 3);
     }
-    if (ctid == 0) trace_stamp(p, 1);
-    if (touched) flush_tensor();
-    if (ctid == 0) trace_stamp(p, 2);
-    if (!p.separate_decode) decode_units(p, pv, sm, n_tiles, lane, NF_KGRAB);     // help finish pass B
-    if (ctid == 0) trace_stamp(p, 3);
+
+    // ---- the grid's last CTA resets the cursors and the completion counters: the plan is clean again ----
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        const int old = atomicAdd(&hdr->finish_count, 1);
+        const int last = (old == (int)gridDim.x - 1) ? 1 : 0;
+        if (last) __threadfence();
+        sm.flag[2] = last;
+    }
+    __syncthreads();
+    if (sm.flag[2]) {
+        for (int t = tid; t < p.T; t += kFThreads) pv.done[t] = 0;
+        if (tid == 0) { hdr->tile_cursor = 0; hdr->unit_cursor = 0; hdr->finish_count = 0; }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1078,9 +1201,13 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
     const size_t smem = fused_smem_bytes(stages, p.W);
     static bool configured = false;
     if (!configured) {
-        const size_t a = fused_smem_bytes(kStages, 64), b = fused_smem_bytes(2, 255);
+        size_t mx = 0;
+        for (int w = 1; w <= 255; ++w) {
+            const size_t b = fused_smem_bytes(w > 64 ? 2 : kStages, w);
+            mx = b > mx ? b : mx;
+        }
         cudaError_t e = cudaFuncSetAttribute(fused_passA_kernel<HEALTH, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)(a > b ? a : b));
+                                             (int)mx);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -1088,8 +1215,9 @@ static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t
     if (work <= 0) return cudaSuccess;
     int64_t grid = device_sm_count();                        // persistent: one CTA per SM
     if (grid > work) grid = work;
-    cudaError_t e = launch_kernel_ex(fused_passA_kernel<HEALTH, MULTI>, (unsigned)grid, kFThreads, smem, s, p.pdl != 0,
-                                     p.inkernel_route != 0, p, stages);
+    // No cooperative launch: no CTA ever waits for a CTA that has not started, so the grid need
+    // not be co-resident (other kernels may hold SMs, two calls may share the device).
+    cudaError_t e = launch_kernel(fused_passA_kernel<HEALTH, MULTI>, (unsigned)grid, kFThreads, smem, s, true, p, stages);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

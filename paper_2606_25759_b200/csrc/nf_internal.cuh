@@ -30,11 +30,32 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     int64_t n;
     int64_t Wd;                            // total packed words per worker plane
     int32_t n_tiles;
-    int32_t pad0;
-    int32_t tile_cursor;                   // fused path: next pass-A tile (dynamic scheduling over the CTAs)
+    int32_t finish_count;                  // fused path: CTAs that have finished (the last one resets the state below)
+    int32_t tile_cursor;                   // fused path: next pass-A scheduling unit (dynamic scheduling over the CTAs)
     int32_t unit_cursor;                   // fused path: next pass-B unit (half tile)
-    int64_t pad1[2];
+    unsigned long long clean;              // fused path: clean_token(T, W) while cursors, done[] and acc[] are all zero
+    int64_t acc_slots;                     // capacity of the acc region in (replica, tensor) slots
 };
+static_assert(sizeof(PlanHeader) == 64, "plan header layout");
+
+// ---------------------------------------------------------------------------------------------
+// Deterministic per-(worker, tensor) totals. abs_sum / sumsq are sums over millions of elements gathered by
+// many CTAs in an order that depends on the dynamic tile scheduling; floating-point atomics would make the last
+// bits (and, rarely, the FP32 scale) depend on that order. Instead every partial (a deterministic FP64 value:
+// the fixed-shape sum of one scheduling segment) is added EXACTLY into a wide fixed-point accumulator with
+// 64-bit integer atomics (integer addition commutes), and the tensor's last arriver rounds the exact total to
+// FP64 once. One slot = 32 x uint64 per (worker, tensor):
+//   words  0..9   sum |x|, word k holds the bits [2^(-149 + 32k), 2^(-149 + 32k + 32)) (+ deferred carries):
+//                 FP32 magnitudes are multiples of 2^-149 and 2^40 of them stay below 2^168;
+//   words 10..28  sum x^2 over finite x, same scheme from 2^-298 (up to 2^296);
+//   word  29 / 30 number of NaN / +-Inf elements;  word 31 unused.
+// A slot is all-zero between calls: whoever rounds it also clears it.
+// ---------------------------------------------------------------------------------------------
+constexpr int kAccWords = 32;
+constexpr int kAccAbs = 0, kAccAbsWords = 10, kAccAbsBase = -149;
+constexpr int kAccSq = 10, kAccSqWords = 19, kAccSqBase = -298;
+constexpr int kAccNan = 29, kAccInf = 30;
+constexpr int kDoneFinal = 0x40000000;     // done[t] bit: the tensor's totals and scale are published
 
 // Offsets (bytes) of the plan arrays for a bucket of T tensors.
 struct PlanLayout {
@@ -43,7 +64,8 @@ struct PlanLayout {
     size_t lt_woff;                        // int64 [T+1]   woff of the L tensors, lt_woff[nL] = Wd
     size_t scale;                          // float [T]     per-tensor scale scratch
     size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
-    size_t total;
+    size_t acc;                            // uint64 [R*T][kAccWords]  exact accumulators (R = workers / replicas)
+    size_t total;                          // without the acc region
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -56,8 +78,15 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
     L.lt_woff = o;     o = align_up(o + sizeof(int64_t) * (size_t)(T + 1), 16);
     L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
     L.done = o;        o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
-    L.total = o;
+    L.acc = align_up(o, 256);
+    L.total = L.acc;
     return L;
+}
+__host__ __device__ inline size_t plan_bytes_for(int T, int R) {
+    return plan_layout(T).acc + sizeof(unsigned long long) * kAccWords * (size_t)(T > 0 ? T : 1) * (size_t)(R > 0 ? R : 1);
+}
+__host__ __device__ inline unsigned long long clean_token(int T, int W) {
+    return 0x4e46434c45414e00ull ^ ((unsigned long long)(unsigned)T << 20) ^ (unsigned long long)(unsigned)W;
 }
 
 struct PlanView {
@@ -67,6 +96,7 @@ struct PlanView {
     const int64_t *lt_woff;
     float *scale;
     int32_t *done;
+    unsigned long long *acc;
 };
 
 __host__ __device__ inline PlanView plan_view(void *plan, int T) {
@@ -79,6 +109,7 @@ __host__ __device__ inline PlanView plan_view(void *plan, int T) {
     v.lt_woff = (const int64_t *)(p + L.lt_woff);
     v.scale = (float *)(p + L.scale);
     v.done = (int32_t *)(p + L.done);
+    v.acc = (unsigned long long *)(p + L.acc);
     return v;
 }
 
@@ -109,9 +140,7 @@ struct StreamParams {
     float *scale_out;          // [T] or NULL (fused path: the in-kernel decode publishes the scales)
     uint8_t *dirs;             // workspace: one byte per 4 low-bit elements (lo nibble +, hi nibble -)
     void *plan;
-    int separate_decode;       // A/B aid: 1 = no decode inside nf_fused.cu (decode_kernel does everything)
     unsigned long long *trace; // debug: per-CTA globaltimer stamps [grid][8], or NULL
-    int pdl;                   // launch with programmatic stream serialization (fused path)
     // in-kernel routing (fused path, T <= kMetaCap): step a1 is computed by the fused kernel itself
     int inkernel_route;
     const uint8_t *elig;       // [T]
@@ -120,6 +149,7 @@ struct StreamParams {
     uint8_t *route_w;          // [T] out
     int64_t *woff_w;           // [T] out
     int64_t *summary;          // [NF_SUM_LEN] out
+    int64_t acc_slots;         // capacity of the plan's accumulator region, in (replica, tensor) slots
 };
 
 enum : int {
@@ -146,24 +176,20 @@ struct ReduceParams {
     uint8_t *cpos;
     uint8_t *cneg;
     float *scale_out;
-    const uint8_t *dirs;       // decode pass of the fused path
     const uint32_t *cnt_pos;   // NEXT-1 merge: bit-sliced partial counts [(g*B + b)*count_stride + k], else NULL
     const uint32_t *cnt_neg;
     int64_t count_stride;
     int G, B;
-    int pdl;                   // launch with programmatic stream serialization (fused path)
     void *plan;
 };
 
 // launchers (each returns a cudaError_t from the launch)
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
-                         nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
-                         double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, int64_t worker_stride, int pdl, cudaStream_t s);
+                         nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan, size_t plan_bytes,
+                         int pdl, int zero_acc, cudaStream_t s);
 cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_fused_passA(bool health, const StreamParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s);
-cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s);
 cudaError_t launch_partial_count(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int Wg, int64_t Wd,
                                  int ternary, int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride,
                                  cudaStream_t s);
@@ -256,6 +282,46 @@ __device__ __forceinline__ int upper_tensor(const I *__restrict__ prefix, int T,
         if (__ldg(prefix + mid) <= x) lo = mid; else hi = mid;
     }
     return lo;
+}
+
+// ---- exact accumulators (see kAccWords above) -------------------------------------------------
+// acc += v for a finite v > 0 that is a multiple of 2^base: the 53-bit mantissa is cut at the 32-bit window
+// boundaries and every piece is added with a 64-bit integer atomic (no return value: RED)
+__device__ __forceinline__ void acc_add(unsigned long long *w, int nwords, int base, double v) {
+    const long long b = __double_as_longlong(v);
+    const int e = (int)((b >> 52) & 0x7ff);
+    if (e == 0 || e == 0x7ff) return;                    // 0 / denormal double / non-finite: not a partial we produce
+    unsigned long long m = ((unsigned long long)b & 0xfffffffffffffull) | (1ull << 52);
+    int p = e - 1075 - base;                             // position of the mantissa's bit 0 in the accumulator
+    if (p < 0) { m >>= -p; p = 0; }                      // (the bits shifted out are zero: v is a multiple of 2^base)
+    const int k = p >> 5, s = p & 31;
+    const unsigned long long lo = m << s;
+    const unsigned long long hi = s ? (m >> (64 - s)) : 0ull;
+    const unsigned long long p0 = lo & 0xffffffffull, p1 = lo >> 32;
+    if (p0 && k < nwords) atomicAdd(w + k, p0);
+    if (p1 && k + 1 < nwords) atomicAdd(w + k + 1, p1);
+    if (hi && k + 2 < nwords) atomicAdd(w + k + 2, hi);
+}
+// the exact total of `nwords` accumulator words rounded once (to nearest even) to FP64
+static __device__ __noinline__ double acc_round(const unsigned long long *w, int nwords, int base) {
+    unsigned long long d[20];
+    unsigned long long carry = 0ull;
+    int top = -1;
+    for (int k = 0; k < nwords; ++k) {
+        const unsigned long long t = w[k] + carry;
+        d[k] = t & 0xffffffffull;
+        carry = t >> 32;
+        if (d[k]) top = k;
+    }
+    if (top < 0) return 0.0;
+    const unsigned long long hi64 = (d[top] << 32) | (top >= 1 ? d[top - 1] : 0ull);
+    const unsigned long long lo32 = top >= 2 ? d[top - 2] : 0ull;
+    bool sticky = false;
+    for (int k = 0; k < top - 2; ++k) sticky |= d[k] != 0ull;
+    const int lz = __clzll((long long)hi64);             // 0..31: d[top] != 0
+    unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
+    if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;   // below the rounding position of a 64 -> 53 bit conversion
+    return scalbn(__ull2double_rn(mant), base + 32 * top + 31 - lz - 63);
 }
 
 // S_t = (float)( sum_w (double)(float)(A[w][t]/len_t) / W )   — PAPER L211 "mean-absolute scale",

@@ -1,5 +1,5 @@
-// nf_reduce.cu — step a3 (reducer-side compact sign-count aggregation + decode) and pass B of the
-// fused path (expand 2-bit directions by the per-tensor scale). PAPER §5.2 L211 ("sum these
+// nf_reduce.cu — step a3 (reducer-side compact sign-count aggregation + decode) and the two levels of
+// the hierarchical count (NEXT-1). PAPER §5.2 L211 ("sum these
 // indicators across workers ... majority voting ... writes the scaled aggregate direction back"),
 // §6.1 L247 ("recovering per-coordinate sign counts rather than numerically adding packed
 // machine words"), L76 (endpoint service = counting compact updates under fan-in W).
@@ -10,7 +10,6 @@
 // per 8 words, ~3 LOP3 per word), which leaves the per-element counts as 8 bit-planes; the
 // majority test with margin is then a bit-sliced compare that decides 32 elements at once.
 // The FP32 output is written warp-cooperatively (lane = element) so stores are 128-byte coalesced.
-#include <stdlib.h>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -117,20 +116,6 @@ __device__ __forceinline__ void count_words2(const uint32_t *__restrict__ P, con
             if (TERNARY) cn.add8(reinterpret_cast<const uint32_t(&)[8]>(xn[h]));
         }
     }
-}
-
-// every CTA computes the scales of the L tensors it may touch into shared memory; CTA 0 publishes
-__device__ __forceinline__ void compute_scales(const ReduceParams &p, const PlanView &pv, float *s_scale) {
-    for (int t = threadIdx.x; t < p.T; t += blockDim.x) {
-        float S = 0.f;
-        if (p.route[t] == NF_ROUTE_L) S = tensor_scale(p.abs_sum, p.W, p.T, t, p.len[t]);
-        s_scale[t] = S;
-        if (blockIdx.x == 0) {
-            pv.scale[t] = S;
-            if (p.scale_out) p.scale_out[t] = S;
-        }
-    }
-    __syncthreads();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -321,8 +306,7 @@ __device__ __forceinline__ void publish_wordless_scales(const ReduceParams &p, c
 
 // ---------------------------------------------------------------------------------------------
 // a3, register-staged variant: one thread walks the W words of its word position with plain loads.
-// Used for the level-2 merge of NEXT-1 (MERGE), for planes the bulk-copy engine cannot take (rows not
-// 16-byte aligned) and as the A/B comparator of the ring kernel below (NF_CR_LDG=1).
+// Used for planes / partial-count planes the bulk-copy engine cannot take (rows not 16-byte aligned).
 // resident CTAs per SM of the deep-round variant: 3 (80 registers, no spills) measured 20-25 % faster than 2
 // at W >= 32 (a thread walks W serially, so the bytes in flight per SM come from occupancy)
 // ---------------------------------------------------------------------------------------------
@@ -336,6 +320,7 @@ __global__ void __launch_bounds__(kRThreads, ROUND == 8 ? 4 : NF_CR_MINB) count_
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     const int64_t Wd = pv.hdr->Wd;
+    if (MERGE ? Wd > p.count_stride : Wd > p.plane_stride) return;     // rows shorter than the packed words: nothing is read
     const int nL = pv.hdr->nL;
     const int lane = threadIdx.x & 31;
     const int W = p.W;
@@ -438,6 +423,7 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
     const int64_t Wd = pv.hdr->Wd;
+    if (MERGE ? Wd > p.count_stride : Wd > p.plane_stride) return;     // rows shorter than the packed words: nothing is read
     const int nL = pv.hdr->nL;
     const int W = p.W;
     const bool ternary = p.ternary != 0;
@@ -532,91 +518,6 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     }
 }
 
-// Pass B of the fused path: out[off_t+i] = S_t * d for every low-bit element, d from the 2-bit
-// directions pass A left in the workspace (one byte per 4 elements: low nibble +, high nibble -).
-// Write-bound (4 B/element out, 0.25 B/element in). 128-thread CTAs; a warp owns 512 consecutive
-// elements of a tile: each lane loads one 32-bit word of directions (16 elements), the bytes are
-// redistributed by shuffle so that every store instruction writes 512 contiguous bytes; 4 tiles
-// are in flight per thread to cover the load latency.
-constexpr int kDThreads = 128;
-constexpr int kDUnroll = 4;
-
-struct DecodeTensor {
-    int tile_b, tile_e;
-    int64_t off_t, len_t, woff_t;
-    bool isL;
-    float S;
-};
-
-__global__ void __launch_bounds__(kDThreads) decode_kernel(const ReduceParams p) {
-    extern __shared__ float s_scale[];
-    pdl_launch_dependents();
-    pdl_wait();
-    const PlanView pv = plan_view(p.plan, p.T);
-    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    compute_scales(p, pv, s_scale);
-    const int n_tiles = pv.hdr->n_tiles;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    DecodeTensor c{0, 0, 0, 0, 0, false, 0.f};
-    for (int base = blockIdx.x * kDUnroll; base < n_tiles; base += gridDim.x * kDUnroll) {
-        uint32_t dw[kDUnroll];
-        int64_t obase[kDUnroll], rem[kDUnroll];
-        float S[kDUnroll];
-#pragma unroll
-        for (int k = 0; k < kDUnroll; ++k) {
-            const int tile = base + k;
-            rem[k] = 0; dw[k] = 0u; obase[k] = 0; S[k] = 0.f;
-            if (tile >= n_tiles) continue;
-            if (tile >= c.tile_e || tile < c.tile_b) {
-                const int t = upper_tensor<int32_t>(pv.tile_prefix, p.T, tile);
-                c.tile_b = __ldg(pv.tile_prefix + t);
-                c.tile_e = __ldg(pv.tile_prefix + t + 1);
-                c.off_t = __ldg(p.off + t);
-                c.len_t = __ldg(p.len + t);
-                c.isL = __ldg(p.route + t) == NF_ROUTE_L;
-                c.woff_t = c.isL ? __ldg(p.woff + t) : 0;
-                c.S = s_scale[t];
-            }
-            if (!c.isL) continue;
-            const int64_t wbase = (int64_t)(tile - c.tile_b) * kTile + warp * 512;   // tensor-relative
-            const int64_t i = wbase + lane * 16;
-            if (i < c.len_t)
-                dw[k] = __ldcs(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)c.woff_t * 8 + (size_t)(i >> 2)));
-            obase[k] = c.off_t + wbase;
-            rem[k] = c.len_t - wbase;           // elements of this warp's 512 that exist (may be <= 0)
-            S[k] = c.S;
-        }
-#pragma unroll
-        for (int k = 0; k < kDUnroll; ++k) {
-            if (rem[k] <= 0) continue;          // warp-uniform
-            const bool al = (obase[k] & 3) == 0;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
-                const uint32_t w32 = __shfl_sync(0xffffffffu, dw[k], j * 8 + (lane >> 2));
-                const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
-                const int64_t e0 = j * 128 + lane * 4;
-                const int64_t r = rem[k] - e0;
-                if (r <= 0) continue;
-                float4 v;
-                v.x = __fmul_rn(S[k], (float)((int)(d & 1u) - (int)((d >> 4) & 1u)));
-                v.y = __fmul_rn(S[k], (float)((int)((d >> 1) & 1u) - (int)((d >> 5) & 1u)));
-                v.z = __fmul_rn(S[k], (float)((int)((d >> 2) & 1u) - (int)((d >> 6) & 1u)));
-                v.w = __fmul_rn(S[k], (float)((int)((d >> 3) & 1u) - (int)((d >> 7) & 1u)));
-                float *o = p.out + obase[k] + e0;
-                if (r >= 4 && al) {
-                    __stcs(reinterpret_cast<float4 *>(o), v);
-                } else {
-                    o[0] = v.x;
-                    if (r > 1) o[1] = v.y;
-                    if (r > 2) o[2] = v.z;
-                    if (r > 3) o[3] = v.w;
-                }
-            }
-        }
-    }
-}
-
 // NEXT-1 level 1 ("node-local counting", L267): the bit-sliced per-position counts of one
 // group of Wg workers' packed planes, B planes per sign = the partial-count payload a node sends.
 __global__ void __launch_bounds__(kRThreads, 3)
@@ -653,9 +554,8 @@ static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_
     }
     const int grid = grid_for(units, NF_CRQ_MINB);
     // programmatic stream serialization: the kernel waits (griddepcontrol.wait) for its predecessor on the stream
-    // before it touches global memory; only its launch latency and shared-memory prologue overlap (NF_NO_PDL=1: off)
-    static const bool use_pdl = getenv("NF_NO_PDL") == nullptr;
-    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>, (unsigned)grid, kQThreads, kQSmem, s, use_pdl, p);
+    // before it touches global memory; only its launch latency and shared-memory prologue overlap
+    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>, (unsigned)grid, kQThreads, kQSmem, s, true, p);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -665,13 +565,12 @@ cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s
     const int grid = grid_for(chunks, 8);
     const bool counts = p.cpos || p.cneg;
     const bool small = !p.cnt_pos && p.W <= 16;              // shallow rounds, 4 CTAs per SM
-    static const bool force_ldg = getenv("NF_CR_LDG") != nullptr;       // A/B aid: register-staged kernel
     // the bulk copies need 16-byte-aligned rows: P, N are (nf_sign_count_reduce checks), so plane_stride % 4 == 0
     const int64_t units = (max_words + kQWords - 1) / kQWords;
-    if (!p.cnt_pos && !force_ldg && (p.plane_stride & 3) == 0)
+    if (!p.cnt_pos && (p.plane_stride & 3) == 0)
         return counts ? launch_ring<true, false>(p, units, s) : launch_ring<false, false>(p, units, s);
     // level-2 merge: rows of partial-count planes, same alignment rule
-    if (p.cnt_pos && !force_ldg && (p.count_stride & 3) == 0 && ((uintptr_t)p.cnt_pos & 15) == 0 &&
+    if (p.cnt_pos && (p.count_stride & 3) == 0 && ((uintptr_t)p.cnt_pos & 15) == 0 &&
         (!p.ternary || ((uintptr_t)p.cnt_neg & 15) == 0))
         return counts ? launch_ring<true, true>(p, units, s) : launch_ring<false, true>(p, units, s);
     if (p.cnt_pos) {
@@ -693,15 +592,6 @@ cudaError_t launch_partial_count(const uint32_t *P, const uint32_t *N, int64_t p
     if (Wd <= 0) return cudaSuccess;
     const int grid = grid_for((Wd + kRThreads - 1) / kRThreads, 8);
     partial_count_kernel<<<grid, kRThreads, 0, s>>>(P, N, plane_stride, Wg, Wd, ternary, B, cnt_pos, cnt_neg, count_stride);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_decode(const ReduceParams &p, int64_t n, cudaStream_t s) {
-    const int64_t max_tiles = n / kTile + p.T;
-    const size_t smem = sizeof(float) * (size_t)(p.T > 0 ? p.T : 1);
-    const int grid = grid_for((max_tiles + kDUnroll - 1) / kDUnroll, 16);
-    cudaError_t e = launch_kernel(decode_kernel, (unsigned)grid, kDThreads, smem, s, p.pdl != 0, p);
-    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 

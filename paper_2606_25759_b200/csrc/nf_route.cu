@@ -5,8 +5,9 @@
 //
 // One CTA of 1024 threads: the work is O(T) with T <= 8192 and must not cost a host round trip;
 // tensors are handled in chunks of 1024 with a warp-shuffle block scan carrying three running
-// sums (packed words, tiles, L-tensor count). The same kernel zeroes the accumulating outputs of
-// the fused path so that no separate memset node is needed on the stream.
+// sums (packed words, tiles, L-tensor count). It writes the plan's route-dependent arrays and header
+// fields only: the self-cleaning state of the fused path (cursors, completion counters, exact
+// accumulators, clean token) is never touched here.
 #include <stdlib.h>
 #include "nf_internal.cuh"
 
@@ -59,8 +60,7 @@ __global__ void __launch_bounds__(kRouteThreads, 1)
 route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
              const uint8_t *__restrict__ elig, int T, int64_t n, nf_state st,
              uint8_t *__restrict__ route, int64_t *__restrict__ woff, int64_t *__restrict__ summary,
-             void *plan, double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-             int64_t zcount, int64_t worker_stride) {
+             void *plan, int64_t acc_slots, int zero_acc) {
     pdl_launch_dependents();   // the next kernel may start its prologue
     pdl_wait();                // the previous call's kernels still read the plan / accumulators
     __shared__ Scan3 s_scan[33];
@@ -71,14 +71,11 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     int32_t *lt_index = (int32_t *)(pb + L.lt_index);
     int64_t *lt_woff = (int64_t *)(pb + L.lt_woff);
 
-    int32_t *done = (int32_t *)(pb + L.done);
-    for (int i = threadIdx.x; i < T; i += kRouteThreads) done[i] = 0;
-    // zero the accumulating outputs of the fused path (abs_sum, sumsq, nan, inf)
-    for (int64_t i = threadIdx.x; i < zcount; i += kRouteThreads) {
-        if (z0) z0[i] = 0.0;
-        if (z1) z1[i] = 0.0;
-        if (z2) z2[i] = 0ull;
-        if (z3) z3[i] = 0ull;
+    // stand-alone use (nf_route_bucket): the exact accumulators the streaming calls add into start from zero
+    // (they clear what they use, but the buffer may be fresh); the fused path keeps them clean itself
+    if (zero_acc) {
+        unsigned long long *acc = (unsigned long long *)(pb + L.acc);
+        for (int64_t i = threadIdx.x; i < acc_slots * kAccWords; i += kRouteThreads) acc[i] = 0ull;
     }
 
     Scan3 carry{0, 0, 0};
@@ -147,9 +144,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
         hdr->n = n;
         hdr->Wd = carry.words;
         hdr->n_tiles = (status == NF_OK) ? (int32_t)carry.tiles : 0;
-        hdr->pad0 = 0;
-        hdr->tile_cursor = 0;
-        hdr->unit_cursor = 0;
+        hdr->acc_slots = acc_slots;
         summary[NF_SUM_WD] = carry.words;
         summary[NF_SUM_NL] = carry.nl;
         summary[NF_SUM_NF] = (int64_t)s_tal[0];
@@ -162,11 +157,12 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
 }
 
 cudaError_t launch_route(const int64_t *off, const int64_t *len, const uint8_t *elig, int T, int64_t n,
-                         nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan,
-                         double *z0, double *z1, unsigned long long *z2, unsigned long long *z3,
-                         int64_t zcount, int64_t worker_stride, int pdl, cudaStream_t s) {
+                         nf_state st, uint8_t *route, int64_t *woff, int64_t *summary, void *plan, size_t plan_bytes,
+                         int pdl, int zero_acc, cudaStream_t s) {
+    const size_t base = plan_layout(T).acc;
+    const int64_t acc_slots = plan_bytes > base ? (int64_t)((plan_bytes - base) / (sizeof(unsigned long long) * kAccWords)) : 0;
     cudaError_t e = launch_kernel(route_kernel, 1, kRouteThreads, 0, s, pdl != 0, off, len, elig, T, n, st, route, woff, summary,
-                                  plan, z0, z1, z2, z3, zcount, worker_stride);
+                                  plan, acc_slots, zero_acc);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

@@ -1,6 +1,6 @@
-// nf_stream.cu — the streaming kernel family: steps a2 (pack), a4a (FP32 route), a4b (health) and
-// pass A of the fused path (route-aware pack + sign count + majority vote + FP32 sum + health from
-// ONE read of the W x n gradients). PAPER §5.2, §3.3; SURVEY §8(a).
+// nf_stream.cu — the stand-alone streaming calls: steps a2 (pack), a4a (FP32 route) and a4b (health),
+// each one read of its input. PAPER §5.2, §3.3; SURVEY §8(a). (The fused path, which does
+// all of them and the count/vote/decode from ONE read of the W x n gradients, is nf_fused.cu.)
 //
 // HBM-bound elementwise streaming (no contraction -> no tensor cores). Design for sm_100a:
 //  * persistent grid (multiple of the SM count), CTAs walk tiles of ONE tensor (tensor-relative
@@ -11,9 +11,10 @@
 //    per-position counts are popcounts of that register under a 0x11111111 mask, and the packed
 //    32-bit plane words come from an 8x8 nibble transpose across 8 lanes (3 shuffles);
 //  * per-(worker,tensor) abs-sum / sum-of-squares run in FP32 over 8 elements, then FP64 per
-//    thread, one block reduce-scatter + FP64 atomics per tensor change.
+//    thread, one fixed-shape block reduce-scatter per tensor change, and the block's total goes EXACTLY
+//    into the plan's wide fixed-point accumulators (integer atomics, nf_internal.cuh): the result does
+//    not depend on the order in which the CTAs arrive; finalize_kernel rounds each total to FP64 once.
 #include <float.h>
-#include <stdlib.h>
 #include "nf_internal.cuh"
 
 namespace nf {
@@ -89,10 +90,12 @@ struct FlushCtx {
     double (*s_red)[16];
     unsigned int *s_nan;
     unsigned int *s_inf;
+    unsigned long long *acc;    // the plan's exact accumulators, [W*T][kAccWords]
 };
 
-// Block-reduce the per-thread FP64 partials of one worker group and add them to the global
-// per-(worker,tensor) accumulators. CTA-uniform call.
+// Block-reduce the per-thread FP64 partials of one worker group (fixed shape: with the static tile striding of
+// this kernel the value is a function of the data and the grid size only) and add the block's totals exactly
+// to the per-(worker,tensor) accumulators; NaN / Inf are tallied, never added. CTA-uniform call.
 template <int FLAGS>
 __device__ __forceinline__ void flush_stats(const StreamParams &p, const FlushCtx &c, double (&a)[8],
                                             double (&q)[8], int w0, int nw, int t, bool isL) {
@@ -111,20 +114,20 @@ __device__ __forceinline__ void flush_stats(const StreamParams &p, const FlushCt
 #pragma unroll
         for (int k = 0; k < kThreads / 32; ++k) tot += c.s_red[k][j];
         if (w < nw) {
-            const size_t o = (size_t)(w0 + w) * p.T + t;
+            unsigned long long *slot = c.acc + ((size_t)(w0 + w) * p.T + t) * kAccWords;
             if (j < 8) {
-                if (PACK && isL && p.abs_sum && tot != 0.0) atomicAdd(p.abs_sum + o, tot);
+                if (PACK && isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot);
             } else {
-                if (HEALTH && p.sumsq && tot != 0.0) atomicAdd(p.sumsq + o, tot);
+                if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
             }
         }
-    } else if (HEALTH && threadIdx.x >= 32 && threadIdx.x < 40) {
+    } else if (threadIdx.x >= 32 && threadIdx.x < 40) {
         const int w = threadIdx.x - 32;
         const unsigned int cn = c.s_nan[w], ci = c.s_inf[w];
-        if (w < nw && p.nan_cnt) {
-            const size_t o = (size_t)(w0 + w) * p.T + t;
-            if (cn) atomicAdd(p.nan_cnt + o, (unsigned long long)cn);
-            if (ci) atomicAdd(p.inf_cnt + o, (unsigned long long)ci);
+        if (w < nw && (HEALTH || isL)) {
+            unsigned long long *slot = c.acc + ((size_t)(w0 + w) * p.T + t) * kAccWords;
+            if (cn) atomicAdd(slot + kAccNan, (unsigned long long)cn);
+            if (ci) atomicAdd(slot + kAccInf, (unsigned long long)ci);
         }
         c.s_nan[w] = 0u;
         c.s_inf[w] = 0u;
@@ -150,8 +153,7 @@ __device__ __forceinline__ int tile_elem(int warp, int lane, int u) { return war
 
 template <int FLAGS>
 __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams p) {
-    constexpr bool PACK = FLAGS & kFPack, COUNT = FLAGS & kFCount, FP32 = FLAGS & kFFp32,
-                   HEALTH = FLAGS & kFHealth;
+    constexpr bool PACK = FLAGS & kFPack, FP32 = FLAGS & kFFp32, HEALTH = FLAGS & kFHealth;
     constexpr bool STATS = PACK || HEALTH;
     __shared__ double s_red[kThreads / 32][16];
     __shared__ unsigned int s_nan[8], s_inf[8];
@@ -159,11 +161,13 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
     pdl_wait();
     const PlanView pv = plan_view(p.plan, p.T);
     if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    if (STATS && (int64_t)p.W * p.T > pv.hdr->acc_slots) return;      // plan too small: finalize_kernel reports it
+    if (PACK && p.P && pv.hdr->Wd > p.plane_stride) return;           // plane rows too short: likewise
     const int n_tiles = pv.hdr->n_tiles;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 8) { s_nan[tid] = 0u; s_inf[tid] = 0u; }
     __syncthreads();
-    const FlushCtx fc{s_red, s_nan, s_inf};
+    const FlushCtx fc{s_red, s_nan, s_inf, pv.acc};
     const TransposeCtl tctl = make_transpose_ctl(lane);
 
     const int W = p.W;
@@ -194,7 +198,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
             ntau = -tau;
             aligned = (((off_t | p.worker_stride) & 3) == 0);
         }
-        const bool do_tile = HEALTH || (isL ? (PACK || COUNT) : FP32);
+        const bool do_tile = HEALTH || (isL ? PACK : FP32);
         if (!do_tile) continue;
         if (STATS && !multi && acc_t != t) {
             if (acc_t >= 0) flush_stats<FLAGS>(p, fc, a, q, 0, W, acc_t, acc_isL);
@@ -211,11 +215,10 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
             const int64_t rem = len_t - irel[u];
             valid[u] = rem >= 4 ? 4 : (rem > 0 ? (int)rem : 0);
         }
-        uint32_t cp[kRows], cn[kRows];       // multi-group: byte-packed per-position counts
         uint32_t posR[kRows], negR[kRows];
         float4 acc[kRows];                   // FP32-route running sums
 #pragma unroll
-        for (int u = 0; u < kRows; ++u) { cp[u] = 0u; cn[u] = 0u; acc[u] = make_float4(0.f, 0.f, 0.f, 0.f); }
+        for (int u = 0; u < kRows; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
 
         for (int w0 = 0; w0 < W; w0 += kGroup) {
             const int nw = min(kGroup, W - w0);
@@ -273,7 +276,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                         badmask |= ok ? 0u : (1u << w);
                     }
                     if (KIND != 0) {
-                        if (PACK || COUNT) {
+                        if (PACK) {
 #pragma unroll
                             for (int u = 0; u < kRows; ++u) {
                                 const float4 v = x[u][w];
@@ -313,11 +316,11 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
 #pragma unroll
                             for (int j = 0; j < 4; ++j) {
                                 const float v = e4[j];
-                                a[w] += (double)fabsf(v);
-                                if (HEALTH) {
-                                    if (v != v) atomicAdd(&s_nan[w], 1u);
-                                    else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[w], 1u);
-                                    else q[w] += (double)v * (double)v;
+                                if (v != v) atomicAdd(&s_nan[w], 1u);
+                                else if (fabsf(v) == INFINITY) atomicAdd(&s_inf[w], 1u);
+                                else {
+                                    a[w] += (double)fabsf(v);
+                                    if (HEALTH) q[w] += (double)v * (double)v;
                                 }
                             }
                         }
@@ -335,16 +338,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
                 else body(BoolTag<false>{}, IntTag<0>{});
             }
 
-            if (isL && (PACK || COUNT)) {
-                if (COUNT && multi) {
-#pragma unroll
-                    for (int u = 0; u < kRows; ++u)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            cp[u] += (uint32_t)__popc(posR[u] & (0x11111111u << j)) << (8 * j);
-                            if (ternary) cn[u] += (uint32_t)__popc(negR[u] & (0x11111111u << j)) << (8 * j);
-                        }
-                }
+            if (isL && PACK) {
                 if (PACK && p.P) {
                     const int wq = lane & 7;
                     const int64_t nwords = (len_t + 31) >> 5;
@@ -365,31 +359,7 @@ __global__ void __launch_bounds__(kThreads, 2) stream_kernel(const StreamParams 
             if (multi && STATS) flush_stats<FLAGS>(p, fc, a, q, w0, nw, t, isL);
         }
 
-        if (isL) {
-            if (COUNT) {
-                // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
-#pragma unroll
-                for (int u = 0; u < kRows; ++u) {
-                    uint32_t d = 0u;
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) {
-                        int c_p, c_n;
-                        if (multi) {
-                            c_p = (cp[u] >> (8 * j)) & 0xff;
-                            c_n = (cn[u] >> (8 * j)) & 0xff;
-                        } else {
-                            c_p = __popc(posR[u] & (0x11111111u << j));
-                            c_n = __popc(negR[u] & (0x11111111u << j));
-                        }
-                        if (!ternary) c_n = W - c_p;
-                        const int D = c_p - c_n;
-                        d |= (D > p.margin ? 1u : 0u) << j;
-                        d |= (D < -p.margin ? 1u : 0u) << (4 + j);
-                    }
-                    if (valid[u] > 0) p.dirs[(size_t)woff_t * 8 + (size_t)(irel[u] >> 2)] = (uint8_t)d;
-                }
-            }
-        } else if (FP32) {
+        if (!isL && FP32) {
 #pragma unroll
             for (int u = 0; u < kRows; ++u) {
                 float *o = p.out + off_t + irel[u];
@@ -424,6 +394,51 @@ int device_sm_count() {
     return sms;
 }
 
+// Rounds the exact totals of every (replica, tensor) slot to FP64 once, writes the call's outputs and clears the
+// slots (one thread per slot). FLAGS as in stream_kernel. A plan whose accumulator region is too small for W x T
+// slots is reported by poisoning the plan (status NF_ERR_ARG), like a bad layout.
+template <int FLAGS>
+__global__ void __launch_bounds__(128) finalize_kernel(const StreamParams p) {
+    constexpr bool PACK = FLAGS & kFPack, HEALTH = FLAGS & kFHealth;
+    pdl_launch_dependents();
+    pdl_wait();
+    const PlanView pv = plan_view(p.plan, p.T);
+    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
+    const int64_t slots = (int64_t)p.W * p.T;
+    if (slots > pv.hdr->acc_slots || (PACK && p.P && pv.hdr->Wd > p.plane_stride)) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) const_cast<PlanHeader *>(pv.hdr)->status = NF_ERR_ARG;
+        return;
+    }
+    const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= slots) return;
+    const int t = (int)(o % p.T);
+    unsigned long long wd[kAccWords];
+    ulonglong2 *slot = reinterpret_cast<ulonglong2 *>(pv.acc + (size_t)o * kAccWords);
+#pragma unroll
+    for (int i = 0; i < kAccWords / 2; ++i) {
+        const ulonglong2 v = __ldcg(slot + i);
+        wd[2 * i] = v.x;
+        wd[2 * i + 1] = v.y;
+    }
+#pragma unroll
+    for (int i = 0; i < kAccWords / 2; ++i) __stcg(slot + i, make_ulonglong2(0ull, 0ull));
+    const unsigned long long cn = wd[kAccNan], ci = wd[kAccInf];
+    if (PACK) {
+        double A = 0.0;
+        if (p.route[t] == NF_ROUTE_L) {
+            A = acc_round(wd + kAccAbs, kAccAbsWords, kAccAbsBase);
+            if (cn) A = __longlong_as_double(0x7ff8000000000000ll);          // IEEE: NaN term -> NaN, Inf term -> +Inf
+            else if (ci) A = __longlong_as_double(0x7ff0000000000000ll);
+        }
+        p.abs_sum[o] = A;
+    }
+    if (HEALTH) {
+        p.sumsq[o] = acc_round(wd + kAccSq, kAccSqWords, kAccSqBase);
+        p.nan_cnt[o] = cn;
+        p.inf_cnt[o] = ci;
+    }
+}
+
 template <int FLAGS>
 static cudaError_t launch_stream_t(const StreamParams &p, int64_t n, cudaStream_t s) {
     static int per_sm = 0;
@@ -437,8 +452,13 @@ static cudaError_t launch_stream_t(const StreamParams &p, int64_t n, cudaStream_
     if (max_tiles <= 0) return cudaSuccess;
     int64_t grid = (int64_t)device_sm_count() * per_sm;     // persistent: a multiple of the SM count
     if (grid > max_tiles) grid = max_tiles;
-    cudaError_t e = launch_kernel(stream_kernel<FLAGS>, (unsigned)grid, kThreads, 0, s, p.pdl != 0, p);
+    cudaError_t e = launch_kernel(stream_kernel<FLAGS>, (unsigned)grid, kThreads, 0, s, true, p);
     if (e != cudaSuccess) return e;
+    if (FLAGS & (kFPack | kFHealth)) {
+        const int64_t slots = (int64_t)p.W * p.T;
+        e = launch_kernel(finalize_kernel<FLAGS>, (unsigned)((slots + 127) / 128), 128, 0, s, true, p);
+        if (e != cudaSuccess) return e;
+    }
     return cudaGetLastError();
 }
 
@@ -447,9 +467,6 @@ cudaError_t launch_stream(int flags, const StreamParams &p, int64_t n, cudaStrea
         case kFPack: return launch_stream_t<kFPack>(p, n, s);
         case kFFp32: return launch_stream_t<kFFp32>(p, n, s);
         case kFHealth: return launch_stream_t<kFHealth>(p, n, s);
-        case kFPack | kFCount | kFFp32: return launch_stream_t<kFPack | kFCount | kFFp32>(p, n, s);
-        case kFPack | kFCount | kFFp32 | kFHealth:
-            return launch_stream_t<kFPack | kFCount | kFFp32 | kFHealth>(p, n, s);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -33,6 +33,7 @@ def test_host_side_checks_need_no_gpu(nf):
     assert lib.nf_version() >= 100
     assert nf.status_string(0) == "NF_OK"
     assert nf.nf_plan_bytes(0) >= 64 and nf.nf_plan_bytes(100) > nf.nf_plan_bytes(10)
+    assert nf.nf_plan_bytes(10, 8) - nf.nf_plan_bytes(10, 1) == 7 * 10 * 256      # 256-byte exact accumulator per (replica, tensor)
     assert nf.nf_workspace_bytes(3, 1 << 20) >= (1 << 20) // 4
     st = nf.NfState(1, 0, 1)
     fake = 0x1000                     # never dereferenced: the range/alignment checks come first

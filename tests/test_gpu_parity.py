@@ -204,16 +204,29 @@ def test_host_buffer_entry_point_matches_oracle():
     g_host = torch.empty((cfg.W, stride), dtype=torch.float32, pin_memory=True)
     g_host.copy_(g_dev_src)
     ref = O.aggregate_bucket(np.ascontiguousarray(g_host.numpy()[:, :b.n]), b.off, b.length, b.elig)
-    bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=False, health=True)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, DEV, planes=True, health=True)
     staging = torch.zeros((cfg.W, stride), dtype=torch.float32, device=DEV)
     out_host = torch.full((b.n,), -3.0, dtype=torch.float32).pin_memory()
     nf.nf_aggregate_bucket_host(g_host, staging, stride, cfg.W, b.n, bb.off, bb.len, bb.elig, bb.T, (1, 0, 1),
-                                nf.MODE_GTERNARY, None, 0, 1.0, bb.route, bb.woff, bb.summary, bb.abs_sum, bb.sumsq,
-                                bb.nan_cnt, bb.inf_cnt, bb.out, out_host, bb.plan, bb.workspace)
+                                nf.MODE_GTERNARY, None, 0, 1.0, bb.route, bb.woff, bb.summary, bb.P, bb.N,
+                                bb.plane_stride, bb.abs_sum, bb.sumsq, bb.nan_cnt, bb.inf_cnt, bb.out, out_host, bb.plan,
+                                bb.workspace)
     torch.cuda.synchronize()
-    compare(bb, ref, cfg.W, O.MODE_GTERNARY, check_planes=False, check_scale=False,      # the host call has no scale_out
+    compare(bb, ref, cfg.W, O.MODE_GTERNARY, check_scale=False,      # the host call has no scale_out
             what="host entry point")
     assert np.array_equal(out_host.numpy(), _np(bb.out)[:b.n])
+    # rows `stride` apart with a host / staging buffer that ends with the last row (the copy must not
+    # run past (W-1)*stride + n floats)
+    stride2 = b.n + 8
+    flat = torch.zeros((cfg.W - 1) * stride2 + b.n, dtype=torch.float32).pin_memory()
+    for w in range(cfg.W):
+        flat[w * stride2: w * stride2 + b.n] = g_host[w, :b.n]
+    staging2 = torch.zeros_like(flat, device=DEV)
+    nf.nf_aggregate_bucket_host(flat, staging2, stride2, cfg.W, b.n, bb.off, bb.len, bb.elig, bb.T, (1, 0, 1),
+                                nf.MODE_GTERNARY, None, 0, 1.0, bb.route, bb.woff, bb.summary, None, None, 0,
+                                bb.abs_sum, bb.sumsq, bb.nan_cnt, bb.inf_cnt, bb.out, out_host, bb.plan, bb.workspace)
+    torch.cuda.synchronize()
+    compare(bb, ref, cfg.W, O.MODE_GTERNARY, check_planes=False, check_scale=False, what="host entry point, tight buffer")
 
 
 @pytest.mark.parametrize("seed", range(24))
