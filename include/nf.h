@@ -90,8 +90,10 @@ int nf_version(void);
 /* Bytes of the device "plan" buffer for a bucket of T tensors used with up to R workers / replicas (host
  * call): the route-dependent tile map the streaming kernels walk, per-tensor scratch (scales, completion
  * counters) and R x T exact accumulators of 256 bytes for the per-(replica, tensor) totals. R = the largest
- * W (or R of nf_health_stats) any call will be given this plan with. 16-byte aligned buffer required; its
- * contents need no initialisation and must not be modified by the caller between calls. */
+ * W (or R of nf_health_stats) any call will be given this plan with. 16-byte aligned buffer required. The
+ * buffer must be zero-filled ONCE before its first use (cudaMemset / torch.zeros) and not modified by the caller
+ * afterwards: the fused call recognises a plan whose state it left clean by a 32-bit token in the header and
+ * re-initialises anything else itself. */
 size_t nf_plan_bytes(int T, int R);
 
 /* Bytes of the device workspace nf_aggregate_bucket needs for a bucket of n elements (host call):
@@ -283,10 +285,11 @@ int nf_supervisor_step(nf_supervisor *s /*host*/, double signal, uint64_t nan_co
 /*
  * Debugging aid, NOT part of the data path and NOT thread-safe (one process-global buffer: use it from one host
  * thread, with no nf_aggregate_bucket call in flight on another). nf_debug_trace(1, NULL) allocates a device
- * buffer of 256 x 8 globaltimer stamps that every CTA of the fused kernel fills from then on (kernel entry,
- * after the dependency wait, after the routing and the clean-token check, consumers start, tiles exhausted,
- * last tensor flushed, decode done); with `out` != NULL (room for 2048 uint64, HOST) the stamps are copied out
- * (synchronises the device); nf_debug_trace(0, ...) frees the buffer.
+ * buffer of 2 x 256 x 16 globaltimer stamps; from then on every CTA of the fused kernel fills its row (kernel
+ * entry, after the dependency wait, after the routing and the clean-token check, consumers start, tiles
+ * exhausted, last tensor flushed, decode done, kernel end), successive calls alternating between the two halves;
+ * with `out` != NULL (room for 8192 uint64, HOST) the stamps are copied out (synchronises the device);
+ * nf_debug_trace(0, ...) frees the buffer.
  */
 int nf_debug_trace(int on, unsigned long long *out /*host*/);
 

@@ -272,10 +272,11 @@ class Supervisor:
 
 
 def nf_debug_trace(on: int, fetch: bool = False):
-    """Debugging aid (single-threaded): per-CTA globaltimer stamps of the fused kernel, [256][8] uint64 or None."""
+    """Debugging aid (single-threaded): per-CTA globaltimer stamps of the last two fused
+    kernels, [2][256][16] uint64, or None."""
     import numpy as np
-    buf = np.zeros(2048, np.uint64) if fetch else None
+    buf = np.zeros(2 * 256 * 16, np.uint64) if fetch else None
     rc = lib().nf_debug_trace(int(on), buf.ctypes.data if fetch else None)
     if rc != NF_OK:
         raise NfError("nf_debug_trace", rc)
-    return buf.reshape(256, 8) if fetch else None
+    return buf.reshape(2, 256, 16) if fetch else None

@@ -6,6 +6,7 @@ using namespace nf;
 
 namespace {
 
+unsigned g_trace_calls = 0;
 unsigned long long *g_trace = nullptr;   // debug (nf_debug_trace, single-threaded use): per-CTA time stamps of the fused kernel
 inline bool misaligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 inline int cuda_rc(cudaError_t e) { return e == cudaSuccess ? NF_OK : NF_ERR_CUDA; }
@@ -222,7 +223,7 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
     p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
     p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
     p.scale_out = scale_out;
-    p.trace = g_trace;
+    p.trace = g_trace ? g_trace + (size_t)(g_trace_calls++ & 1) * 256 * 16 : nullptr;
     p.inkernel_route = inkernel ? 1 : 0;
     p.elig = elig; p.st = state; p.n = n; p.route_w = route; p.woff_w = woff; p.summary = summary;
     p.acc_slots = (int64_t)((plan_bytes - plan_layout(T).acc) / (sizeof(unsigned long long) * kAccWords));
@@ -232,8 +233,13 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
 // debug aid (nf.h): enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;
 // with `out` != NULL the stamps are copied to the host (synchronises).
 int nf_debug_trace(int on, unsigned long long *out) {
-    if (on && !g_trace) { if (cudaMalloc(&g_trace, 256 * 8 * 8) != cudaSuccess) return NF_ERR_CUDA; cudaMemset(g_trace, 0, 256 * 8 * 8); }
-    if (out && g_trace && cudaMemcpy(out, g_trace, 256 * 8 * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return NF_ERR_CUDA;
+    const size_t bytes = 2 * 256 * 16 * sizeof(unsigned long long);
+    if (on && !g_trace) {
+        if (cudaMalloc(&g_trace, bytes) != cudaSuccess) return NF_ERR_CUDA;
+        cudaMemset(g_trace, 0, bytes);
+        g_trace_calls = 0;
+    }
+    if (out && g_trace && cudaMemcpy(out, g_trace, bytes, cudaMemcpyDeviceToHost) != cudaSuccess) return NF_ERR_CUDA;
     if (!on && g_trace) { cudaFree(g_trace); g_trace = nullptr; }
     return NF_OK;
 }

@@ -38,9 +38,6 @@ constexpr int kCThreads = kCW * 32;              // 512 threads x 4 elements = o
 #ifndef NF_KKT
 #define NF_KKT 4
 #endif
-#ifndef NF_KGRAB
-#define NF_KGRAB 2                       // decode units a consumer warp takes per trip to the cursor at the end
-#endif
 #ifndef NF_KCHUNK
 #define NF_KCHUNK 4                      // longest run of consecutive tiles one CTA takes at a time
 #endif
@@ -451,7 +448,7 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
     if (p.trace) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-        p.trace[(size_t)blockIdx.x * 8 + slot] = t;
+        p.trace[(size_t)blockIdx.x * 16 + slot] = t;
     }
 }
 
@@ -460,113 +457,142 @@ __device__ __forceinline__ void trace_stamp(const StreamParams &p, int slot) {
 __device__ __noinline__ void report_timeout(const StreamParams &p) {
     PlanHeader *hdr = (PlanHeader *)p.plan;
     hdr->status = NF_ERR_CUDA;
-    hdr->clean = 0ull;
+    hdr->sched = 0ull;
     if (p.summary) p.summary[NF_SUM_STATUS] = NF_ERR_CUDA;
     __threadfence();
 }
 
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
-// pass B inside the kernel: out[off_t+i] = S_t * d for the low-bit tiles this CTA owns, as soon as
-// tensor t is complete (all its tiles published by every CTA: plan.done[t] == tiles of t). A unit
-// is half a tile (1024 elements); warps take kDU units at a time from a per-CTA cursor in shared
-// memory, in tile order, so the wait is always on the earliest unfinished tensor. The dedicated
-// decode warps overlap their stores with the consumers' reads of later tensors; the consumers
-// join when their own tiles are done. Every store instruction writes 512 contiguous bytes.
+// pass B inside the kernel: out[off_t+i] = S_t * d for the low-bit tiles, as soon as tensor t is complete and
+// finalised (plan.fin[t] != 0: every CTA's tiles of t are published and the tensor's last arriver has rounded
+// the totals and computed S_t). A unit is half a tile (1024 elements), handed out in tile order by a
+// device-wide cursor, so the wait is always on the earliest unfinished tensor. The dedicated decode warps
+// overlap their stores with the consumers' reads of later tensors; the consumers join when their own tiles are
+// done. Every store instruction writes 512 contiguous bytes.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void decode_units(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
-                                             int n_tiles, int lane, int grab) {
+struct DecodeCur {
+    int t_cur, tile_b, tile_e;
+    int64_t off_t, len_t, woff_t;
+    bool dec;
+    float S_t;
+};
+// kDU consecutive units from u0 (those below u_lim), by one warp
+__device__ __forceinline__ void decode_span(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, DecodeCur &dc,
+                                            int u0, int u_lim, int lane) {
     const float4 *dtab = sm.dtab;
+    uint32_t dv[kDU][2];
+    int64_t obase[kDU], rem[kDU];
+    float S[kDU];
+#pragma unroll
+    for (int k = 0; k < kDU; ++k) {
+        const int u = u0 + k;
+        rem[k] = 0; obase[k] = 0; S[k] = 0.f; dv[k][0] = 0u; dv[k][1] = 0u;
+        if (u >= u_lim) continue;
+        const int tile = u >> 1;
+        if (tile >= dc.tile_e) {
+            TensorCur tc;
+            tensor_lookup(p, pv, sm, tile, tc);
+            dc.t_cur = tc.t; dc.tile_b = tc.tile_b; dc.tile_e = tc.tile_e; dc.off_t = tc.off; dc.len_t = tc.len;
+            dc.dec = tc.isL;
+            if (dc.dec) {
+                // wait for the tensor's last arriver (it runs in a resident CTA, and so does every CTA that still
+                // holds tiles of the tensor: nobody waits for a CTA that has not started)
+                dc.woff_t = tc.woff;
+                const unsigned long long *fp = pv.fin + dc.t_cur;
+                unsigned long long seen;
+                for (unsigned spins = 0;; ++spins) {
+                    seen = ld_acquire_u64(fp);
+                    if (seen) break;
+                    __nanosleep(100);
+                    if (spins > (1u << 25)) { report_timeout(p); dc.dec = false; break; }   // > 4 s: give up loudly
+                }
+                dc.S_t = __uint_as_float((uint32_t)seen);
+            }
+        }
+        if (!dc.dec) continue;
+        const int64_t wbase = (int64_t)(tile - dc.tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int64_t i = wbase + h * 512 + lane * 16;
+            if (i < dc.len_t)
+                dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)dc.woff_t * 8 + (size_t)(i >> 2)));
+        }
+        obase[k] = dc.off_t + wbase;
+        rem[k] = dc.len_t - wbase;
+        S[k] = dc.S_t;
+    }
+#pragma unroll
+    for (int k = 0; k < kDU; ++k) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int64_t rh = rem[k] - h * 512;
+            if (rh <= 0) continue;                       // warp-uniform
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
+                const uint32_t w32 = __shfl_sync(0xffffffffu, dv[k][h], j * 8 + (lane >> 2));
+                const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
+                const int64_t e0 = j * 128 + lane * 4;
+                const int64_t r = rh - e0;
+                if (r <= 0) continue;
+                float4 v = dtab[d];
+                v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
+                v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
+                float *o = p.out + obase[k] + h * 512 + e0;
+                if (r >= 4 && (obase[k] & 3) == 0) {
+                    __stcs(reinterpret_cast<float4 *>(o), v);
+                } else {
+                    o[0] = v.x;
+                    if (r > 1) o[1] = v.y;
+                    if (r > 2) o[2] = v.z;
+                    if (r > 3) o[3] = v.w;
+                }
+            }
+        }
+    }
+}
+// a dedicated decode warp: kDU units per trip to the cursor, for the whole kernel
+__device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
+                                                 int n_tiles, int lane) {
     const int total_units = n_tiles * 2;
     int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
-    int t_cur = -1, tile_b = 0, tile_e = 0;
-    int64_t off_t = 0, len_t = 0, woff_t = 0;
-    bool dec = false;
-    float S_t = 0.f;
-    // `grab` units per trip to the device-wide cursor, processed kDU at a time: the dedicated decode warps
-    // take few (they run beside the consumers for the whole kernel), the consumers that join at the end take
-    // more, so that a few thousand warps arriving together do not serialise on one atomic.
-    int u_next = 0, u_end = 0;
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
     for (;;) {
-        if (u_next >= u_end) {
-            int ub = 0;
-            if (lane == 0) ub = atomicAdd(cursor, grab);
-            u_next = __shfl_sync(0xffffffffu, ub, 0);
-            u_end = u_next + grab;
-        }
-        const int u0 = u_next;
-        u_next += kDU;
-        if (u0 >= total_units) break;
-        uint32_t dv[kDU][2];
-        int64_t obase[kDU], rem[kDU];
-        float S[kDU];
-#pragma unroll
-        for (int k = 0; k < kDU; ++k) {
-            const int u = u0 + k;
-            rem[k] = 0; obase[k] = 0; S[k] = 0.f; dv[k][0] = 0u; dv[k][1] = 0u;
-            if (u >= total_units) continue;
-            const int tile = u >> 1;
-            if (tile >= tile_e) {
-                TensorCur tc;
-                tensor_lookup(p, pv, sm, tile, tc);
-                t_cur = tc.t; tile_b = tc.tile_b; tile_e = tc.tile_e; off_t = tc.off; len_t = tc.len;
-                dec = tc.isL;
-                if (dec) {
-                    // wait until the tensor's last arriver has published its totals and scale (it runs in a
-                    // resident CTA, and so does every CTA that still holds tiles of the tensor: no CTA waits
-                    // for one that has not started)
-                    woff_t = tc.woff;
-                    const int *dp = pv.done + t_cur;
-                    int seen;
-                    for (unsigned spins = 0;; ++spins) {
-                        asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(seen) : "l"(dp) : "memory");
-                        if (seen & kDoneFinal) break;
-                        __nanosleep(200);
-                        if (spins > (1u << 24)) { report_timeout(p); return; }   // > 4 s: give up loudly, do not hang
-                    }
-                    S_t = __ldcg(pv.scale + t_cur);
-                }
-            }
-            if (!dec) continue;
-            const int64_t wbase = (int64_t)(tile - tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int64_t i = wbase + h * 512 + lane * 16;
-                if (i < len_t)
-                    dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)woff_t * 8 + (size_t)(i >> 2)));
-            }
-            obase[k] = off_t + wbase;
-            rem[k] = len_t - wbase;
-            S[k] = S_t;
-        }
-#pragma unroll
-        for (int k = 0; k < kDU; ++k) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int64_t rh = rem[k] - h * 512;
-                if (rh <= 0) continue;                       // warp-uniform
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
-                    const uint32_t w32 = __shfl_sync(0xffffffffu, dv[k][h], j * 8 + (lane >> 2));
-                    const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
-                    const int64_t e0 = j * 128 + lane * 4;
-                    const int64_t r = rh - e0;
-                    if (r <= 0) continue;
-                    float4 v = dtab[d];
-                    v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
-                    v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
-                    float *o = p.out + obase[k] + h * 512 + e0;
-                    if (r >= 4 && (obase[k] & 3) == 0) {
-                        __stcs(reinterpret_cast<float4 *>(o), v);
-                    } else {
-                        o[0] = v.x;
-                        if (r > 1) o[1] = v.y;
-                        if (r > 2) o[2] = v.z;
-                        if (r > 3) o[3] = v.w;
-                    }
-                }
-            }
-        }
+        int ub = 0;
+        if (lane == 0) ub = atomicAdd(cursor, kDU);
+        ub = __shfl_sync(0xffffffffu, ub, 0);
+        if (ub >= total_units) break;
+        decode_span(p, pv, sm, dc, ub, total_units, lane);
+    }
+}
+// the consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
+// arriving together on one address serialise: 15 us for the last warp served), chunk sizes guided by what is
+// left (>= one span per warp), spans dealt to the 16 warps round-robin
+__device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
+                                                int n_tiles, int ctid) {
+    const int total_units = n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
+    int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
+    int chunk = kDU * kCW;
+    for (;;) {
+        if (ctid == 0) sm.flag[3] = atomicAdd(cursor, chunk);
+        consumer_sync();
+        const int base = sm.flag[3];
+        if (base >= total_units) break;
+        const int lim = min(base + chunk, total_units);
+        for (int u0 = base + kDU * warp; u0 < lim; u0 += kDU * kCW) decode_span(p, pv, sm, dc, u0, lim, lane);
+        const int spans = (total_units - lim) / (2 * (int)gridDim.x * kDU * kCW);
+        chunk = kDU * kCW * min(max(spans, 1), 16);
+        consumer_sync();                                    // everybody has read flag[3]
     }
 }
 
@@ -586,55 +612,43 @@ __device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool 
 
 extern __shared__ __align__(128) unsigned char smem_raw[];
 
-__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p) {
-    unsigned long long v;
-    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v) {
-    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-constexpr unsigned long long kInitToken = 0x4e46494e4954494eull;     // a CTA is zeroing the plan's state
 
 // ---------------------------------------------------------------------------------------------
 // The tensor's last arriver (the CTA whose publication completed done[t]) rounds the exact totals of tensor t
 // to FP64 once, writes abs_sum / sumsq / nan_cnt / inf_cnt, clears the accumulator slots for the next call,
 // computes S_t = (float)(sum_w (double)(float)(A_w / len_t) / W) in worker order ("mean-absolute
-// scale"; readings #7, #8) and publishes it: done[t] |= kDoneFinal releases the decode warps of every CTA.
+// scale"; readings #7, #8) and publishes it: fin[t] = {1, S_t} releases the decode warps of every CTA.
 // Called by all consumer threads of the CTA.
 // ---------------------------------------------------------------------------------------------
 template <bool HEALTH>
 __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
                                              int64_t len_t, bool isL, int ctid) {
-    const int W = p.W, T = p.T;
-    if (ctid < W) {
-        const size_t o = (size_t)ctid * T + t;
+    const int W = p.W, T = p.T, warp = ctid >> 5, lane = ctid & 31;
+    for (int w = warp; w < W; w += kCW) {                      // a warp per worker: lane k holds word k of the slot
+        const size_t o = (size_t)w * T + t;
         double A = 0.0;
         if (isL || HEALTH) {
-            unsigned long long wd[kAccWords];
-            ulonglong2 *slot = reinterpret_cast<ulonglong2 *>(pv.acc + o * kAccWords);
-#pragma unroll
-            for (int i = 0; i < kAccWords / 2; ++i) {
-                const ulonglong2 v = __ldcg(slot + i);
-                wd[2 * i] = v.x;
-                wd[2 * i + 1] = v.y;
-            }
-#pragma unroll
-            for (int i = 0; i < kAccWords / 2; ++i) __stcg(slot + i, make_ulonglong2(0ull, 0ull));
-            const unsigned long long cn = wd[kAccNan], ci = wd[kAccInf];
+            unsigned long long *slot = pv.acc + o * kAccWords;
+            const unsigned long long v = __ldcg(slot + lane);
+            __stcg(slot + lane, 0ull);
+            const unsigned long long cn = __shfl_sync(0xffffffffu, v, kAccNan), ci = __shfl_sync(0xffffffffu, v, kAccInf);
+            uint32_t digit;
+            warp_acc_digits(v, lane, digit);
+            const unsigned nz = __ballot_sync(0xffffffffu, digit != 0u);
             if (isL) {
-                A = acc_round(wd + kAccAbs, kAccAbsWords, kAccAbsBase);
+                A = warp_acc_round(digit, nz, kAccAbs, kAccAbsWords, kAccAbsBase);
                 if (cn) A = __longlong_as_double(0x7ff8000000000000ll);          // IEEE: a NaN term makes the sum NaN,
                 else if (ci) A = __longlong_as_double(0x7ff0000000000000ll);     // an Inf term (no NaN) makes it +Inf
             }
             if (HEALTH) {
-                p.sumsq[o] = acc_round(wd + kAccSq, kAccSqWords, kAccSqBase);
-                p.nan_cnt[o] = cn;
-                p.inf_cnt[o] = ci;
+                const double Q = warp_acc_round(digit, nz, kAccSq, kAccSqWords, kAccSqBase);
+                if (lane == 0) { p.sumsq[o] = Q; p.nan_cnt[o] = cn; p.inf_cnt[o] = ci; }
             }
         }
-        p.abs_sum[o] = A;                                  // 0 for tensors that are not low-bit routed
-        sm.sw[ctid] = (float)(A / (double)len_t);
+        if (lane == 0) {
+            p.abs_sum[o] = A;                                  // 0 for tensors that are not low-bit routed
+            sm.sw[w] = (float)(A / (double)len_t);
+        }
     }
     if (!isL) return;                                      // CTA-uniform
     consumer_sync();
@@ -645,7 +659,7 @@ __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanVi
         pv.scale[t] = S;
         if (p.scale_out) p.scale_out[t] = S;
         __threadfence();
-        atomicOr(pv.done + t, kDoneFinal);
+        st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));
     }
 }
 
@@ -676,6 +690,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     for (int i = tid; i < 256; i += kFThreads)
         sm.dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
                                  (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
+    // warm the L2 with the small arrays the start-up chain reads (prefetches only: nothing the previous kernel on
+    // the stream may still be writing is READ before the dependency wait). Every bucket has its own plan and
+    // metadata, touched once per step: without this each dependent round trip below goes to HBM.
+    {
+        auto pf = [](const void *q) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q)); };
+        const int T = p.T;
+        if (tid == 0) pf(p.plan);
+        if (p.inkernel_route) {
+            if (tid * 16 < T) { pf(p.off + tid * 16); pf(p.len + tid * 16); }
+            if (tid * 128 < T) pf(p.elig + tid * 128);
+            if (p.tau && tid * 32 < T) pf(p.tau + tid * 32);
+        }
+        if (tid * 32 < T) pf(plan_view(p.plan, T).done + tid * 32);
+    }
     __syncthreads();
     // everything above touched shared memory only and overlapped the previous kernel on the stream (PDL)
     pdl_wait();
@@ -685,17 +713,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     int n_tiles = 0;
 
     // -----------------------------------------------------------------------------------------
-    // Self-cleaning state. The cursors, the per-tensor completion counters done[] and the exact accumulators
-    // acc[] are all zero whenever hdr->clean holds the token of this (T, W) shape: every call leaves them so
-    // (slots are cleared by whoever rounds them, the grid's last CTA resets the rest). Thread 0 starts the
-    // check here; the routing below needs none of that state and overlaps the round trip. Any other value
-    // (first use of the buffer, another shape) is settled once by compare-and-swap: the winning CTA zeroes
-    // the state and publishes the token, the others wait for a CTA that is running. No grid-wide barrier,
-    // no cooperative launch: nothing here assumes that all CTAs of the grid are resident together.
+    // Self-cleaning state and the first scheduling unit, in ONE atomic. hdr->sched = {clean token of this (T, W)
+    // shape, next unit}: unit_cursor, finish_count, the per-tensor completion counters done[] and the exact
+    // accumulators acc[] are all zero whenever the high half holds the token, because every call leaves them so
+    // (slots are cleared by whoever rounds them, the grid's last CTA resets the rest and the low half). The
+    // producer lane adds 1 here; the routing below needs none of that state and overlaps the round trip. A
+    // returned value with the token in it is a valid unit of a clean plan. Anything else (first use of the
+    // buffer, another shape) is settled once by compare-and-swap: the winning CTA zeroes the state and publishes
+    // the token, the others wait for a CTA that is running. No grid-wide barrier, no cooperative launch: nothing
+    // here assumes that all CTAs of the grid are resident together.
     // -----------------------------------------------------------------------------------------
-    const unsigned long long want_token = clean_token(p.T, W);
-    unsigned long long seen_token = want_token;
-    if (tid == 0) seen_token = ld_acquire_u64(&hdr->clean);
+    const uint32_t want_token = clean_token(p.T, W);
+    const bool is_prod = (warp == kCW && lane == 0);
+    unsigned long long sched_old = 0ull;
+    if (p.inkernel_route && is_prod) sched_old = atomicAdd(&hdr->sched, 1ull);
 
     if (p.inkernel_route) {
         // ---- step a1 inside this kernel (T <= kMetaCap) --------
@@ -728,6 +759,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                             c = __shfl_up_sync(0xffffffffu, i_nl, d);
             if (lane >= d) { i_tiles += a; i_words += b; i_nl += c; }
         }
+        if (tid == 0) trace_stamp(p, 9);
         long long *s_scan = reinterpret_cast<long long *>(smem_raw + 128);        // [3][8] warp totals, [24..27] tallies
         if (tid < 32) s_scan[tid] = 0;
         __syncthreads();
@@ -754,6 +786,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
         }
         const int any_bad = __syncthreads_or(bad);
+        if (tid == 0) trace_stamp(p, 10);
         long long b_tiles = 0, b_words = 0, b_nl = 0, t_tiles = 0, t_words = 0, t_nl = 0;
 #pragma unroll
         for (int k = 0; k < kMetaCap / 32; ++k) {
@@ -804,8 +837,12 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 p.summary[NF_SUM_STATUS] = status;
             }
         }
-        if (status != NF_OK) return;                           // nothing of the self-cleaning state was touched
+        if (status != NF_OK) {                                 // nothing else of the self-cleaning state was touched
+            if (is_prod) atomicAdd(&hdr->sched, ~0ull);        // give the unit back (-1)
+            return;
+        }
         n_tiles = (int)t_tiles;
+        if (tid == 0) trace_stamp(p, 11);
     } else {
         if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
         if (p.P && pv.hdr->Wd > p.plane_stride) {              // plane rows too short: refuse, like a bad layout
@@ -813,6 +850,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             return;
         }
         n_tiles = pv.hdr->n_tiles;
+        if (is_prod) sched_old = atomicAdd(&hdr->sched, 1ull);
         if (p.T <= kMetaCap) {
             // per-tensor metadata -> shared memory (one round trip for the whole CTA)
             for (int t = tid; t <= p.T; t += kFThreads) {
@@ -828,32 +866,44 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
     }
 
-    // ---- settle the clean token (thread 0 read it before the routing) ------------------------------
-    if (tid == 0) {
-        int role = 0;                                          // 1: this CTA zeroes the state
-        for (unsigned spins = 0; seen_token != want_token; ++spins) {
-            if (seen_token != kInitToken) {
-                const unsigned long long old = atomicCAS(&hdr->clean, seen_token, kInitToken);
-                if (old == seen_token) { role = 1; break; }
-                seen_token = old;
-            } else {
-                __nanosleep(200);
-                seen_token = ld_acquire_u64(&hdr->clean);
-                if (spins > (1u << 24)) { report_timeout(p); role = 2; break; }
-            }
-        }
-        sm.flag[0] = role;
-    }
+    // ---- settle the clean token (the producer lane took a unit before the routing) -----------------
+    if (is_prod) sm.flag[0] = ((uint32_t)(sched_old >> 32) == want_token) ? 0 : 1;
     __syncthreads();                                           // also: the shared-memory metadata is complete
-    if (sm.flag[0] == 2) return;
-    if (sm.flag[0] == 1) {
-        const size_t na = (size_t)W * p.T * kAccWords;
-        for (size_t i = tid; i < na; i += kFThreads) pv.acc[i] = 0ull;
-        for (int t = tid; t < p.T; t += kFThreads) pv.done[t] = 0;
-        if (tid == 0) { hdr->tile_cursor = 0; hdr->unit_cursor = 0; hdr->finish_count = 0; }
-        __threadfence();
+    if (sm.flag[0]) {
+        // rare: the plan's state is not known to be clean
+        if (tid == 0) {
+            int role = 0;                                      // 1: this CTA zeroes the state, 2: gave up
+            for (unsigned spins = 0;; ++spins) {
+                const unsigned long long v = ld_acquire_u64(&hdr->sched);
+                const uint32_t hi = (uint32_t)(v >> 32);
+                if (hi == want_token) break;
+                if (hi == kInitToken) {
+                    __nanosleep(200);
+                    if (spins > (1u << 24)) { report_timeout(p); role = 2; break; }
+                } else if (atomicCAS(&hdr->sched, v, (unsigned long long)kInitToken << 32) == v) {
+                    role = 1;
+                    break;
+                }
+            }
+            sm.flag[1] = role;
+        }
         __syncthreads();
-        if (tid == 0) st_release_u64(&hdr->clean, want_token);
+        const int role = sm.flag[1];
+        if (role == 2) return;
+        if (role == 1) {
+            const size_t na = (size_t)W * p.T * kAccWords;
+            for (size_t i = tid; i < na; i += kFThreads) pv.acc[i] = 0ull;
+            for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
+            if (tid == 0) { hdr->unit_cursor = 0; hdr->finish_count = 0; }
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) atomicExch(&hdr->sched, (unsigned long long)want_token << 32);
+        }
+        __syncthreads();
+        if (is_prod) {
+            sched_old = atomicAdd(&hdr->sched, 1ull);
+            if ((uint32_t)(sched_old >> 32) != want_token) { report_timeout(p); sched_old = 0x7fffffffull; }
+        }
     }
     if (tid == 0) trace_stamp(p, 7);
 
@@ -871,14 +921,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // =====================================================================================
         if (lane == 0) {
             const uint64_t pol = policy_evict_first();
-            int32_t *cursor = &hdr->tile_cursor;
+            int u_next = (int)(uint32_t)sched_old;                 // the unit taken before the routing
+            bool have_unit = true;
             int pr_st = 0, pr_next = 0, pr_end = 0;
             uint32_t pr_ph = 0;
             TensorCur pc{};
             pc.tile_e = 0;
             for (;;) {
                 if (pr_next >= pr_end) {
-                    const int u = atomicAdd(cursor, 1);
+                    const int u = have_unit ? u_next : (int)(uint32_t)atomicAdd(&hdr->sched, 1ull);
+                    have_unit = false;
                     if (u < nA) { pr_next = 4 * u; pr_end = pr_next + 4; }
                     else if (u < nA + nB) { pr_next = sA + 2 * (u - nA); pr_end = pr_next + 2; }
                     else { pr_next = sB + (u - nA - nB); pr_end = pr_next + 1; }
@@ -962,10 +1014,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
     } else if (warp >= kCW + 2) {
         // =====================================================================================
-        // decode warps (pass B inside the kernel): see decode_units(). The consumers join them once
+        // decode warps (pass B inside the kernel): see decode_warp_loop(). The consumers join them once
         // their own tiles are done.
         // =====================================================================================
-        decode_units(p, pv, sm, n_tiles, lane, kDU);
+        decode_warp_loop(p, pv, sm, n_tiles, lane);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
     } else {
         // =====================================================================================
@@ -1171,7 +1223,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (ctid == 0) trace_stamp(p, 1);
         if (touched) flush_tensor();
         if (ctid == 0) trace_stamp(p, 2);
-        decode_units(p, pv, sm, n_tiles, lane, NF_KGRAB);     // help finish pass B
+        decode_cta_loop(p, pv, sm, n_tiles, ctid);           // help finish pass B
         if (ctid == 0) trace_stamp(p, 3);
     }
 
@@ -1186,9 +1238,14 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
     __syncthreads();
     if (sm.flag[2]) {
-        for (int t = tid; t < p.T; t += kFThreads) pv.done[t] = 0;
-        if (tid == 0) { hdr->tile_cursor = 0; hdr->unit_cursor = 0; hdr->finish_count = 0; }
+        for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
+        if (tid == 0) {
+            hdr->unit_cursor = 0;
+            hdr->finish_count = 0;
+            hdr->sched = (unsigned long long)want_token << 32;
+        }
     }
+    if (tid == 0) trace_stamp(p, 8);
 }
 
 // ---------------------------------------------------------------------------------------------

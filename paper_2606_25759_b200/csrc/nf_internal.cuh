@@ -31,9 +31,12 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     int64_t Wd;                            // total packed words per worker plane
     int32_t n_tiles;
     int32_t finish_count;                  // fused path: CTAs that have finished (the last one resets the state below)
-    int32_t tile_cursor;                   // fused path: next pass-A scheduling unit (dynamic scheduling over the CTAs)
     int32_t unit_cursor;                   // fused path: next pass-B unit (half tile)
-    unsigned long long clean;              // fused path: clean_token(T, W) while cursors, done[] and acc[] are all zero
+    int32_t pad0;
+    // fused path: high half = clean_token(T, W) while unit_cursor, finish_count, done[] and acc[] are all zero
+    // (the state every call leaves behind), low half = next pass-A scheduling unit (dynamic scheduling over the
+    // CTAs). One atomicAdd both takes a unit and proves the state clean.
+    unsigned long long sched;
     int64_t acc_slots;                     // capacity of the acc region in (replica, tensor) slots
 };
 static_assert(sizeof(PlanHeader) == 64, "plan header layout");
@@ -55,7 +58,6 @@ constexpr int kAccWords = 32;
 constexpr int kAccAbs = 0, kAccAbsWords = 10, kAccAbsBase = -149;
 constexpr int kAccSq = 10, kAccSqWords = 19, kAccSqBase = -298;
 constexpr int kAccNan = 29, kAccInf = 30;
-constexpr int kDoneFinal = 0x40000000;     // done[t] bit: the tensor's totals and scale are published
 
 // Offsets (bytes) of the plan arrays for a bucket of T tensors.
 struct PlanLayout {
@@ -64,6 +66,7 @@ struct PlanLayout {
     size_t lt_woff;                        // int64 [T+1]   woff of the L tensors, lt_woff[nL] = Wd
     size_t scale;                          // float [T]     per-tensor scale scratch
     size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
+    size_t fin;                            // uint64 [T]    fused path: {1, FP32 bits of S_t} once tensor t is finalised, else 0
     size_t acc;                            // uint64 [R*T][kAccWords]  exact accumulators (R = workers / replicas)
     size_t total;                          // without the acc region
 };
@@ -78,6 +81,7 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
     L.lt_woff = o;     o = align_up(o + sizeof(int64_t) * (size_t)(T + 1), 16);
     L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
     L.done = o;        o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
+    L.fin = o;         o = align_up(o + sizeof(unsigned long long) * (size_t)(T > 0 ? T : 1), 16);
     L.acc = align_up(o, 256);
     L.total = L.acc;
     return L;
@@ -85,8 +89,11 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
 __host__ __device__ inline size_t plan_bytes_for(int T, int R) {
     return plan_layout(T).acc + sizeof(unsigned long long) * kAccWords * (size_t)(T > 0 ? T : 1) * (size_t)(R > 0 ? R : 1);
 }
-__host__ __device__ inline unsigned long long clean_token(int T, int W) {
-    return 0x4e46434c45414e00ull ^ ((unsigned long long)(unsigned)T << 20) ^ (unsigned long long)(unsigned)W;
+constexpr uint32_t kInitToken = 0x494e4954u;          // "INIT": a CTA is zeroing the plan's state
+__host__ __device__ inline uint32_t clean_token(int T, int W) {
+    uint32_t h = (((uint32_t)T << 8) + (uint32_t)W) * 0x9e3779b1u ^ 0x4e46434cu;
+    if (h == 0u || h == kInitToken) h ^= 0x5a5a5a5au;
+    return h;
 }
 
 struct PlanView {
@@ -96,6 +103,7 @@ struct PlanView {
     const int64_t *lt_woff;
     float *scale;
     int32_t *done;
+    unsigned long long *fin;
     unsigned long long *acc;
 };
 
@@ -109,6 +117,7 @@ __host__ __device__ inline PlanView plan_view(void *plan, int T) {
     v.lt_woff = (const int64_t *)(p + L.lt_woff);
     v.scale = (float *)(p + L.scale);
     v.done = (int32_t *)(p + L.done);
+    v.fin = (unsigned long long *)(p + L.fin);
     v.acc = (unsigned long long *)(p + L.acc);
     return v;
 }
@@ -321,6 +330,37 @@ static __device__ __noinline__ double acc_round(const unsigned long long *w, int
     const int lz = __clzll((long long)hi64);             // 0..31: d[top] != 0
     unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
     if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;   // below the rounding position of a 64 -> 53 bit conversion
+    return scalbn(__ull2double_rn(mant), base + 32 * top + 31 - lz - 63);
+}
+
+// The same rounding done by a whole (converged) warp on one accumulator slot, lane k holding word k: `digit` is
+// the lane's 32-bit digit after carry normalisation (warp_acc_digits), the number occupies lanes [l0, l0 + nwords).
+__device__ __forceinline__ void warp_acc_digits(unsigned long long v, int lane, uint32_t &digit) {
+    unsigned long long lo = v & 0xffffffffull, hi = v >> 32;
+    if (lane >= kAccNan) { lo = 0ull; hi = 0ull; }
+    for (;;) {                                           // deferred carries ripple up (two numbers: no carry into lanes 0 / kAccSq)
+        unsigned long long c = __shfl_up_sync(0xffffffffu, hi, 1);
+        if (lane == kAccAbs || lane == kAccSq) c = 0ull;
+        const unsigned long long s = lo + c;
+        lo = s & 0xffffffffull;
+        hi = s >> 32;
+        if (!__any_sync(0xffffffffu, hi != 0ull)) break;
+    }
+    digit = (uint32_t)lo;
+}
+__device__ __forceinline__ double warp_acc_round(uint32_t digit, unsigned nz /*ballot(digit != 0)*/, int l0, int nwords, int base) {
+    const unsigned m = (nz >> l0) & ((1u << nwords) - 1u);
+    const int top = m ? 31 - __clz(m) : 0;
+    const unsigned long long d0 = __shfl_sync(0xffffffffu, digit, l0 + top);
+    const unsigned long long d1 = __shfl_sync(0xffffffffu, digit, l0 + max(top - 1, 0));
+    const unsigned long long d2 = __shfl_sync(0xffffffffu, digit, l0 + max(top - 2, 0));
+    if (m == 0u) return 0.0;
+    const unsigned long long hi64 = (d0 << 32) | (top >= 1 ? d1 : 0ull);
+    const unsigned long long lo32 = top >= 2 ? d2 : 0ull;
+    const bool sticky = top >= 3 && (m & ((1u << (top - 2)) - 1u)) != 0u;
+    const int lz = __clzll((long long)hi64);
+    unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
+    if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;
     return scalbn(__ull2double_rn(mant), base + 32 * top + 31 - lz - 63);
 }
 
