@@ -240,22 +240,27 @@ def run_nf(args):
     peak, peak_src = measured_peak()
     # dominant kernel: nf::fused_passA_kernel = pass A + pass B of one bucket in one launch, so its
     # algorithmic bytes are the whole path's (SURVEY 8(d) "fused floor" + planes)
-    achieved = all_bytes / (fused_ms * 1e-3) / 1e9
+    # Inside a step the kernels of consecutive buckets overlap (the tail of bucket k is drained by the kernel of
+    # bucket k+1), so the kernel's average duration in the timed region is the step time over the launches: the
+    # timed region contains nothing but these launches, on the stream the CUDA events were recorded on.
+    achieved = all_bytes / (ms_per_step * 1e-3) / 1e9
     traffic = ncu_traffic()
     roofline = {"bound": "hbm", "kernel": "nf::fused_passA_kernel (pass A + pass B of one bucket, TMA ring)",
                 "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                 "frac": round(achieved / peak, 4), "peak_source": peak_src,
                 "frac_of_nominal_8TBs": round(achieved / HBM_NOMINAL_GBS, 4),
                 "algorithmic_bytes_per_step": all_bytes, "launches_per_step": nb,
-                "avg_launch_ms": round(fused_ms / nb, 4),
+                "avg_launch_ms": round(ms_per_step / nb, 4),
+                "avg_launch_ms_unchained": round(fused_ms / nb, 4),
                 "traffic": (traffic or {}).get("dram_bytes_per_launch_avg"),
                 "traffic_note": (traffic or {}).get("note"),
                 "whole_path": {"algorithmic_bytes_per_step": all_bytes,
                                "achieved": round(all_bytes / (ms_per_step * 1e-3) / 1e9, 1),
                                "frac": round(all_bytes / (ms_per_step * 1e-3) / 1e9 / peak, 4)},
-                "kernel_ms_per_step": {"fused": round(fused_ms, 4)},
-                "note": "kernel time = CUDA events around each launch on the launching stream; the events "
-                        "break the PDL chain between consecutive launches, so their sum exceeds ms_per_step"}
+                "kernel_ms_per_step": {"fused_in_step": round(ms_per_step, 4), "fused_unchained_sum": round(fused_ms, 4)},
+                "note": "avg_launch_ms = timed region (CUDA events on the launching stream) / launches: the step is "
+                        "nothing but these launches. avg_launch_ms_unchained = the same kernel as stand-alone "
+                        "nf_aggregate_bucket calls, one CUDA event pair per launch (no overlap between buckets)"}
 
     # ---- e2e: same metric through the C-ABI call with HOST buffers (H2D + D2H inside the region)
     e2e = None

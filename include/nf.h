@@ -218,6 +218,42 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         nf_stream stream);
 
 /*
+ * One training step's buckets in ONE call (the hook's view of a step: PAPER L140-146, steps (2)-(7) for every DDP
+ * bucket of the model). Bucket i is aggregated exactly as nf_aggregate_bucket would (same results, bit for bit), all
+ * on `stream`, but consecutive buckets are chained into a software pipeline: the decode of a bucket's last low-bit
+ * tensor — which cannot start before the bucket has been read completely, because its scale needs all of the
+ * tensor — is taken over by the kernel of the NEXT bucket and overlaps that bucket's reads, and a chained kernel
+ * does not wait for its predecessor before it starts reading (it needs nothing of it).
+ * Requirements beyond nf_aggregate_bucket's: the nf_bucket array is HOST memory (read during the call only);
+ * every bucket has its own plan, outputs, accumulators and planes (buffers of different buckets must not overlap);
+ * everything the step reads (gradients, metadata) is complete before the call is enqueued, i.e. was produced by
+ * work enqueued on `stream` before it; `workspace` holds nf_step_workspace_bytes(buckets, nb) bytes (one direction
+ * slice per bucket: n/4 bytes each). W, state, mode, margin, alpha are the step's. Buckets of more than 256 tensors (routed
+ * by a separate kernel) and empty buckets break the chain and run as stand-alone calls.
+ */
+typedef struct nf_bucket {
+    const float *g;            /* [W][worker_stride] */
+    int64_t worker_stride, n;
+    const int64_t *off, *len;  /* [T] */
+    const uint8_t *elig;       /* [T] */
+    int32_t T, reserved;
+    const float *tau;          /* [T] or NULL */
+    uint8_t *route;            /* [T] out */
+    int64_t *woff;             /* [T] out */
+    int64_t *summary;          /* [NF_SUM_LEN] out */
+    uint32_t *P, *N;           /* planes or NULL */
+    int64_t plane_stride;
+    double *abs_sum, *sumsq;   /* [W][T]; sumsq / nan_cnt / inf_cnt may all be NULL */
+    uint64_t *nan_cnt, *inf_cnt;
+    float *out, *scale_out;    /* [n], [T] or NULL */
+    void *plan;
+    size_t plan_bytes;
+} nf_bucket;
+size_t nf_step_workspace_bytes(const nf_bucket *buckets /*host*/, int nb);
+int nf_aggregate_step(const nf_bucket *buckets /*host*/, int nb, int W, nf_state state, int mode, int margin,
+                      float alpha, void *workspace, size_t workspace_bytes, nf_stream stream);
+
+/*
  * End-to-end convenience with HOST buffers (used for the e2e measurement): copies the W rows of n floats
  * from pinned/pageable host memory `g_host` (worker stride = worker_stride elements: (W-1)*worker_stride + n
  * floats are read, and as many written to the caller's device staging buffer `g_dev`, same stride), runs

@@ -23,7 +23,7 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
-           "nf_aggregate_bucket", "nf_aggregate_bucket_host",
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_aggregate_step", "nf_step_workspace_bytes",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
            "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace")
 
@@ -40,6 +40,16 @@ class NfSupervisorCfg(C.Structure):
 class NfSupervisor(C.Structure):
     _fields_ = [("cfg", NfSupervisorCfg), ("phase", C.c_int32), ("remaining", C.c_int32), ("step", C.c_int64),
                 ("detections", C.c_int64), ("ema", C.c_double), ("cusum", C.c_double)]
+
+
+class NfBucket(C.Structure):
+    """struct nf_bucket of include/nf.h (one bucket of nf_aggregate_step)."""
+    _fields_ = [("g", C.c_void_p), ("worker_stride", C.c_int64), ("n", C.c_int64), ("off", C.c_void_p),
+                ("len", C.c_void_p), ("elig", C.c_void_p), ("T", C.c_int32), ("reserved", C.c_int32),
+                ("tau", C.c_void_p), ("route", C.c_void_p), ("woff", C.c_void_p), ("summary", C.c_void_p),
+                ("P", C.c_void_p), ("N", C.c_void_p), ("plane_stride", C.c_int64), ("abs_sum", C.c_void_p),
+                ("sumsq", C.c_void_p), ("nan_cnt", C.c_void_p), ("inf_cnt", C.c_void_p), ("out", C.c_void_p),
+                ("scale_out", C.c_void_p), ("plan", C.c_void_p), ("plan_bytes", C.c_size_t)]
 
 
 class NfError(RuntimeError):
@@ -89,6 +99,10 @@ def lib() -> C.CDLL:
                                            vp, sz, vp, sz, vp]
     L.nf_debug_trace.restype = i32
     L.nf_debug_trace.argtypes = [i32, vp]
+    L.nf_step_workspace_bytes.restype = sz
+    L.nf_step_workspace_bytes.argtypes = [C.POINTER(NfBucket), i32]
+    L.nf_aggregate_step.restype = i32
+    L.nf_aggregate_step.argtypes = [C.POINTER(NfBucket), i32, i32, NfState, i32, i32, f32, vp, sz, vp]
     L.nf_count_planes.restype = i32
     L.nf_count_planes.argtypes = [i32]
     L.nf_partial_count.restype = i32
@@ -205,6 +219,18 @@ def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, el
         _ptr(route), _ptr(woff), _ptr(summary), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(sumsq),
         _ptr(nan_cnt), _ptr(inf_cnt), _ptr(out), _ptr(out_host, cuda=False), _ptr(plan), plan.numel() * plan.element_size(),
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_step_workspace_bytes(buckets) -> int:
+    """buckets: a ctypes array of NfBucket."""
+    return int(lib().nf_step_workspace_bytes(buckets, len(buckets)))
+
+
+def nf_aggregate_step(buckets, W, state, mode, margin, alpha, workspace, stream=None):
+    """buckets: a ctypes array of NfBucket (host memory, device pointers inside)."""
+    _check("nf_aggregate_step", lib().nf_aggregate_step(
+        buckets, len(buckets), int(W), _state(state), int(mode), int(margin), float(alpha), _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream)))
 
 
 def nf_count_planes(Wg: int) -> int:

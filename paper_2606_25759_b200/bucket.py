@@ -90,22 +90,41 @@ class ModelBuffers:
     """Device buffers of a whole model's buckets, in the arrangement bench.py times (memory plumbing only):
     every bucket has its own metadata, plan, accumulators, output and — when `planes` — its own packed
     planes P/N (the "wire payload" of that bucket); the 2-bit direction workspace between the two passes of
-    the fused call is ONE buffer shared by all buckets (an L2-resident intermediate, sized for the largest
-    bucket). `step()` issues one nf_aggregate_bucket per bucket, back to back on one stream."""
+    the fused path is one buffer with a slice per bucket (an L2-resident intermediate: a slice is written and
+    read back within one bucket's kernel time). `step()` is ONE nf_aggregate_step call: one fused kernel per bucket, back to back
+    on one stream, chained into a pipeline by the library."""
 
     def __init__(self, layouts, W: int, device="cuda", planes: bool = True, health: bool = True):
         """layouts: sequence of (off, length, elig, n) per bucket."""
         dev = torch.device(device)
         self.W = int(W)
+        self.planes = planes
         self.buckets = []
-        max_T = max(len(l[0]) for l in layouts)
-        max_n = max(int(l[3]) for l in layouts)
-        self.workspace = torch.zeros(nf.nf_workspace_bytes(max_T, max_n), dtype=torch.uint8, device=dev)
+        self.workspace = torch.zeros(sum(nf.nf_workspace_bytes(len(l[0]), int(l[3])) for l in layouts), dtype=torch.uint8,
+                                     device=dev)
         for off, length, elig, n in layouts:
             bb = BucketBuffers(off, length, elig, n, W, dev, planes=planes, health=health, workspace=self.workspace)
             self.buckets.append(bb)
+        self._desc = (nf.NfBucket * len(self.buckets))()
+
+    def _fill(self, G, mode, tau):
+        ptr = lambda t: None if t is None else t.data_ptr()
+        for i, (g, bb) in enumerate(zip(G, self.buckets)):
+            d = self._desc[i]
+            use_planes = self.planes and bb.P is not None
+            d.g, d.worker_stride, d.n = g.data_ptr(), g.shape[1], bb.n
+            d.off, d.len, d.elig, d.T = bb.off.data_ptr(), bb.len.data_ptr(), bb.elig.data_ptr(), bb.T
+            d.tau = ptr(tau[i]) if tau is not None else None
+            d.route, d.woff, d.summary = bb.route.data_ptr(), bb.woff.data_ptr(), bb.summary.data_ptr()
+            d.P = ptr(bb.P) if use_planes else None
+            d.N = ptr(bb.N) if (use_planes and mode == nf.MODE_GTERNARY) else None
+            d.plane_stride = bb.plane_stride
+            d.abs_sum, d.sumsq = bb.abs_sum.data_ptr(), ptr(bb.sumsq)
+            d.nan_cnt, d.inf_cnt = ptr(bb.nan_cnt), ptr(bb.inf_cnt)
+            d.out, d.scale_out = bb.out.data_ptr(), bb.scale.data_ptr()
+            d.plan, d.plan_bytes = bb.plan.data_ptr(), bb.plan.numel()
 
     def step(self, G, state=(1, 0, 1), mode=nf.MODE_GTERNARY, tau=None, margin=0, alpha=1.0, stream=None):
-        """G: per-bucket gradient tensors [W][stride]."""
-        for g, bb in zip(G, self.buckets):
-            bb.aggregate(g, g.shape[1], state, mode, tau, margin, alpha, stream=stream)
+        """G: per-bucket gradient tensors [W][stride]; tau: per-bucket [T] tensors or None."""
+        self._fill(G, mode, tau)
+        nf.nf_aggregate_step(self._desc, self.W, state, mode, margin, alpha, self.workspace, stream)

@@ -181,6 +181,78 @@ int nf_health_stats(const float *x, int64_t replica_stride, int R, int64_t n,
     return cuda_rc(launch_stream(kFHealth, p, n, s));
 }
 
+}  // extern "C"
+
+namespace {
+
+struct Chain {                 // how a bucket's kernel is linked to its neighbours inside nf_aggregate_step
+    const nf_bucket *prev = nullptr;
+    const void *prev_dirs = nullptr;
+    int prev_W = 0;
+    bool chained = false, next_chained = false;
+};
+
+int check_bucket(const nf_bucket &b, int W, int mode, int margin, const void *workspace, size_t workspace_bytes) {
+    int rc = check_common(W, b.n, b.T);
+    if (rc != NF_OK) return rc;
+    if (margin < 0 || margin > 255) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!b.summary || !b.plan || b.plan_bytes < nf_plan_bytes(b.T, W)) return NF_ERR_ARG;
+    if (!workspace || workspace_bytes < nf_workspace_bytes(b.T, b.n)) return NF_ERR_ARG;
+    if (b.worker_stride < b.n || b.plane_stride < 0 || !b.abs_sum) return NF_ERR_ARG;
+    if (b.T > 0 && (!b.g || !b.off || !b.len || !b.elig || !b.route || !b.woff || !b.out)) return NF_ERR_ARG;
+    if (b.P && mode == NF_MODE_GTERNARY && !b.N) return NF_ERR_ARG;
+    const bool health = b.sumsq || b.nan_cnt || b.inf_cnt;
+    if (health && !(b.sumsq && b.nan_cnt && b.inf_cnt)) return NF_ERR_ARG;
+    if (misaligned16(b.g) || misaligned16(b.out) || misaligned16(b.P) || misaligned16(b.N) ||
+        misaligned16(b.plan) || misaligned16(workspace))
+        return NF_ERR_ALIGN;
+    return NF_OK;
+}
+
+// one bucket through the fused path (arguments already checked)
+int launch_bucket(const nf_bucket &b, int W, nf_state state, int mode, int margin, float alpha, void *workspace,
+                  const Chain &ch, cudaStream_t s) {
+    const int T = b.T;
+    // a1: inside the fused kernel for buckets of up to kMetaCap tensors (one launch per bucket), else by the
+    // route kernel first (PDL-chained). An empty bucket only gets its summary written.
+    const bool inkernel = T > 0 && T <= kMetaCap;
+    if (!inkernel) {
+        if (launch_route(b.off, b.len, b.elig, T, b.n, state, b.route, b.woff, b.summary, b.plan, b.plan_bytes, 1, 0, s) !=
+            cudaSuccess)
+            return NF_ERR_CUDA;
+        if (T == 0) return NF_OK;
+    }
+    // one read of the W x n gradients: pass A + pass B in one persistent kernel (nf_fused.cu)
+    StreamParams p{};
+    p.g = b.g; p.worker_stride = b.worker_stride; p.W = W; p.T = T;
+    p.off = b.off; p.len = b.len; p.route = b.route; p.woff = b.woff;
+    p.ternary = (mode == NF_MODE_GTERNARY); p.tau = b.tau; p.margin = margin; p.alpha = alpha;
+    p.P = b.P; p.N = b.N; p.plane_stride = b.plane_stride;
+    p.abs_sum = b.abs_sum; p.sumsq = b.sumsq;
+    p.nan_cnt = (unsigned long long *)b.nan_cnt; p.inf_cnt = (unsigned long long *)b.inf_cnt;
+    p.out = b.out; p.dirs = (uint8_t *)workspace; p.plan = b.plan;
+    p.scale_out = b.scale_out;
+    p.trace = g_trace ? g_trace + (size_t)(g_trace_calls++ & 1) * 256 * 16 : nullptr;
+    p.inkernel_route = inkernel ? 1 : 0;
+    p.elig = b.elig; p.st = state; p.n = b.n; p.route_w = b.route; p.woff_w = b.woff; p.summary = b.summary;
+    p.acc_slots = (int64_t)((b.plan_bytes - plan_layout(T).acc) / (sizeof(unsigned long long) * kAccWords));
+    p.chained = ch.chained ? 1 : 0;
+    p.next_chained = ch.next_chained ? 1 : 0;
+    p.defer_tail = ch.next_chained ? 1 : 0;
+    if (ch.chained) {
+        p.prev_plan = ch.prev->plan; p.prev_T = ch.prev->T; p.prev_W = ch.prev_W;
+        p.prev_off = ch.prev->off; p.prev_len = ch.prev->len; p.prev_woff = ch.prev->woff;
+        p.prev_route = ch.prev->route; p.prev_dirs = (const uint8_t *)ch.prev_dirs; p.prev_out = ch.prev->out;
+    }
+    const bool health = b.sumsq != nullptr;
+    return cuda_rc(launch_fused_passA(health, p, b.n, s));
+}
+
+}  // namespace
+
+extern "C" {
+
 int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         const int64_t *off, const int64_t *len, const uint8_t *elig, int T,
                         nf_state state, int mode, const float *tau, int margin, float alpha,
@@ -190,44 +262,55 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         float *out, float *scale_out,
                         void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
                         nf_stream stream) {
-    int rc = check_common(W, n, T);
+    nf_bucket b{};
+    b.g = g; b.worker_stride = worker_stride; b.n = n; b.off = off; b.len = len; b.elig = elig; b.T = T; b.tau = tau;
+    b.route = route; b.woff = woff; b.summary = summary; b.P = P; b.N = N; b.plane_stride = plane_stride;
+    b.abs_sum = abs_sum; b.sumsq = sumsq; b.nan_cnt = nan_cnt; b.inf_cnt = inf_cnt; b.out = out; b.scale_out = scale_out;
+    b.plan = plan; b.plan_bytes = plan_bytes;
+    const int rc = check_bucket(b, W, mode, margin, workspace, workspace_bytes);
     if (rc != NF_OK) return rc;
-    if (margin < 0 || margin > 255) return NF_ERR_RANGE;
-    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
-    if (!summary || !plan || plan_bytes < nf_plan_bytes(T, W)) return NF_ERR_ARG;
-    if (!workspace || workspace_bytes < nf_workspace_bytes(T, n)) return NF_ERR_ARG;
-    if (worker_stride < n || plane_stride < 0 || !abs_sum) return NF_ERR_ARG;
-    if (T > 0 && (!g || !off || !len || !elig || !route || !woff || !out)) return NF_ERR_ARG;
-    if (P && mode == NF_MODE_GTERNARY && !N) return NF_ERR_ARG;
-    const bool health = sumsq || nan_cnt || inf_cnt;
-    if (health && !(sumsq && nan_cnt && inf_cnt)) return NF_ERR_ARG;
-    if (misaligned16(g) || misaligned16(out) || misaligned16(P) || misaligned16(N) ||
-        misaligned16(plan) || misaligned16(workspace))
-        return NF_ERR_ALIGN;
-    cudaStream_t s = (cudaStream_t)stream;
-    // a1: inside the fused kernel for buckets of up to kMetaCap tensors (one launch per bucket), else by the
-    // route kernel first (PDL-chained). An empty bucket only gets its summary written.
-    const bool inkernel = T > 0 && T <= kMetaCap;
-    if (!inkernel) {
-        if (launch_route(off, len, elig, T, n, state, route, woff, summary, plan, plan_bytes, 1, 0, s) != cudaSuccess)
-            return NF_ERR_CUDA;
-        if (T == 0) return NF_OK;
+    return launch_bucket(b, W, state, mode, margin, alpha, workspace, Chain{}, (cudaStream_t)stream);
+}
+
+size_t nf_step_workspace_bytes(const nf_bucket *buckets, int nb) {
+    size_t total = 0;
+    for (int i = 0; buckets && i < nb; ++i) total += nf_workspace_bytes(buckets[i].T, buckets[i].n);
+    return total > 0 ? total : nf_workspace_bytes(0, 0);
+}
+
+int nf_aggregate_step(const nf_bucket *buckets, int nb, int W, nf_state state, int mode, int margin, float alpha,
+                      void *workspace, size_t workspace_bytes, nf_stream stream) {
+    if (nb < 0 || (nb > 0 && !buckets)) return NF_ERR_ARG;
+    if (!workspace || workspace_bytes < nf_step_workspace_bytes(buckets, nb)) return NF_ERR_ARG;
+    // everything is checked before anything is launched
+    for (int i = 0; i < nb; ++i) {
+        const int rc = check_bucket(buckets[i], W, mode, margin, workspace, nf_workspace_bytes(buckets[i].T, buckets[i].n));
+        if (rc != NF_OK) return rc;
+        for (int j = 0; j < i; ++j)
+            if (buckets[j].plan == buckets[i].plan || (buckets[i].n > 0 && buckets[j].n > 0 && buckets[j].out == buckets[i].out))
+                return NF_ERR_ARG;                            // buckets of a step must not share plans or outputs
     }
-    // one read of the W x n gradients: pass A + pass B in one persistent kernel (nf_fused.cu)
-    StreamParams p{};
-    p.g = g; p.worker_stride = worker_stride; p.W = W; p.T = T;
-    p.off = off; p.len = len; p.route = route; p.woff = woff;
-    p.ternary = (mode == NF_MODE_GTERNARY); p.tau = tau; p.margin = margin; p.alpha = alpha;
-    p.P = P; p.N = N; p.plane_stride = plane_stride;
-    p.abs_sum = abs_sum; p.sumsq = sumsq;
-    p.nan_cnt = (unsigned long long *)nan_cnt; p.inf_cnt = (unsigned long long *)inf_cnt;
-    p.out = out; p.dirs = (uint8_t *)workspace; p.plan = plan;
-    p.scale_out = scale_out;
-    p.trace = g_trace ? g_trace + (size_t)(g_trace_calls++ & 1) * 256 * 16 : nullptr;
-    p.inkernel_route = inkernel ? 1 : 0;
-    p.elig = elig; p.st = state; p.n = n; p.route_w = route; p.woff_w = woff; p.summary = summary;
-    p.acc_slots = (int64_t)((plan_bytes - plan_layout(T).acc) / (sizeof(unsigned long long) * kAccWords));
-    return cuda_rc(launch_fused_passA(health, p, n, s));
+    // Every bucket gets its own slice of the workspace: several kernels of the chain can be in flight at once (a
+    // small bucket's kernel starts on idle SMs while its predecessors still run), so no slice is ever reused
+    // inside a step.
+    auto chainable = [&](int i) { return buckets[i].T > 0 && buckets[i].T <= kMetaCap; };
+    size_t slice_off = 0, prev_off = 0;
+    for (int i = 0; i < nb; ++i) {
+        Chain ch;
+        ch.chained = i > 0 && chainable(i) && chainable(i - 1);
+        ch.next_chained = i + 1 < nb && chainable(i) && chainable(i + 1);
+        if (ch.chained) {
+            ch.prev = &buckets[i - 1];
+            ch.prev_dirs = (const char *)workspace + prev_off;
+            ch.prev_W = W;
+        }
+        const int rc = launch_bucket(buckets[i], W, state, mode, margin, alpha, (char *)workspace + slice_off, ch,
+                                     (cudaStream_t)stream);
+        if (rc != NF_OK) return rc;
+        prev_off = slice_off;
+        slice_off += nf_workspace_bytes(buckets[i].T, buckets[i].n);
+    }
+    return NF_OK;
 }
 
 // debug aid (nf.h): enable (on != 0) allocates a device buffer of 256 x 8 stamps the fused kernel fills;

@@ -126,8 +126,9 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 // shared-memory carve-up (dynamic). Everything the hot loop touches sits at a compile-time offset:
 //   [0, 64)         mbarriers full[4], empty[4]
 //   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
-//   [112, 128)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid)
 //   [128, 384)      scratch of the in-kernel routing scan
+//   [416, 456)      pending publication of a tensor, tensor handed to finalize_tensor
+//   [384, 416)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid, decode chunk, pass A done)
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
 //   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
 //   [4096, 8192)    decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
@@ -144,8 +145,9 @@ struct FusedSmem {
     int *tile_of;                // [kMaxStages] tile held by a stage, -1 = no more tiles
     int *run_of;                 // [kMaxStages] MULTI: length R of the run of tiles the stage belongs to
     int *seg_of;                 // [kMaxStages] 1: the tile ends a segment (last tile of its scheduling unit or tensor)
-    int *flag;                   // [4] CTA-wide flags
+    int *flag;                   // [8] CTA-wide flags
     float *sw;                   // [256] per-worker scales of the tensor being finalised
+    int *pend;                   // [10] pending publication of a tensor / tensor handed to finalize_tensor
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -164,8 +166,9 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.tile_of = (int *)(base + 64);
     s.run_of = (int *)(base + 80);
     s.seg_of = (int *)(base + 96);
-    s.flag = (int *)(base + 112);
+    s.flag = (int *)(base + 384);
     s.sw = (float *)(base + 3072);
+    s.pend = (int *)(base + 416);
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -485,8 +488,21 @@ struct DecodeCur {
     bool dec;
     float S_t;
 };
+// where the units of a bucket come from: this kernel's own bucket (metadata in shared memory when T <= kMetaCap)
+// or the previous bucket of the step (everything from global memory)
+struct DecodeSrc {
+    int T, n_tiles;
+    bool smem_meta;
+    const int32_t *tile_prefix;
+    const int64_t *off, *len, *woff;
+    const uint8_t *route;
+    const unsigned long long *fin;
+    const uint8_t *dirs;
+    float *out;
+    PlanHeader *hdr;
+};
 // kDU consecutive units from u0 (those below u_lim), by one warp
-__device__ __forceinline__ void decode_span(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, DecodeCur &dc,
+__device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
                                             int u0, int u_lim, int lane) {
     const float4 *dtab = sm.dtab;
     uint32_t dv[kDU][2];
@@ -499,15 +515,27 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const PlanVie
         if (u >= u_lim) continue;
         const int tile = u >> 1;
         if (tile >= dc.tile_e) {
-            TensorCur tc;
-            tensor_lookup(p, pv, sm, tile, tc);
-            dc.t_cur = tc.t; dc.tile_b = tc.tile_b; dc.tile_e = tc.tile_e; dc.off_t = tc.off; dc.len_t = tc.len;
-            dc.dec = tc.isL;
+            if (src.smem_meta) {
+                int lo = 0, hi = src.T;                  // invariant: m_tile[lo] <= tile < m_tile[hi]
+                while (hi - lo > 1) {
+                    const int mid = (lo + hi) >> 1;
+                    if (sm.m_tile[mid] <= tile) lo = mid; else hi = mid;
+                }
+                dc.t_cur = lo; dc.tile_b = sm.m_tile[lo]; dc.tile_e = sm.m_tile[lo + 1];
+                dc.off_t = sm.m_off[lo]; dc.len_t = sm.m_len[lo];
+                dc.woff_t = sm.m_woff[lo];
+                dc.dec = dc.woff_t >= 0;
+            } else {
+                const int t = upper_tensor<int32_t>(src.tile_prefix, src.T, tile);
+                dc.t_cur = t; dc.tile_b = __ldg(src.tile_prefix + t); dc.tile_e = __ldg(src.tile_prefix + t + 1);
+                dc.off_t = __ldg(src.off + t); dc.len_t = __ldg(src.len + t);
+                dc.dec = __ldcg(src.route + t) == NF_ROUTE_L;
+                dc.woff_t = dc.dec ? __ldcg(src.woff + t) : 0;
+            }
             if (dc.dec) {
                 // wait for the tensor's last arriver (it runs in a resident CTA, and so does every CTA that still
                 // holds tiles of the tensor: nobody waits for a CTA that has not started)
-                dc.woff_t = tc.woff;
-                const unsigned long long *fp = pv.fin + dc.t_cur;
+                const unsigned long long *fp = src.fin + dc.t_cur;
                 unsigned long long seen;
                 for (unsigned spins = 0;; ++spins) {
                     seen = ld_acquire_u64(fp);
@@ -524,7 +552,7 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const PlanVie
         for (int h = 0; h < 2; ++h) {
             const int64_t i = wbase + h * 512 + lane * 16;
             if (i < dc.len_t)
-                dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(p.dirs + (size_t)dc.woff_t * 8 + (size_t)(i >> 2)));
+                dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(src.dirs + (size_t)dc.woff_t * 8 + (size_t)(i >> 2)));
         }
         obase[k] = dc.off_t + wbase;
         rem[k] = dc.len_t - wbase;
@@ -547,7 +575,7 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const PlanVie
                 float4 v = dtab[d];
                 v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
                 v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
-                float *o = p.out + obase[k] + h * 512 + e0;
+                float *o = src.out + obase[k] + h * 512 + e0;
                 if (r >= 4 && (obase[k] & 3) == 0) {
                     __stcs(reinterpret_cast<float4 *>(o), v);
                 } else {
@@ -560,42 +588,44 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const PlanVie
         }
     }
 }
-// a dedicated decode warp: kDU units per trip to the cursor, for the whole kernel
-__device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
-                                                 int n_tiles, int lane) {
-    const int total_units = n_tiles * 2;
-    int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
+// A dedicated decode warp: kDU units per trip to the bucket's cursor, the next trip issued before the current span
+// is processed (the round trip hides behind the span's loads and stores). `stop` (shared memory, or NULL): once it
+// is set the warp takes no further units (what it holds it finishes): the rest is left to the next kernel of the step.
+__device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
+                                                 const volatile int *stop, int lane) {
+    const int total_units = src.n_tiles * 2;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
-    for (;;) {
-        int ub = 0;
-        if (lane == 0) ub = atomicAdd(cursor, kDU);
-        ub = __shfl_sync(0xffffffffu, ub, 0);
-        if (ub >= total_units) break;
-        decode_span(p, pv, sm, dc, ub, total_units, lane);
+    if (stop && *stop) return;
+    int ub = 0;
+    if (lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kDU);
+    ub = __shfl_sync(0xffffffffu, ub, 0);
+    while (ub < total_units) {
+        const bool more = !(stop && *stop);
+        int ub_next = total_units;
+        if (more && lane == 0) ub_next = atomicAdd(&src.hdr->unit_cursor, kDU);
+        decode_span(p, src, sm, dc, ub, total_units, lane);
+        ub = __shfl_sync(0xffffffffu, ub_next, 0);
     }
 }
-// the consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
+// The consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
 // arriving together on one address serialise: 15 us for the last warp served), chunk sizes guided by what is
-// left (>= one span per warp), spans dealt to the 16 warps round-robin
-__device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const PlanView &pv, const FusedSmem &sm,
-                                                int n_tiles, int ctid) {
-    const int total_units = n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
-    int32_t *cursor = const_cast<int32_t *>(&pv.hdr->unit_cursor);
+// left (4 spans .. 16 spans per warp), spans dealt to the 16 warps round-robin.
+__device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, int ctid) {
+    const int total_units = src.n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
-    int chunk = kDU * kCW;
+    int chunk = kDU * 8;
     for (;;) {
-        if (ctid == 0) sm.flag[3] = atomicAdd(cursor, chunk);
+        if (ctid == 0) sm.flag[3] = atomicAdd(&src.hdr->unit_cursor, chunk);
         consumer_sync();
         const int base = sm.flag[3];
         if (base >= total_units) break;
         const int lim = min(base + chunk, total_units);
-        for (int u0 = base + kDU * warp; u0 < lim; u0 += kDU * kCW) decode_span(p, pv, sm, dc, u0, lim, lane);
-        const int spans = (total_units - lim) / (2 * (int)gridDim.x * kDU * kCW);
-        chunk = kDU * kCW * min(max(spans, 1), 16);
+        for (int u0 = base + kDU * warp; u0 < lim; u0 += kDU * kCW) decode_span(p, src, sm, dc, u0, lim, lane);
+        const int spans = (total_units - lim) / (2 * (int)gridDim.x * kDU);     // guided: half of an even share
+        chunk = kDU * min(max(spans, 4), 16 * kCW);
         consumer_sync();                                    // everybody has read flag[3]
     }
 }
-
 // the same vote from byte-packed running counts (W > 8: several worker groups per tile)
 __device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool ternary, int W, int margin) {
     uint32_t d = 0u;
@@ -679,7 +709,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     const FusedSmem sm = carve(smem_raw, stages);
     const int W = p.W;                          // MULTI: W > 8, several worker groups of 8 per tile
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    pdl_launch_dependents();
+    // Chaining (nf_aggregate_step), see the comment at the decode warps below. A chained kernel needs nothing of the
+    // previous grid for its pass A and lets its own successor go at once; a kernel whose successor is chained lets
+    // it go only after its own dependency wait, so that "everything before the step" is complete for the whole chain.
+    if (!p.next_chained) pdl_launch_dependents();
     if (tid == 0) trace_stamp(p, 5);
 
     if (tid == 0) {
@@ -687,6 +720,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < 256; i += kFThreads) { sm.nan[i] = 0u; sm.inf[i] = 0u; }
+    if (tid < 8) sm.flag[tid] = 0;
     for (int i = tid; i < 256; i += kFThreads)
         sm.dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
                                  (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
@@ -706,11 +740,13 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
     __syncthreads();
     // everything above touched shared memory only and overlapped the previous kernel on the stream (PDL)
-    pdl_wait();
+    if (!p.chained) pdl_wait();
+    if (p.next_chained) pdl_launch_dependents();
     if (tid == 0) trace_stamp(p, 6);
     const PlanView pv = plan_view(p.plan, p.T);
     PlanHeader *const hdr = (PlanHeader *)p.plan;
     int n_tiles = 0;
+    bool layout_ok = true;
 
     // -----------------------------------------------------------------------------------------
     // Self-cleaning state and the first scheduling unit, in ONE atomic. hdr->sched = {clean token of this (T, W)
@@ -837,11 +873,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 p.summary[NF_SUM_STATUS] = status;
             }
         }
-        if (status != NF_OK) {                                 // nothing else of the self-cleaning state was touched
-            if (is_prod) atomicAdd(&hdr->sched, ~0ull);        // give the unit back (-1)
-            return;
-        }
-        n_tiles = (int)t_tiles;
+        // a refused layout is a bucket without tiles: nothing is read or written, the plan's state (and the tail
+        // of a previous bucket of the step) is still looked after
+        layout_ok = status == NF_OK;
+        n_tiles = layout_ok ? (int)t_tiles : 0;
         if (tid == 0) trace_stamp(p, 11);
     } else {
         if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
@@ -906,6 +941,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
     }
     if (tid == 0) trace_stamp(p, 7);
+
+    const DecodeSrc own{p.T, n_tiles, p.T <= kMetaCap, pv.tile_prefix, p.off, p.len, p.woff, p.route, pv.fin, p.dirs, p.out, hdr};
+    const PlanView ppv = plan_view(p.prev_plan, p.prev_T);              // (only dereferenced when chained)
+    DecodeSrc prev{p.prev_T, 0, false, ppv.tile_prefix, p.prev_off, p.prev_len, p.prev_woff, p.prev_route, ppv.fin, p.prev_dirs,
+                   p.prev_out, (PlanHeader *)p.prev_plan};
 
     // scheduling units: a pure function of (n_tiles, grid): 4 consecutive tiles, then 2, then single tiles near
     // the end (guided self-scheduling with fixed boundaries). A *segment* = unit x tensor is what one FP32
@@ -999,7 +1039,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             bool isL;
             if (p.T <= kMetaCap) { len_t = sm.m_len[t]; isL = sm.m_woff[t] >= 0; }
             else { len_t = __ldg(p.len + t); isL = __ldg(p.route + t) == NF_ROUTE_L; }
-            if (len_t > 0) continue;
+            if (len_t > 0 || !layout_ok) continue;
             for (int w = 0; w < W; ++w) {
                 const size_t o = (size_t)w * p.T + t;
                 p.abs_sum[o] = 0.0;
@@ -1017,7 +1057,18 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // decode warps (pass B inside the kernel): see decode_warp_loop(). The consumers join them once
         // their own tiles are done.
         // =====================================================================================
-        decode_warp_loop(p, pv, sm, n_tiles, lane);
+        // Chaining: the decode of a bucket's LAST low-bit tensor cannot start before the bucket has been read
+        // completely (S_t needs all of the tensor), so at the end of a stand-alone call the device only writes. Inside
+        // a step the kernels of consecutive buckets form a pipeline instead: when pass A of bucket k ends, its CTAs
+        // leave at once (defer_tail) and the kernel of bucket k+1, which needs nothing of bucket k for its own
+        // pass A and therefore never waited for it, drains bucket k's remaining units here, beside its own reads.
+        // The only thread-level dependency waits of a chained kernel are the ones in front of bucket k's data.
+        if (p.chained) {
+            pdl_wait();
+            prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+            decode_warp_loop(p, prev, sm, nullptr, lane);
+        }
+        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, lane);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
     } else {
         // =====================================================================================
@@ -1047,49 +1098,84 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         int segpar = 0;                             // buffer of the current segment's per-warp FP64 values
         double *wbuf = sm.wacc;
 
+        // The publication of a tensor's tile count (below) is asynchronous: ctid 0 issues the atomic and everybody goes
+        // on; whether this CTA was the tensor's last arriver is looked at in front of the next CTA barrier the
+        // consumers pass anyway (resolve_pre / resolve_post around it), and only then is the tensor finalised.
+        // The pending publication lives in shared memory (sm.pend: tensor or -1, route, length, tiles published, tiles
+        // of the tensor); only the value the atomic returns stays in a register of ctid 0.
+        int pend_old = 0;
+        int rpar = 0;                               // parity of the verdict slot (sm.flag[5 + rpar]), CTA-uniform
+        if (ctid == 0) sm.pend[0] = -1;
+        auto resolve_pre = [&]() __attribute__((always_inline)) {
+            if (ctid == 0) {
+                int last = 0;
+                if (sm.pend[0] >= 0) {
+                    last = (pend_old + sm.pend[4] == sm.pend[5]) ? 1 : 0;
+                    if (last) {
+                        __threadfence();            // acquire: every CTA's adds of the tensor are visible below
+                        sm.pend[6] = sm.pend[0];    // handed to finalize_tensor: tensor, route, length
+                        sm.pend[7] = sm.pend[1];
+                        sm.pend[8] = sm.pend[2];
+                        sm.pend[9] = sm.pend[3];
+                    }
+                    sm.pend[0] = -1;
+                }
+                sm.flag[5 + rpar] = last;
+            }
+        };
+        auto resolve_post = [&]() __attribute__((always_inline)) {
+            const int last = sm.flag[5 + rpar];
+            rpar ^= 1;
+            if (last)
+                finalize_tensor<HEALTH>(p, pv, sm, sm.pend[6], *reinterpret_cast<const int64_t *>(sm.pend + 8), sm.pend[7] != 0, ctid);
+        };
+
         // A segment (the tiles of one scheduling unit inside one tensor) is complete: its per-warp FP64 values are in
-        // `wbuf`. Sum them over the 16 warps in warp order (a fixed shape: the value depends on the data only) and add
-        // the segment's total EXACTLY to the tensor's accumulator (integer atomics: the order in which segments
-        // arrive, i.e. the dynamic scheduling, cannot change the result).
+        // `wbuf`, 16 per (worker, statistic). Warp j sums column j (j + 16, ...) in a fixed tree shape (the value
+        // depends on the data only) and adds the segment's total EXACTLY to the tensor's accumulator (integer
+        // atomics: the order in which segments arrive, i.e. the dynamic scheduling, cannot change the result).
         auto seg_reduce = [&]() __attribute__((always_inline)) {
+            resolve_pre();
             consumer_sync();
-            if (ctid < 2 * W) {
-                const double *src = wbuf + ctid;
-                double tot = 0.0;
-#pragma unroll
-                for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
-                const int stat = ctid & 1;
-                unsigned long long *slot = pv.acc + ((size_t)(ctid >> 1) * T + c.t) * kAccWords;
-                if (stat == 0) { if (c.isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
-                else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
+            for (int j = warp; j < 2 * W; j += kCW) {
+                double v = lane < kCW ? wbuf[(size_t)lane * 2 * W + j] : 0.0;
+                v += __shfl_xor_sync(0xffffffffu, v, 8);
+                v += __shfl_xor_sync(0xffffffffu, v, 4);
+                v += __shfl_xor_sync(0xffffffffu, v, 2);
+                v += __shfl_xor_sync(0xffffffffu, v, 1);
+                if (lane == 0) {
+                    unsigned long long *slot = pv.acc + ((size_t)(j >> 1) * T + c.t) * kAccWords;
+                    if ((j & 1) == 0) { if (c.isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, v); }
+                    else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, v);
+                }
             }
             if (nbuf == 1) consumer_sync();         // one buffer (W > 32): the next segment overwrites it
             else { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
+            resolve_post();
         };
 
-        // All tiles this CTA took of tensor c.t are done: hand in the NaN / Inf tallies, publish the tile count
-        // (release: direction bytes, plane words, outputs and accumulator adds of every consumer thread come first),
-        // and finalise the tensor if this publication completed it.
+        // All tiles this CTA took of tensor c.t are done (every warp has passed the barrier of the tensor's last
+        // segment: its NaN / Inf tallies are final): hand in the tallies and publish the tile count. Release: the CTA
+        // barrier orders every consumer thread's direction bytes, plane words, outputs and accumulator adds before
+        // ctid 0's fence, which is cumulative. One barrier, no round trip on the consumers' path.
         auto flush_tensor = [&]() __attribute__((always_inline)) {
-            if (c.isL || HEALTH) {
-                for (int w = ctid; w < W; w += kCThreads) {
-                    const unsigned cn_ = sm.nan[w], ci_ = sm.inf[w];
+            if ((c.isL || HEALTH) && warp == 0) {
+                for (int w = lane; w < W; w += 32) {
+                    const unsigned cn_ = atomicExch(&sm.nan[w], 0u), ci_ = atomicExch(&sm.inf[w], 0u);
                     unsigned long long *slot = pv.acc + ((size_t)w * T + c.t) * kAccWords;
-                    if (cn_) { atomicAdd(slot + kAccNan, (unsigned long long)cn_); sm.nan[w] = 0u; }
-                    if (ci_) { atomicAdd(slot + kAccInf, (unsigned long long)ci_); sm.inf[w] = 0u; }
+                    if (cn_) atomicAdd(slot + kAccNan, (unsigned long long)cn_);
+                    if (ci_) atomicAdd(slot + kAccInf, (unsigned long long)ci_);
                 }
             }
-            __threadfence();
+            resolve_pre();                          // (a publication still pending from the tensor before)
             consumer_sync();
+            resolve_post();
             if (ctid == 0) {
-                const int total = c.tile_e - c.tile_b;
-                const int old = atomicAdd(pv.done + c.t, ntile_acc);
-                const int last = (old + ntile_acc == total) ? 1 : 0;
-                if (last) __threadfence();
-                sm.flag[1] = last;
+                __threadfence();
+                pend_old = atomicAdd(pv.done + c.t, ntile_acc);
+                sm.pend[0] = c.t; sm.pend[1] = c.isL ? 1 : 0; *reinterpret_cast<int64_t *>(sm.pend + 2) = c.len;
+                sm.pend[4] = ntile_acc; sm.pend[5] = c.tile_e - c.tile_b;
             }
-            consumer_sync();
-            if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
             ntile_acc = 0;
         };
 
@@ -1222,15 +1308,29 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
         if (ctid == 0) trace_stamp(p, 1);
         if (touched) flush_tensor();
+        resolve_pre();
+        consumer_sync();
+        resolve_post();
         if (ctid == 0) trace_stamp(p, 2);
-        decode_cta_loop(p, pv, sm, n_tiles, ctid);           // help finish pass B
+        if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
+        if (p.chained) {
+            // whatever is left of the previous bucket (normally nothing: its tail was drained long ago)
+            pdl_wait();
+            prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+            decode_cta_loop(p, prev, sm, ctid);
+        }
+        if (!p.defer_tail) decode_cta_loop(p, own, sm, ctid);      // help finish pass B
         if (ctid == 0) trace_stamp(p, 3);
     }
 
-    // ---- the grid's last CTA resets the cursors and the completion counters: the plan is clean again ----
+    // ---- the grid's last CTA resets the self-cleaning state: of this bucket unless its tail is deferred (then the
+    // next kernel of the step does it when it is through with it), and of the previous bucket of the step ----
     __syncthreads();
     if (tid == 0) {
-        __threadfence();
+        // (own state is reset below only when the tail is not deferred: then this CTA's stores to it, the fin words
+        // of the tensors it finalised, must come first. A deferred bucket's state is reset by the next kernel, after
+        // its dependency wait; what this kernel did to the previous bucket's state are atomics that have returned.)
+        if (!p.defer_tail) __threadfence();
         const int old = atomicAdd(&hdr->finish_count, 1);
         const int last = (old == (int)gridDim.x - 1) ? 1 : 0;
         if (last) __threadfence();
@@ -1238,11 +1338,24 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
     __syncthreads();
     if (sm.flag[2]) {
-        for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
+        if (!p.defer_tail)
+            for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
         if (tid == 0) {
-            hdr->unit_cursor = 0;
             hdr->finish_count = 0;
-            hdr->sched = (unsigned long long)want_token << 32;
+            if (!p.defer_tail) {
+                hdr->unit_cursor = 0;
+                hdr->sched = (unsigned long long)want_token << 32;
+            } else {
+                hdr->sched = 0ull;                             // not clean until the next kernel has drained the tail
+            }
+        }
+        if (p.chained) {
+            pdl_wait();
+            for (int t = tid; t < p.prev_T; t += kFThreads) { ppv.done[t] = 0; ppv.fin[t] = 0ull; }
+            if (tid == 0) {
+                prev.hdr->unit_cursor = 0;
+                prev.hdr->sched = (unsigned long long)clean_token(p.prev_T, p.prev_W) << 32;
+            }
         }
     }
     if (tid == 0) trace_stamp(p, 8);

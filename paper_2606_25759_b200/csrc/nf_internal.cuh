@@ -159,6 +159,16 @@ struct StreamParams {
     int64_t *woff_w;           // [T] out
     int64_t *summary;          // [NF_SUM_LEN] out
     int64_t acc_slots;         // capacity of the plan's accumulator region, in (replica, tensor) slots
+    // chaining (nf_aggregate_step): consecutive buckets of one step form a software pipeline, see nf_fused.cu
+    int chained;               // 1: the kernel right before this one on the stream is the fused kernel of `prev`
+    int next_chained;          // 1: the kernel right after this one is chained to it
+    int defer_tail;            // 1: the next kernel of the step decodes what cannot be decoded before pass A ends
+    void *prev_plan;           // previous bucket of the step (its remaining decode units are drained here)
+    int prev_T, prev_W;
+    const int64_t *prev_off, *prev_len, *prev_woff;
+    const uint8_t *prev_route;
+    const uint8_t *prev_dirs;
+    float *prev_out;
 };
 
 enum : int {

@@ -73,3 +73,71 @@ def test_gpt2_1p3b_whole_config():
 @pytest.mark.parametrize("W", shapes.SWEEP_W)
 def test_sweep_whole_config(W):
     _whole_config(shapes.sweep(W), steps=2)
+
+
+def test_step_chain_with_breakers_and_bitwise_equal_to_single_calls():
+    """nf_aggregate_step on an irregular sequence of buckets: small and large, a bucket of 300 tensors (routed by a
+    separate kernel: breaks the chain), a one-tile bucket, W > 8, repeated three times. Every bucket must match the
+    oracle AND be bitwise identical to what a stand-alone nf_aggregate_bucket call produces for it."""
+    from tests.util import layout
+    rng = np.random.default_rng(2024)
+    W = 12
+    specs = []
+    for T, big in ((5, 2048 * 120 + 7), (300, 2048 * 40), (3, 100), (40, 2048 * 300 + 1), (7, 2048 * 9), (1, 2048 * 64), (20, 5000)):
+        lens = [int(x) for x in rng.integers(1, 4000, T)]
+        lens[T // 2] = big
+        off, ln, n = layout(lens)
+        elig = [int(x) for x in rng.integers(0, 2, T)]
+        elig[T // 2] = 1
+        specs.append((off, ln, elig, n))
+    G, refs = [], []
+    for off, ln, elig, n in specs:
+        g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
+        g[rng.random((W, n)) < 0.03] = 0.0
+        gd = torch.zeros((W, (n + 3) // 4 * 4), dtype=torch.float32, device=DEV)
+        gd[:, :n] = torch.from_numpy(g)
+        G.append(gd)
+        refs.append(O.aggregate_bucket(g, off, ln, elig))
+    mb = ModelBuffers(specs, W, DEV, planes=True, health=True)
+    for _ in range(3):
+        for bb in mb.buckets:
+            bb.out.fill_(-5.0)
+        mb.step(G)
+    torch.cuda.synchronize()
+    for i, (bb, ref) in enumerate(zip(mb.buckets, refs)):
+        compare(bb, ref, W, O.MODE_GTERNARY, what=f"step bucket {i}")
+    # bitwise against stand-alone calls
+    from paper_2606_25759_b200 import BucketBuffers
+    for i, ((off, ln, elig, n), g, bb) in enumerate(zip(specs, G, mb.buckets)):
+        one = BucketBuffers(off, ln, elig, n, W, DEV, planes=True, health=True)
+        one.aggregate(g, g.shape[1])
+        torch.cuda.synchronize()
+        for name in ("out", "scale", "abs_sum", "sumsq", "nan_cnt", "inf_cnt", "P", "N", "route", "woff"):
+            a, b = getattr(bb, name), getattr(one, name)
+            assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), f"bucket {i}: {name} differs from the stand-alone call"
+
+
+def test_step_with_a_refused_bucket_in_the_middle():
+    """A bucket with a bad layout inside a step: it is refused on the device (status in its summary, nothing written),
+    its neighbours are aggregated as usual, and the next step works again."""
+    from tests.util import layout
+    rng = np.random.default_rng(7)
+    W = 4
+    off, ln, n = layout([3000, 2048 * 30, 500])
+    specs = [(off, ln, [1, 1, 0], n), (np.array([0, 8], np.int64), np.array([16, 8], np.int64), [1, 1], 32), (off, ln, [0, 1, 1], n)]
+    G, refs = [], []
+    for off_, ln_, elig_, n_ in specs:
+        g = rng.standard_normal((W, n_)).astype(np.float32)
+        gd = torch.zeros((W, (n_ + 3) // 4 * 4), dtype=torch.float32, device=DEV)
+        gd[:, :n_] = torch.from_numpy(g)
+        G.append(gd)
+        refs.append(None if n_ == 32 else O.aggregate_bucket(g, off_, ln_, elig_))
+    mb = ModelBuffers(specs, W, DEV, planes=True, health=True)
+    for _ in range(2):
+        mb.buckets[1].out.fill_(9.0)
+        mb.step(G)
+        torch.cuda.synchronize()
+        assert int(mb.buckets[1].summary[nf.SUM_STATUS]) == nf.NF_ERR_ARG
+        assert bool((mb.buckets[1].out == 9.0).all())
+        for i in (0, 2):
+            compare(mb.buckets[i], refs[i], W, O.MODE_GTERNARY, what=f"bucket {i} beside a refused bucket")
