@@ -127,7 +127,6 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [0, 64)         mbarriers full[4], empty[4]
 //   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
 //   [128, 384)      scratch of the in-kernel routing scan
-//   [416, 456)      pending publication of a tensor, tensor handed to finalize_tensor
 //   [384, 416)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid, decode chunk, pass A done)
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
 //   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
@@ -147,7 +146,6 @@ struct FusedSmem {
     int *seg_of;                 // [kMaxStages] 1: the tile ends a segment (last tile of its scheduling unit or tensor)
     int *flag;                   // [8] CTA-wide flags
     float *sw;                   // [256] per-worker scales of the tensor being finalised
-    int *pend;                   // [10] pending publication of a tensor / tensor handed to finalize_tensor
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -168,7 +166,6 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.seg_of = (int *)(base + 96);
     s.flag = (int *)(base + 384);
     s.sw = (float *)(base + 3072);
-    s.pend = (int *)(base + 416);
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -699,6 +696,9 @@ __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanVi
 #ifndef NF_TAIL4
 #define NF_TAIL4 12                       // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
 #endif
+#ifndef NF_GRAB
+#define NF_GRAB 1                         // most scheduling units a producer takes per trip to the cursor
+#endif
 #ifndef NF_TAIL2
 #define NF_TAIL2 4                        // the last NF_TAIL2 x grid tiles are handed out one at a time
 #endif
@@ -961,16 +961,25 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // =====================================================================================
         if (lane == 0) {
             const uint64_t pol = policy_evict_first();
+            // Units are taken several at a time while plenty are left (guided: a share of what remains when the
+            // previous trip was made, 1 .. NF_GRAB): fewer trips to one address, and a CTA walks longer contiguous
+            // stretches of the W rows (DRAM pages, TLB entries). The segment boundaries are those of the units, so
+            // how many are taken at once changes nothing in the values.
             int u_next = (int)(uint32_t)sched_old;                 // the unit taken before the routing
-            bool have_unit = true;
+            int u_end = u_next + 1;
+            const int n_units = nA + nB + (n_tiles - sB);
             int pr_st = 0, pr_next = 0, pr_end = 0;
             uint32_t pr_ph = 0;
             TensorCur pc{};
             pc.tile_e = 0;
             for (;;) {
                 if (pr_next >= pr_end) {
-                    const int u = have_unit ? u_next : (int)(uint32_t)atomicAdd(&hdr->sched, 1ull);
-                    have_unit = false;
+                    if (u_next >= u_end) {
+                        const int g = min(max((n_units - u_end) / (4 * (int)gridDim.x), 1), NF_GRAB);
+                        u_next = (int)(uint32_t)atomicAdd(&hdr->sched, (unsigned long long)g);
+                        u_end = u_next + g;
+                    }
+                    const int u = u_next++;
                     if (u < nA) { pr_next = 4 * u; pr_end = pr_next + 4; }
                     else if (u < nA + nB) { pr_next = sA + 2 * (u - nA); pr_end = pr_next + 2; }
                     else { pr_next = sB + (u - nA - nB); pr_end = pr_next + 1; }
@@ -1098,44 +1107,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         int segpar = 0;                             // buffer of the current segment's per-warp FP64 values
         double *wbuf = sm.wacc;
 
-        // The publication of a tensor's tile count (below) is asynchronous: ctid 0 issues the atomic and everybody goes
-        // on; whether this CTA was the tensor's last arriver is looked at in front of the next CTA barrier the
-        // consumers pass anyway (resolve_pre / resolve_post around it), and only then is the tensor finalised.
-        // The pending publication lives in shared memory (sm.pend: tensor or -1, route, length, tiles published, tiles
-        // of the tensor); only the value the atomic returns stays in a register of ctid 0.
-        int pend_old = 0;
-        int rpar = 0;                               // parity of the verdict slot (sm.flag[5 + rpar]), CTA-uniform
-        if (ctid == 0) sm.pend[0] = -1;
-        auto resolve_pre = [&]() __attribute__((always_inline)) {
-            if (ctid == 0) {
-                int last = 0;
-                if (sm.pend[0] >= 0) {
-                    last = (pend_old + sm.pend[4] == sm.pend[5]) ? 1 : 0;
-                    if (last) {
-                        __threadfence();            // acquire: every CTA's adds of the tensor are visible below
-                        sm.pend[6] = sm.pend[0];    // handed to finalize_tensor: tensor, route, length
-                        sm.pend[7] = sm.pend[1];
-                        sm.pend[8] = sm.pend[2];
-                        sm.pend[9] = sm.pend[3];
-                    }
-                    sm.pend[0] = -1;
-                }
-                sm.flag[5 + rpar] = last;
-            }
-        };
-        auto resolve_post = [&]() __attribute__((always_inline)) {
-            const int last = sm.flag[5 + rpar];
-            rpar ^= 1;
-            if (last)
-                finalize_tensor<HEALTH>(p, pv, sm, sm.pend[6], *reinterpret_cast<const int64_t *>(sm.pend + 8), sm.pend[7] != 0, ctid);
-        };
-
         // A segment (the tiles of one scheduling unit inside one tensor) is complete: its per-warp FP64 values are in
         // `wbuf`, 16 per (worker, statistic). Warp j sums column j (j + 16, ...) in a fixed tree shape (the value
         // depends on the data only) and adds the segment's total EXACTLY to the tensor's accumulator (integer
         // atomics: the order in which segments arrive, i.e. the dynamic scheduling, cannot change the result).
         auto seg_reduce = [&]() __attribute__((always_inline)) {
-            resolve_pre();
             consumer_sync();
             for (int j = warp; j < 2 * W; j += kCW) {
                 double v = lane < kCW ? wbuf[(size_t)lane * 2 * W + j] : 0.0;
@@ -1151,13 +1127,12 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
             if (nbuf == 1) consumer_sync();         // one buffer (W > 32): the next segment overwrites it
             else { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
-            resolve_post();
         };
 
         // All tiles this CTA took of tensor c.t are done (every warp has passed the barrier of the tensor's last
-        // segment: its NaN / Inf tallies are final): hand in the tallies and publish the tile count. Release: the CTA
+        // segment: its NaN / Inf tallies are final): hand in the tallies, publish the tile count (release: the CTA
         // barrier orders every consumer thread's direction bytes, plane words, outputs and accumulator adds before
-        // ctid 0's fence, which is cumulative. One barrier, no round trip on the consumers' path.
+        // ctid 0's fence, which is cumulative), and finalise the tensor if this publication completed it.
         auto flush_tensor = [&]() __attribute__((always_inline)) {
             if ((c.isL || HEALTH) && warp == 0) {
                 for (int w = lane; w < W; w += 32) {
@@ -1167,15 +1142,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     if (ci_) atomicAdd(slot + kAccInf, (unsigned long long)ci_);
                 }
             }
-            resolve_pre();                          // (a publication still pending from the tensor before)
             consumer_sync();
-            resolve_post();
             if (ctid == 0) {
                 __threadfence();
-                pend_old = atomicAdd(pv.done + c.t, ntile_acc);
-                sm.pend[0] = c.t; sm.pend[1] = c.isL ? 1 : 0; *reinterpret_cast<int64_t *>(sm.pend + 2) = c.len;
-                sm.pend[4] = ntile_acc; sm.pend[5] = c.tile_e - c.tile_b;
+                const int old = atomicAdd(pv.done + c.t, ntile_acc);
+                const int last = (old + ntile_acc == c.tile_e - c.tile_b) ? 1 : 0;
+                if (last) __threadfence();          // acquire: every CTA's adds of the tensor are visible below
+                sm.flag[1] = last;
             }
+            consumer_sync();
+            if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
             ntile_acc = 0;
         };
 
@@ -1308,9 +1284,6 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
         if (ctid == 0) trace_stamp(p, 1);
         if (touched) flush_tensor();
-        resolve_pre();
-        consumer_sync();
-        resolve_post();
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
