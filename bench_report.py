@@ -86,27 +86,33 @@ def fused_bytes(cfg, planes=True, p=2):
 
 
 def run_config(cfg, iters, dev):
-    """Whole model per iteration through nf_aggregate_bucket; small models are replicated so that
-    one iteration touches more than L2."""
+    """Whole model per iteration: ONE nf_aggregate_step call over all buckets (the kernels of consecutive buckets
+    chained by the library), and for comparison one nf_aggregate_bucket call per bucket; small models are
+    replicated so that one iteration touches more than L2 (the step then runs over all copies)."""
     import torch
-    from paper_2606_25759_b200 import BucketBuffers, binding as nf
+    from paper_2606_25759_b200 import ModelBuffers, binding as nf
     from workloads import gen
     in_bytes = sum(4 * cfg.W * b.n for b in cfg.buckets)
     copies = max(1, -(-2 * L2_BYTES // in_bytes)) if in_bytes < 2 * L2_BYTES else 1
-    G, BB = [], []
+    G, layouts = [], []
     for _ in range(copies):
         for b in cfg.buckets:
             G.append(gen.gen_bucket(cfg, b, dev))
-            BB.append(BucketBuffers(b.off, b.length, b.elig, b.n, cfg.W, dev, planes=True, health=True))
+            layouts.append((b.off, b.length, b.elig, b.n))
+    mb = ModelBuffers(layouts, cfg.W, dev, planes=True, health=True)
 
     def step():
-        for g, bb in zip(G, BB):
+        mb.step(G, (1, 0, 1), nf.MODE_GTERNARY)
+
+    def calls():
+        for g, bb in zip(G, mb.buckets):
             bb.aggregate(g, g.shape[1], (1, 0, 1), nf.MODE_GTERNARY)
     ms = time_fn(step, iters) / copies
     ms_graph = time_fn(step, iters, graph=True) / copies
-    del G, BB
+    ms_calls = time_fn(calls, iters, graph=True) / copies
+    del G, mb
     torch.cuda.empty_cache()
-    return ms, ms_graph, copies
+    return ms, ms_graph, ms_calls, copies
 
 
 def table_configs(args, dev, peak):
@@ -115,20 +121,22 @@ def table_configs(args, dev, peak):
     rows = []
     for nme in names:
         cfg = shapes.get(nme)
-        ms, msg, copies = run_config(cfg, args.iters if cfg.n_params < 5e8 else max(5, args.iters // 4), dev)
-        rows.append((cfg.name, cfg.W, cfg.n_params, len(cfg.buckets), ms, msg, copies, fused_bytes(cfg)))
+        ms, msg, msc, copies = run_config(cfg, args.iters if cfg.n_params < 5e8 else max(5, args.iters // 4), dev)
+        rows.append((cfg.name, cfg.W, cfg.n_params, len(cfg.buckets), ms, msg, msc, copies, fused_bytes(cfg)))
     for n in (131_072, 524_288):
         cfg = shapes.paper_local_count(n)
-        ms, msg, copies = run_config(cfg, args.iters, dev)
-        rows.append((cfg.name + " (PAPER L456 shape)", cfg.W, cfg.n_params, 1, ms, msg, copies, fused_bytes(cfg)))
-    out = ["| config | W | n (elements) | buckets | time / step | FP32-grad GB/s | elements/s | algorithmic bytes | % of 8000 GB/s | "
-           f"% of {peak:.1f} GB/s | same calls replayed from a CUDA graph | note |", "|---|---|---|---|---|---|---|---|---|---|---|---|"]
-    for name, W, n, nb, ms, msg, copies, ab in rows:
+        ms, msg, msc, copies = run_config(cfg, args.iters, dev)
+        rows.append((cfg.name + " (PAPER L456 shape)", cfg.W, cfg.n_params, 1, ms, msg, msc, copies, fused_bytes(cfg)))
+    out = ["| config | W | n (elements) | buckets | time / step (nf_aggregate_step, eager) | FP32-grad GB/s | elements/s | algorithmic bytes | "
+           f"% of 8000 GB/s | % of {peak:.1f} GB/s | nf_aggregate_step replayed from a CUDA graph | one nf_aggregate_bucket call per bucket, "
+           "graph replay | note |", "|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    for name, W, n, nb, ms, msg, msc, copies, ab in rows:
         t = ms * 1e-3
-        note = f"{copies} rotating copies (input < 2 x L2)" if copies > 1 else "input > L2"
+        note = f"{copies} rotating copies (input < 2 x L2), chained into one step" if copies > 1 else "input > L2"
         out.append(f"| {name} | {W} | {n:,} | {nb} | {ms * 1e3:.1f} us | {4 * W * n / t / 1e9:.1f} | {n / t:.3e} | "
                    f"{ab / 1e6:.1f} MB | {100 * ab / t / 1e9 / NOMINAL:.1f} | {100 * ab / t / 1e9 / peak:.1f} | "
-                   f"{msg * 1e3:.1f} us, {100 * ab / (msg * 1e-3) / 1e9 / peak:.1f} % | {note} |")
+                   f"{msg * 1e3:.1f} us, {100 * ab / (msg * 1e-3) / 1e9 / peak:.1f} % | "
+                   f"{msc * 1e3:.1f} us, {100 * ab / (msc * 1e-3) / 1e9 / peak:.1f} % | {note} |")
     return "\n".join(out)
 
 
@@ -199,7 +207,7 @@ def table_hier(args, dev, peak):
     from paper_2606_25759_b200 import BucketBuffers, binding as nf
     from workloads import shapes, gen
     out = ["| W | G (nodes) | workers/node | B planes | payload per node: packed signs -> partial counts | level 1 (one node) | "
-           "level 2 merge + decode | flat count-reduce | NEXT-2: stock packed-sign, W replicated counts | hierarchical, all nodes "
+           "level 2 merge + decode | flat count-reduce | NEXT-2: stock packed-sign (all-gather of the planes to W replicas + W local counts) | hierarchical, all nodes "
            "(G x level 1 + level 2) | NEXT-3: measured endpoint service rate | guard verdict at 12.5 / 50 / 400 GB/s per node |",
            "|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for W, G in ((32, 4), (32, 8), (128, 4), (128, 8), (128, 16)):
@@ -247,9 +255,23 @@ def table_hier(args, dev, peak):
             for bb in BBs:
                 bb.sign_count_reduce(nf.MODE_GTERNARY)
 
-        def stock():      # NEXT-2: every worker receives all W sign streams and counts them itself
-            for i in range(W):
-                BBs[i % rc].sign_count_reduce(nf.MODE_GTERNARY)
+        # NEXT-2: stock packed-sign transport: every worker receives all W sign streams (W gathered
+        # copies of the planes, device-to-device) and counts them itself into its own output (nf_stock_packed_sign)
+        bb0 = BBs[0]
+        recvP = torch.empty((W, W, bb0.plane_stride), dtype=torch.int32, device=dev)
+        recvN = torch.empty_like(recvP)
+        ostride = (n + 3) // 4 * 4
+        outs = torch.zeros((W, ostride), dtype=torch.float32, device=dev)
+
+        def stock():
+            nf.nf_stock_packed_sign(bb0.P, bb0.N, bb0.plane_stride, W, n, bb0.off, bb0.len, bb0.route, bb0.woff, bb0.T,
+                                    nf.MODE_GTERNARY, 0, bb0.abs_sum, recvP, recvN, outs, ostride, bb0.plan)
+        stock()
+        merge(bb0, CPs[0], CNs[0])
+        torch.cuda.synchronize()
+        for r in range(W):      # every replica reconstructs the same aggregate, and it is the hierarchical path's
+            assert torch.equal(outs[r, :n].view(torch.int32), bb0.out[:n].view(torch.int32)), f"replica {r} differs"
+        gathered = 2 * W * W * Wd * 4
 
         def hier_all():   # all G nodes count locally, one merge + decode
             for bb, cp, cn in zip(BBs, CPs, CNs):
@@ -258,11 +280,12 @@ def table_hier(args, dev, peak):
         t1, t2, t3, t4, t5 = (time_fn(f, args.iters if f is not stock else max(3, args.iters // 5), reps=1, graph=True) * 1e3 / div
                               for f, div in ((level1, rc * G), (level2, rc), (flat, rc), (stock, 1), (hier_all, rc)))
         packed, partial = 2 * Wg * Wd * 4, 2 * B * Wd * 4
-        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | {t4:.0f} us | {t5:.1f} us | "
+        out.append(f"| {W} | {G} | {Wg} | {B} | {packed / 1e6:.1f} MB -> {partial / 1e6:.1f} MB | {t1:.1f} us | {t2:.1f} us | {t3:.1f} us | "
+                   f"{t4:.0f} us ({gathered / 1e9:.2f} GB gathered, {W} outputs, all identical) | {t5:.1f} us | "
                    f"{packed / (t1 * 1e-6) / 1e9:.0f} GB/s | "
                    + " / ".join("admit" if nf.nf_capacity_guard(n, G, Wg, packed / (t1 * 1e-6), bw, 2)[0] else "FP32"
                                 for bw in (12.5e9, 50e9, 400e9)) + " |")
-        del g, bb, cp, cn, BBs, CPs, CNs
+        del g, bb, cp, cn, BBs, CPs, CNs, recvP, recvN, outs
         torch.cuda.empty_cache()
     return "\n".join(out)
 

@@ -174,6 +174,23 @@ int nf_partial_count_merge(const uint32_t *cnt_pos, const uint32_t *cnt_neg, int
                            nf_stream stream);
 
 /*
+ * NEXT-2: the stock packed-sign path the paper compares against — PAPER L245 ("packed-sign all-gather
+ * followed by local unpack-and-count"), L267 ("aggregation remains replicated: each worker receives sign streams and
+ * reconstructs the same count locally"), Fig. 3. Emulated on one GPU with the W workers as replicas: for every
+ * replica r < W, (1) the all-gather: all W workers' packed planes are copied into replica r's own receive buffer
+ * recvP + r*W*plane_stride (recvN likewise; G-Ternary only) — device-to-device copies standing in for the wire —
+ * and (2) the local unpack-and-count: the flat count + vote + decode of nf_sign_count_reduce over the received
+ * planes into replica r's own output out + r*out_stride. All W outputs must come out identical (and identical to
+ * nf_sign_count_reduce / the hierarchical path): that is what "the same count" means. Bytes gathered =
+ * W * W * Wd * 4 per plane. recvP / recvN: [W][W][plane_stride] words; out: [W][out_stride] floats, out_stride >= n
+ * and a multiple of 4; only low-bit positions are written. Same plan / metadata arguments as nf_sign_count_reduce.
+ */
+int nf_stock_packed_sign(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int W, int64_t n,
+                         const int64_t *off, const int64_t *len, const uint8_t *route, const int64_t *woff, int T,
+                         int mode, int margin, const double *abs_sum, uint32_t *recvP, uint32_t *recvN,
+                         float *out, int64_t out_stride, void *plan, nf_stream stream);
+
+/*
  * a4a FP32 route — PAPER L50, L66, L144 (oracle O4a). For every P/F tensor:
  * out[i] = alpha * (((g_0[i] + g_1[i]) + g_2[i]) + ... + g_{W-1}[i]) in FP32, fixed worker order.
  */

@@ -250,3 +250,19 @@ def aggregate_bucket(g, off, length, elig, state=(1, 0, 1), mode=MODE_GTERNARY, 
     fp32_reduce(g, off, length, r.route, alpha, out)
     Q, cn, ci = health_stats(g, off, length)
     return BucketResult(r, P, N, A, out, cpos, cneg, scale, Q, cn, ci)
+
+
+def stock_packed_sign(P, N, W, n, off, length, route, woff, mode, margin, abs_sum):
+    """NEXT-2, the stock packed-sign path ("packed-sign all-gather followed by local unpack-and-count",
+    L267 "each worker receives sign streams and reconstructs the same count locally"), written out: every replica r
+    gets its own copy of all W workers' planes (the all-gather) and runs O3 on it. Returns (out [W][n], gathered
+    bytes). That the W results are equal is NOT assumed here: the tests check it."""
+    outs = []
+    gathered = 0
+    for _ in range(W):
+        rP = np.array(P, copy=True)
+        rN = None if N is None else np.array(N, copy=True)
+        gathered += rP.nbytes + (0 if rN is None else rN.nbytes)
+        out, _, _, _ = sign_count_reduce(rP, rN, W, n, off, length, route, woff, mode, margin, abs_sum)
+        outs.append(out)
+    return np.stack(outs), gathered

@@ -23,7 +23,7 @@ SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = r
 
 EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_bytes", "nf_route_bucket",
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
-           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_aggregate_step", "nf_step_workspace_bytes",
+           "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_aggregate_step", "nf_step_workspace_bytes", "nf_stock_packed_sign",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
            "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace")
 
@@ -103,6 +103,8 @@ def lib() -> C.CDLL:
     L.nf_step_workspace_bytes.argtypes = [C.POINTER(NfBucket), i32]
     L.nf_aggregate_step.restype = i32
     L.nf_aggregate_step.argtypes = [C.POINTER(NfBucket), i32, i32, NfState, i32, i32, f32, vp, sz, vp]
+    L.nf_stock_packed_sign.restype = i32
+    L.nf_stock_packed_sign.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp, i64, vp, vp]
     L.nf_count_planes.restype = i32
     L.nf_count_planes.argtypes = [i32]
     L.nf_partial_count.restype = i32
@@ -231,6 +233,14 @@ def nf_aggregate_step(buckets, W, state, mode, margin, alpha, workspace, stream=
     _check("nf_aggregate_step", lib().nf_aggregate_step(
         buckets, len(buckets), int(W), _state(state), int(mode), int(margin), float(alpha), _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_stock_packed_sign(P, N, plane_stride, W, n, off, length, route, woff, T, mode, margin, abs_sum, recvP, recvN,
+                         out, out_stride, plan, stream=None):
+    _check("nf_stock_packed_sign", lib().nf_stock_packed_sign(
+        _ptr(P), _ptr(N), int(plane_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(route), _ptr(woff), int(T),
+        int(mode), int(margin), _ptr(abs_sum), _ptr(recvP), _ptr(recvN), _ptr(out), int(out_stride), _ptr(plan),
+        _stream(stream)))
 
 
 def nf_count_planes(Wg: int) -> int:

@@ -146,6 +146,43 @@ int nf_partial_count_merge(const uint32_t *cnt_pos, const uint32_t *cnt_neg, int
     return cuda_rc(launch_count_reduce(p, n, (cudaStream_t)stream));
 }
 
+int nf_stock_packed_sign(const uint32_t *P, const uint32_t *N, int64_t plane_stride, int W, int64_t n,
+                         const int64_t *off, const int64_t *len, const uint8_t *route, const int64_t *woff, int T,
+                         int mode, int margin, const double *abs_sum, uint32_t *recvP, uint32_t *recvN,
+                         float *out, int64_t out_stride, void *plan, nf_stream stream) {
+    int rc = check_common(W, n, T);
+    if (rc != NF_OK) return rc;
+    if (margin < 0 || margin > 255) return NF_ERR_RANGE;
+    if (mode != NF_MODE_GBINARY && mode != NF_MODE_GTERNARY) return NF_ERR_ARG;
+    if (!plan || plane_stride < 0 || out_stride < n || (out_stride & 3)) return NF_ERR_ARG;
+    if (T > 0 && (!P || !recvP || !off || !len || !route || !woff || !abs_sum || !out)) return NF_ERR_ARG;
+    if (mode == NF_MODE_GTERNARY && T > 0 && (!N || !recvN)) return NF_ERR_ARG;
+    if (misaligned16(P) || misaligned16(N) || misaligned16(recvP) || misaligned16(recvN) || misaligned16(out) ||
+        misaligned16(plan) || (plane_stride & 3))
+        return NF_ERR_ALIGN;
+    if (T == 0) return NF_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t plane_words = (size_t)W * (size_t)plane_stride;
+    for (int r = 0; r < W; ++r) {
+        // (1) all-gather: replica r receives every worker's packed planes
+        uint32_t *rp = recvP + (size_t)r * plane_words, *rn = recvN ? recvN + (size_t)r * plane_words : nullptr;
+        if (plane_words > 0) {
+            if (cudaMemcpyAsync(rp, P, plane_words * 4, cudaMemcpyDeviceToDevice, s) != cudaSuccess) return NF_ERR_CUDA;
+            if (mode == NF_MODE_GTERNARY &&
+                cudaMemcpyAsync(rn, N, plane_words * 4, cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+                return NF_ERR_CUDA;
+        }
+        // (2) local unpack-and-count over the received streams
+        ReduceParams p{};
+        p.P = rp; p.N = rn; p.plane_stride = plane_stride; p.W = W; p.T = T;
+        p.off = off; p.len = len; p.route = route; p.woff = woff;
+        p.ternary = (mode == NF_MODE_GTERNARY); p.margin = margin; p.abs_sum = abs_sum;
+        p.out = out + (size_t)r * (size_t)out_stride; p.plan = plan;
+        if (launch_count_reduce(p, n, s) != cudaSuccess) return NF_ERR_CUDA;
+    }
+    return NF_OK;
+}
+
 int nf_fp32_reduce(const float *g, int64_t worker_stride, int W, int64_t n,
                    const int64_t *off, const int64_t *len, const uint8_t *route, int T,
                    float alpha, float *out, void *plan, nf_stream stream) {

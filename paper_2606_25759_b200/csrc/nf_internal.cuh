@@ -200,6 +200,9 @@ struct ReduceParams {
     int64_t count_stride;
     int G, B;
     void *plan;
+    // NEXT-1 level 1 through the ring kernel (PARTIAL): the B count planes of this group of W workers are the output
+    uint32_t *part_pos, *part_neg;
+    int64_t part_Wd;           // packed words per plane (no plan, no tensor metadata on this path)
 };
 
 // launchers (each returns a cudaError_t from the launch)

@@ -404,7 +404,7 @@ constexpr int kQHdr = 256 + 4096;                  // mbarriers, direction table
 constexpr size_t kQSmem = kQHdr + (size_t)kQStages * kQStageWords * 4;
 static_assert(2 * kQStages * 8 <= 256, "mbarriers fit the header");
 
-template <bool WRITE_COUNTS, bool MERGE>
+template <bool WRITE_COUNTS, bool MERGE, bool PARTIAL>
 __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kernel(const __grid_constant__ ReduceParams p) {
     extern __shared__ __align__(128) unsigned char q_smem[];
     uint64_t *full = reinterpret_cast<uint64_t *>(q_smem);
@@ -420,11 +420,13 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     for (int i = tid; i < 256; i += kQThreads) fill_direction_table(s_dtab, i);
     __syncthreads();
     pdl_wait();                              // everything above touched shared memory only
-    const PlanView pv = plan_view(p.plan, p.T);
-    if (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK) return;
-    const int64_t Wd = pv.hdr->Wd;
+    // PARTIAL (NEXT-1 level 1, "node-local counting"): the bit-sliced counts of this group's W workers are
+    // the OUTPUT (B planes per sign); no plan, no tensors, no vote: the word count comes with the call
+    const PlanView pv = PARTIAL ? PlanView{} : plan_view(p.plan, p.T);
+    if (!PARTIAL && (pv.hdr->magic != kPlanMagic || pv.hdr->status != NF_OK)) return;
+    const int64_t Wd = PARTIAL ? p.part_Wd : pv.hdr->Wd;
     if (MERGE ? Wd > p.count_stride : Wd > p.plane_stride) return;     // rows shorter than the packed words: nothing is read
-    const int nL = pv.hdr->nL;
+    const int nL = PARTIAL ? 0 : pv.hdr->nL;
     const int W = p.W;
     const bool ternary = p.ternary != 0;
     const int64_t n_units = (Wd + kQWords - 1) / kQWords;
@@ -475,16 +477,19 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
     }
 
     // ---- consumers: thread = word position ----
-    publish_wordless_scales(p, pv, W, kQWords);
+    if (!PARTIAL) publish_wordless_scales(p, pv, W, kQWords);
     int st = 0;
     uint32_t ph = 0;
     TensorCache tc{-1, 0, 0, 0, 0, 0.f};
     for (int64_t unit = blockIdx.x; unit < n_units; unit += gridDim.x) {
         const int64_t k = unit * kQWords + tid;
         WordMeta m{0, -1, 0};
-        const bool hit = cached_meta(tc, k, lane, m);
-        if (!hit) m = word_meta(p, pv, nL, Wd, k);                     // overlaps the copies in flight,
-        const float S = warp_scales(p, pv, W, lane, k, m, hit, tc);    // and so does the chain of W abs-sums
+        float S = 0.f;
+        if (!PARTIAL) {
+            const bool hit = cached_meta(tc, k, lane, m);
+            if (!hit) m = word_meta(p, pv, nL, Wd, k);                 // overlaps the copies in flight,
+            S = warp_scales(p, pv, W, lane, k, m, hit, tc);            // and so does the chain of W abs-sums
+        }
         SlicedCounter cpv, cnv;
         cpv.clear(); cnv.clear();
         for (int g = 0; g < n_stg; ++g) {
@@ -511,6 +516,17 @@ __global__ void __launch_bounds__(kQThreads, NF_CRQ_MINB) count_reduce_ring_kern
                 else if (nb > 0) cpv.add8(xb);
             }
             if (++st == kQStages) { st = 0; ph ^= 1u; }
+        }
+        if (PARTIAL) {
+            if (k < Wd) {
+#pragma unroll
+                for (int b = 0; b < 8; ++b) {
+                    if (b >= p.B) break;
+                    p.part_pos[(size_t)b * p.count_stride + k] = cpv.c[b];
+                    if (ternary) p.part_neg[(size_t)b * p.count_stride + k] = cnv.c[b];
+                }
+            }
+            continue;
         }
         uint32_t dpos = 0u, dneg = 0u;
         if (k < Wd) vote_masks(p, W, cpv, cnv, m.nvalid, dpos, dneg);
@@ -543,11 +559,11 @@ static int grid_for(int64_t units, int per_sm) {
     return (int)(g < 1 ? 1 : g);
 }
 
-template <bool WRITE_COUNTS, bool MERGE>
+template <bool WRITE_COUNTS, bool MERGE, bool PARTIAL>
 static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_t s) {
     static bool attr_set = false;                    // per template instance
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>,
+        cudaError_t e = cudaFuncSetAttribute(count_reduce_ring_kernel<WRITE_COUNTS, MERGE, PARTIAL>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kQSmem);
         if (e != cudaSuccess) return e;
         attr_set = true;
@@ -555,7 +571,7 @@ static cudaError_t launch_ring(const ReduceParams &p, int64_t units, cudaStream_
     const int grid = grid_for(units, NF_CRQ_MINB);
     // programmatic stream serialization: the kernel waits (griddepcontrol.wait) for its predecessor on the stream
     // before it touches global memory; only its launch latency and shared-memory prologue overlap
-    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS, MERGE>, (unsigned)grid, kQThreads, kQSmem, s, true, p);
+    cudaError_t e = launch_kernel(count_reduce_ring_kernel<WRITE_COUNTS, MERGE, PARTIAL>, (unsigned)grid, kQThreads, kQSmem, s, true, p);
     return e != cudaSuccess ? e : cudaGetLastError();
 }
 
@@ -568,11 +584,11 @@ cudaError_t launch_count_reduce(const ReduceParams &p, int64_t n, cudaStream_t s
     // the bulk copies need 16-byte-aligned rows: P, N are (nf_sign_count_reduce checks), so plane_stride % 4 == 0
     const int64_t units = (max_words + kQWords - 1) / kQWords;
     if (!p.cnt_pos && (p.plane_stride & 3) == 0)
-        return counts ? launch_ring<true, false>(p, units, s) : launch_ring<false, false>(p, units, s);
+        return counts ? launch_ring<true, false, false>(p, units, s) : launch_ring<false, false, false>(p, units, s);
     // level-2 merge: rows of partial-count planes, same alignment rule
     if (p.cnt_pos && (p.count_stride & 3) == 0 && ((uintptr_t)p.cnt_pos & 15) == 0 &&
         (!p.ternary || ((uintptr_t)p.cnt_neg & 15) == 0))
-        return counts ? launch_ring<true, true>(p, units, s) : launch_ring<false, true>(p, units, s);
+        return counts ? launch_ring<true, true, false>(p, units, s) : launch_ring<false, true, false>(p, units, s);
     if (p.cnt_pos) {
         if (counts) count_reduce_kernel<true, true, 16><<<grid, kRThreads, 0, s>>>(p);
         else count_reduce_kernel<false, true, 16><<<grid, kRThreads, 0, s>>>(p);
@@ -590,6 +606,14 @@ cudaError_t launch_partial_count(const uint32_t *P, const uint32_t *N, int64_t p
                                  int ternary, int B, uint32_t *cnt_pos, uint32_t *cnt_neg, int64_t count_stride,
                                  cudaStream_t s) {
     if (Wd <= 0) return cudaSuccess;
+    // rows the bulk-copy engine can take (16-byte aligned): the same ring kernel as the flat reduce, the count planes
+    // as its output; anything else: the register-staged kernel
+    if ((plane_stride & 3) == 0 && ((uintptr_t)P & 15) == 0 && (!ternary || ((uintptr_t)N & 15) == 0)) {
+        ReduceParams p{};
+        p.P = P; p.N = N; p.plane_stride = plane_stride; p.W = Wg; p.ternary = ternary; p.B = B;
+        p.part_pos = cnt_pos; p.part_neg = cnt_neg; p.count_stride = count_stride; p.part_Wd = Wd;
+        return launch_ring<false, false, true>(p, (Wd + kQWords - 1) / kQWords, s);
+    }
     const int grid = grid_for((Wd + kRThreads - 1) / kRThreads, 8);
     partial_count_kernel<<<grid, kRThreads, 0, s>>>(P, N, plane_stride, Wg, Wd, ternary, B, cnt_pos, cnt_neg, count_stride);
     return cudaGetLastError();

@@ -15,12 +15,15 @@ pytestmark = pytest.mark.gpu
 DEV = "cuda"
 
 
-def _hier(cfg, b, groups, mode, margin=0, cs_pad=0):
+def _hier(cfg, b, groups, mode, margin=0, cs_pad=0, ps_pad=0):
     W = cfg.W
     assert sum(groups) == W
     g = gen.gen_bucket(cfg, b, DEV)
     ref = O.aggregate_bucket(np.ascontiguousarray(_np(g)[:, :b.n]), b.off, b.length, b.elig, (1, 0, 1), mode, None, margin)
-    bb = BucketBuffers(b.off, b.length, b.elig, b.n, W, DEV, planes=True, counts=True, health=True)
+    # plane_stride a multiple of 4 words: level 1 runs on the bulk-copy ring kernel; anything else: register-staged
+    Wd0 = sum((int(l) + 31) // 32 for l, e in zip(b.length, b.elig) if e)
+    bb = BucketBuffers(b.off, b.length, b.elig, b.n, W, DEV, planes=True, counts=True, health=True,
+                       plane_stride=(Wd0 + 3) // 4 * 4 + ps_pad)
     bb.route_bucket((1, 0, 1))
     bb.sign_pack(g, g.shape[1], mode)
     bb.fp32_reduce(g, g.shape[1])
@@ -83,6 +86,8 @@ def test_tiny_hierarchical(groups, mode):
     _hier(cfg, cfg.buckets[0], groups, mode)
     _hier(cfg, cfg.buckets[0], groups, mode, margin=1)
     _hier(cfg, cfg.buckets[0], groups, mode, cs_pad=2)
+    _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=1)
+    _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=3, margin=1)
 
 
 @pytest.mark.parametrize("name,groups", [("resnet50", [4, 4]), ("vit_b16", [8, 8]), ("vit_b16", [4, 4, 4, 4]),
@@ -98,3 +103,46 @@ def test_sweep_full_size_hierarchical():
     """Config 5 at full size (n = 6,553,600), W = 32 as 4 nodes of 8."""
     cfg = shapes.sweep(32)
     _hier(cfg, cfg.buckets[0], [8, 8, 8, 8], nf.MODE_GTERNARY)
+
+
+@pytest.mark.parametrize("mode", [nf.MODE_GBINARY, nf.MODE_GTERNARY])
+@pytest.mark.parametrize("name", ["tiny", "resnet50", "vit_b16", "sweep_w32"])
+def test_stock_packed_sign_replicated_counting(name, mode):
+    """NEXT-2 (Fig. 3): nf_stock_packed_sign — W gathered copies of the planes, W local
+    unpack-and-count passes into W outputs. Every replica's output matches the oracle's replica, all W are bitwise
+    identical to each other, to the flat nf_sign_count_reduce and to the two-level hierarchical path."""
+    cfg = shapes.get(name, small=(name != "tiny"))
+    W = cfg.W
+    for b in cfg.buckets[:2]:
+        g = gen.gen_bucket(cfg, b, DEV)
+        ref = O.aggregate_bucket(np.ascontiguousarray(_np(g)[:, :b.n]), b.off, b.length, b.elig, (1, 0, 1), mode)
+        ref_outs, gathered = O.stock_packed_sign(ref.P, ref.N if mode == O.MODE_GTERNARY else None, W, b.n, b.off, b.length,
+                                                 ref.route.route, ref.route.woff, mode, 0, ref.abs_sum)
+        bb = BucketBuffers(b.off, b.length, b.elig, b.n, W, DEV, planes=True, counts=False, health=True)
+        bb.route_bucket((1, 0, 1))
+        bb.sign_pack(g, g.shape[1], mode)
+        ternary = mode == nf.MODE_GTERNARY
+        recvP = torch.zeros((W, W, bb.plane_stride), dtype=torch.int32, device=DEV)
+        recvN = torch.zeros_like(recvP) if ternary else None
+        stride = (b.n + 3) // 4 * 4
+        outs = torch.full((W, max(stride, 4)), -9.0, dtype=torch.float32, device=DEV)
+        nf.nf_stock_packed_sign(bb.P, bb.N if ternary else None, bb.plane_stride, W, b.n, bb.off, bb.len, bb.route, bb.woff,
+                                bb.T, mode, 0, bb.abs_sum, recvP, recvN, outs, outs.shape[1], bb.plan)
+        bb.out.fill_(-9.0)
+        bb.sign_count_reduce(mode)
+        torch.cuda.synchronize()
+        Wd = ref.route.Wd
+        assert gathered == W * W * Wd * 4 * (2 if ternary else 1)
+        for r in range(W):                                           # the gathered streams are the workers' planes
+            assert np.array_equal(_np(recvP[r]).view(np.uint32)[:, :Wd], ref.P)
+        isL = np.zeros(b.n, bool)
+        for o, l, rt in zip(b.off, b.length, ref.route.route):
+            if rt == O.ROUTE_L:
+                isL[o:o + l] = True
+        flat = _np(bb.out)[:b.n]
+        from tests.util import assert_float_match
+        for r in range(W):
+            got = _np(outs[r])[:b.n]
+            assert_float_match(got[isL], ref_outs[r][isL], 1e-6, f"{cfg.name} bucket {b.index} replica {r}")
+            assert np.array_equal(got[isL], flat[isL], equal_nan=True), f"replica {r} differs from the flat reduce"
+            assert np.all(got[~isL] == -9.0)                         # only low-bit positions are written

@@ -93,3 +93,31 @@ def test_hierarchical_equals_flat(W, groups, mode):
         hier = O.partial_count_merge(cp, cn, W, n, off, ln, r.route, r.woff, mode, margin, A)
         for a, b in zip(flat, hier):
             assert np.array_equal(a, b, equal_nan=True)
+
+
+@pytest.mark.parametrize("mode", [O.MODE_GBINARY, O.MODE_GTERNARY])
+def test_stock_packed_sign_every_replica_reconstructs_the_same_aggregate(mode):
+    """NEXT-2: with stock packed-sign transport every worker unpacks and counts all W streams itself and
+    must arrive at the same aggregate: W identical outputs, equal to the flat reduce, whose counts equal the
+    brute-force counts taken straight from the floats (no words involved)."""
+    rng = np.random.default_rng(11)
+    W = 5
+    lens = [70, 33, 400]
+    off, ln, n = layout(lens)
+    g = rng.standard_normal((W, n)).astype(np.float32)
+    g[rng.random((W, n)) < 0.2] = 0.0
+    r = O.route_bucket(off, ln, [1, 0, 1], n)
+    P, N, A = O.sign_pack(g, off, ln, r.route, r.woff, mode, None, r.Wd)
+    outs, gathered = O.stock_packed_sign(P, N, W, n, off, ln, r.route, r.woff, mode, 0, A)
+    assert outs.shape == (W, n)
+    assert gathered == W * W * r.Wd * 4 * (2 if mode == O.MODE_GTERNARY else 1)
+    flat, cpos, cneg, scale = O.sign_count_reduce(P, N, W, n, off, ln, r.route, r.woff, mode, 0, A)
+    for rr in range(W):
+        assert np.array_equal(outs[rr], flat)
+    # brute force from the floats for the two low-bit tensors
+    for t in (0, 2):
+        x = g[:, off[t]:off[t] + ln[t]]
+        cp = (x > 0).sum(0)
+        cn = (x < 0).sum(0) if mode == O.MODE_GTERNARY else W - cp
+        d = np.sign(cp.astype(int) - cn.astype(int)).astype(np.float32)
+        assert np.array_equal(outs[0][off[t]:off[t] + ln[t]], scale[t] * d)
