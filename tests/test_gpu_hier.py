@@ -86,8 +86,9 @@ def test_tiny_hierarchical(groups, mode):
     _hier(cfg, cfg.buckets[0], groups, mode)
     _hier(cfg, cfg.buckets[0], groups, mode, margin=1)
     _hier(cfg, cfg.buckets[0], groups, mode, cs_pad=2)
-    _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=1)
-    _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=3, margin=1)
+    if len(groups) == 1:          # (several groups: their base pointers must stay 16-byte aligned)
+        _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=1)
+        _hier(cfg, cfg.buckets[0], groups, mode, ps_pad=3, margin=1)
 
 
 @pytest.mark.parametrize("name,groups", [("resnet50", [4, 4]), ("vit_b16", [8, 8]), ("vit_b16", [4, 4, 4, 4]),
