@@ -57,6 +57,10 @@ constexpr int kMaxStages = 4;
 constexpr int kStages = 3;                       // ring depth: 3 x 64 KB
 static_assert(kTile == kCThreads * 4, "one float4 per consumer thread per worker and tile");
 
+// named barriers 2 + b: hand-over of segment buffer b from the 16 consumer warps (arrive, never wait) to the reducer
+// warp (sync: a hardware wait, no polling)
+__device__ __forceinline__ void seg_bar_arrive(int b) { asm volatile("bar.arrive %0, %1;" ::"r"(2 + b), "n"(kCW * 32 + 32) : "memory"); }
+__device__ __forceinline__ void seg_bar_sync(int b) { asm volatile("bar.sync %0, %1;" ::"r"(2 + b), "n"(kCW * 32 + 32) : "memory"); }
 // barrier among the consumer warps only (the producer / decode warps never join it)
 __device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(kCThreads) : "memory"); }
 
@@ -127,6 +131,7 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [0, 64)         mbarriers full[4], empty[4]
 //   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
 //   [128, 384)      scratch of the in-kernel routing scan
+//   [416, 448)      segment buffers: mbarriers free[2], tensor and route of the segment held
 //   [384, 416)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid, decode chunk, pass A done)
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
 //   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
@@ -146,6 +151,8 @@ struct FusedSmem {
     int *seg_of;                 // [kMaxStages] 1: the tile ends a segment (last tile of its scheduling unit or tensor)
     int *flag;                   // [8] CTA-wide flags
     float *sw;                   // [256] per-worker scales of the tensor being finalised
+    uint64_t *seg_free;          // [2] mbarriers: the reducer warp is through with a segment buffer
+    int *seg_t, *seg_isL;        // [2] tensor (-1: no more segments) and route of the segment in a buffer
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -166,6 +173,9 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.seg_of = (int *)(base + 96);
     s.flag = (int *)(base + 384);
     s.sw = (float *)(base + 3072);
+    s.seg_free = (uint64_t *)(base + 416);
+    s.seg_t = (int *)(base + 432);
+    s.seg_isL = s.seg_t + 2;
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -717,6 +727,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
 
     if (tid == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(sm.full + s, 1); mbar_init(sm.empty + s, kCW); }
+        for (int b = 0; b < 2; ++b) mbar_init(sm.seg_free + b, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < 256; i += kFThreads) { sm.nan[i] = 0u; sm.inf[i] = 0u; }
@@ -1061,6 +1072,36 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
+        // ---- then the reducer of the CTA's segments. A segment (the tiles of one scheduling unit inside one
+        // tensor) leaves the 16 consumer warps as 16 FP64 values per (worker, statistic) in a buffer; one lane per
+        // (worker, statistic) sums them in warp order (a fixed shape: the value depends on the data only) and adds
+        // the segment's total EXACTLY to the tensor's accumulator (integer atomics: the order in which segments
+        // arrive, i.e. the dynamic scheduling, cannot change the result). The consumers never wait for each other
+        // here: a warp arrives on the buffer's named barrier and goes on; it waits on the buffer's "free" mbarrier
+        // only when it comes back to the same buffer (two buffers when W <= 32).
+        {
+            const int nbuf = fused_nbuf(W), T = p.T;
+            int b = 0;
+            for (;;) {
+                seg_bar_sync(b);
+                const int t = sm.seg_t[b];
+                if (t < 0) break;
+                const bool isL = sm.seg_isL[b] != 0;
+                const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
+                for (int j = lane; j < 2 * W; j += 32) {
+                    const double *src = src0 + j;
+                    double tot = 0.0;
+#pragma unroll
+                    for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
+                    unsigned long long *slot = pv.acc + ((size_t)(j >> 1) * T + t) * kAccWords;
+                    if ((j & 1) == 0) { if (isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
+                    else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(sm.seg_free + b);   // (release: the adds are ordered before whoever waits)
+                if (nbuf == 2) b ^= 1;
+            }
+        }
     } else if (warp >= kCW + 2) {
         // =====================================================================================
         // decode warps (pass B inside the kernel): see decode_warp_loop(). The consumers join them once
@@ -1107,24 +1148,23 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         int segpar = 0;                             // buffer of the current segment's per-warp FP64 values
         double *wbuf = sm.wacc;
 
-        // A segment (the tiles of one scheduling unit inside one tensor) is complete: its per-warp FP64 values are in
-        // `wbuf`, 16 per (worker, statistic). One thread per (worker, statistic) sums them in warp order (a fixed
-        // shape: the value depends on the data only) and adds the segment's total EXACTLY to the tensor's accumulator
-        // (integer atomics: the order in which segments arrive, i.e. the dynamic scheduling, cannot change the
-        // result). (Spreading the sum over the warps with shuffles was 5 - 11 % slower at W >= 32.)
-        auto seg_reduce = [&]() __attribute__((always_inline)) {
-            consumer_sync();
-            if (ctid < 2 * W) {
-                const double *src = wbuf + ctid;
-                double tot = 0.0;
-#pragma unroll
-                for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
-                unsigned long long *slot = pv.acc + ((size_t)(ctid >> 1) * T + c.t) * kAccWords;
-                if ((ctid & 1) == 0) { if (c.isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
-                else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
-            }
-            if (nbuf == 1) consumer_sync();         // one buffer (W > 32): the next segment overwrites it
-            else { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
+        uint32_t seguse0 = 0u, seguse1 = 0u;        // uses of each segment buffer so far
+        // before the first stat_flush of a segment: the reducer warp is through with the buffer's previous segment
+        auto seg_acquire = [&]() __attribute__((always_inline)) {
+            const uint32_t u = segpar ? seguse1 : seguse0;
+            mbar_wait(sm.seg_free + segpar, (u & 1u) ^ 1u);            // first use: passes at once
+        };
+        // after the last stat_flush of a segment: hand the buffer to the reducer warp (see there) and go on
+        auto seg_publish = [&](int t, bool isL) __attribute__((always_inline)) {
+            if (ctid == 0) { sm.seg_t[segpar] = t; sm.seg_isL[segpar] = isL ? 1 : 0; }
+            seg_bar_arrive(segpar);
+            if (segpar) ++seguse1; else ++seguse0;
+            if (nbuf == 2) { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
+        };
+        // every segment handed over so far has been added to the accumulators
+        auto seg_drain = [&]() __attribute__((always_inline)) {
+            if (seguse0 > 0u) mbar_wait(sm.seg_free + 0, (seguse0 - 1u) & 1u);
+            if (seguse1 > 0u) mbar_wait(sm.seg_free + 1, (seguse1 - 1u) & 1u);
         };
 
         // All tiles this CTA took of tensor c.t are done (every warp has passed the barrier of the tensor's last
@@ -1132,6 +1172,9 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // barrier orders every consumer thread's direction bytes, plane words, outputs and accumulator adds before
         // ctid 0's fence, which is cumulative), and finalise the tensor if this publication completed it.
         auto flush_tensor = [&]() __attribute__((always_inline)) {
+            // (the reducer warp takes a segment only after all 16 warps have handed it over: once it is through with
+            // the tensor's last segment, every warp's exact_redo tallies of the tensor are in and all its adds are out)
+            if (c.isL || HEALTH) seg_drain();
             if ((c.isL || HEALTH) && warp == 0) {
                 for (int w = lane; w < W; w += 32) {
                     const unsigned cn_ = atomicExch(&sm.nan[w], 0u), ci_ = atomicExch(&sm.inf[w], 0u);
@@ -1235,8 +1278,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                         }
                     }
                 }
-                if (MULTI && stats)
+                if (MULTI && stats) {
+                    if (w0 == 0) seg_acquire();
                     stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
+                }
             }
             if (c.isL) {
                 // majority vote with margin m and ties -> 0 (readings #3, #5, #6)
@@ -1272,16 +1317,19 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             if (!MULTI) ++kcnt;
             if (stats && seg_end) {
                 if (!MULTI) {
+                    seg_acquire();
                     stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
                     kcnt = 0;
                 }
-                seg_reduce();
+                seg_publish(c.t, c.isL);
             } else if (!MULTI && seg_end) {
                 kcnt = 0;
             }
         }
         if (ctid == 0) trace_stamp(p, 1);
         if (touched) flush_tensor();
+        seg_acquire();
+        seg_publish(-1, false);                     // no more segments: the reducer warp leaves
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
