@@ -508,17 +508,20 @@ struct DecodeSrc {
     float *out;
     PlanHeader *hdr;
 };
-// kDU consecutive units from u0 (those below u_lim), by one warp
-__device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
-                                            int u0, int u_lim, int lane) {
-    const float4 *dtab = sm.dtab;
+// A span = kDU consecutive units, by one warp, in two phases so that a warp can have the loads of its next span in
+// flight while it stores the current one: decode_load (tensor lookup, wait for the tensor's scale, direction words)
+// and decode_store (expand and write).
+struct DecodeSpan {
     uint32_t dv[kDU][2];
     int64_t obase[kDU], rem[kDU];
     float S[kDU];
+};
+__device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
+                                            int u0, int u_lim, int lane, DecodeSpan &sp) {
 #pragma unroll
     for (int k = 0; k < kDU; ++k) {
         const int u = u0 + k;
-        rem[k] = 0; obase[k] = 0; S[k] = 0.f; dv[k][0] = 0u; dv[k][1] = 0u;
+        sp.rem[k] = 0; sp.obase[k] = 0; sp.S[k] = 0.f; sp.dv[k][0] = 0u; sp.dv[k][1] = 0u;
         if (u >= u_lim) continue;
         const int tile = u >> 1;
         if (tile >= dc.tile_e) {
@@ -559,31 +562,34 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
         for (int h = 0; h < 2; ++h) {
             const int64_t i = wbase + h * 512 + lane * 16;
             if (i < dc.len_t)
-                dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(src.dirs + (size_t)dc.woff_t * 8 + (size_t)(i >> 2)));
+                sp.dv[k][h] = __ldcg(reinterpret_cast<const uint32_t *>(src.dirs + (size_t)dc.woff_t * 8 + (size_t)(i >> 2)));
         }
-        obase[k] = dc.off_t + wbase;
-        rem[k] = dc.len_t - wbase;
-        S[k] = dc.S_t;
+        sp.obase[k] = dc.off_t + wbase;
+        sp.rem[k] = dc.len_t - wbase;
+        sp.S[k] = dc.S_t;
     }
+}
+__device__ __forceinline__ void decode_store(const DecodeSrc &src, const FusedSmem &sm, int lane, const DecodeSpan &sp) {
+    const float4 *dtab = sm.dtab;
 #pragma unroll
     for (int k = 0; k < kDU; ++k) {
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const int64_t rh = rem[k] - h * 512;
+            const int64_t rh = sp.rem[k] - h * 512;
             if (rh <= 0) continue;                       // warp-uniform
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 // store j covers elements j*128 + lane*4 .. +3: direction byte (j*32 + lane)
-                const uint32_t w32 = __shfl_sync(0xffffffffu, dv[k][h], j * 8 + (lane >> 2));
+                const uint32_t w32 = __shfl_sync(0xffffffffu, sp.dv[k][h], j * 8 + (lane >> 2));
                 const uint32_t d = (w32 >> (8 * (lane & 3))) & 0xffu;
                 const int64_t e0 = j * 128 + lane * 4;
                 const int64_t r = rh - e0;
                 if (r <= 0) continue;
                 float4 v = dtab[d];
-                v.x = __fmul_rn(S[k], v.x); v.y = __fmul_rn(S[k], v.y);
-                v.z = __fmul_rn(S[k], v.z); v.w = __fmul_rn(S[k], v.w);
-                float *o = src.out + obase[k] + h * 512 + e0;
-                if (r >= 4 && (obase[k] & 3) == 0) {
+                v.x = __fmul_rn(sp.S[k], v.x); v.y = __fmul_rn(sp.S[k], v.y);
+                v.z = __fmul_rn(sp.S[k], v.z); v.w = __fmul_rn(sp.S[k], v.w);
+                float *o = src.out + sp.obase[k] + h * 512 + e0;
+                if (r >= 4 && (sp.obase[k] & 3) == 0) {
                     __stcs(reinterpret_cast<float4 *>(o), v);
                 } else {
                     o[0] = v.x;
@@ -595,23 +601,37 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
         }
     }
 }
-// A dedicated decode warp: kDU units per trip to the bucket's cursor, the next trip issued before the current span
-// is processed (the round trip hides behind the span's loads and stores). `stop` (shared memory, or NULL): once it
+__device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
+                                            int u0, int u_lim, int lane) {
+    DecodeSpan sp;
+    decode_load(p, src, sm, dc, u0, u_lim, lane, sp);
+    decode_store(src, sm, lane, sp);
+}
+// A dedicated decode warp: kDU units per trip to the bucket's cursor, software-pipelined: the trip for span i+2 and
+// the loads of span i+1 are in flight while span i is expanded and stored. `stop` (shared memory, or NULL): once it
 // is set the warp takes no further units (what it holds it finishes): the rest is left to the next kernel of the step.
 __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
                                                  const volatile int *stop, int lane) {
     const int total_units = src.n_tiles * 2;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
-    if (stop && *stop) return;
-    int ub = 0;
-    if (lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kDU);
-    ub = __shfl_sync(0xffffffffu, ub, 0);
-    while (ub < total_units) {
-        const bool more = !(stop && *stop);
-        int ub_next = total_units;
-        if (more && lane == 0) ub_next = atomicAdd(&src.hdr->unit_cursor, kDU);
-        decode_span(p, src, sm, dc, ub, total_units, lane);
-        ub = __shfl_sync(0xffffffffu, ub_next, 0);
+    auto grab = [&]() -> int {
+        int ub = total_units;
+        if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kDU);
+        return ub;                                          // (lane 0's value is the one that counts)
+    };
+    int ub = __shfl_sync(0xffffffffu, grab(), 0);
+    if (ub >= total_units) return;
+    int ub_next = grab();                                   // in flight while the first span is loaded
+    DecodeSpan cur;
+    decode_load(p, src, sm, dc, ub, total_units, lane, cur);
+    for (;;) {
+        const int u1 = __shfl_sync(0xffffffffu, ub_next, 0);
+        if (u1 >= total_units) { decode_store(src, sm, lane, cur); break; }
+        ub_next = grab();
+        DecodeSpan nxt;
+        decode_load(p, src, sm, dc, u1, total_units, lane, nxt);     // its direction words travel while `cur` is stored
+        decode_store(src, sm, lane, cur);
+        cur = nxt;
     }
 }
 // The consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
