@@ -10,7 +10,8 @@ CUSUM ... fallback, cooldown, and guarded readmission"; L143 (4)/(6): admission,
 
 Readings (DESIGN.md §2 #15-#19; the paper gives no formulas, so everything below the CUSUM recursion itself
 is "parity unpinned by the paper"):
-  #15 smoothing: m_0 = x_0, m_k = beta*m_{k-1} + (1-beta)*x_k
+  #15 smoothing: m_0 = the first finite x (a NaN / Inf signal is a fault, reading #18, and never enters the
+      smoothed signal), m_k = beta*m_{k-1} + (1-beta)*x_k
   #16 CUSUM (Page's one-sided test, the paper's ref [21]): y_k = m_k - m_{k-1};
       S_k = max(0, S_{k-1} + y_k - slack); alarm iff S_k > threshold
   #17 phases: WARMUP (admitted=0) for warmup_steps steps -> ADMITTED -> alarm -> COOLDOWN (veto=1) for
@@ -33,7 +34,7 @@ class Supervisor:
         self.cooldown_steps, self.guard_steps = int(cooldown_steps), int(guard_steps)
         self.phase = WARMUP if self.warmup_steps > 0 else ADMITTED
         self.step_no = 0
-        self.ema = 0.0
+        self.ema = None                 # not seeded yet
         self.cusum = 0.0
         self.remaining = self.warmup_steps
         self.detections = 0
@@ -44,7 +45,7 @@ class Supervisor:
         finite = math.isfinite(signal)
         fault = (nan_count > 0) or (inf_count > 0) or (not finite)
         if finite:
-            if self.step_no == 0:
+            if self.ema is None:
                 self.ema, y = float(signal), 0.0
             else:
                 new = self.beta * self.ema + (1.0 - self.beta) * float(signal)

@@ -27,7 +27,7 @@ int nf_supervisor_init(nf_supervisor *s, const nf_supervisor_cfg *cfg) {
     s->remaining = cfg->warmup_steps;
     s->step = 0;
     s->detections = 0;
-    s->ema = 0.0;
+    s->ema = NAN;                      // not seeded yet (reading #15: the first FINITE signal seeds it)
     s->cusum = 0.0;
     return NF_OK;
 }
@@ -39,8 +39,8 @@ int nf_supervisor_step(nf_supervisor *s, double signal, uint64_t nan_count, uint
     const bool fault = nan_count != 0 || inf_count != 0 || !finite;           // reading #18
     double y = 0.0;                                                            // increase of the smoothed signal
     if (finite) {
-        if (s->step == 0) {
-            s->ema = signal;                                                   // reading #15: m_0 = x_0
+        if (isnan(s->ema)) {
+            s->ema = signal;                                                   // reading #15: m_0 = the first finite x
         } else {
             const double m = s->cfg.ema_beta * s->ema + (1.0 - s->cfg.ema_beta) * signal;
             y = m - s->ema;

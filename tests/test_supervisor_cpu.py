@@ -124,3 +124,23 @@ def test_library_supervisor_matches_oracle_step_for_step(nf, seed):
         assert a == b, i
         assert lib.phase == ora.phase and lib.detections == ora.detections
         assert lib.cusum == ora.cusum and lib.ema == ora.ema          # same FP64 operations in the same order
+
+
+def test_non_finite_first_signals_do_not_seed_the_smoothed_signal(nf):
+    """Reading #15: the smoothed signal starts at the FIRST FINITE value. A NaN / Inf at step 0 must not
+    leave m at 0 (the next finite x would then look like a jump of (1 - beta) x and, once admitted, like a long climb:
+    spurious alarms). Closed form: NaN, Inf, then a constant c for ever -> m = c exactly, y = 0, S = 0, no alarm after
+    the faults' own; oracle and library agree step for step."""
+    cfg = dict(warmup_steps=0, ema_beta=0.9, slack=0.0, threshold=0.05, cooldown_steps=2, guard_steps=0)
+    ora, lib = S.Supervisor(**cfg), nf.Supervisor(**cfg)
+    c = 2.5
+    xs = [float("nan"), float("inf")] + [c] * 40
+    for i, x in enumerate(xs):
+        a, b = ora.step(x), lib.step(x)
+        assert a == b, i
+        if i >= 2:
+            assert ora.ema == c and lib.ema == c and ora.cusum == 0.0 and lib.cusum == 0.0
+    # the two non-finite signals were faults (reading #18): admitted from the start, so exactly one detection (the
+    # second fault falls into the cooldown of the first), none from the constant stretch
+    assert ora.detections == 1 and lib.detections == 1
+    assert ora.phase == S.ADMITTED and lib.phase == S.ADMITTED
