@@ -375,9 +375,27 @@ def cpu_baseline(cfg, G, budget_s=20.0):
         del gh
     if not used:
         return None
-    return {"value": round(done_bytes / t_total / 1e9, 4), "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"buckets {used} of {cfg.name} ({done_bytes / 1e9:.2f} GB of FP32 gradient input, "
-                      f"{t_total:.1f} s single-threaded, host has {os.cpu_count()} cores)"}
+    out = {"value": round(done_bytes / t_total / 1e9, 4), "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"buckets {used} of {cfg.name} ({done_bytes / 1e9:.2f} GB of FP32 gradient input, "
+                     f"{t_total:.1f} s single-threaded, host has {os.cpu_count()} cores)"}
+    # the same (unchanged, single-threaded) oracle on all host cores at once: one bucket per thread, the C calls run
+    # outside the GIL; reported beside the 1-core figure, never as the target
+    try:
+        from concurrent.futures import ThreadPoolExecutor
+        nthr = max(1, min(os.cpu_count() or 1, len(used), 16))
+        todo = [(b, g.cpu().numpy()[:, :b.n].copy()) for b, g in zip(cfg.buckets, G) if b.index in used[:nthr]]
+        t0 = time.perf_counter()
+        with ThreadPoolExecutor(max_workers=nthr) as ex:
+            list(ex.map(lambda bg: O.aggregate_bucket(bg[1], bg[0].off, bg[0].length, bg[0].elig, (1, 0, 1),
+                                                      O.MODE_GTERNARY) and None, todo))
+        dt = time.perf_counter() - t0
+        nb = sum(4 * cfg.W * b.n for b, _ in todo)
+        out["all_cores"] = {"value": round(nb / dt / 1e9, 4), "unit": UNIT, "cores": nthr,
+                            "sample": f"buckets {[b.index for b, _ in todo]} concurrently, one oracle call per thread "
+                                      f"({nb / 1e9:.2f} GB in {dt:.1f} s)"}
+    except Exception as e:                                   # the 1-core figure stands on its own
+        out["all_cores"] = {"error": str(e)[:200]}
+    return out
 
 
 def run_reference(args):
@@ -390,15 +408,16 @@ def run_reference(args):
     from oracle import nf_oracle as O
     from workloads import shapes, gen
     cfg = shapes.get(args.config, small=args.small)
-    # bounded sample: the first mixed low-bit bucket of the workload (bucket 1: 33.6 M elements x W)
-    b = cfg.buckets[min(1, len(cfg.buckets) - 1)]
+    # bounded sample: the first bucket of the workload (GPT config: bucket 0, 33.6 M elements x W = 8, two 16.8 M
+    # low-bit weight matrices + biases / LayerNorm on the FP32 route, no injected NaN: a clean, typical bucket)
+    b = cfg.buckets[0]
     dev = "cuda" if torch.cuda.is_available() else "cpu"
     gh = gen.gen_bucket(cfg, b, dev).cpu().numpy()[:, :b.n].copy()
     in_bytes = 4 * cfg.W * b.n
 
     def step():
         O.aggregate_bucket(gh, b.off, b.length, b.elig, (1, 0, 1), O.MODE_GTERNARY)
-    for _ in range(min(args.warmup, 1)):
+    for _ in range(args.warmup):
         step()
     t0 = time.perf_counter()
     for _ in range(args.steps):
@@ -406,9 +425,9 @@ def run_reference(args):
     dt = (time.perf_counter() - t0) / args.steps
     val = round(in_bytes / dt / 1e9, 4)
     sample = (f"bucket {b.index} of {cfg.name} per step ({in_bytes / 1e9:.2f} GB of FP32 gradient input, "
-              f"{b.n} elements x W={cfg.W}); single-threaded C oracle; host has {os.cpu_count()} cores")
+              f"{b.n} elements x W={cfg.W}, no injected NaN); single-threaded C oracle; host has {os.cpu_count()} cores")
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
-                      "n_gpus": args.gpus, "steps": args.steps, "warmup": min(args.warmup, 1),
+                      "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
                       "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True, "scaling": "weak",
                       "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                       "config": {"workload": f"{cfg.name}: W={cfg.W}, bounded sample = {sample}"},
