@@ -131,7 +131,7 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [0, 64)         mbarriers full[4], empty[4]
 //   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
 //   [128, 384)      scratch of the in-kernel routing scan
-//   [416, 448)      segment buffers: mbarriers free[2], tensor and route of the segment held
+//   [416, 512)      segment buffers: mbarriers free[2]; the record handed over with each buffer [2][8]
 //   [384, 416)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid, decode chunk, pass A done)
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
 //   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
@@ -152,7 +152,7 @@ struct FusedSmem {
     int *flag;                   // [8] CTA-wide flags
     float *sw;                   // [256] per-worker scales of the tensor being finalised
     uint64_t *seg_free;          // [2] mbarriers: the reducer warp is through with a segment buffer
-    int *seg_t, *seg_isL;        // [2] tensor (-1: no more segments) and route of the segment in a buffer
+    int *seg_rec;                // [2][8] record handed over with a buffer: tensor (-1: no more), kind, route, tiles, ...
     unsigned int *nan, *inf;     // [256] each
     float4 *dtab;                // [256]
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
@@ -174,8 +174,7 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.flag = (int *)(base + 384);
     s.sw = (float *)(base + 3072);
     s.seg_free = (uint64_t *)(base + 416);
-    s.seg_t = (int *)(base + 432);
-    s.seg_isL = s.seg_t + 2;
+    s.seg_rec = (int *)(base + 448);
     s.nan = (unsigned int *)(base + 1024);
     s.inf = s.nan + 256;
     s.dtab = (float4 *)(base + 4096);
@@ -407,7 +406,7 @@ __device__ __forceinline__ uint32_t vote4(uint32_t posR, uint32_t negR, int W, i
 // totals: |x| sums finite, squares neither over- nor underflowed; otherwise the warp re-reads
 // exactly those elements in FP64 (and tallies NaN / Inf).
 template <bool HEALTH>
-__device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, double *wbuf, float (&af)[8],
+__device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, double *wbuf, int tally0, float (&af)[8],
                                            float (&qf)[8], int64_t off_t, int64_t len_t, int tile_b, int w0, int nw,
                                            int cnt, int4 recent, int ctid, bool aligned) {
     const int lane = ctid & 31, warp = ctid >> 5, W = p.W;
@@ -438,7 +437,7 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
                 double2 e = make_double2((double)a_t, (double)q_t);
                 if (!ok_t)
                     e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, recent, cnt, ctid, sm.nan,
-                                           sm.inf, w0 + w, aligned);
+                                           sm.inf, tally0 + w0 + w, aligned);
                 const double ea = warp_sum(e.x), eq = warp_sum(e.y);
                 if (lane == 0) { slot[w * 2] = ea; slot[w * 2 + 1] = eq; }
             } else if ((lane & 1) == 0 && wl == w) {
@@ -611,7 +610,7 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
 // the loads of span i+1 are in flight while span i is expanded and stored. `stop` (shared memory, or NULL): once it
 // is set the warp takes no further units (what it holds it finishes): the rest is left to the next kernel of the step.
 __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
-                                                 const volatile int *stop, int lane) {
+                                                 const volatile int *stop, volatile int *hint, int lane) {
     const int total_units = src.n_tiles * 2;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
     auto grab = [&]() -> int {
@@ -626,6 +625,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
     decode_load(p, src, sm, dc, ub, total_units, lane, cur);
     for (;;) {
         const int u1 = __shfl_sync(0xffffffffu, ub_next, 0);
+        if (lane == 0 && hint) *hint = u1;                  // (where the cursor stands: the consumers size their first chunk by it)
         if (u1 >= total_units) { decode_store(src, sm, lane, cur); break; }
         ub_next = grab();
         DecodeSpan nxt;
@@ -637,14 +637,18 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
 // The consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
 // arriving together on one address serialise: 15 us for the last warp served), chunk sizes guided by what is
 // left (4 spans .. 16 spans per warp), spans dealt to the 16 warps round-robin.
-__device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, int ctid) {
+__device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, int ctid,
+                                                int cursor_hint) {
     const int total_units = src.n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
-    int chunk = kDU * 8;
+    // first chunk: an even share of what was left when this CTA's decode warps last looked (a backlog of many units is
+    // then taken in one trip per CTA), at least 8 spans
+    int chunk = kDU * min(max((total_units - cursor_hint) / ((int)gridDim.x * kDU), 8), 16 * kCW);
     for (;;) {
-        if (ctid == 0) sm.flag[3] = atomicAdd(&src.hdr->unit_cursor, chunk);
+        if (ctid == 0) { sm.flag[3] = atomicAdd(&src.hdr->unit_cursor, chunk); sm.flag[6] = chunk; }
         consumer_sync();
         const int base = sm.flag[3];
+        chunk = sm.flag[6];                                  // (ctid 0's: the hint the first chunk is sized by is racy)
         if (base >= total_units) break;
         const int lim = min(base + chunk, total_units);
         for (int u0 = base + kDU * warp; u0 < lim; u0 += kDU * kCW) decode_span(p, src, sm, dc, u0, lim, lane);
@@ -675,8 +679,123 @@ extern __shared__ __align__(128) unsigned char smem_raw[];
 // to FP64 once, writes abs_sum / sumsq / nan_cnt / inf_cnt, clears the accumulator slots for the next call,
 // computes S_t = (float)(sum_w (double)(float)(A_w / len_t) / W) in worker order ("mean-absolute
 // scale"; readings #7, #8) and publishes it: fin[t] = {1, S_t} releases the decode warps of every CTA.
-// Called by all consumer threads of the CTA.
+// Done by ONE warp (the CTA's reducer warp), so that the consumers never stop for it.
+//  * W <= 32: lane k holds word k of a worker's slot (one coalesced 256-byte load per worker, the loads of up to 8
+//    workers in flight together), carries and rounding by shuffles;
+//  * wider fan-in: lane = worker, 32 workers per pass, each lane walking its own slot (acc_round).
 // ---------------------------------------------------------------------------------------------
+template <bool HEALTH>
+__device__ __noinline__ void finalize_tensor_warp(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
+                                                  int64_t len_t, bool isL, int lane) {
+    const int W = p.W, T = p.T;
+    const bool read = isL || HEALTH;
+    if (W <= 32) {
+        for (int w0 = 0; w0 < W; w0 += 8) {
+            unsigned long long v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                v[i] = 0ull;
+                if (read && w0 + i < W) v[i] = __ldcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane);
+            }
+            // (the clearing stores come after ALL the loads have been issued: a store behind a load of the same word
+            // would serialise the eight round trips)
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+                if (read && w0 + i < W) __stcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane, 0ull);
+            // the eight workers' carry chains and roundings are walked together (independent shuffle chains overlap)
+            unsigned long long cn[8], ci[8], lo[8], hi[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                cn[i] = __shfl_sync(0xffffffffu, v[i], kAccNan);
+                ci[i] = __shfl_sync(0xffffffffu, v[i], kAccInf);
+                lo[i] = lane >= kAccNan ? 0ull : (v[i] & 0xffffffffull);
+                hi[i] = lane >= kAccNan ? 0ull : (v[i] >> 32);
+            }
+            for (;;) {                                   // deferred carries ripple up (no carry into lanes 0 / kAccSq)
+                bool more = false;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    unsigned long long c = __shfl_up_sync(0xffffffffu, hi[i], 1);
+                    if (lane == kAccAbs || lane == kAccSq) c = 0ull;
+                    const unsigned long long x = lo[i] + c;
+                    lo[i] = x & 0xffffffffull;
+                    hi[i] = x >> 32;
+                    more |= hi[i] != 0ull;
+                }
+                if (!__any_sync(0xffffffffu, more)) break;
+            }
+            double A[8], Q[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const uint32_t digit = (uint32_t)lo[i];
+                const unsigned nz = __ballot_sync(0xffffffffu, digit != 0u);
+                A[i] = 0.0;
+                Q[i] = 0.0;
+                if (read && isL) {
+                    A[i] = warp_acc_round(digit, nz, kAccAbs, kAccAbsWords, kAccAbsBase);
+                    if (cn[i]) A[i] = __longlong_as_double(0x7ff8000000000000ll);      // IEEE: a NaN term makes the sum NaN,
+                    else if (ci[i]) A[i] = __longlong_as_double(0x7ff0000000000000ll); // an Inf term (no NaN) makes it +Inf
+                }
+                if (read && HEALTH) Q[i] = warp_acc_round(digit, nz, kAccSq, kAccSqWords, kAccSqBase);
+            }
+            if (lane < 8 && w0 + lane < W) {             // lane i writes worker w0 + i's results
+                double a = 0.0, q = 0.0;
+                unsigned long long n_ = 0ull, i_ = 0ull;
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    if (lane == i) { a = A[i]; q = Q[i]; n_ = cn[i]; i_ = ci[i]; }
+                const size_t o = (size_t)(w0 + lane) * T + t;
+                if (HEALTH) { p.sumsq[o] = q; p.nan_cnt[o] = n_; p.inf_cnt[o] = i_; }
+                p.abs_sum[o] = a;                                  // 0 for tensors that are not low-bit routed
+                sm.sw[w0 + lane] = (float)(a / (double)len_t);
+            }
+        }
+    } else {
+        for (int w = lane; w < W; w += 32) {
+            const size_t o = (size_t)w * T + t;
+            double A = 0.0;
+            if (read) {
+                unsigned long long wd[kAccWords];
+                ulonglong2 *slot = reinterpret_cast<ulonglong2 *>(pv.acc + o * kAccWords);
+#pragma unroll
+                for (int i = 0; i < kAccWords / 2; ++i) {
+                    const ulonglong2 x = __ldcg(slot + i);
+                    wd[2 * i] = x.x;
+                    wd[2 * i + 1] = x.y;
+                }
+#pragma unroll
+                for (int i = 0; i < kAccWords / 2; ++i) __stcg(slot + i, make_ulonglong2(0ull, 0ull));
+                const unsigned long long cn = wd[kAccNan], ci = wd[kAccInf];
+                if (isL) {
+                    A = acc_round(wd + kAccAbs, kAccAbsWords, kAccAbsBase);
+                    if (cn) A = __longlong_as_double(0x7ff8000000000000ll);
+                    else if (ci) A = __longlong_as_double(0x7ff0000000000000ll);
+                }
+                if (HEALTH) {
+                    p.sumsq[o] = acc_round(wd + kAccSq, kAccSqWords, kAccSqBase);
+                    p.nan_cnt[o] = cn;
+                    p.inf_cnt[o] = ci;
+                }
+            }
+            p.abs_sum[o] = A;
+            sm.sw[w] = (float)(A / (double)len_t);
+        }
+    }
+    if (!isL) return;
+    __syncwarp();
+    if (lane == 0) {
+        double s = 0.0;
+        for (int w = 0; w < W; ++w) s += (double)sm.sw[w];
+        const float S = (float)(s / (double)W);
+        pv.scale[t] = S;
+        if (p.scale_out) p.scale_out[t] = S;
+        st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));    // (release: a fence of its own)
+    }
+    __syncwarp();
+}
+
+// The same by the CTA's 16 consumer warps, a warp per worker (used at the end of the kernel, when the consumers have
+// nothing else to do and the tensor's decode is the critical path). Called by all consumer threads.
 template <bool HEALTH>
 __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
                                              int64_t len_t, bool isL, int ctid) {
@@ -1071,19 +1190,22 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         }
     } else if (warp == kCW + 1) {
         // =====================================================================================
-        // housekeeping warp: the outputs of the tensors that own no tile (len = 0): totals 0, scale 0 on the
-        // FP32 route and the oracle's 0/0 on the low-bit route (every other tensor is finalised by its last arriver)
+        // housekeeping warp: the outputs nobody else writes. Tensors that own no tile (len = 0): totals 0, scale 0 on
+        // the FP32 route and the oracle's 0/0 on the low-bit route. FP32-route tensors: scale 0, and abs_sum 0 when no
+        // health statistics are gathered (with them, the tensor is finalised like any other by its last arriver).
         // =====================================================================================
-        for (int t = blockIdx.x * 32 + lane; t < p.T; t += (int)gridDim.x * 32) {
+        for (int t = blockIdx.x * 32 + lane; t < p.T && layout_ok; t += (int)gridDim.x * 32) {
             int64_t len_t;
             bool isL;
             if (p.T <= kMetaCap) { len_t = sm.m_len[t]; isL = sm.m_woff[t] >= 0; }
             else { len_t = __ldg(p.len + t); isL = __ldg(p.route + t) == NF_ROUTE_L; }
-            if (len_t > 0 || !layout_ok) continue;
-            for (int w = 0; w < W; ++w) {
-                const size_t o = (size_t)w * p.T + t;
-                p.abs_sum[o] = 0.0;
-                if (HEALTH) { p.sumsq[o] = 0.0; p.nan_cnt[o] = 0ull; p.inf_cnt[o] = 0ull; }
+            if (len_t > 0 && isL) continue;
+            if (len_t <= 0 || !HEALTH) {
+                for (int w = 0; w < W; ++w) {
+                    const size_t o = (size_t)w * p.T + t;
+                    p.abs_sum[o] = 0.0;
+                    if (HEALTH) { p.sumsq[o] = 0.0; p.nan_cnt[o] = 0ull; p.inf_cnt[o] = 0ull; }
+                }
             }
             double s = 0.0;
             const double zero = 0.0, dl = (double)len_t;
@@ -1092,33 +1214,61 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
-        // ---- then the reducer of the CTA's segments. A segment (the tiles of one scheduling unit inside one
-        // tensor) leaves the 16 consumer warps as 16 FP64 values per (worker, statistic) in a buffer; one lane per
-        // (worker, statistic) sums them in warp order (a fixed shape: the value depends on the data only) and adds
-        // the segment's total EXACTLY to the tensor's accumulator (integer atomics: the order in which segments
-        // arrive, i.e. the dynamic scheduling, cannot change the result). The consumers never wait for each other
-        // here: a warp arrives on the buffer's named barrier and goes on; it waits on the buffer's "free" mbarrier
-        // only when it comes back to the same buffer (two buffers when W <= 32).
+        // ---- then the CTA's reducer and publisher. The 16 consumer warps hand it records through two buffers (one
+        // when W > 32): a warp arrives on the buffer's named barrier and goes on (it waits on the buffer's "free"
+        // mbarrier only when it comes back to the same buffer), so the consumers never wait for each other here.
+        //  * data record = a SEGMENT (the tiles of one scheduling unit inside one tensor): 16 FP64 values per (worker,
+        //    statistic), one per consumer warp; a lane per (worker, statistic) sums them in warp order (a fixed shape:
+        //    the value depends on the data only) and adds the segment's total EXACTLY to the tensor's accumulator
+        //    (integer atomics: the order in which segments arrive, i.e. the dynamic scheduling, cannot change the
+        //    result); the NaN / Inf tallies of the segment go the same way.
+        //  * flush record = this CTA is through with tensor t for now (`n` tiles since its last flush): publish the
+        //    count (release: every consumer warp arrived after its last store of the tensor; this warp's fence is
+        //    cumulative) and, if that completed the tensor, finalise it (finalize_tensor_warp).
         {
             const int nbuf = fused_nbuf(W), T = p.T;
             int b = 0;
             for (;;) {
                 seg_bar_sync(b);
-                const int t = sm.seg_t[b];
+                const int *rec = sm.seg_rec + 8 * b;
+                const int t = rec[0];
                 if (t < 0) break;
-                const bool isL = sm.seg_isL[b] != 0;
-                const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
-                for (int j = lane; j < 2 * W; j += 32) {
-                    const double *src = src0 + j;
-                    double tot = 0.0;
+                const bool isL = rec[2] != 0;
+                if (rec[1] == 0) {
+                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
+                    for (int j = lane; j < 2 * W; j += 32) {
+                        const double *src = src0 + j;
+                        double tot = 0.0;
 #pragma unroll
-                    for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
-                    unsigned long long *slot = pv.acc + ((size_t)(j >> 1) * T + t) * kAccWords;
-                    if ((j & 1) == 0) { if (isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
-                    else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
+                        for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
+                        unsigned long long *slot = pv.acc + ((size_t)(j >> 1) * T + t) * kAccWords;
+                        if ((j & 1) == 0) { if (isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
+                        else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
+                    }
+                    for (int w = lane; w < W; w += 32) {
+                        const unsigned cn_ = atomicExch(&sm.nan[b * 32 + w], 0u), ci_ = atomicExch(&sm.inf[b * 32 + w], 0u);
+                        unsigned long long *slot = pv.acc + ((size_t)w * T + t) * kAccWords;
+                        if (cn_) atomicAdd(slot + kAccNan, (unsigned long long)cn_);
+                        if (ci_) atomicAdd(slot + kAccInf, (unsigned long long)ci_);
+                    }
+                } else {
+                    const int n = rec[3], total = rec[4];
+                    const int64_t len_t = *reinterpret_cast<const int64_t *>(rec + 6);
+                    __threadfence();
+                    __syncwarp();
+                    int old = 0;
+                    if (lane == 0) old = atomicAdd(pv.done + t, n);
+                    old = __shfl_sync(0xffffffffu, old, 0);
+                    if (old + n == total) {
+                        // (every other CTA's adds of the tensor were fenced before its own count reached done[t]; the
+                        // slots are read from L2, after the value the atomic returned: control dependency)
+                        if (lane == 0) trace_stamp(p, 12);
+                        finalize_tensor_warp<HEALTH>(p, pv, sm, t, len_t, isL, lane);
+                        if (lane == 0) trace_stamp(p, 13);
+                    }
                 }
                 __syncwarp();
-                if (lane == 0) mbar_arrive(sm.seg_free + b);   // (release: the adds are ordered before whoever waits)
+                if (lane == 0) mbar_arrive(sm.seg_free + b);   // (release: what was done is ordered before whoever waits)
                 if (nbuf == 2) b ^= 1;
             }
         }
@@ -1136,9 +1286,9 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (p.chained) {
             pdl_wait();
             prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
-            decode_warp_loop(p, prev, sm, nullptr, lane);
+            decode_warp_loop(p, prev, sm, nullptr, nullptr, lane);
         }
-        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, lane);
+        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, sm.flag + 7, lane);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
     } else {
         // =====================================================================================
@@ -1148,7 +1298,6 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (ctid == 0) trace_stamp(p, 0);
         const TCtl tctl = make_tctl(lane);
         const bool ternary = p.ternary != 0;
-        const int T = p.T;
         float af[8], qf[8];                         // FP32 partials of the current worker group
 #pragma unroll
         for (int i = 0; i < 8; ++i) { af[i] = 0.f; qf[i] = 0.f; }
@@ -1172,47 +1321,27 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // before the first stat_flush of a segment: the reducer warp is through with the buffer's previous segment
         auto seg_acquire = [&]() __attribute__((always_inline)) {
             const uint32_t u = segpar ? seguse1 : seguse0;
-            mbar_wait(sm.seg_free + segpar, (u & 1u) ^ 1u);            // first use: passes at once
+            mbar_wait_backoff(sm.seg_free + segpar, (u & 1u) ^ 1u);    // first use: passes at once
         };
         // after the last stat_flush of a segment: hand the buffer to the reducer warp (see there) and go on
-        auto seg_publish = [&](int t, bool isL) __attribute__((always_inline)) {
-            if (ctid == 0) { sm.seg_t[segpar] = t; sm.seg_isL[segpar] = isL ? 1 : 0; }
+        auto seg_publish = [&](int t, int kind, bool isL, int n, int total, int64_t len_t) __attribute__((always_inline)) {
+            if (ctid == 0) {
+                int *rec = sm.seg_rec + 8 * segpar;
+                rec[0] = t; rec[1] = kind; rec[2] = isL ? 1 : 0; rec[3] = n; rec[4] = total;
+                *reinterpret_cast<int64_t *>(rec + 6) = len_t;
+            }
             seg_bar_arrive(segpar);
             if (segpar) ++seguse1; else ++seguse0;
             if (nbuf == 2) { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
         };
-        // every segment handed over so far has been added to the accumulators
-        auto seg_drain = [&]() __attribute__((always_inline)) {
-            if (seguse0 > 0u) mbar_wait(sm.seg_free + 0, (seguse0 - 1u) & 1u);
-            if (seguse1 > 0u) mbar_wait(sm.seg_free + 1, (seguse1 - 1u) & 1u);
-        };
-
-        // All tiles this CTA took of tensor c.t are done (every warp has passed the barrier of the tensor's last
-        // segment: its NaN / Inf tallies are final): hand in the tallies, publish the tile count (release: the CTA
-        // barrier orders every consumer thread's direction bytes, plane words, outputs and accumulator adds before
-        // ctid 0's fence, which is cumulative), and finalise the tensor if this publication completed it.
+        // All tiles this CTA took of tensor c.t so far are done: tell the reducer warp (a flush record: it publishes the
+        // tile count and finalises the tensor if that completed it). No barrier, no round trip on the consumers' path:
+        // every warp arrives after its own last store of the tensor.
         auto flush_tensor = [&]() __attribute__((always_inline)) {
-            // (the reducer warp takes a segment only after all 16 warps have handed it over: once it is through with
-            // the tensor's last segment, every warp's exact_redo tallies of the tensor are in and all its adds are out)
-            if (c.isL || HEALTH) seg_drain();
-            if ((c.isL || HEALTH) && warp == 0) {
-                for (int w = lane; w < W; w += 32) {
-                    const unsigned cn_ = atomicExch(&sm.nan[w], 0u), ci_ = atomicExch(&sm.inf[w], 0u);
-                    unsigned long long *slot = pv.acc + ((size_t)w * T + c.t) * kAccWords;
-                    if (cn_) atomicAdd(slot + kAccNan, (unsigned long long)cn_);
-                    if (ci_) atomicAdd(slot + kAccInf, (unsigned long long)ci_);
-                }
+            if (c.isL || HEALTH) {
+                seg_acquire();
+                seg_publish(c.t, 1, c.isL, ntile_acc, c.tile_e - c.tile_b, c.len);
             }
-            consumer_sync();
-            if (ctid == 0) {
-                __threadfence();
-                const int old = atomicAdd(pv.done + c.t, ntile_acc);
-                const int last = (old + ntile_acc == c.tile_e - c.tile_b) ? 1 : 0;
-                if (last) __threadfence();          // acquire: every CTA's adds of the tensor are visible below
-                sm.flag[1] = last;
-            }
-            consumer_sync();
-            if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
             ntile_acc = 0;
         };
 
@@ -1300,7 +1429,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 }
                 if (MULTI && stats) {
                     if (w0 == 0) seg_acquire();
-                    stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
+                    stat_flush<HEALTH>(p, sm, wbuf, segpar * 32, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
                 }
             }
             if (c.isL) {
@@ -1338,27 +1467,40 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             if (stats && seg_end) {
                 if (!MULTI) {
                     seg_acquire();
-                    stat_flush<HEALTH>(p, sm, wbuf, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
+                    stat_flush<HEALTH>(p, sm, wbuf, segpar * 32, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
                     kcnt = 0;
                 }
-                seg_publish(c.t, c.isL);
+                seg_publish(c.t, 0, c.isL, 0, 0, 0);
             } else if (!MULTI && seg_end) {
                 kcnt = 0;
             }
         }
         if (ctid == 0) trace_stamp(p, 1);
-        if (touched) flush_tensor();
+        if (touched && (c.isL || HEALTH)) {
+            // the last tensor this CTA worked on: its decode is now the critical path and the consumers are free, so
+            // they publish and finalise it themselves (16 warps) once the reducer warp is through with every record
+            if (seguse0 > 0u) mbar_wait_backoff(sm.seg_free + 0, (seguse0 - 1u) & 1u);
+            if (seguse1 > 0u) mbar_wait_backoff(sm.seg_free + 1, (seguse1 - 1u) & 1u);
+            consumer_sync();
+            if (ctid == 0) {
+                __threadfence();
+                const int old = atomicAdd(pv.done + c.t, ntile_acc);
+                sm.flag[1] = (old + ntile_acc == c.tile_e - c.tile_b) ? 1 : 0;
+            }
+            consumer_sync();
+            if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
+        }
         seg_acquire();
-        seg_publish(-1, false);                     // no more segments: the reducer warp leaves
+        seg_publish(-1, 0, false, 0, 0, 0);         // no more records: the reducer warp leaves
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
             // whatever is left of the previous bucket (normally nothing: its tail was drained long ago)
             pdl_wait();
             prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
-            decode_cta_loop(p, prev, sm, ctid);
+            decode_cta_loop(p, prev, sm, ctid, 0);
         }
-        if (!p.defer_tail) decode_cta_loop(p, own, sm, ctid);      // help finish pass B
+        if (!p.defer_tail) decode_cta_loop(p, own, sm, ctid, *(volatile int *)(sm.flag + 7));      // help finish pass B
         if (ctid == 0) trace_stamp(p, 3);
     }
 

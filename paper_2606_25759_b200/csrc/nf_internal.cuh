@@ -279,6 +279,19 @@ __device__ __forceinline__ void mbar_wait(uint64_t *b, uint32_t parity) {
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
         "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"(smem_u32(b)), "r"(parity) : "memory");
 }
+// the same wait for a warp that may have to wait LONG for another warp of its own CTA: poll, and sleep in between,
+// so that the waiting warps do not take the issue slots the warp they wait for needs
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t *b, uint32_t parity) {
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+        if (ok) break;
+        __nanosleep(100);
+    }
+}
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
