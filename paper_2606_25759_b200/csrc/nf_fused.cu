@@ -606,32 +606,34 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
     decode_load(p, src, sm, dc, u0, u_lim, lane, sp);
     decode_store(src, sm, lane, sp);
 }
-// A dedicated decode warp: kDU units per trip to the bucket's cursor, software-pipelined: the trip for span i+2 and
-// the loads of span i+1 are in flight while span i is expanded and stored. `stop` (shared memory, or NULL): once it
-// is set the warp takes no further units (what it holds it finishes): the rest is left to the next kernel of the step.
+// A dedicated decode warp: one span (kDU units) per trip to the bucket's cursor, the next trip issued before the span
+// is processed (its round trip hides behind the span's loads and stores). More in flight per warp (2 or 4 spans per
+// trip, or the next span's loads ahead of the current span's stores) made every config slower: the decode warps then
+// take issue slots and L2 bandwidth the consumers need. `stop` (shared memory, or NULL): once it is set the warp
+// takes no further units (what it holds it finishes): the rest is left to the next kernel of the step.
+#ifndef NF_DSPANS
+#define NF_DSPANS 1
+#endif
 __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
                                                  const volatile int *stop, volatile int *hint, int lane) {
+    constexpr int kGU = NF_DSPANS * kDU;                    // units per trip
     const int total_units = src.n_tiles * 2;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
     auto grab = [&]() -> int {
         int ub = total_units;
-        if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kDU);
+        if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kGU);
         return ub;                                          // (lane 0's value is the one that counts)
     };
     int ub = __shfl_sync(0xffffffffu, grab(), 0);
-    if (ub >= total_units) return;
-    int ub_next = grab();                                   // in flight while the first span is loaded
-    DecodeSpan cur;
-    decode_load(p, src, sm, dc, ub, total_units, lane, cur);
-    for (;;) {
-        const int u1 = __shfl_sync(0xffffffffu, ub_next, 0);
-        if (lane == 0 && hint) *hint = u1;                  // (where the cursor stands: the consumers size their first chunk by it)
-        if (u1 >= total_units) { decode_store(src, sm, lane, cur); break; }
-        ub_next = grab();
-        DecodeSpan nxt;
-        decode_load(p, src, sm, dc, u1, total_units, lane, nxt);     // its direction words travel while `cur` is stored
-        decode_store(src, sm, lane, cur);
-        cur = nxt;
+    while (ub < total_units) {
+        const int ub_next = grab();                         // in flight while this trip's spans are processed
+        DecodeSpan sp[NF_DSPANS];
+#pragma unroll
+        for (int k = 0; k < NF_DSPANS; ++k) decode_load(p, src, sm, dc, ub + k * kDU, total_units, lane, sp[k]);
+#pragma unroll
+        for (int k = 0; k < NF_DSPANS; ++k) decode_store(src, sm, lane, sp[k]);
+        ub = __shfl_sync(0xffffffffu, ub_next, 0);
+        if (lane == 0 && hint) *hint = ub;                  // (where the cursor stands: the consumers size their first chunk by it)
     }
 }
 // The consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
