@@ -1236,7 +1236,43 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 const int t = rec[0];
                 if (t < 0) break;
                 const bool isL = rec[2] != 0;
-                if (rec[1] == 0) {
+                if (rec[1] == 2) {
+                    // the segment is the whole tensor: its sums ARE the totals (exactly what rounding the accumulator
+                    // of a single addend gives)
+                    const int64_t len_t = *reinterpret_cast<const int64_t *>(rec + 6);
+                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
+                    for (int j0 = 0; j0 < 2 * W; j0 += 32) {
+                        const int j = j0 + lane, w = j >> 1;
+                        double tot = 0.0;
+                        if (j < 2 * W) {
+#pragma unroll
+                            for (int k = 0; k < kCW; ++k) tot += src0[(size_t)k * 2 * W + j];
+                        }
+                        const double other = __shfl_xor_sync(0xffffffffu, tot, 1);      // even lane: sum |x|, odd lane: sum x^2
+                        if (j < 2 * W && (j & 1) == 0) {
+                            const unsigned cn_ = atomicExch(&sm.nan[b * 32 + w], 0u), ci_ = atomicExch(&sm.inf[b * 32 + w], 0u);
+                            const size_t o = (size_t)w * T + t;
+                            double A = 0.0;
+                            if (isL) {
+                                A = tot;
+                                if (cn_) A = __longlong_as_double(0x7ff8000000000000ll);
+                                else if (ci_) A = __longlong_as_double(0x7ff0000000000000ll);
+                            }
+                            p.abs_sum[o] = A;
+                            if (HEALTH) { p.sumsq[o] = other; p.nan_cnt[o] = cn_; p.inf_cnt[o] = ci_; }
+                            sm.sw[w] = (float)(A / (double)len_t);
+                        }
+                    }
+                    __syncwarp();
+                    if (isL && lane == 0) {
+                        double sacc = 0.0;
+                        for (int w = 0; w < W; ++w) sacc += (double)sm.sw[w];
+                        const float S = (float)(sacc / (double)W);
+                        pv.scale[t] = S;
+                        if (p.scale_out) p.scale_out[t] = S;
+                        st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));
+                    }
+                } else if (rec[1] == 0) {
                     const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
                     for (int j = lane; j < 2 * W; j += 32) {
                         const double *src = src0 + j;
@@ -1467,12 +1503,17 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             ntile_acc += R;
             if (!MULTI) ++kcnt;
             if (stats && seg_end) {
+                // a segment that IS the whole tensor (small tensors: norms, biases): this CTA is its only arriver, so
+                // the reducer warp writes the tensor's results straight from the segment's sums (record kind 2): no
+                // accumulator, no fence, no completion count, no flush record
+                const bool whole = (MULTI ? R : kcnt) == c.tile_e - c.tile_b;
                 if (!MULTI) {
                     seg_acquire();
                     stat_flush<HEALTH>(p, sm, wbuf, segpar * 32, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
                     kcnt = 0;
                 }
-                seg_publish(c.t, 0, c.isL, 0, 0, 0);
+                seg_publish(c.t, whole ? 2 : 0, c.isL, 0, 0, c.len);
+                if (whole) { touched = false; ntile_acc = 0; }
             } else if (!MULTI && seg_end) {
                 kcnt = 0;
             }
