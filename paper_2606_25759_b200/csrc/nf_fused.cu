@@ -997,11 +997,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             int32_t *tile_prefix = (int32_t *)(pb + PL.tile_prefix);
             int32_t *lt_index = (int32_t *)(pb + PL.lt_index);
             int64_t *lt_woff = (int64_t *)(pb + PL.lt_woff);
+            LtRec *lt_rec = (LtRec *)(pb + PL.lt_rec);
             if (tid < T) {
                 p.route_w[tid] = (uint8_t)r;
                 p.woff_w[tid] = r == NF_ROUTE_L ? ex_words : -1;
                 tile_prefix[tid] = (int32_t)ex_tiles;
-                if (r == NF_ROUTE_L) { lt_index[ex_nl] = tid; lt_woff[ex_nl] = ex_words; }
+                if (r == NF_ROUTE_L) {
+                    lt_index[ex_nl] = tid;
+                    lt_woff[ex_nl] = ex_words;
+                    lt_rec[ex_nl] = LtRec{tid, o, l, ex_words, ex_words + v_words, 0};
+                }
             }
             if (tid == 0) {
                 const unsigned long long *tal = reinterpret_cast<const unsigned long long *>(s_scan + 24);

@@ -59,11 +59,22 @@ constexpr int kAccAbs = 0, kAccAbsWords = 10, kAccAbsBase = -149;
 constexpr int kAccSq = 10, kAccSqWords = 19, kAccSqBase = -298;
 constexpr int kAccNan = 29, kAccInf = 30;
 
+// One low-bit tensor as step a3 sees it (index li in the plan's list of L tensors): a warp that enters a tensor reads
+// this record instead of walking lt_index -> len / off / lt_woff[li], lt_woff[li + 1] (a chain of dependent L2 round trips).
+struct __align__(16) LtRec {
+    int64_t t;                             // tensor index
+    int64_t off, len;                      // bucket offset and length in elements
+    int64_t kfirst, kend;                  // packed word range [kfirst, kend)
+    int64_t pad;
+};
+static_assert(sizeof(LtRec) == 48, "LtRec layout");
+
 // Offsets (bytes) of the plan arrays for a bucket of T tensors.
 struct PlanLayout {
     size_t tile_prefix;                    // int32 [T+1]
     size_t lt_index;                       // int32 [T]     ids of the L tensors, in order
     size_t lt_woff;                        // int64 [T+1]   woff of the L tensors, lt_woff[nL] = Wd
+    size_t lt_rec;                         // LtRec [T]     everything a3 needs of an L tensor in one 48-byte record
     size_t scale;                          // float [T]     per-tensor scale scratch
     size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
     size_t fin;                            // uint64 [T]    fused path: {1, FP32 bits of S_t} once tensor t is finalised, else 0
@@ -79,6 +90,7 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
     L.tile_prefix = o; o = align_up(o + sizeof(int32_t) * (size_t)(T + 1), 16);
     L.lt_index = o;    o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
     L.lt_woff = o;     o = align_up(o + sizeof(int64_t) * (size_t)(T + 1), 16);
+    L.lt_rec = o;      o = align_up(o + sizeof(LtRec) * (size_t)(T > 0 ? T : 1), 16);
     L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
     L.done = o;        o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
     L.fin = o;         o = align_up(o + sizeof(unsigned long long) * (size_t)(T > 0 ? T : 1), 16);
@@ -101,6 +113,7 @@ struct PlanView {
     const int32_t *tile_prefix;
     const int32_t *lt_index;
     const int64_t *lt_woff;
+    const LtRec *lt_rec;
     float *scale;
     int32_t *done;
     unsigned long long *fin;
@@ -115,6 +128,7 @@ __host__ __device__ inline PlanView plan_view(void *plan, int T) {
     v.tile_prefix = (const int32_t *)(p + L.tile_prefix);
     v.lt_index = (const int32_t *)(p + L.lt_index);
     v.lt_woff = (const int64_t *)(p + L.lt_woff);
+    v.lt_rec = (const LtRec *)(p + L.lt_rec);
     v.scale = (float *)(p + L.scale);
     v.done = (int32_t *)(p + L.done);
     v.fin = (unsigned long long *)(p + L.fin);

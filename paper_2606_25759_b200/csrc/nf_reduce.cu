@@ -127,15 +127,20 @@ struct WordMeta {
     int64_t obase;     // bucket position of the word's first element
 };
 
+__device__ __forceinline__ LtRec load_rec(const LtRec *r) {
+    const longlong2 *q = reinterpret_cast<const longlong2 *>(r);
+    const longlong2 a = __ldg(q), b = __ldg(q + 1), c = __ldg(q + 2);
+    return LtRec{a.x, a.y, b.x, b.y, c.x, c.y};
+}
 __device__ __forceinline__ WordMeta word_meta(const ReduceParams &p, const PlanView &pv, int nL, int64_t Wd, int64_t k) {
     WordMeta m{0, -1, 0};
     if (k < Wd) {
         const int li = upper_tensor<int64_t>(pv.lt_woff, nL, k);
-        const int t = __ldg(pv.lt_index + li);
-        const int64_t i0 = (k - __ldg(pv.lt_woff + li)) * 32;  // tensor-relative first element
-        const int64_t rem = __ldg(p.len + t) - i0;
+        const LtRec r = load_rec(pv.lt_rec + li);              // one 48-byte record instead of four dependent lookups
+        const int64_t i0 = (k - r.kfirst) * 32;                // tensor-relative first element
+        const int64_t rem = r.len - i0;
         m.nvalid = rem >= 32 ? 32 : (int)rem;
-        m.obase = __ldg(p.off + t) + i0;
+        m.obase = r.off + i0;
         m.li = li;
     }
     return m;
@@ -206,20 +211,20 @@ __device__ __forceinline__ float warp_scales(const ReduceParams &p, const PlanVi
 #pragma unroll
         for (int d = 16; d >= 1; d >>= 1) li_hi = max(li_hi, __shfl_xor_sync(0xffffffffu, li_hi, d));
         for (int li = li_lo; li >= 0 && li <= li_hi; ++li) {
-            const int t = __ldg(pv.lt_index + li);
-            const float St = warp_tensor_scale(p.abs_sum, W, p.T, t, __ldg(p.len + t), lane);
+            const LtRec r = load_rec(pv.lt_rec + li);
+            const int t = (int)r.t;
+            const float St = warp_tensor_scale(p.abs_sum, W, p.T, t, r.len, lane);
             if (m.li == li) S = St;
-            const int64_t kfirst = __ldg(pv.lt_woff + li);
-            if (lane == 0 && kfirst >= k && kfirst < k + 32) {      // this warp holds the tensor's first word
+            if (lane == 0 && r.kfirst >= k && r.kfirst < k + 32) {  // this warp holds the tensor's first word
                 pv.scale[t] = St;
                 if (p.scale_out) p.scale_out[t] = St;
             }
             if (li == li_hi) {                                      // remember the last tensor seen (warp-uniform)
                 tc.li = li;
-                tc.kfirst = kfirst;
-                tc.kend = __ldg(pv.lt_woff + li + 1);
-                tc.len = __ldg(p.len + t);
-                tc.off = __ldg(p.off + t);
+                tc.kfirst = r.kfirst;
+                tc.kend = r.kend;
+                tc.len = r.len;
+                tc.off = r.off;
                 tc.S = St;
             }
         }

@@ -70,6 +70,7 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
     int32_t *tile_prefix = (int32_t *)(pb + L.tile_prefix);
     int32_t *lt_index = (int32_t *)(pb + L.lt_index);
     int64_t *lt_woff = (int64_t *)(pb + L.lt_woff);
+    LtRec *lt_rec = (LtRec *)(pb + L.lt_rec);
 
     // stand-alone use (nf_route_bucket): the exact accumulators the streaming calls add into start from zero
     // (they clear what they use, but the buffer may be fresh); the fused path keeps them clean itself
@@ -110,7 +111,11 @@ route_kernel(const int64_t *__restrict__ off, const int64_t *__restrict__ len,
             route[t] = (uint8_t)r;
             woff[t] = (r == NF_ROUTE_L) ? ex.words : -1;
             tile_prefix[t] = (int32_t)ex.tiles;
-            if (r == NF_ROUTE_L) { lt_index[ex.nl] = t; lt_woff[ex.nl] = ex.words; }
+            if (r == NF_ROUTE_L) {
+                lt_index[ex.nl] = t;
+                lt_woff[ex.nl] = ex.words;
+                lt_rec[ex.nl] = LtRec{t, off[t], l, ex.words, ex.words + v.words, 0};
+            }
         }
         carry = add3(carry, total);
     }
