@@ -845,13 +845,13 @@ __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanVi
 // the kernel
 // ---------------------------------------------------------------------------------------------
 #ifndef NF_TAIL4
-#define NF_TAIL4 12                       // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
+#define NF_TAIL4 4                        // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
 #endif
 #ifndef NF_GRAB
 #define NF_GRAB 1                         // most scheduling units a producer takes per trip to the cursor
 #endif
 #ifndef NF_TAIL2
-#define NF_TAIL2 4                        // the last NF_TAIL2 x grid tiles are handed out one at a time
+#define NF_TAIL2 1                        // the last NF_TAIL2 x grid tiles are handed out one at a time
 #endif
 
 template <bool HEALTH, bool MULTI>
