@@ -61,7 +61,8 @@ typedef enum nf_status {
     NF_ERR_ARG = -1,    /* NULL where a pointer is required, bad mode, bad bucket layout, plan too small */
     NF_ERR_ALIGN = -2,  /* a base pointer is not 16-byte aligned */
     NF_ERR_RANGE = -3,  /* W, margin, T or n outside the supported range */
-    NF_ERR_CUDA = -4    /* a CUDA runtime call or kernel launch failed */
+    NF_ERR_CUDA = -4,   /* a CUDA runtime call or kernel launch failed */
+    NF_ERR_TOO_LARGE = -5 /* nf_aggregate_bucket_noalloc: the bucket needs more scratch than NF_NOALLOC_WORKSPACE_BYTES */
 } nf_status;
 
 /* Route codes: L = low-bit executed, F = FP32 fallback of an admitted route under
@@ -233,6 +234,34 @@ int nf_aggregate_bucket(const float *g, int64_t worker_stride, int W, int64_t n,
                         float *out, float *scale_out,
                         void *plan, size_t plan_bytes, void *workspace, size_t workspace_bytes,
                         nf_stream stream);
+
+/*
+ * nf_aggregate_bucket for callers that cannot provide scratch memory of their own because they may not call
+ * cudaMalloc where the call is made (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * allocation). Same arguments, results and errors as nf_aggregate_bucket, minus (workspace, workspace_bytes): the
+ * fused kernel's direction workspace (one byte per 4 low-bit elements, written by pass A and read back by pass B of
+ * the same launch) is a file-scope static device array of NF_NOALLOC_WORKSPACE_BYTES inside the library, which
+ * every GPU that loads the library holds until the process exits. The call allocates nothing (no cudaMalloc /
+ * cudaFree / allocating library routine); inputs, outputs and the plan are still the caller's.
+ *  - Limit: nf_workspace_bytes(T, n) <= NF_NOALLOC_WORKSPACE_BYTES, i.e. n/32 + T + 1 <= 2 Mi words: buckets of up
+ *    to about 67 M elements (256 MB of FP32 gradients per worker). A larger bucket is refused with
+ *    NF_ERR_TOO_LARGE before anything is launched.
+ *  - The array's device address is looked up once per device, on that device's first call (with that device
+ *    current); a failure of that lookup is NF_ERR_CUDA. The first call on a device should therefore be made
+ *    outside stream capture.
+ *  - Every call on a device shares the one array, and it keeps the previous call's contents. Nothing in it has
+ *    to start at zero: pass A writes every byte pass B reads. Calls that overlap on the GPU (different streams,
+ *    or a stream beside a graph launch) race on it and produce garbage: order them on one stream.
+ */
+#define NF_NOALLOC_WORKSPACE_BYTES ((size_t)16 << 20)
+int nf_aggregate_bucket_noalloc(const float *g, int64_t worker_stride, int W, int64_t n,
+                                const int64_t *off, const int64_t *len, const uint8_t *elig, int T,
+                                nf_state state, int mode, const float *tau, int margin, float alpha,
+                                uint8_t *route, int64_t *woff, int64_t *summary,
+                                uint32_t *P, uint32_t *N, int64_t plane_stride,
+                                double *abs_sum, double *sumsq, uint64_t *nan_cnt, uint64_t *inf_cnt,
+                                float *out, float *scale_out,
+                                void *plan, size_t plan_bytes, nf_stream stream);
 
 /*
  * One training step's buckets in ONE call (the hook's view of a step: PAPER L140-146, steps (2)-(7) for every DDP

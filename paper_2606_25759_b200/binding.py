@@ -16,7 +16,8 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libnf.so")
 
-NF_OK, NF_ERR_ARG, NF_ERR_ALIGN, NF_ERR_RANGE, NF_ERR_CUDA = 0, -1, -2, -3, -4
+NF_OK, NF_ERR_ARG, NF_ERR_ALIGN, NF_ERR_RANGE, NF_ERR_CUDA, NF_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5
+NF_NOALLOC_WORKSPACE_BYTES = 16 << 20   # nf.h: the static scratch array behind nf_aggregate_bucket_noalloc
 ROUTE_P, ROUTE_L, ROUTE_F = 0, 1, 2
 MODE_GBINARY, MODE_GTERNARY = 1, 2
 SUM_WD, SUM_NL, SUM_NF, SUM_NP, SUM_E, SUM_F, SUM_TILES, SUM_STATUS, SUM_LEN = range(9)
@@ -25,7 +26,7 @@ EXPORTS = ("nf_status_string", "nf_version", "nf_plan_bytes", "nf_workspace_byte
            "nf_sign_pack", "nf_sign_count_reduce", "nf_fp32_reduce", "nf_health_stats",
            "nf_aggregate_bucket", "nf_aggregate_bucket_host", "nf_aggregate_step", "nf_step_workspace_bytes", "nf_stock_packed_sign",
            "nf_count_planes", "nf_partial_count", "nf_partial_count_merge", "nf_supervisor_init",
-           "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace")
+           "nf_supervisor_step", "nf_mgtr", "nf_capacity_guard", "nf_debug_trace", "nf_aggregate_bucket_noalloc")
 
 
 class NfState(C.Structure):
@@ -93,6 +94,10 @@ def lib() -> C.CDLL:
     L.nf_aggregate_bucket.argtypes = [vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32, f32,
                                       vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp,
                                       vp, sz, vp, sz, vp]
+    L.nf_aggregate_bucket_noalloc.restype = i32
+    L.nf_aggregate_bucket_noalloc.argtypes = [vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32, f32,
+                                              vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp,
+                                              vp, sz, vp]
     L.nf_aggregate_bucket_host.restype = i32
     L.nf_aggregate_bucket_host.argtypes = [vp, vp, i64, i32, i64, vp, vp, vp, i32, NfState, i32, vp, i32,
                                            f32, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp,
@@ -210,6 +215,18 @@ def nf_aggregate_bucket(g, worker_stride, W, n, off, length, elig, T, state, mod
         _ptr(summary), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt),
         _ptr(inf_cnt), _ptr(out), _ptr(scale_out), _ptr(plan), plan.numel() * plan.element_size(),
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def nf_aggregate_bucket_noalloc(g, worker_stride, W, n, off, length, elig, T, state, mode, tau, margin, alpha,
+                                route, woff, summary, P, N, plane_stride, abs_sum, sumsq, nan_cnt, inf_cnt,
+                                out, scale_out, plan, stream=None):
+    """nf_aggregate_bucket with the direction workspace in the library's static device array (nf.h): no buffer to
+    pass, nothing allocated; buckets beyond NF_NOALLOC_WORKSPACE_BYTES of scratch raise NF_ERR_TOO_LARGE."""
+    _check("nf_aggregate_bucket_noalloc", lib().nf_aggregate_bucket_noalloc(
+        _ptr(g), int(worker_stride), int(W), int(n), _ptr(off), _ptr(length), _ptr(elig), int(T),
+        _state(state), int(mode), _ptr(tau), int(margin), float(alpha), _ptr(route), _ptr(woff),
+        _ptr(summary), _ptr(P), _ptr(N), int(plane_stride), _ptr(abs_sum), _ptr(sumsq), _ptr(nan_cnt),
+        _ptr(inf_cnt), _ptr(out), _ptr(scale_out), _ptr(plan), plan.numel() * plan.element_size(), _stream(stream)))
 
 
 def nf_aggregate_bucket_host(g_host, g_dev, worker_stride, W, n, off, length, elig, T, state, mode, tau,

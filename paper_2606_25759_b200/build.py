@@ -14,7 +14,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libnf.so")
-SOURCES = ["nf_route.cu", "nf_stream.cu", "nf_fused.cu", "nf_reduce.cu", "nf_api.cu", "nf_supervisor.cu", "nf_guard.cu"]
+SOURCES = ["nf_route.cu", "nf_stream.cu", "nf_fused.cu", "nf_reduce.cu", "nf_api.cu", "nf_supervisor.cu", "nf_guard.cu",
+           "nf_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 # no --use_fast_math; the FP32 route uses explicit __fadd_rn/__fmul_rn so contraction cannot touch it
 EXTRA = os.environ.get("NF_EXTRA_NVCC", "").split()   # tuning aid, e.g. NF_EXTRA_NVCC="-DNF_KDW=3"
@@ -39,7 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         subprocess.check_call([NVCC, *NVCC_FLAGS, *EXTRA, *extra, "-c", os.path.join(CSRC, src), "-o", obj])
         return obj
 
-    with ThreadPoolExecutor(max_workers=7) as ex:
+    with ThreadPoolExecutor(max_workers=8) as ex:
         objs = list(ex.map(cc, SOURCES))
     tmp = LIB + ".tmp.%d" % os.getpid()
     subprocess.check_call([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs])

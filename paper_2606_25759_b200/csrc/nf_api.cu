@@ -29,6 +29,7 @@ const char *nf_status_string(int status) {
         case NF_ERR_ALIGN: return "NF_ERR_ALIGN: base pointer not 16-byte aligned";
         case NF_ERR_RANGE: return "NF_ERR_RANGE: W, margin, T or n out of range";
         case NF_ERR_CUDA: return "NF_ERR_CUDA: CUDA runtime / launch failure";
+        case NF_ERR_TOO_LARGE: return "NF_ERR_TOO_LARGE: bucket needs more scratch than the static NF_NOALLOC_WORKSPACE_BYTES array holds";
         default: return "unknown nf_status";
     }
 }
