@@ -493,6 +493,7 @@ struct DecodeCur {
     int64_t off_t, len_t, woff_t;
     bool dec;
     float S_t;
+    bool handed_on;              // the tensor was not final when this CTA had to leave: its units go to the next kernel
 };
 // where the units of a bucket come from: this kernel's own bucket (metadata in shared memory when T <= kMetaCap)
 // or the previous bucket of the step (everything from global memory)
@@ -506,6 +507,7 @@ struct DecodeSrc {
     const uint8_t *dirs;
     float *out;
     PlanHeader *hdr;
+    int32_t *orph;
 };
 // A span = kDU consecutive units, by one warp, in two phases so that a warp can have the loads of its next span in
 // flight while it stores the current one: decode_load (tensor lookup, wait for the tensor's scale, direction words)
@@ -515,15 +517,19 @@ struct DecodeSpan {
     int64_t obase[kDU], rem[kDU];
     float S[kDU];
 };
+// `stop` (shared memory, or NULL): set when this CTA leaves the rest of the bucket's pass B to the next kernel of the
+// step. A unit in hand whose tensor is not final by then is not waited for (the CTA would hold its SM for nothing
+// until the tensor's last arriver, somewhere else, is through): it is listed in the plan (orph[]) and the next
+// kernel's decode warps take it first.
 __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
-                                            int u0, int u_lim, int lane, DecodeSpan &sp) {
+                                            int u0, int u_lim, int lane, DecodeSpan &sp, const volatile int *stop = nullptr) {
 #pragma unroll
     for (int k = 0; k < kDU; ++k) {
         const int u = u0 + k;
         sp.rem[k] = 0; sp.obase[k] = 0; sp.S[k] = 0.f; sp.dv[k][0] = 0u; sp.dv[k][1] = 0u;
         if (u >= u_lim) continue;
         const int tile = u >> 1;
-        if (tile >= dc.tile_e) {
+        if (tile >= dc.tile_e || tile < dc.tile_b) {             // (handed-on units do not come in tile order)
             if (src.smem_meta) {
                 int lo = 0, hi = src.T;                  // invariant: m_tile[lo] <= tile < m_tile[hi]
                 while (hi - lo > 1) {
@@ -541,6 +547,7 @@ __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeS
                 dc.dec = __ldcg(src.route + t) == NF_ROUTE_L;
                 dc.woff_t = dc.dec ? __ldcg(src.woff + t) : 0;
             }
+            dc.handed_on = false;
             if (dc.dec) {
                 // wait for the tensor's last arriver (it runs in a resident CTA, and so does every CTA that still
                 // holds tiles of the tensor: nobody waits for a CTA that has not started)
@@ -549,6 +556,7 @@ __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeS
                 for (unsigned spins = 0;; ++spins) {
                     seen = ld_acquire_u64(fp);
                     if (seen) break;
+                    if (stop && *stop) { dc.handed_on = true; break; }
                     __nanosleep(100);
                     if (spins > (1u << 25)) { report_timeout(p); dc.dec = false; break; }   // > 4 s: give up loudly
                 }
@@ -556,6 +564,27 @@ __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeS
             }
         }
         if (!dc.dec) continue;
+        if (dc.handed_on) {
+            int slot = 0;
+            if (lane == 0) slot = atomicAdd(&src.hdr->n_orph, 1);
+            slot = __shfl_sync(0xffffffffu, slot, 0);
+            if (slot < kMaxOrphans) {
+                if (lane == 0) src.orph[slot] = u;
+                continue;
+            }
+            // (the list is sized for every decode warp of a grid of 256 CTAs; beyond that: wait after all)
+            const unsigned long long *fp = src.fin + dc.t_cur;
+            unsigned long long seen;
+            for (unsigned spins = 0;; ++spins) {
+                seen = ld_acquire_u64(fp);
+                if (seen) break;
+                __nanosleep(100);
+                if (spins > (1u << 25)) { report_timeout(p); dc.dec = false; break; }
+            }
+            if (!dc.dec) continue;
+            dc.S_t = __uint_as_float((uint32_t)seen);
+            dc.handed_on = false;
+        }
         const int64_t wbase = (int64_t)(tile - dc.tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -618,7 +647,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
                                                  const volatile int *stop, volatile int *hint, int lane) {
     constexpr int kGU = NF_DSPANS * kDU;                    // units per trip
     const int total_units = src.n_tiles * 2;
-    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
     auto grab = [&]() -> int {
         int ub = total_units;
         if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kGU);
@@ -629,7 +658,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
         const int ub_next = grab();                         // in flight while this trip's spans are processed
         DecodeSpan sp[NF_DSPANS];
 #pragma unroll
-        for (int k = 0; k < NF_DSPANS; ++k) decode_load(p, src, sm, dc, ub + k * kDU, total_units, lane, sp[k]);
+        for (int k = 0; k < NF_DSPANS; ++k) decode_load(p, src, sm, dc, ub + k * kDU, total_units, lane, sp[k], stop);
 #pragma unroll
         for (int k = 0; k < NF_DSPANS; ++k) decode_store(src, sm, lane, sp[k]);
         ub = __shfl_sync(0xffffffffu, ub_next, 0);
@@ -642,7 +671,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
 __device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, int ctid,
                                                 int cursor_hint) {
     const int total_units = src.n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
-    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
     // first chunk: an even share of what was left when this CTA's decode warps last looked (a backlog of many units is
     // then taken in one trip per CTA), at least 8 spans
     int chunk = kDU * min(max((total_units - cursor_hint) / ((int)gridDim.x * kDU), 8), 16 * kCW);
@@ -674,6 +703,34 @@ __device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool 
 }
 
 extern __shared__ __align__(128) unsigned char smem_raw[];
+
+// A chained kernel's accounting for the PREVIOUS bucket of the step, whose decode tail it drains. Called by a whole
+// warp that is through with that bucket: its cursor is exhausted (every unit has a taker) and what the warp took it has
+// written. The parties of a CTA are its decode warps and, only if they registered as helpers before any decode warp
+// was through (sm.flag[5] = helpers << 8 | parties through), its consumers. The CTA's last party counts the CTA in the
+// previous bucket's plan, and the grid's last CTA resets that bucket's self-cleaning state. For the decode warps this
+// happens early in the kernel, on nobody's critical path: a chained kernel ends without a device-wide round trip.
+__device__ __forceinline__ void through_with_prev(const StreamParams &p, PlanHeader *prev_hdr, const PlanView &ppv,
+                                                  const FusedSmem &sm, int lane) {
+    __syncwarp();
+    int last_party = 0;
+    if (lane == 0) {
+        const int old = atomicAdd(sm.flag + 5, 1);
+        last_party = ((old & 0xff) + 1 == kDW + (old >> 8)) ? 1 : 0;
+    }
+    if (!__shfl_sync(0xffffffffu, last_party, 0)) return;
+    int last = 0;
+    if (lane == 0) last = atomicAdd(&prev_hdr->finish_count, 1) == (int)gridDim.x - 1;
+    if (!__shfl_sync(0xffffffffu, last, 0)) return;
+    for (int t = lane; t < p.prev_T; t += 32) { ppv.done[t] = 0; ppv.fin[t] = 0ull; }
+    if (lane == 0) {
+        prev_hdr->unit_cursor = 0;
+        prev_hdr->finish_count = 0;
+        prev_hdr->n_orph = 0;
+        prev_hdr->orph_taken = 0;
+        prev_hdr->sched = (unsigned long long)clean_token(p.prev_T, p.prev_W) << 32;
+    }
+}
 
 
 // ---------------------------------------------------------------------------------------------
@@ -726,30 +783,61 @@ __device__ __noinline__ void finalize_tensor_warp(const StreamParams &p, const P
                 }
                 if (!__any_sync(0xffffffffu, more)) break;
             }
-            double A[8], Q[8];
+            // The 16 roundings (8 workers x {sum |x|, sum x^2}) are done by 16 lanes AT ONCE, lane q = (worker q >> 1,
+            // statistic q & 1): each lane fetches the three leading digits of its own accumulator from the lanes that
+            // hold them and rounds once. (One after the other, by the whole warp, they were a chain of a few thousand
+            // dependent instructions: 25 - 30 us for a warp that competes with 16 busy consumer warps, during which the
+            // tensor's decode could not start.)
+            uint32_t dg[8];
+            unsigned nzb[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const uint32_t digit = (uint32_t)lo[i];
-                const unsigned nz = __ballot_sync(0xffffffffu, digit != 0u);
-                A[i] = 0.0;
-                Q[i] = 0.0;
-                if (read && isL) {
-                    A[i] = warp_acc_round(digit, nz, kAccAbs, kAccAbsWords, kAccAbsBase);
-                    if (cn[i]) A[i] = __longlong_as_double(0x7ff8000000000000ll);      // IEEE: a NaN term makes the sum NaN,
-                    else if (ci[i]) A[i] = __longlong_as_double(0x7ff0000000000000ll); // an Inf term (no NaN) makes it +Inf
-                }
-                if (read && HEALTH) Q[i] = warp_acc_round(digit, nz, kAccSq, kAccSqWords, kAccSqBase);
+                dg[i] = (uint32_t)lo[i];
+                nzb[i] = __ballot_sync(0xffffffffu, dg[i] != 0u);
             }
-            if (lane < 8 && w0 + lane < W) {             // lane i writes worker w0 + i's results
-                double a = 0.0, q = 0.0;
-                unsigned long long n_ = 0ull, i_ = 0ull;
+            const int wi = (lane & 15) >> 1, stat = lane & 1;
+            const int l0 = stat ? kAccSq : kAccAbs, nwords = stat ? kAccSqWords : kAccAbsWords;
+            unsigned my_nz = 0u;
+            unsigned long long my_cn = 0ull, my_ci = 0ull;
 #pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (lane == i) { a = A[i]; q = Q[i]; n_ = cn[i]; i_ = ci[i]; }
-                const size_t o = (size_t)(w0 + lane) * T + t;
-                if (HEALTH) { p.sumsq[o] = q; p.nan_cnt[o] = n_; p.inf_cnt[o] = i_; }
-                p.abs_sum[o] = a;                                  // 0 for tensors that are not low-bit routed
-                sm.sw[w0 + lane] = (float)(a / (double)len_t);
+            for (int i = 0; i < 8; ++i)
+                if (wi == i) { my_nz = nzb[i]; my_cn = cn[i]; my_ci = ci[i]; }
+            const unsigned m = (my_nz >> l0) & ((1u << nwords) - 1u);
+            const int top = m ? 31 - __clz(m) : 0;
+            const int s0 = l0 + top, s1 = l0 + max(top - 1, 0), s2 = l0 + max(top - 2, 0);
+            unsigned long long d0 = 0ull, d1 = 0ull, d2 = 0ull;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const uint32_t a = __shfl_sync(0xffffffffu, dg[i], s0), b = __shfl_sync(0xffffffffu, dg[i], s1),
+                               c = __shfl_sync(0xffffffffu, dg[i], s2);
+                if (wi == i) { d0 = a; d1 = b; d2 = c; }
+            }
+            double val = 0.0;                            // the same arithmetic as warp_acc_round()
+            if (m != 0u) {
+                const unsigned long long hi64 = (d0 << 32) | (top >= 1 ? d1 : 0ull);
+                const unsigned long long lo32 = top >= 2 ? d2 : 0ull;
+                const bool sticky = top >= 3 && (m & ((1u << (top - 2)) - 1u)) != 0u;
+                const int lz = __clzll((long long)hi64);
+                unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
+                if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;
+                val = scalbn(__ull2double_rn(mant), (stat ? kAccSqBase : kAccAbsBase) + 32 * top + 31 - lz - 63);
+            }
+            if (lane < 16 && w0 + wi < W) {
+                const size_t o = (size_t)(w0 + wi) * T + t;
+                if (stat == 0) {
+                    double a = 0.0;                                // 0 for tensors that are not low-bit routed
+                    if (read && isL) {
+                        a = val;
+                        if (my_cn) a = __longlong_as_double(0x7ff8000000000000ll);      // IEEE: a NaN term makes the sum NaN,
+                        else if (my_ci) a = __longlong_as_double(0x7ff0000000000000ll); // an Inf term (no NaN) makes it +Inf
+                    }
+                    p.abs_sum[o] = a;
+                    sm.sw[w0 + wi] = (float)(a / (double)len_t);
+                } else if (HEALTH) {
+                    p.sumsq[o] = read ? val : 0.0;
+                    p.nan_cnt[o] = my_cn;
+                    p.inf_cnt[o] = my_ci;
+                }
             }
         }
     } else {
@@ -865,6 +953,22 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // it go only after its own dependency wait, so that "everything before the step" is complete for the whole chain.
     if (!p.next_chained) pdl_launch_dependents();
     if (tid == 0) trace_stamp(p, 5);
+    // A chained kernel reads its bucket's layout at once: like the gradients, it was complete before the step was
+    // enqueued (nf.h), and the step's first kernel has waited for that. The round trip overlaps the set-up below.
+#ifndef NF_EARLY_META
+#define NF_EARLY_META 1
+#endif
+    const bool early_meta = NF_EARLY_META && p.chained && p.inkernel_route;
+    long long m_o = 0, m_l = 0, m_pe = 0;
+    int m_el = 0;
+    float m_tau = 0.f;
+    if (early_meta && tid < p.T) {
+        m_o = __ldg(p.off + tid);
+        m_l = __ldg(p.len + tid);
+        m_pe = tid == 0 ? 0 : __ldg(p.off + tid - 1) + __ldg(p.len + tid - 1);
+        m_el = __ldg(p.elig + tid);
+        if (p.tau) m_tau = __ldg(p.tau + tid);
+    }
 
     if (tid == 0) {
         for (int s = 0; s < stages; ++s) { mbar_init(sm.full + s, 1); mbar_init(sm.empty + s, kCW); }
@@ -927,13 +1031,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         int r = NF_ROUTE_P;
         int bad = 0;
         if (tid < T) {
-            o = __ldg(p.off + tid);
-            l = __ldg(p.len + tid);
-            const long long prev_end = tid == 0 ? 0 : __ldg(p.off + tid - 1) + __ldg(p.len + tid - 1);
+            if (!early_meta) {
+                m_o = __ldg(p.off + tid);
+                m_l = __ldg(p.len + tid);
+                m_pe = tid == 0 ? 0 : __ldg(p.off + tid - 1) + __ldg(p.len + tid - 1);
+                m_el = __ldg(p.elig + tid);
+                if (p.tau) m_tau = __ldg(p.tau + tid);
+            }
+            o = m_o;
+            l = m_l;
+            const long long prev_end = m_pe;
             if (l < 0 || o < prev_end || o + l > p.n) bad = 1;
             if (l < 0) l = 0;
             if (!p.st.admitted) r = NF_ROUTE_P;
-            else if (__ldg(p.elig + tid) == 0) r = NF_ROUTE_P;
+            else if (m_el == 0) r = NF_ROUTE_P;
             else if (p.st.veto || !p.st.capacity_ok) r = NF_ROUTE_F;
             else r = NF_ROUTE_L;
             v_tiles = (l + kTile - 1) / kTile;
@@ -990,7 +1101,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             sm.m_off[tid] = o;
             sm.m_len[tid] = l;
             sm.m_woff[tid] = r == NF_ROUTE_L ? ex_words : -1;
-            sm.m_tau[tid] = (p.tau && r == NF_ROUTE_L) ? __ldg(p.tau + tid) : 0.f;
+            sm.m_tau[tid] = (p.tau && r == NF_ROUTE_L) ? m_tau : 0.f;
         }
         if (tid == 0) sm.m_tile[T] = (int32_t)t_tiles;
         if (blockIdx.x == 0) {
@@ -1086,7 +1197,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             const size_t na = (size_t)W * p.T * kAccWords;
             for (size_t i = tid; i < na; i += kFThreads) pv.acc[i] = 0ull;
             for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
-            if (tid == 0) { hdr->unit_cursor = 0; hdr->finish_count = 0; }
+            if (tid == 0) { hdr->unit_cursor = 0; hdr->finish_count = 0; hdr->n_orph = 0; hdr->orph_taken = 0; }
             __threadfence();
             __syncthreads();
             if (tid == 0) atomicExch(&hdr->sched, (unsigned long long)want_token << 32);
@@ -1099,10 +1210,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
     if (tid == 0) trace_stamp(p, 7);
 
-    const DecodeSrc own{p.T, n_tiles, p.T <= kMetaCap, pv.tile_prefix, p.off, p.len, p.woff, p.route, pv.fin, p.dirs, p.out, hdr};
+    const DecodeSrc own{p.T, n_tiles, p.T <= kMetaCap, pv.tile_prefix, p.off, p.len, p.woff, p.route, pv.fin, p.dirs, p.out, hdr, pv.orph};
     const PlanView ppv = plan_view(p.prev_plan, p.prev_T);              // (only dereferenced when chained)
     DecodeSrc prev{p.prev_T, 0, false, ppv.tile_prefix, p.prev_off, p.prev_len, p.prev_woff, p.prev_route, ppv.fin, p.prev_dirs,
-                   p.prev_out, (PlanHeader *)p.prev_plan};
+                   p.prev_out, (PlanHeader *)p.prev_plan, ppv.orph};
 
     // scheduling units: a pure function of (n_tiles, grid): 4 consecutive tiles, then 2, then single tiles near
     // the end (guided self-scheduling with fixed boundaries). A *segment* = unit x tensor is what one FP32
@@ -1124,6 +1235,15 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             // how many are taken at once changes nothing in the values.
             int u_next = (int)(uint32_t)sched_old;                 // the unit taken before the routing
             int u_end = u_next + 1;
+            // Deferred tail: this bucket's state stays in use after the kernel, so the clean token must go (a call that
+            // found it would take the state for clean). It may go once no CTA of this grid will look at it again, i.e.
+            // when every CTA has made its first draw: finish_count counts the CTAs that have (this one's draw has
+            // returned: its token was checked above); the last one to start takes the token away when it leaves.
+            int started = -1;
+#ifndef NF_STARTED
+#define NF_STARTED 1
+#endif
+            if (NF_STARTED && p.defer_tail) started = atomicAdd(&hdr->finish_count, 1);
             const int n_units = nA + nB + (n_tiles - sB);
             int pr_st = 0, pr_next = 0, pr_end = 0;
             uint32_t pr_ph = 0;
@@ -1146,6 +1266,10 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     mbar_wait(sm.empty + pr_st, pr_ph ^ 1u);
                     sm.tile_of[pr_st] = -1;                            // sentinel: the consumers stop
                     mbar_arrive(sm.full + pr_st);
+                    if (started == (int)gridDim.x - 1) {
+                        hdr->finish_count = 0;
+                        atomicAnd(&hdr->sched, 0xffffffffull);         // not clean until the next kernel has drained the tail
+                    }
                     break;
                 }
                 if (pr_tile >= pc.tile_e) tensor_lookup(p, pv, sm, pr_tile, pc);
@@ -1329,7 +1453,21 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (p.chained) {
             pdl_wait();
             prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+            {
+                // first the units the previous kernel's decode warps had taken and handed on (all final by now)
+                const int n_orph = min(__ldcg(&prev.hdr->n_orph), kMaxOrphans);
+                DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
+                while (n_orph > 0) {
+                    int i = 0;
+                    if (lane == 0) i = atomicAdd(&prev.hdr->orph_taken, 1);
+                    i = __shfl_sync(0xffffffffu, i, 0);
+                    if (i >= n_orph) break;
+                    const int u = __ldcg(prev.orph + i);
+                    decode_span(p, prev, sm, dc, u, u + 1, lane);
+                }
+            }
             decode_warp_loop(p, prev, sm, nullptr, nullptr, lane);
+            through_with_prev(p, prev.hdr, ppv, sm, lane);
         }
         decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, sm.flag + 7, lane);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
@@ -1543,47 +1681,44 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
-            // whatever is left of the previous bucket (normally nothing: its tail was drained long ago)
-            pdl_wait();
-            prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
-            decode_cta_loop(p, prev, sm, ctid, 0);
+            // The previous bucket's tail: normally drained long ago by the decode warps. If none of them has seen its
+            // cursor exhausted yet there is a backlog (the decode warps alone do not keep up with two large tensors per
+            // bucket): the consumers register as helpers and take a share with all 16 warps.
+            if (ctid == 0) sm.flag[2] = (atomicCAS(sm.flag + 5, 0, 0x100) == 0) ? 1 : 0;
+            consumer_sync();
+            if (sm.flag[2]) {
+                pdl_wait();
+                prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+                decode_cta_loop(p, prev, sm, ctid, 0);
+                if (warp == 0) through_with_prev(p, prev.hdr, ppv, sm, lane);
+            }
         }
         if (!p.defer_tail) decode_cta_loop(p, own, sm, ctid, *(volatile int *)(sm.flag + 7));      // help finish pass B
         if (ctid == 0) trace_stamp(p, 3);
     }
 
-    // ---- the grid's last CTA resets the self-cleaning state: of this bucket unless its tail is deferred (then the
-    // next kernel of the step does it when it is through with it), and of the previous bucket of the step ----
-    __syncthreads();
-    if (tid == 0) {
-        // (own state is reset below only when the tail is not deferred: then this CTA's stores to it, the fin words
-        // of the tensors it finalised, must come first. A deferred bucket's state is reset by the next kernel, after
-        // its dependency wait; what this kernel did to the previous bucket's state are atomics that have returned.)
-        if (!p.defer_tail) __threadfence();
-        const int old = atomicAdd(&hdr->finish_count, 1);
-        const int last = (old == (int)gridDim.x - 1) ? 1 : 0;
-        if (last) __threadfence();
-        sm.flag[2] = last;
-    }
-    __syncthreads();
-    if (sm.flag[2]) {
-        if (!p.defer_tail)
-            for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
+    // ---- the self-cleaning state at the end of the kernel. Tail not deferred (a stand-alone call, the last bucket of a
+    // step): the grid's last CTA resets this bucket's state. Tail deferred: nothing to do here (the next kernel of the
+    // step resets it when it is through with the tail; the last CTA to START took the clean token away, see the
+    // producer), so such a CTA leaves without a device-wide round trip. The previous bucket's state was reset by the
+    // decode warps. ----
+    if (!p.defer_tail) {
+        __syncthreads();
         if (tid == 0) {
-            hdr->finish_count = 0;
-            if (!p.defer_tail) {
+            // (this CTA's stores to the state, the fin words of the tensors it finalised, must come first)
+            __threadfence();
+            const int old = atomicAdd(&hdr->finish_count, 1);
+            const int last = (old == (int)gridDim.x - 1) ? 1 : 0;
+            if (last) __threadfence();
+            sm.flag[2] = last;
+        }
+        __syncthreads();
+        if (sm.flag[2]) {
+            for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
+            if (tid == 0) {
+                hdr->finish_count = 0;
                 hdr->unit_cursor = 0;
                 hdr->sched = (unsigned long long)want_token << 32;
-            } else {
-                hdr->sched = 0ull;                             // not clean until the next kernel has drained the tail
-            }
-        }
-        if (p.chained) {
-            pdl_wait();
-            for (int t = tid; t < p.prev_T; t += kFThreads) { ppv.done[t] = 0; ppv.fin[t] = 0ull; }
-            if (tid == 0) {
-                prev.hdr->unit_cursor = 0;
-                prev.hdr->sched = (unsigned long long)clean_token(p.prev_T, p.prev_W) << 32;
             }
         }
     }

@@ -22,7 +22,9 @@ constexpr int kGroup = 8;                  // workers per register group (8 x 4-
 constexpr uint32_t kPlanMagic = 0x4e46504cu;  // "NFPL"
 constexpr int kMetaCap = 256;              // fused kernel: tensors whose metadata lives in shared memory
 
-struct PlanHeader {                        // 64 bytes, at plan + 0
+constexpr int kMaxOrphans = 2048;          // fused path, chained kernels: pass-B units handed on to the next kernel (see orph)
+
+struct PlanHeader {                        // 80 bytes, at plan + 0
     uint32_t magic;
     int32_t status;                        // NF_OK or NF_ERR_ARG (bad layout): later kernels no-op
     int32_t T;
@@ -38,8 +40,14 @@ struct PlanHeader {                        // 64 bytes, at plan + 0
     // CTAs). One atomicAdd both takes a unit and proves the state clean.
     unsigned long long sched;
     int64_t acc_slots;                     // capacity of the acc region in (replica, tensor) slots
+    // fused path, a bucket whose decode tail is left to the next kernel of the step: pass-B units a decode warp had
+    // taken but could not finish before its CTA left (their tensor was not final yet) are listed in orph[] for the
+    // next kernel, which takes them one by one (orph_taken). Both zero in the clean state.
+    int32_t n_orph;
+    int32_t orph_taken;
+    int64_t pad1;
 };
-static_assert(sizeof(PlanHeader) == 64, "plan header layout");
+static_assert(sizeof(PlanHeader) == 80, "plan header layout");
 
 // ---------------------------------------------------------------------------------------------
 // Deterministic per-(worker, tensor) totals. abs_sum / sumsq are sums over millions of elements gathered by
@@ -78,6 +86,7 @@ struct PlanLayout {
     size_t scale;                          // float [T]     per-tensor scale scratch
     size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
     size_t fin;                            // uint64 [T]    fused path: {1, FP32 bits of S_t} once tensor t is finalised, else 0
+    size_t orph;                           // int32 [kMaxOrphans]  fused path: handed-on pass-B units (header: n_orph)
     size_t acc;                            // uint64 [R*T][kAccWords]  exact accumulators (R = workers / replicas)
     size_t total;                          // without the acc region
 };
@@ -94,6 +103,7 @@ __host__ __device__ inline PlanLayout plan_layout(int T) {
     L.scale = o;       o = align_up(o + sizeof(float) * (size_t)(T > 0 ? T : 1), 16);
     L.done = o;        o = align_up(o + sizeof(int32_t) * (size_t)(T > 0 ? T : 1), 16);
     L.fin = o;         o = align_up(o + sizeof(unsigned long long) * (size_t)(T > 0 ? T : 1), 16);
+    L.orph = o;        o = align_up(o + sizeof(int32_t) * (size_t)kMaxOrphans, 16);
     L.acc = align_up(o, 256);
     L.total = L.acc;
     return L;
@@ -117,6 +127,7 @@ struct PlanView {
     float *scale;
     int32_t *done;
     unsigned long long *fin;
+    int32_t *orph;
     unsigned long long *acc;
 };
 
@@ -132,6 +143,7 @@ __host__ __device__ inline PlanView plan_view(void *plan, int T) {
     v.scale = (float *)(p + L.scale);
     v.done = (int32_t *)(p + L.done);
     v.fin = (unsigned long long *)(p + L.fin);
+    v.orph = (int32_t *)(p + L.orph);
     v.acc = (unsigned long long *)(p + L.acc);
     return v;
 }
