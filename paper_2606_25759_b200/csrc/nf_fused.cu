@@ -138,8 +138,8 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [4096, 8192)    decode table: byte of 4 (+,-) flag pairs -> float4 of directions in {-1, 0, +1}
 //   [8192, 17408)   per-tensor metadata of the first kMetaCap tensors (tile prefix, off, len, woff, tau)
 //   [17408, ...)    ring [stages][8][kPitch] floats
-//   after the ring  per-warp FP64 totals {abs, sq} per worker of one segment, [nbuf][kCW][2*W] doubles
-//                   (double-buffered by segment parity when W <= 32: one CTA barrier per segment instead of two)
+//   after the ring  per-warp FP64 totals {abs, sq} per worker of one record, [2][kCW][2*min(W, kRecW)] doubles: a
+//                   segment is handed to the reducer warp in records of at most kRecW workers, double-buffered
 // ---------------------------------------------------------------------------------------------
 constexpr int kSmemMeta = 8192;
 constexpr int kSmemHdr = kSmemMeta + 9216;       // 4*(cap+1) + 3*8*cap + 4*cap = 8196 bytes, padded
@@ -158,11 +158,12 @@ struct FusedSmem {
     int32_t *m_tile;             // [kMetaCap + 1] exclusive tile prefix
     int64_t *m_off, *m_len, *m_woff;   // [kMetaCap]; woff = -1 when the tensor is not low-bit routed
     float *m_tau;                // [kMetaCap]
-    double *wacc;                // [kCW][2*W]
+    double *wacc;                // [2][kCW][2*min(W, kRecW)]
 };
-__host__ __device__ inline int fused_nbuf(int W) { return W <= 32 ? 2 : 1; }
+constexpr int kRecW = 32;                        // workers per record handed to the reducer warp
+__host__ __device__ inline int fused_recw(int W) { return W < kRecW ? W : kRecW; }
 __host__ __device__ inline size_t fused_smem_bytes(int stages, int W) {
-    return (size_t)kSmemHdr + (size_t)stages * kStageBytes + sizeof(double) * kCW * 2 * (size_t)W * fused_nbuf(W);
+    return (size_t)kSmemHdr + (size_t)stages * kStageBytes + sizeof(double) * kCW * 2 * (size_t)fused_recw(W) * 2;
 }
 __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     FusedSmem s;
@@ -409,7 +410,8 @@ template <bool HEALTH>
 __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSmem &sm, double *wbuf, int tally0, float (&af)[8],
                                            float (&qf)[8], int64_t off_t, int64_t len_t, int tile_b, int w0, int nw,
                                            int cnt, int4 recent, int ctid, bool aligned) {
-    const int lane = ctid & 31, warp = ctid >> 5, W = p.W;
+    // (wbuf, tally0: the record buffer and its NaN / Inf tallies, both indexed by worker - first worker of the record)
+    const int lane = ctid & 31, warp = ctid >> 5, W = p.W, wr0 = w0 % kRecW;
     float v16[16];
 #pragma unroll
     for (int i = 0; i < 8; ++i) { v16[i] = af[i]; v16[i + 8] = qf[i]; }
@@ -420,7 +422,7 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
     const bool ok = HEALTH ? ((A <= FLT_MAX) && (((Q >= 1e-30f) && (Q <= FLT_MAX)) || A == 0.f))
                            : (A <= FLT_MAX);
     const unsigned bad = __ballot_sync(0xffffffffu, !ok && wl < nw);
-    double *slot = wbuf + (size_t)warp * 2 * W + (size_t)w0 * 2;
+    double *slot = wbuf + (size_t)warp * 2 * fused_recw(W) + (size_t)wr0 * 2;
     if (bad == 0u) {
         if ((lane & 1) == 0 && wl < nw) slot[wl * 2 + stat] = (double)r;
     } else {
@@ -437,7 +439,7 @@ __device__ __forceinline__ void stat_flush(const StreamParams &p, const FusedSme
                 double2 e = make_double2((double)a_t, (double)q_t);
                 if (!ok_t)
                     e = exact_redo<HEALTH>(p.g, p.worker_stride, w0 + w, off_t, len_t, tile_b, recent, cnt, ctid, sm.nan,
-                                           sm.inf, tally0 + w0 + w, aligned);
+                                           sm.inf, tally0 + wr0 + w, aligned);
                 const double ea = warp_sum(e.x), eq = warp_sum(e.y);
                 if (lane == 0) { slot[w * 2] = ea; slot[w * 2 + 1] = eq; }
             } else if ((lane & 1) == 0 && wl == w) {
@@ -743,103 +745,111 @@ __device__ __forceinline__ void through_with_prev(const StreamParams &p, PlanHea
 //    workers in flight together), carries and rounding by shuffles;
 //  * wider fan-in: lane = worker, 32 workers per pass, each lane walking its own slot (acc_round).
 // ---------------------------------------------------------------------------------------------
+// Eight workers' accumulators of tensor t, [w0, w0 + 8), rounded and written by ONE warp: lane k holds word k of each
+// worker's slot (eight coalesced 256-byte loads in flight together), carries by shuffles, the 16 roundings by 16 lanes
+// at once. Leaves sm.sw[w] = (float)(A_w / len_t) for the scale.
+template <bool HEALTH>
+__device__ __forceinline__ void finalize8(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t, int64_t len_t,
+                                          bool isL, bool read, int w0, int lane) {
+    const int W = p.W, T = p.T;
+    unsigned long long v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        v[i] = 0ull;
+        if (read && w0 + i < W) v[i] = __ldcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane);
+    }
+    // (the clearing stores come after ALL the loads have been issued: a store behind a load of the same word
+    // would serialise the eight round trips)
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        if (read && w0 + i < W) __stcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane, 0ull);
+    // the eight workers' carry chains and roundings are walked together (independent shuffle chains overlap)
+    unsigned long long cn[8], ci[8], lo[8], hi[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        cn[i] = __shfl_sync(0xffffffffu, v[i], kAccNan);
+        ci[i] = __shfl_sync(0xffffffffu, v[i], kAccInf);
+        lo[i] = lane >= kAccNan ? 0ull : (v[i] & 0xffffffffull);
+        hi[i] = lane >= kAccNan ? 0ull : (v[i] >> 32);
+    }
+    for (;;) {                                   // deferred carries ripple up (no carry into lanes 0 / kAccSq)
+        bool more = false;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            unsigned long long c = __shfl_up_sync(0xffffffffu, hi[i], 1);
+            if (lane == kAccAbs || lane == kAccSq) c = 0ull;
+            const unsigned long long x = lo[i] + c;
+            lo[i] = x & 0xffffffffull;
+            hi[i] = x >> 32;
+            more |= hi[i] != 0ull;
+        }
+        if (!__any_sync(0xffffffffu, more)) break;
+    }
+    // The 16 roundings (8 workers x {sum |x|, sum x^2}) are done by 16 lanes AT ONCE, lane q = (worker q >> 1,
+    // statistic q & 1): each lane fetches the three leading digits of its own accumulator from the lanes that
+    // hold them and rounds once. (One after the other, by the whole warp, they were a chain of a few thousand
+    // dependent instructions: 25 - 30 us for a warp that competes with 16 busy consumer warps, during which the
+    // tensor's decode could not start.)
+    uint32_t dg[8];
+    unsigned nzb[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        dg[i] = (uint32_t)lo[i];
+        nzb[i] = __ballot_sync(0xffffffffu, dg[i] != 0u);
+    }
+    const int wi = (lane & 15) >> 1, stat = lane & 1;
+    const int l0 = stat ? kAccSq : kAccAbs, nwords = stat ? kAccSqWords : kAccAbsWords;
+    unsigned my_nz = 0u;
+    unsigned long long my_cn = 0ull, my_ci = 0ull;
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        if (wi == i) { my_nz = nzb[i]; my_cn = cn[i]; my_ci = ci[i]; }
+    const unsigned m = (my_nz >> l0) & ((1u << nwords) - 1u);
+    const int top = m ? 31 - __clz(m) : 0;
+    const int s0 = l0 + top, s1 = l0 + max(top - 1, 0), s2 = l0 + max(top - 2, 0);
+    unsigned long long d0 = 0ull, d1 = 0ull, d2 = 0ull;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const uint32_t a = __shfl_sync(0xffffffffu, dg[i], s0), b = __shfl_sync(0xffffffffu, dg[i], s1),
+                       c = __shfl_sync(0xffffffffu, dg[i], s2);
+        if (wi == i) { d0 = a; d1 = b; d2 = c; }
+    }
+    double val = 0.0;                            // the same arithmetic as warp_acc_round()
+    if (m != 0u) {
+        const unsigned long long hi64 = (d0 << 32) | (top >= 1 ? d1 : 0ull);
+        const unsigned long long lo32 = top >= 2 ? d2 : 0ull;
+        const bool sticky = top >= 3 && (m & ((1u << (top - 2)) - 1u)) != 0u;
+        const int lz = __clzll((long long)hi64);
+        unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
+        if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;
+        val = scalbn(__ull2double_rn(mant), (stat ? kAccSqBase : kAccAbsBase) + 32 * top + 31 - lz - 63);
+    }
+    if (lane < 16 && w0 + wi < W) {
+        const size_t o = (size_t)(w0 + wi) * T + t;
+        if (stat == 0) {
+            double a = 0.0;                                // 0 for tensors that are not low-bit routed
+            if (read && isL) {
+                a = val;
+                if (my_cn) a = __longlong_as_double(0x7ff8000000000000ll);      // IEEE: a NaN term makes the sum NaN,
+                else if (my_ci) a = __longlong_as_double(0x7ff0000000000000ll); // an Inf term (no NaN) makes it +Inf
+            }
+            p.abs_sum[o] = a;
+            sm.sw[w0 + wi] = (float)(a / (double)len_t);
+        } else if (HEALTH) {
+            p.sumsq[o] = read ? val : 0.0;
+            p.nan_cnt[o] = my_cn;
+            p.inf_cnt[o] = my_ci;
+        }
+    }
+}
+
 template <bool HEALTH>
 __device__ __noinline__ void finalize_tensor_warp(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
                                                   int64_t len_t, bool isL, int lane) {
     const int W = p.W, T = p.T;
     const bool read = isL || HEALTH;
     if (W <= 32) {
-        for (int w0 = 0; w0 < W; w0 += 8) {
-            unsigned long long v[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                v[i] = 0ull;
-                if (read && w0 + i < W) v[i] = __ldcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane);
-            }
-            // (the clearing stores come after ALL the loads have been issued: a store behind a load of the same word
-            // would serialise the eight round trips)
-#pragma unroll
-            for (int i = 0; i < 8; ++i)
-                if (read && w0 + i < W) __stcg(pv.acc + ((size_t)(w0 + i) * T + t) * kAccWords + lane, 0ull);
-            // the eight workers' carry chains and roundings are walked together (independent shuffle chains overlap)
-            unsigned long long cn[8], ci[8], lo[8], hi[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                cn[i] = __shfl_sync(0xffffffffu, v[i], kAccNan);
-                ci[i] = __shfl_sync(0xffffffffu, v[i], kAccInf);
-                lo[i] = lane >= kAccNan ? 0ull : (v[i] & 0xffffffffull);
-                hi[i] = lane >= kAccNan ? 0ull : (v[i] >> 32);
-            }
-            for (;;) {                                   // deferred carries ripple up (no carry into lanes 0 / kAccSq)
-                bool more = false;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    unsigned long long c = __shfl_up_sync(0xffffffffu, hi[i], 1);
-                    if (lane == kAccAbs || lane == kAccSq) c = 0ull;
-                    const unsigned long long x = lo[i] + c;
-                    lo[i] = x & 0xffffffffull;
-                    hi[i] = x >> 32;
-                    more |= hi[i] != 0ull;
-                }
-                if (!__any_sync(0xffffffffu, more)) break;
-            }
-            // The 16 roundings (8 workers x {sum |x|, sum x^2}) are done by 16 lanes AT ONCE, lane q = (worker q >> 1,
-            // statistic q & 1): each lane fetches the three leading digits of its own accumulator from the lanes that
-            // hold them and rounds once. (One after the other, by the whole warp, they were a chain of a few thousand
-            // dependent instructions: 25 - 30 us for a warp that competes with 16 busy consumer warps, during which the
-            // tensor's decode could not start.)
-            uint32_t dg[8];
-            unsigned nzb[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                dg[i] = (uint32_t)lo[i];
-                nzb[i] = __ballot_sync(0xffffffffu, dg[i] != 0u);
-            }
-            const int wi = (lane & 15) >> 1, stat = lane & 1;
-            const int l0 = stat ? kAccSq : kAccAbs, nwords = stat ? kAccSqWords : kAccAbsWords;
-            unsigned my_nz = 0u;
-            unsigned long long my_cn = 0ull, my_ci = 0ull;
-#pragma unroll
-            for (int i = 0; i < 8; ++i)
-                if (wi == i) { my_nz = nzb[i]; my_cn = cn[i]; my_ci = ci[i]; }
-            const unsigned m = (my_nz >> l0) & ((1u << nwords) - 1u);
-            const int top = m ? 31 - __clz(m) : 0;
-            const int s0 = l0 + top, s1 = l0 + max(top - 1, 0), s2 = l0 + max(top - 2, 0);
-            unsigned long long d0 = 0ull, d1 = 0ull, d2 = 0ull;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const uint32_t a = __shfl_sync(0xffffffffu, dg[i], s0), b = __shfl_sync(0xffffffffu, dg[i], s1),
-                               c = __shfl_sync(0xffffffffu, dg[i], s2);
-                if (wi == i) { d0 = a; d1 = b; d2 = c; }
-            }
-            double val = 0.0;                            // the same arithmetic as warp_acc_round()
-            if (m != 0u) {
-                const unsigned long long hi64 = (d0 << 32) | (top >= 1 ? d1 : 0ull);
-                const unsigned long long lo32 = top >= 2 ? d2 : 0ull;
-                const bool sticky = top >= 3 && (m & ((1u << (top - 2)) - 1u)) != 0u;
-                const int lz = __clzll((long long)hi64);
-                unsigned long long mant = lz ? ((hi64 << lz) | (lo32 >> (32 - lz))) : hi64;
-                if (sticky || ((lo32 << lz) & 0xffffffffull)) mant |= 1ull;
-                val = scalbn(__ull2double_rn(mant), (stat ? kAccSqBase : kAccAbsBase) + 32 * top + 31 - lz - 63);
-            }
-            if (lane < 16 && w0 + wi < W) {
-                const size_t o = (size_t)(w0 + wi) * T + t;
-                if (stat == 0) {
-                    double a = 0.0;                                // 0 for tensors that are not low-bit routed
-                    if (read && isL) {
-                        a = val;
-                        if (my_cn) a = __longlong_as_double(0x7ff8000000000000ll);      // IEEE: a NaN term makes the sum NaN,
-                        else if (my_ci) a = __longlong_as_double(0x7ff0000000000000ll); // an Inf term (no NaN) makes it +Inf
-                    }
-                    p.abs_sum[o] = a;
-                    sm.sw[w0 + wi] = (float)(a / (double)len_t);
-                } else if (HEALTH) {
-                    p.sumsq[o] = read ? val : 0.0;
-                    p.nan_cnt[o] = my_cn;
-                    p.inf_cnt[o] = my_ci;
-                }
-            }
-        }
+        for (int w0 = 0; w0 < W; w0 += 8) finalize8<HEALTH>(p, pv, sm, t, len_t, isL, read, w0, lane);
     } else {
         for (int w = lane; w < W; w += 32) {
             const size_t o = (size_t)w * T + t;
@@ -890,7 +900,11 @@ template <bool HEALTH>
 __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanView &pv, const FusedSmem &sm, int t,
                                              int64_t len_t, bool isL, int ctid) {
     const int W = p.W, T = p.T, warp = ctid >> 5, lane = ctid & 31;
-    for (int w = warp; w < W; w += kCW) {                      // a warp per worker: lane k holds word k of the slot
+    // wide fan-in: a warp per 8 workers, their loads in flight together (a warp per worker walks W / 16 slots one after
+    // the other: 16 us at W = 64 between the last tile and the tensor's decode)
+    if (W > kCW)
+        for (int w0 = warp * 8; w0 < W; w0 += kCW * 8) finalize8<HEALTH>(p, pv, sm, t, len_t, isL, isL || HEALTH, w0, lane);
+    for (int w = warp; w < W && W <= kCW; w += kCW) {          // a warp per worker: lane k holds word k of the slot
         const size_t o = (size_t)w * T + t;
         double A = 0.0;
         if (isL || HEALTH) {
@@ -924,8 +938,7 @@ __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanVi
         const float S = (float)(s / (double)W);
         pv.scale[t] = S;
         if (p.scale_out) p.scale_out[t] = S;
-        __threadfence();
-        st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));
+        st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));    // (release: a fence of its own)
     }
 }
 
@@ -1357,7 +1370,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         //    count (release: every consumer warp arrived after its last store of the tensor; this warp's fence is
         //    cumulative) and, if that completed the tensor, finalise it (finalize_tensor_warp).
         {
-            const int nbuf = fused_nbuf(W), T = p.T;
+            const int T = p.T, Wc = fused_recw(W);
             int b = 0;
             for (;;) {
                 seg_bar_sync(b);
@@ -1365,21 +1378,22 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 const int t = rec[0];
                 if (t < 0) break;
                 const bool isL = rec[2] != 0;
+                const int wbase = rec[5], wc = min(Wc, W - wbase);     // data records: the workers the record covers
                 if (rec[1] == 2) {
                     // the segment is the whole tensor: its sums ARE the totals (exactly what rounding the accumulator
                     // of a single addend gives)
                     const int64_t len_t = *reinterpret_cast<const int64_t *>(rec + 6);
-                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
-                    for (int j0 = 0; j0 < 2 * W; j0 += 32) {
-                        const int j = j0 + lane, w = j >> 1;
+                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * Wc;
+                    for (int j0 = 0; j0 < 2 * wc; j0 += 32) {
+                        const int j = j0 + lane, wr = j >> 1, w = wbase + wr;
                         double tot = 0.0;
-                        if (j < 2 * W) {
+                        if (j < 2 * wc) {
 #pragma unroll
-                            for (int k = 0; k < kCW; ++k) tot += src0[(size_t)k * 2 * W + j];
+                            for (int k = 0; k < kCW; ++k) tot += src0[(size_t)k * 2 * Wc + j];
                         }
                         const double other = __shfl_xor_sync(0xffffffffu, tot, 1);      // even lane: sum |x|, odd lane: sum x^2
-                        if (j < 2 * W && (j & 1) == 0) {
-                            const unsigned cn_ = atomicExch(&sm.nan[b * 32 + w], 0u), ci_ = atomicExch(&sm.inf[b * 32 + w], 0u);
+                        if (j < 2 * wc && (j & 1) == 0) {
+                            const unsigned cn_ = atomicExch(&sm.nan[b * 32 + wr], 0u), ci_ = atomicExch(&sm.inf[b * 32 + wr], 0u);
                             const size_t o = (size_t)w * T + t;
                             double A = 0.0;
                             if (isL) {
@@ -1393,7 +1407,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                         }
                     }
                     __syncwarp();
-                    if (isL && lane == 0) {
+                    if (isL && lane == 0 && wbase + wc == W) {             // the tensor's last record: all W scales are in
                         double sacc = 0.0;
                         for (int w = 0; w < W; ++w) sacc += (double)sm.sw[w];
                         const float S = (float)(sacc / (double)W);
@@ -1402,19 +1416,19 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                         st_release_u64(pv.fin + t, (1ull << 32) | (unsigned long long)__float_as_uint(S));
                     }
                 } else if (rec[1] == 0) {
-                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * W;
-                    for (int j = lane; j < 2 * W; j += 32) {
+                    const double *src0 = sm.wacc + (size_t)b * kCW * 2 * Wc;
+                    for (int j = lane; j < 2 * wc; j += 32) {
                         const double *src = src0 + j;
                         double tot = 0.0;
 #pragma unroll
-                        for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * W];
-                        unsigned long long *slot = pv.acc + ((size_t)(j >> 1) * T + t) * kAccWords;
+                        for (int k = 0; k < kCW; ++k) tot += src[(size_t)k * 2 * Wc];
+                        unsigned long long *slot = pv.acc + ((size_t)(wbase + (j >> 1)) * T + t) * kAccWords;
                         if ((j & 1) == 0) { if (isL) acc_add(slot + kAccAbs, kAccAbsWords, kAccAbsBase, tot); }
                         else if (HEALTH) acc_add(slot + kAccSq, kAccSqWords, kAccSqBase, tot);
                     }
-                    for (int w = lane; w < W; w += 32) {
+                    for (int w = lane; w < wc; w += 32) {
                         const unsigned cn_ = atomicExch(&sm.nan[b * 32 + w], 0u), ci_ = atomicExch(&sm.inf[b * 32 + w], 0u);
-                        unsigned long long *slot = pv.acc + ((size_t)w * T + t) * kAccWords;
+                        unsigned long long *slot = pv.acc + ((size_t)(wbase + w) * T + t) * kAccWords;
                         if (cn_) atomicAdd(slot + kAccNan, (unsigned long long)cn_);
                         if (ci_) atomicAdd(slot + kAccInf, (unsigned long long)ci_);
                     }
@@ -1436,7 +1450,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(sm.seg_free + b);   // (release: what was done is ordered before whoever waits)
-                if (nbuf == 2) b ^= 1;
+                b ^= 1;
             }
         }
     } else if (warp >= kCW + 2) {
@@ -1494,8 +1508,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         uint32_t *pP = nullptr, *pN = nullptr;      // this thread's plane-word / direction / output slots
         uint8_t *pD = nullptr;                      //   of tile 0 of the current tensor
         float *pO = nullptr;
-        const int nbuf = fused_nbuf(W);
-        int segpar = 0;                             // buffer of the current segment's per-warp FP64 values
+        int segpar = 0;                             // buffer of the current record's per-warp FP64 values
         double *wbuf = sm.wacc;
 
         uint32_t seguse0 = 0u, seguse1 = 0u;        // uses of each segment buffer so far
@@ -1505,15 +1518,16 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             mbar_wait_backoff(sm.seg_free + segpar, (u & 1u) ^ 1u);    // first use: passes at once
         };
         // after the last stat_flush of a segment: hand the buffer to the reducer warp (see there) and go on
-        auto seg_publish = [&](int t, int kind, bool isL, int n, int total, int64_t len_t) __attribute__((always_inline)) {
+        auto seg_publish = [&](int t, int kind, bool isL, int n, int total, int64_t len_t, int wbase) __attribute__((always_inline)) {
             if (ctid == 0) {
                 int *rec = sm.seg_rec + 8 * segpar;
-                rec[0] = t; rec[1] = kind; rec[2] = isL ? 1 : 0; rec[3] = n; rec[4] = total;
+                rec[0] = t; rec[1] = kind; rec[2] = isL ? 1 : 0; rec[3] = n; rec[4] = total; rec[5] = wbase;
                 *reinterpret_cast<int64_t *>(rec + 6) = len_t;
             }
             seg_bar_arrive(segpar);
             if (segpar) ++seguse1; else ++seguse0;
-            if (nbuf == 2) { segpar ^= 1; wbuf = sm.wacc + (size_t)segpar * kCW * 2 * W; }
+            segpar ^= 1;
+            wbuf = sm.wacc + (size_t)segpar * kCW * 2 * fused_recw(W);
         };
         // All tiles this CTA took of tensor c.t so far are done: tell the reducer warp (a flush record: it publishes the
         // tile count and finalises the tensor if that completed it). No barrier, no round trip on the consumers' path:
@@ -1521,7 +1535,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         auto flush_tensor = [&]() __attribute__((always_inline)) {
             if (c.isL || HEALTH) {
                 seg_acquire();
-                seg_publish(c.t, 1, c.isL, ntile_acc, c.tile_e - c.tile_b, c.len);
+                seg_publish(c.t, 1, c.isL, ntile_acc, c.tile_e - c.tile_b, c.len, 0);
             }
             ntile_acc = 0;
         };
@@ -1609,8 +1623,12 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     }
                 }
                 if (MULTI && stats) {
-                    if (w0 == 0) seg_acquire();
+                    // a segment goes to the reducer warp in records of at most kRecW workers (the last one after the
+                    // votes below)
+                    if (w0 % kRecW == 0) seg_acquire();
                     stat_flush<HEALTH>(p, sm, wbuf, segpar * 32, af, qf, c.off, c.len, c.tile_b, w0, nw, R, recent, ctid, c.aligned);
+                    if ((w0 + kGroup) % kRecW == 0 && w0 + kGroup < W)
+                        seg_publish(c.t, R == c.tile_e - c.tile_b ? 2 : 0, c.isL, 0, 0, c.len, w0 + kGroup - kRecW);
                 }
             }
             if (c.isL) {
@@ -1655,7 +1673,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     stat_flush<HEALTH>(p, sm, wbuf, segpar * 32, af, qf, c.off, c.len, c.tile_b, 0, W, kcnt, recent, ctid, c.aligned);
                     kcnt = 0;
                 }
-                seg_publish(c.t, whole ? 2 : 0, c.isL, 0, 0, c.len);
+                seg_publish(c.t, whole ? 2 : 0, c.isL, 0, 0, c.len, MULTI ? (W - 1) / kRecW * kRecW : 0);
                 if (whole) { touched = false; ntile_acc = 0; }
             } else if (!MULTI && seg_end) {
                 kcnt = 0;
@@ -1677,7 +1695,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             if (sm.flag[1]) finalize_tensor<HEALTH>(p, pv, sm, c.t, c.len, c.isL, ctid);
         }
         seg_acquire();
-        seg_publish(-1, 0, false, 0, 0, 0);         // no more records: the reducer warp leaves
+        seg_publish(-1, 0, false, 0, 0, 0, 0);      // no more records: the reducer warp leaves
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
@@ -1730,16 +1748,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
 // ---------------------------------------------------------------------------------------------
 template <bool HEALTH, bool MULTI>
 static cudaError_t launch_fused_t(const StreamParams &p, int64_t n, cudaStream_t s) {
-    // ring depth: 3 stages unless the per-warp FP64 slots of a very wide fan-in need the room
-    const int stages = (MULTI && p.W > 64) ? 2 : kStages;
+    const int stages = kStages;                              // (the record buffers are at most 16 KB at any fan-in)
     const size_t smem = fused_smem_bytes(stages, p.W);
     static bool configured = false;
     if (!configured) {
-        size_t mx = 0;
-        for (int w = 1; w <= 255; ++w) {
-            const size_t b = fused_smem_bytes(w > 64 ? 2 : kStages, w);
-            mx = b > mx ? b : mx;
-        }
+        const size_t mx = fused_smem_bytes(kStages, kRecW);
         cudaError_t e = cudaFuncSetAttribute(fused_passA_kernel<HEALTH, MULTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)mx);
         if (e != cudaSuccess) return e;
