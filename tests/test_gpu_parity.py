@@ -35,7 +35,7 @@ def test_handworked_bucket_on_gpu():
         assert np.array_equal(ref.out[:8], np.array([S * int(x) for x in d[dkey]], np.float32))
 
 
-@pytest.mark.parametrize("W", [1, 2, 3, 4, 8, 9, 17, 255])
+@pytest.mark.parametrize("W", [1, 2, 3, 4, 8, 9, 17, 32, 33, 64, 100, 255])     # (records of 32 workers: whole, one over, ragged)
 @pytest.mark.parametrize("mode", [O.MODE_GBINARY, O.MODE_GTERNARY])
 def test_adversarial_lengths_and_offsets(W, mode):
     """Lengths 1, 31, 32, 33, 4099, a multi-tile tensor, offsets that are not multiples of 4,
