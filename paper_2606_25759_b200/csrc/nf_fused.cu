@@ -495,7 +495,16 @@ struct DecodeCur {
     int64_t off_t, len_t, woff_t;
     bool dec;
     float S_t;
-    bool handed_on;              // the tensor was not final when this CTA had to leave: its units go to the next kernel
+};
+// Units a decode warp hands on to the next kernel of the step when its CTA leaves (`stop`): every decode warp of the
+// grid owns kHandOn entries of the plan's orph[] (unit + 1, 0 = empty; entries of CTA c, decode warp d at
+// (c * kDW + d) * kHandOn), written with plain stores and read, then cleared, by the same warp of the next kernel:
+// no atomics, no round trip before the CTA can go.
+constexpr int kHandOn = 4;                       // <= 2 spans of kDU units in hand (the current one, the prefetched one)
+struct HandOn {
+    const volatile int *stop;                    // shared memory: this CTA takes no more units (NULL: never)
+    int32_t *slots;                              // this warp's entries (NULL: hand nothing on, wait instead)
+    int n;                                       // entries used so far
 };
 // where the units of a bucket come from: this kernel's own bucket (metadata in shared memory when T <= kMetaCap)
 // or the previous bucket of the step (everything from global memory)
@@ -519,17 +528,21 @@ struct DecodeSpan {
     int64_t obase[kDU], rem[kDU];
     float S[kDU];
 };
-// `stop` (shared memory, or NULL): set when this CTA leaves the rest of the bucket's pass B to the next kernel of the
-// step. A unit in hand whose tensor is not final by then is not waited for (the CTA would hold its SM for nothing
-// until the tensor's last arriver, somewhere else, is through): it is listed in the plan (orph[]) and the next
-// kernel's decode warps take it first.
+// `ho` (or NULL): once its stop flag is set (this CTA leaves the rest of the bucket's pass B to the next kernel of the
+// step), units in hand that have not been started are not decoded any more, let alone waited for (the CTA would hold
+// its SM for nothing until a tensor's last arriver, somewhere else, is through): they are handed on.
 __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, DecodeCur &dc,
-                                            int u0, int u_lim, int lane, DecodeSpan &sp, const volatile int *stop = nullptr) {
+                                            int u0, int u_lim, int lane, DecodeSpan &sp, HandOn *ho = nullptr) {
 #pragma unroll
     for (int k = 0; k < kDU; ++k) {
         const int u = u0 + k;
         sp.rem[k] = 0; sp.obase[k] = 0; sp.S[k] = 0.f; sp.dv[k][0] = 0u; sp.dv[k][1] = 0u;
         if (u >= u_lim) continue;
+        if (ho && ho->slots && ho->n < kHandOn && *ho->stop) {
+            if (lane == 0) ho->slots[ho->n] = u + 1;
+            ++ho->n;
+            continue;
+        }
         const int tile = u >> 1;
         if (tile >= dc.tile_e || tile < dc.tile_b) {             // (handed-on units do not come in tile order)
             if (src.smem_meta) {
@@ -549,44 +562,30 @@ __device__ __forceinline__ void decode_load(const StreamParams &p, const DecodeS
                 dc.dec = __ldcg(src.route + t) == NF_ROUTE_L;
                 dc.woff_t = dc.dec ? __ldcg(src.woff + t) : 0;
             }
-            dc.handed_on = false;
             if (dc.dec) {
                 // wait for the tensor's last arriver (it runs in a resident CTA, and so does every CTA that still
                 // holds tiles of the tensor: nobody waits for a CTA that has not started)
                 const unsigned long long *fp = src.fin + dc.t_cur;
                 unsigned long long seen;
+                bool handed = false;
                 for (unsigned spins = 0;; ++spins) {
                     seen = ld_acquire_u64(fp);
                     if (seen) break;
-                    if (stop && *stop) { dc.handed_on = true; break; }
+                    if (ho && ho->slots && ho->n < kHandOn && *ho->stop) { handed = true; break; }
                     __nanosleep(100);
                     if (spins > (1u << 25)) { report_timeout(p); dc.dec = false; break; }   // > 4 s: give up loudly
+                }
+                if (handed) {
+                    if (lane == 0) ho->slots[ho->n] = u + 1;
+                    ++ho->n;
+                    dc.tile_e = 0;                           // (nothing is known of this tensor: look again next time)
+                    dc.tile_b = 0;
+                    continue;
                 }
                 dc.S_t = __uint_as_float((uint32_t)seen);
             }
         }
         if (!dc.dec) continue;
-        if (dc.handed_on) {
-            int slot = 0;
-            if (lane == 0) slot = atomicAdd(&src.hdr->n_orph, 1);
-            slot = __shfl_sync(0xffffffffu, slot, 0);
-            if (slot < kMaxOrphans) {
-                if (lane == 0) src.orph[slot] = u;
-                continue;
-            }
-            // (the list is sized for every decode warp of a grid of 256 CTAs; beyond that: wait after all)
-            const unsigned long long *fp = src.fin + dc.t_cur;
-            unsigned long long seen;
-            for (unsigned spins = 0;; ++spins) {
-                seen = ld_acquire_u64(fp);
-                if (seen) break;
-                __nanosleep(100);
-                if (spins > (1u << 25)) { report_timeout(p); dc.dec = false; break; }
-            }
-            if (!dc.dec) continue;
-            dc.S_t = __uint_as_float((uint32_t)seen);
-            dc.handed_on = false;
-        }
         const int64_t wbase = (int64_t)(tile - dc.tile_b) * kTile + (u & 1) * 1024;     // tensor-relative
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -646,10 +645,13 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
 #define NF_DSPANS 1
 #endif
 __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
-                                                 const volatile int *stop, volatile int *hint, int lane) {
+                                                 const volatile int *stop, volatile int *hint, int lane, int dwarp) {
     constexpr int kGU = NF_DSPANS * kDU;                    // units per trip
     const int total_units = src.n_tiles * 2;
-    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
+    // (a grid beyond the list's capacity: the warps of the CTAs past it wait for their tensors instead)
+    const int my_slot = ((int)blockIdx.x * kDW + dwarp) * kHandOn;
+    HandOn ho{stop, (stop && my_slot + kHandOn <= kMaxOrphans) ? src.orph + my_slot : nullptr, 0};
     auto grab = [&]() -> int {
         int ub = total_units;
         if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kGU);
@@ -660,7 +662,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
         const int ub_next = grab();                         // in flight while this trip's spans are processed
         DecodeSpan sp[NF_DSPANS];
 #pragma unroll
-        for (int k = 0; k < NF_DSPANS; ++k) decode_load(p, src, sm, dc, ub + k * kDU, total_units, lane, sp[k], stop);
+        for (int k = 0; k < NF_DSPANS; ++k) decode_load(p, src, sm, dc, ub + k * kDU, total_units, lane, sp[k], &ho);
 #pragma unroll
         for (int k = 0; k < NF_DSPANS; ++k) decode_store(src, sm, lane, sp[k]);
         ub = __shfl_sync(0xffffffffu, ub_next, 0);
@@ -673,7 +675,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
 __device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm, int ctid,
                                                 int cursor_hint) {
     const int total_units = src.n_tiles * 2, lane = ctid & 31, warp = ctid >> 5;
-    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
+    DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
     // first chunk: an even share of what was left when this CTA's decode warps last looked (a backlog of many units is
     // then taken in one trip per CTA), at least 8 spans
     int chunk = kDU * min(max((total_units - cursor_hint) / ((int)gridDim.x * kDU), 8), 16 * kCW);
@@ -728,8 +730,6 @@ __device__ __forceinline__ void through_with_prev(const StreamParams &p, PlanHea
     if (lane == 0) {
         prev_hdr->unit_cursor = 0;
         prev_hdr->finish_count = 0;
-        prev_hdr->n_orph = 0;
-        prev_hdr->orph_taken = 0;
         prev_hdr->sched = (unsigned long long)clean_token(p.prev_T, p.prev_W) << 32;
     }
 }
@@ -1210,7 +1210,8 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             const size_t na = (size_t)W * p.T * kAccWords;
             for (size_t i = tid; i < na; i += kFThreads) pv.acc[i] = 0ull;
             for (int t = tid; t < p.T; t += kFThreads) { pv.done[t] = 0; pv.fin[t] = 0ull; }
-            if (tid == 0) { hdr->unit_cursor = 0; hdr->finish_count = 0; hdr->n_orph = 0; hdr->orph_taken = 0; }
+            for (int i = tid; i < kMaxOrphans; i += kFThreads) pv.orph[i] = 0;
+            if (tid == 0) { hdr->unit_cursor = 0; hdr->finish_count = 0; }
             __threadfence();
             __syncthreads();
             if (tid == 0) atomicExch(&hdr->sched, (unsigned long long)want_token << 32);
@@ -1279,6 +1280,9 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     mbar_wait(sm.empty + pr_st, pr_ph ^ 1u);
                     sm.tile_of[pr_st] = -1;                            // sentinel: the consumers stop
                     mbar_arrive(sm.full + pr_st);
+                    // deferred tail: the CTA's decode warps wind down now (they need a few us to finish the span they
+                    // are storing and to hand on what else they hold), while the consumers work off the ring
+                    if (p.defer_tail) *(volatile int *)(sm.flag + 4) = 1;
                     if (started == (int)gridDim.x - 1) {
                         hdr->finish_count = 0;
                         atomicAnd(&hdr->sched, 0xffffffffull);         // not clean until the next kernel has drained the tail
@@ -1464,26 +1468,29 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         // leave at once (defer_tail) and the kernel of bucket k+1, which needs nothing of bucket k for its own
         // pass A and therefore never waited for it, drains bucket k's remaining units here, beside its own reads.
         // The only thread-level dependency waits of a chained kernel are the ones in front of bucket k's data.
+        const int dwarp = warp - (kCW + 2);
         if (p.chained) {
             pdl_wait();
             prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
             {
-                // first the units the previous kernel's decode warps had taken and handed on (all final by now)
-                const int n_orph = min(__ldcg(&prev.hdr->n_orph), kMaxOrphans);
-                DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f, false};
-                while (n_orph > 0) {
-                    int i = 0;
-                    if (lane == 0) i = atomicAdd(&prev.hdr->orph_taken, 1);
-                    i = __shfl_sync(0xffffffffu, i, 0);
-                    if (i >= n_orph) break;
-                    const int u = __ldcg(prev.orph + i);
-                    decode_span(p, prev, sm, dc, u, u + 1, lane);
+                // first the units the previous kernel's decode warps had in hand when their CTAs left (all final by
+                // now): this warp takes, and clears, the entries of the same warp of CTAs c, c + grid, ...
+                DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
+                for (int c = (int)blockIdx.x; (c * kDW + dwarp + 1) * kHandOn <= kMaxOrphans; c += (int)gridDim.x) {
+                    int4 *e = reinterpret_cast<int4 *>(prev.orph + (c * kDW + dwarp) * kHandOn);
+                    const int4 v = __ldcg(e);
+                    if ((v.x | v.y | v.z | v.w) == 0) continue;
+                    if (lane == 0) __stcg(e, make_int4(0, 0, 0, 0));
+                    if (v.x) decode_span(p, prev, sm, dc, v.x - 1, v.x, lane);
+                    if (v.y) decode_span(p, prev, sm, dc, v.y - 1, v.y, lane);
+                    if (v.z) decode_span(p, prev, sm, dc, v.z - 1, v.z, lane);
+                    if (v.w) decode_span(p, prev, sm, dc, v.w - 1, v.w, lane);
                 }
             }
-            decode_warp_loop(p, prev, sm, nullptr, nullptr, lane);
+            decode_warp_loop(p, prev, sm, nullptr, nullptr, lane, dwarp);
             through_with_prev(p, prev.hdr, ppv, sm, lane);
         }
-        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, sm.flag + 7, lane);
+        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, sm.flag + 7, lane, dwarp);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
     } else {
         // =====================================================================================

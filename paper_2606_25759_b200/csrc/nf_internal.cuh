@@ -40,12 +40,7 @@ struct PlanHeader {                        // 80 bytes, at plan + 0
     // CTAs). One atomicAdd both takes a unit and proves the state clean.
     unsigned long long sched;
     int64_t acc_slots;                     // capacity of the acc region in (replica, tensor) slots
-    // fused path, a bucket whose decode tail is left to the next kernel of the step: pass-B units a decode warp had
-    // taken but could not finish before its CTA left (their tensor was not final yet) are listed in orph[] for the
-    // next kernel, which takes them one by one (orph_taken). Both zero in the clean state.
-    int32_t n_orph;
-    int32_t orph_taken;
-    int64_t pad1;
+    int64_t pad1[2];
 };
 static_assert(sizeof(PlanHeader) == 80, "plan header layout");
 
@@ -86,7 +81,9 @@ struct PlanLayout {
     size_t scale;                          // float [T]     per-tensor scale scratch
     size_t done;                           // int32 [T]     tiles of the tensor whose pass-A results are published
     size_t fin;                            // uint64 [T]    fused path: {1, FP32 bits of S_t} once tensor t is finalised, else 0
-    size_t orph;                           // int32 [kMaxOrphans]  fused path: handed-on pass-B units (header: n_orph)
+    size_t orph;                           // int32 [kMaxOrphans]  fused path: pass-B units (+ 1, 0 = none) the decode warps of a
+                                           // kernel whose tail is deferred had in hand when their CTAs left: 4 entries per
+                                           // (CTA, decode warp), taken and cleared by the next kernel of the step
     size_t acc;                            // uint64 [R*T][kAccWords]  exact accumulators (R = workers / replicas)
     size_t total;                          // without the acc region
 };
