@@ -225,6 +225,7 @@ namespace {
 
 struct Chain {                 // how a bucket's kernel is linked to its neighbours inside nf_aggregate_step
     const nf_bucket *prev = nullptr;
+    const nf_bucket *pp = nullptr;   // the bucket before prev, when prev's kernel was chained to it
     const void *prev_dirs = nullptr;
     int prev_W = 0;
     bool chained = false, next_chained = false;
@@ -280,6 +281,7 @@ int launch_bucket(const nf_bucket &b, int W, nf_state state, int mode, int margi
     p.defer_tail = ch.next_chained ? 1 : 0;
     if (ch.chained) {
         p.prev_plan = ch.prev->plan; p.prev_T = ch.prev->T; p.prev_W = ch.prev_W;
+        if (ch.pp) { p.pp_plan = ch.pp->plan; p.pp_T = ch.pp->T; p.pp_W = ch.prev_W; }
         p.prev_off = ch.prev->off; p.prev_len = ch.prev->len; p.prev_woff = ch.prev->woff;
         p.prev_route = ch.prev->route; p.prev_dirs = (const uint8_t *)ch.prev_dirs; p.prev_out = ch.prev->out;
     }
@@ -339,6 +341,7 @@ int nf_aggregate_step(const nf_bucket *buckets, int nb, int W, nf_state state, i
         ch.next_chained = i + 1 < nb && chainable(i) && chainable(i + 1);
         if (ch.chained) {
             ch.prev = &buckets[i - 1];
+            if (i >= 2 && chainable(i - 2)) ch.pp = &buckets[i - 2];      // (kernel i-1 was chained to i-2)
             ch.prev_dirs = (const char *)workspace + prev_off;
             ch.prev_W = W;
         }

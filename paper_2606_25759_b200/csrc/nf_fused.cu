@@ -150,6 +150,7 @@ struct FusedSmem {
     int *run_of;                 // [kMaxStages] MULTI: length R of the run of tiles the stage belongs to
     int *seg_of;                 // [kMaxStages] 1: the tile ends a segment (last tile of its scheduling unit or tensor)
     int *flag;                   // [8] CTA-wide flags
+    int *aux;                    // [4] [0]: tiles of the previous bucket + 1 (0: not read yet)
     float *sw;                   // [256] per-worker scales of the tensor being finalised
     uint64_t *seg_free;          // [2] mbarriers: the reducer warp is through with a segment buffer
     int *seg_rec;                // [2][8] record handed over with a buffer: tensor (-1: no more), kind, route, tiles, ...
@@ -173,6 +174,7 @@ __device__ __forceinline__ FusedSmem carve(unsigned char *base, int stages) {
     s.run_of = (int *)(base + 80);
     s.seg_of = (int *)(base + 96);
     s.flag = (int *)(base + 384);
+    s.aux = (int *)(base + 432);
     s.sw = (float *)(base + 3072);
     s.seg_free = (uint64_t *)(base + 416);
     s.seg_rec = (int *)(base + 448);
@@ -644,16 +646,18 @@ __device__ __forceinline__ void decode_span(const StreamParams &p, const DecodeS
 #ifndef NF_DSPANS
 #define NF_DSPANS 1
 #endif
-__device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
-                                                 const volatile int *stop, volatile int *hint, int lane, int dwarp) {
+// Returns whether the warp saw the cursor exhausted (false: it left because of `stop`).
+__device__ __forceinline__ bool decode_warp_loop(const StreamParams &p, const DecodeSrc &src, const FusedSmem &sm,
+                                                 const volatile int *stop, bool hand_on, volatile int *hint, int lane, int dwarp) {
     constexpr int kGU = NF_DSPANS * kDU;                    // units per trip
     const int total_units = src.n_tiles * 2;
     DecodeCur dc{-1, 0, 0, 0, 0, 0, false, 0.f};
     // (a grid beyond the list's capacity: the warps of the CTAs past it wait for their tensors instead)
     const int my_slot = ((int)blockIdx.x * kDW + dwarp) * kHandOn;
-    HandOn ho{stop, (stop && my_slot + kHandOn <= kMaxOrphans) ? src.orph + my_slot : nullptr, 0};
+    HandOn ho{stop, (stop && hand_on && my_slot + kHandOn <= kMaxOrphans) ? src.orph + my_slot : nullptr, 0};
+    constexpr int kStopped = 0x7fffffff;
     auto grab = [&]() -> int {
-        int ub = total_units;
+        int ub = kStopped;
         if (!(stop && *stop) && lane == 0) ub = atomicAdd(&src.hdr->unit_cursor, kGU);
         return ub;                                          // (lane 0's value is the one that counts)
     };
@@ -668,6 +672,7 @@ __device__ __forceinline__ void decode_warp_loop(const StreamParams &p, const De
         ub = __shfl_sync(0xffffffffu, ub_next, 0);
         if (lane == 0 && hint) *hint = ub;                  // (where the cursor stands: the consumers size their first chunk by it)
     }
+    return ub != kStopped;
 }
 // The consumers once their tiles are exhausted: ONE trip to the cursor per CTA and chunk (a few thousand warps
 // arriving together on one address serialise: 15 us for the last warp served), chunk sizes guided by what is
@@ -708,7 +713,22 @@ __device__ __forceinline__ uint32_t vote4_packed(uint32_t cp, uint32_t cn, bool 
 
 extern __shared__ __align__(128) unsigned char smem_raw[];
 
-// A chained kernel's accounting for the PREVIOUS bucket of the step, whose decode tail it drains. Called by a whole
+// The self-cleaning state of a bucket whose decode tail was drained by a later kernel, back to "clean" (by one warp,
+// once nothing uses the state any more). The hand-on entries were cleared by whoever took them.
+__device__ __forceinline__ void reset_bucket_state(void *plan, int T, int W, int lane) {
+    const PlanView v = plan_view(plan, T);
+    PlanHeader *h = (PlanHeader *)plan;
+    for (int t = lane; t < T; t += 32) { v.done[t] = 0; v.fin[t] = 0ull; }
+    if (lane == 0) {
+        h->unit_cursor = 0;
+        h->finish_count = 0;
+        h->sched = (unsigned long long)clean_token(T, W) << 32;
+    }
+}
+
+// A chained kernel's accounting for the PREVIOUS bucket of the step, whose decode tail it drains. Only the LAST kernel of
+// a chain needs it: in the middle of a chain the state of bucket k-1 is reset by kernel k+1 (whose dependency wait on
+// kernel k, which waited on kernel k-1, proves that nothing uses it any more), without any counting. Called by a whole
 // warp that is through with that bucket: its cursor is exhausted (every unit has a taker) and what the warp took it has
 // written. The parties of a CTA are its decode warps and, only if they registered as helpers before any decode warp
 // was through (sm.flag[5] = helpers << 8 | parties through), its consumers. The CTA's last party counts the CTA in the
@@ -726,12 +746,7 @@ __device__ __forceinline__ void through_with_prev(const StreamParams &p, PlanHea
     int last = 0;
     if (lane == 0) last = atomicAdd(&prev_hdr->finish_count, 1) == (int)gridDim.x - 1;
     if (!__shfl_sync(0xffffffffu, last, 0)) return;
-    for (int t = lane; t < p.prev_T; t += 32) { ppv.done[t] = 0; ppv.fin[t] = 0ull; }
-    if (lane == 0) {
-        prev_hdr->unit_cursor = 0;
-        prev_hdr->finish_count = 0;
-        prev_hdr->sched = (unsigned long long)clean_token(p.prev_T, p.prev_W) << 32;
-    }
+    reset_bucket_state(p.prev_plan, p.prev_T, p.prev_W, lane);
 }
 
 
@@ -990,6 +1005,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     }
     for (int i = tid; i < 256; i += kFThreads) { sm.nan[i] = 0u; sm.inf[i] = 0u; }
     if (tid < 8) sm.flag[tid] = 0;
+    if (tid < 4) sm.aux[tid] = 0;
     for (int i = tid; i < 256; i += kFThreads)
         sm.dtab[i] = make_float4((float)((i & 1) - ((i >> 4) & 1)), (float)(((i >> 1) & 1) - ((i >> 5) & 1)),
                                  (float)(((i >> 2) & 1) - ((i >> 6) & 1)), (float)(((i >> 3) & 1) - ((i >> 7) & 1)));
@@ -1472,6 +1488,9 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (p.chained) {
             pdl_wait();
             prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+            if (lane == 0) sm.aux[0] = prev.n_tiles + 1;
+            // the bucket before the previous one: kernel k-1 is complete, and it had waited for kernel k-2
+            if (p.pp_plan && blockIdx.x == 0 && dwarp == 0) reset_bucket_state(p.pp_plan, p.pp_T, p.pp_W, lane);
             {
                 // first the units the previous kernel's decode warps had in hand when their CTAs left (all final by
                 // now): this warp takes, and clears, the entries of the same warp of CTAs c, c + grid, ...
@@ -1487,10 +1506,17 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
                     if (v.w) decode_span(p, prev, sm, dc, v.w - 1, v.w, lane);
                 }
             }
-            decode_warp_loop(p, prev, sm, nullptr, nullptr, lane, dwarp);
-            through_with_prev(p, prev.hdr, ppv, sm, lane);
+            if (p.next_chained) {
+                // middle of a chain: the warp leaves the previous bucket when this CTA's pass A is about to end (what
+                // is left then, the consumers take, see there); flag[5] = some decode warp saw the cursor exhausted
+                const bool exhausted = decode_warp_loop(p, prev, sm, sm.flag + 4, false, nullptr, lane, dwarp);
+                if (exhausted && lane == 0) *(volatile int *)(sm.flag + 5) = 1;
+            } else {
+                decode_warp_loop(p, prev, sm, nullptr, false, nullptr, lane, dwarp);
+                through_with_prev(p, prev.hdr, ppv, sm, lane);
+            }
         }
-        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, sm.flag + 7, lane, dwarp);
+        decode_warp_loop(p, own, sm, p.defer_tail ? sm.flag + 4 : nullptr, true, sm.flag + 7, lane, dwarp);
         if (warp == kCW + 2 && lane == 0) trace_stamp(p, 4);
     } else {
         // =====================================================================================
@@ -1706,16 +1732,20 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
         if (ctid == 0) trace_stamp(p, 2);
         if (p.defer_tail && ctid == 0) *(volatile int *)(sm.flag + 4) = 1;   // this CTA's decode warps take no more units
         if (p.chained) {
-            // The previous bucket's tail: normally drained long ago by the decode warps. If none of them has seen its
-            // cursor exhausted yet there is a backlog (the decode warps alone do not keep up with two large tensors per
-            // bucket): the consumers register as helpers and take a share with all 16 warps.
-            if (ctid == 0) sm.flag[2] = (atomicCAS(sm.flag + 5, 0, 0x100) == 0) ? 1 : 0;
+            // The previous bucket's tail. If no decode warp of this CTA has seen its cursor exhausted there is a backlog
+            // (the decode warps alone do not keep up with a bucket's worth of decoding per kernel): the consumers take
+            // a share with all 16 warps. In the middle of a chain nothing is counted (see through_with_prev); the last
+            // kernel of a chain counts its CTAs: there the consumers register as a third party before they help.
+            if (ctid == 0)
+                sm.flag[2] = p.next_chained ? (*(volatile int *)(sm.flag + 5) == 0 ? 1 : 0)
+                                            : ((atomicCAS(sm.flag + 5, 0, 0x100) == 0) ? 1 : 0);
             consumer_sync();
             if (sm.flag[2]) {
                 pdl_wait();
-                prev.n_tiles = __ldcg(&prev.hdr->n_tiles);
+                const int seen = *(volatile int *)sm.aux;           // (read by the decode warps long ago)
+                prev.n_tiles = seen ? seen - 1 : __ldcg(&prev.hdr->n_tiles);
                 decode_cta_loop(p, prev, sm, ctid, 0);
-                if (warp == 0) through_with_prev(p, prev.hdr, ppv, sm, lane);
+                if (!p.next_chained && warp == 0) through_with_prev(p, prev.hdr, ppv, sm, lane);
             }
         }
         if (!p.defer_tail) decode_cta_loop(p, own, sm, ctid, *(volatile int *)(sm.flag + 7));      // help finish pass B

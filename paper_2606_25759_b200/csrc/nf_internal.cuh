@@ -188,6 +188,8 @@ struct StreamParams {
     int defer_tail;            // 1: the next kernel of the step decodes what cannot be decoded before pass A ends
     void *prev_plan;           // previous bucket of the step (its remaining decode units are drained here)
     int prev_T, prev_W;
+    void *pp_plan;             // the bucket before that, when it was chained too (else NULL): this kernel resets its
+    int pp_T, pp_W;            //   self-cleaning state (everything that used it is complete once kernel i-1 is)
     const int64_t *prev_off, *prev_len, *prev_woff;
     const uint8_t *prev_route;
     const uint8_t *prev_dirs;
