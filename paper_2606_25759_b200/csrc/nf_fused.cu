@@ -961,7 +961,13 @@ __device__ __noinline__ void finalize_tensor(const StreamParams &p, const PlanVi
 // the kernel
 // ---------------------------------------------------------------------------------------------
 #ifndef NF_TAIL4
-#define NF_TAIL4 4                        // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
+#define NF_TAIL4 2                        // the last NF_TAIL4 x grid tiles are not handed out 4 at a time
+#endif
+#ifndef NF_TAIL4_M
+#define NF_TAIL4_M 6                      // the same for W > 8, where a tile is W / 8 ring stages: no single-tile units
+#endif
+#ifndef NF_TAIL2_M
+#define NF_TAIL2_M 0
 #endif
 #ifndef NF_GRAB
 #define NF_GRAB 1                         // most scheduling units a producer takes per trip to the cursor
@@ -1248,8 +1254,8 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     // scheduling units: a pure function of (n_tiles, grid): 4 consecutive tiles, then 2, then single tiles near
     // the end (guided self-scheduling with fixed boundaries). A *segment* = unit x tensor is what one FP32
     // partial spans, so the value of every partial depends on the data only, not on which CTA took the unit.
-    const int sA = max(0, n_tiles - NF_TAIL4 * (int)gridDim.x) & ~3, nA = sA >> 2;
-    const int sB = sA + (max(0, n_tiles - NF_TAIL2 * (int)gridDim.x - sA) & ~1), nB = (sB - sA) >> 1;
+    const int sA = max(0, n_tiles - (MULTI ? NF_TAIL4_M : NF_TAIL4) * (int)gridDim.x) & ~3, nA = sA >> 2;
+    const int sB = sA + (max(0, n_tiles - (MULTI ? NF_TAIL2_M : NF_TAIL2) * (int)gridDim.x - sA) & ~1), nB = (sB - sA) >> 1;
 
     if (warp == kCW) {
         // =====================================================================================
