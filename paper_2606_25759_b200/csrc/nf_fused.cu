@@ -670,7 +670,7 @@ __device__ __forceinline__ bool decode_warp_loop(const StreamParams &p, const De
 #pragma unroll
         for (int k = 0; k < NF_DSPANS; ++k) decode_store(src, sm, lane, sp[k]);
         ub = __shfl_sync(0xffffffffu, ub_next, 0);
-        if (lane == 0 && hint) *hint = ub;                  // (where the cursor stands: the consumers size their first chunk by it)
+        if (lane == 0 && hint && ub != kStopped) *hint = ub;      // (where the cursor stands: the consumers size their first chunk by it)
     }
     return ub != kStopped;
 }
@@ -692,6 +692,7 @@ __device__ __forceinline__ void decode_cta_loop(const StreamParams &p, const Dec
         if (base >= total_units) break;
         const int lim = min(base + chunk, total_units);
         for (int u0 = base + kDU * warp; u0 < lim; u0 += kDU * kCW) decode_span(p, src, sm, dc, u0, lim, lane);
+        if (lim >= total_units) break;                      // this chunk reached the end: no trip to find that out
         const int spans = (total_units - lim) / (2 * (int)gridDim.x * kDU);     // guided: half of an even share
         chunk = kDU * min(max(spans, 4), 16 * kCW);
         consumer_sync();                                    // everybody has read flag[3]
@@ -1719,7 +1720,12 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             }
         }
         if (ctid == 0) trace_stamp(p, 1);
-        if (touched && (c.isL || HEALTH)) {
+        if (touched && (c.isL || HEALTH) && p.next_chained) {
+            // middle of a chain: the last tensor goes to the reducer warp like any other (its fence and its atomic are
+            // two round trips: they overlap what the consumers do next, the previous bucket's backlog; the tensor's
+            // decode is the next kernel's business anyway)
+            flush_tensor();
+        } else if (touched && (c.isL || HEALTH)) {
             // the last tensor this CTA worked on: its decode is now the critical path and the consumers are free, so
             // they publish and finalise it themselves (16 warps) once the reducer warp is through with every record
             if (seguse0 > 0u) mbar_wait_backoff(sm.seg_free + 0, (seguse0 - 1u) & 1u);
