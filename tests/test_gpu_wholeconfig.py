@@ -141,3 +141,61 @@ def test_step_with_a_refused_bucket_in_the_middle():
         assert bool((mb.buckets[1].out == 9.0).all())
         for i in (0, 2):
             compare(mb.buckets[i], refs[i], W, O.MODE_GTERNARY, what=f"bucket {i} beside a refused bucket")
+
+
+@pytest.mark.parametrize("seed,W", [(1, 4), (2, 12), (3, 40), (4, 8)])
+def test_random_step_chains_bitwise_equal_to_single_calls(seed, W):
+    """Random sequences of buckets through nf_aggregate_step: runs of tiny buckets (kernels of a few CTAs that overlap
+    their neighbours, grids of different sizes handing decode units on to each other), large ones, chain breakers
+    (T > 256, empty buckets), all-FP32 and all-low-bit buckets, four steps in a row on the same plans. Every output of
+    every bucket must be bitwise what a stand-alone nf_aggregate_bucket call produces (itself checked against the
+    oracle elsewhere), after the last step and after the first."""
+    from tests.util import layout
+    from paper_2606_25759_b200 import BucketBuffers
+    rng = np.random.default_rng(9000 + seed)
+    specs = []
+    for _ in range(int(rng.integers(9, 14))):
+        kind = rng.integers(0, 6)
+        if kind == 0:
+            T = int(rng.integers(1, 4)); lens = [int(x) for x in rng.integers(1, 300, T)]                 # tiny
+        elif kind == 1:
+            T = int(rng.integers(2, 30)); lens = [int(x) for x in rng.integers(1, 6000, T)]               # small
+        elif kind == 2:
+            T = int(rng.integers(1, 6)); lens = [int(x) for x in rng.integers(2048 * 50, 2048 * 400, T)]   # large
+        elif kind == 3:
+            T = int(rng.integers(257, 300)); lens = [int(x) for x in rng.integers(1, 500, T)]              # breaks the chain
+        elif kind == 4:
+            T = 0; lens = []                                                                                # empty bucket
+        else:
+            T = int(rng.integers(3, 12)); lens = [int(x) for x in rng.integers(1, 2048 * 12, T)]
+        off, ln, n = layout(lens)
+        mode = rng.integers(0, 3)
+        elig = [1] * T if mode == 0 else ([0] * T if mode == 1 else [int(x) for x in rng.integers(0, 2, T)])
+        specs.append((off, ln, elig, n))
+    G = []
+    for off, ln, elig, n in specs:
+        g = (rng.standard_normal((W, max(n, 1))) * 10 ** rng.uniform(-4, 0, (1, max(n, 1)))).astype(np.float32)
+        g[rng.random(g.shape) < 0.03] = 0.0
+        gd = torch.zeros((W, (max(n, 1) + 3) // 4 * 4), dtype=torch.float32, device=DEV)
+        gd[:, :g.shape[1]] = torch.from_numpy(g)
+        G.append(gd)
+    names = ("out", "scale", "abs_sum", "sumsq", "nan_cnt", "inf_cnt", "P", "N", "route", "woff", "summary")
+    ones = []
+    for (off, ln, elig, n), g in zip(specs, G):
+        one = BucketBuffers(off, ln, elig, n, W, DEV, planes=True, health=True)
+        one.out.fill_(-5.0)
+        one.aggregate(g, g.shape[1])
+        ones.append(one)
+    mb = ModelBuffers(specs, W, DEV, planes=True, health=True)
+    for step in range(4):
+        for bb in mb.buckets:
+            bb.out.fill_(-5.0)
+        mb.step(G)
+        if step in (0, 3):
+            torch.cuda.synchronize()
+            for i, (bb, one) in enumerate(zip(mb.buckets, ones)):
+                assert int(bb.summary[nf.SUM_STATUS]) == nf.NF_OK
+                for name in names:
+                    a, b = getattr(bb, name), getattr(one, name)
+                    assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), \
+                        f"seed {seed} step {step} bucket {i} (T = {bb.T}, n = {bb.n}): {name} differs from the stand-alone call"
