@@ -990,10 +990,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
     if (tid == 0) trace_stamp(p, 5);
     // A chained kernel reads its bucket's layout at once: like the gradients, it was complete before the step was
     // enqueued (nf.h), and the step's first kernel has waited for that. The round trip overlaps the set-up below.
-#ifndef NF_EARLY_META
-#define NF_EARLY_META 1
-#endif
-    const bool early_meta = NF_EARLY_META && p.chained && p.inkernel_route;
+    const bool early_meta = p.chained && p.inkernel_route;
     long long m_o = 0, m_l = 0, m_pe = 0;
     int m_el = 0;
     float m_tau = 0.f;
@@ -1277,10 +1274,7 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             // when every CTA has made its first draw: finish_count counts the CTAs that have (this one's draw has
             // returned: its token was checked above); the last one to start takes the token away when it leaves.
             int started = -1;
-#ifndef NF_STARTED
-#define NF_STARTED 1
-#endif
-            if (NF_STARTED && p.defer_tail) started = atomicAdd(&hdr->finish_count, 1);
+            if (p.defer_tail) started = atomicAdd(&hdr->finish_count, 1);
             const int n_units = nA + nB + (n_tiles - sB);
             int pr_st = 0, pr_next = 0, pr_end = 0;
             uint32_t pr_ph = 0;
