@@ -20,7 +20,6 @@
 //  * ragged last tiles and tensors whose rows are not 16-byte aligned go through the same ring;
 //  * each CTA publishes its finished tiles per tensor (release); decode warps, and the consumers once
 //    the tiles are exhausted, acquire the per-tensor counter and expand the 2-bit directions.
-#include <cooperative_groups.h>
 #include <float.h>
 #include <utility>
 #include "nf_internal.cuh"
@@ -131,7 +130,7 @@ __device__ __forceinline__ F reduce_scatter16(F (&v)[16], int lane) {
 //   [0, 64)         mbarriers full[4], empty[4]
 //   [64, 112)       per ring stage: tile index, run length (MULTI), end-of-segment flag
 //   [128, 384)      scratch of the in-kernel routing scan
-//   [416, 512)      segment buffers: mbarriers free[2]; the record handed over with each buffer [2][8]
+//   [416, 512)      segment buffers: mbarriers free[2]; [432, 448) aux words; the record handed over with each buffer [2][8]
 //   [384, 416)      CTA-wide flags (init role, last arriver of a tensor, last CTA of the grid, decode chunk, pass A done)
 //   [1024, 3072)    NaN / Inf tallies, 256 workers each
 //   [3072, 4096)    per-worker scales s_w of the tensor being finalised, 256 floats
@@ -1379,10 +1378,11 @@ __global__ void __maxnreg__(96) fused_passA_kernel(const __grid_constant__ Strea
             pv.scale[t] = S;
             if (p.scale_out) p.scale_out[t] = S;
         }
-        // ---- then the CTA's reducer and publisher. The 16 consumer warps hand it records through two buffers (one
-        // when W > 32): a warp arrives on the buffer's named barrier and goes on (it waits on the buffer's "free"
+        // ---- then the CTA's reducer and publisher. The 16 consumer warps hand it records through two buffers: a warp
+        // arrives on the buffer's named barrier and goes on (it waits on the buffer's "free"
         // mbarrier only when it comes back to the same buffer), so the consumers never wait for each other here.
-        //  * data record = a SEGMENT (the tiles of one scheduling unit inside one tensor): 16 FP64 values per (worker,
+        //  * data record = a SEGMENT (the tiles of one scheduling unit inside one tensor), at most kRecW workers of it
+        //    (wider fan-in: several records per segment): 16 FP64 values per (worker,
         //    statistic), one per consumer warp; a lane per (worker, statistic) sums them in warp order (a fixed shape:
         //    the value depends on the data only) and adds the segment's total EXACTLY to the tensor's accumulator
         //    (integer atomics: the order in which segments arrive, i.e. the dynamic scheduling, cannot change the
