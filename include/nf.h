@@ -90,7 +90,8 @@ int nf_version(void);
 
 /* Bytes of the device "plan" buffer for a bucket of T tensors used with up to R workers / replicas (host
  * call): the route-dependent tile map the streaming kernels walk, per-tensor scratch (scales, completion
- * counters) and R x T exact accumulators of 256 bytes for the per-(replica, tensor) totals. R = the largest
+ * counters), an 8 KB list of decode units handed from one kernel of a step to the next, and R x T exact
+ * accumulators of 256 bytes for the per-(replica, tensor) totals. R = the largest
  * W (or R of nf_health_stats) any call will be given this plan with. 16-byte aligned buffer required. The
  * buffer must be zero-filled ONCE before its first use (cudaMemset / torch.zeros) and not modified by the caller
  * afterwards: the fused call recognises a plan whose state it left clean by a 32-bit token in the header and

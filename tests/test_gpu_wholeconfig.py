@@ -1,7 +1,7 @@
 """`-m gpu` parity of WHOLE configs at BASELINE.json's full sizes, in exactly the buffer arrangement and
-launch sequence `bench.py` times (`ModelBuffers`: every bucket resident in HBM, per-bucket planes and
-accumulators, ONE shared direction workspace, one `nf_aggregate_bucket` per bucket issued back to back on
-one stream with no host synchronisation in between). Two full steps are run before anything is compared, so
+launch sequence `bench.py` times (`ModelBuffers`: every bucket resident in HBM, per-bucket planes,
+accumulators and direction-workspace slices, ONE `nf_aggregate_step` call per step: one fused kernel per bucket,
+chained, on one stream with no host synchronisation in between). Two full steps are run before anything is compared, so
 that what is checked is the steady state (plans, accumulators and workspace reused from the previous step);
 then EVERY bucket of the config is compared with the oracle element by element (planes, abs-sums, decoded and
 FP32-route outputs, scales, health statistics, route codes). PAPER.md L285 / L455-456: zero aggregate-output
