@@ -240,8 +240,12 @@ __device__ __forceinline__ void write_back(const ReduceParams &p, int W, int lan
     // Fast write-back: the warp's 32 words are 1024 consecutive, 16-byte-aligned elements of ONE tensor.
     // Each thread turns its two masks into 8 direction bytes (low nibble +, high nibble -); a byte
     // indexes a shared-memory table of float4 directions, and every store writes 512 contiguous bytes.
+    // (ONE tensor: two low-bit tensors that are adjacent in the bucket, the first a whole number of words long, are
+    // contiguous in `out` too, but each has its own scale)
     const int64_t ob0 = __shfl_sync(0xffffffffu, m.obase, 0);
-    const bool fast = !WRITE_COUNTS && __all_sync(0xffffffffu, m.nvalid == 32 && m.obase == ob0 + 32 * lane) &&
+    const int li0 = __shfl_sync(0xffffffffu, m.li, 0);
+    const bool fast = !WRITE_COUNTS &&
+                      __all_sync(0xffffffffu, m.nvalid == 32 && m.obase == ob0 + 32 * lane && m.li == li0) &&
                       ((ob0 & 3) == 0);
     if (fast) {
         auto spread = [](uint32_t x) {           // 4 nibbles of a 16-bit value -> low nibbles of 4 bytes

@@ -429,3 +429,29 @@ def test_concurrent_calls_on_two_streams_behind_foreign_work(T):
             for k in range(2):
                 compare(bbs[k], refs[k], W, O.MODE_GTERNARY, what=f"concurrent T={T} iteration {it} stream {k}")
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("W", [4, 24])
+def test_adjacent_lowbit_tensors_meeting_inside_a_warp_of_the_count_reduce(W):
+    """Low-bit tensors that are adjacent in the bucket and a whole number of 32-element words long, with word offsets
+    that are not multiples of 32: a warp of nf_sign_count_reduce (32 consecutive word positions) then holds words of
+    two tensors whose elements are contiguous in `out`, and must still give each its own scale (the 512-byte
+    write-back path once took them for one tensor)."""
+    rng = np.random.default_rng(4242 + W)
+    lens = [2080, 4096, 96, 32 * 77, 5000, 32 * 33, 32 * 31, 2048 * 3]
+    off, ln, n = layout(lens)
+    elig = [1, 1, 1, 1, 1, 1, 1, 1]
+    g = (rng.standard_normal((W, n)) * 10 ** rng.uniform(-4, 0, (1, n))).astype(np.float32)
+    for t, (o, l) in enumerate(zip(off, ln)):          # very different scales per tensor
+        g[:, o:o + l] *= 10.0 ** (t - 4)
+    gd = _dev(g)
+    ref = run_both(gd, off, ln, elig, what=f"adjacent low-bit tensors W={W}")
+    # the five calls WITHOUT count outputs: nf_sign_count_reduce then writes back 512 contiguous bytes per store
+    bc = BucketBuffers(off, ln, elig, n, W, gd.device, planes=True, counts=False, health=True)
+    bc.out.fill_(-77.0)
+    bc.route_bucket((1, 0, 1))
+    bc.sign_pack(gd, gd.shape[1], O.MODE_GTERNARY)
+    bc.sign_count_reduce(O.MODE_GTERNARY, 0)
+    bc.fp32_reduce(gd, gd.shape[1], 1.0)
+    bc.health_stats(gd, gd.shape[1])
+    compare(bc, ref, W, O.MODE_GTERNARY, what=f"adjacent low-bit tensors W={W} [5-call, no count outputs]")
