@@ -92,6 +92,20 @@ def run_both(g: torch.Tensor, off, length, elig, state=(1, 0, 1), mode=O.MODE_GT
     bc.fp32_reduce(g, stride, alpha)
     bc.health_stats(g, stride)
     compare(bc, ref, W, mode, check_counts=True, what=what + " [5-call]")
+    # a3 once more WITHOUT count outputs (its 512-byte write-back path): the same bits at every low-bit position,
+    # nothing written elsewhere
+    if ref.route.Wd:
+        out_nc = torch.full_like(bc.out, -123.0)
+        nf.nf_sign_count_reduce(bc.P, bc.N if mode == O.MODE_GTERNARY else None, bc.plane_stride, W, n, bc.off, bc.len,
+                                bc.route, bc.woff, bc.T, mode, margin, bc.abs_sum, out_nc, None, None, None, bc.plan)
+        torch.cuda.synchronize()
+        isL = np.zeros(n, bool)
+        for o, l, r in zip(off, length, ref.route.route):
+            if r == O.ROUTE_L:
+                isL[o:o + l] = True
+        a_nc, b_c = _np(out_nc)[:n], _np(bc.out)[:n]
+        assert np.array_equal(a_nc[isL].view(np.uint32), b_c[isL].view(np.uint32)), what + " a3 without count outputs"
+        assert np.all(a_nc[~isL] == -123.0), what + " a3 without count outputs wrote outside the low-bit tensors"
     # fused == 5-call bit for bit on planes and outputs
     torch.cuda.synchronize()
     if ref.route.Wd:
