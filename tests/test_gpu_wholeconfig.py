@@ -143,13 +143,14 @@ def test_step_with_a_refused_bucket_in_the_middle():
             compare(mb.buckets[i], refs[i], W, O.MODE_GTERNARY, what=f"bucket {i} beside a refused bucket")
 
 
-@pytest.mark.parametrize("seed,W", [(1, 4), (2, 12), (3, 40), (4, 8)])
-def test_random_step_chains_bitwise_equal_to_single_calls(seed, W):
+@pytest.mark.parametrize("seed,W,lean", [(1, 4, False), (2, 12, False), (3, 40, False), (4, 8, False), (5, 8, True), (6, 20, True)])
+def test_random_step_chains_bitwise_equal_to_single_calls(seed, W, lean):
     """Random sequences of buckets through nf_aggregate_step: runs of tiny buckets (kernels of a few CTAs that overlap
     their neighbours, grids of different sizes handing decode units on to each other), large ones, chain breakers
     (T > 256, empty buckets), all-FP32 and all-low-bit buckets, four steps in a row on the same plans. Every output of
     every bucket must be bitwise what a stand-alone nf_aggregate_bucket call produces (itself checked against the
-    oracle elsewhere), after the last step and after the first."""
+    oracle elsewhere), after the last step and after the first. `lean`: G-Binary, no planes, no health statistics (the
+    other template instances of the chained kernel)."""
     from tests.util import layout
     from paper_2606_25759_b200 import BucketBuffers
     rng = np.random.default_rng(9000 + seed)
@@ -179,18 +180,19 @@ def test_random_step_chains_bitwise_equal_to_single_calls(seed, W):
         gd = torch.zeros((W, (max(n, 1) + 3) // 4 * 4), dtype=torch.float32, device=DEV)
         gd[:, :g.shape[1]] = torch.from_numpy(g)
         G.append(gd)
-    names = ("out", "scale", "abs_sum", "sumsq", "nan_cnt", "inf_cnt", "P", "N", "route", "woff", "summary")
+    names = ("out", "scale", "abs_sum", "route", "woff", "summary") + (() if lean else ("sumsq", "nan_cnt", "inf_cnt", "P", "N"))
+    mode = O.MODE_GBINARY if lean else O.MODE_GTERNARY
     ones = []
     for (off, ln, elig, n), g in zip(specs, G):
-        one = BucketBuffers(off, ln, elig, n, W, DEV, planes=True, health=True)
+        one = BucketBuffers(off, ln, elig, n, W, DEV, planes=not lean, health=not lean)
         one.out.fill_(-5.0)
-        one.aggregate(g, g.shape[1])
+        one.aggregate(g, g.shape[1], (1, 0, 1), mode, None, 1 if lean else 0, 1.0)
         ones.append(one)
-    mb = ModelBuffers(specs, W, DEV, planes=True, health=True)
+    mb = ModelBuffers(specs, W, DEV, planes=not lean, health=not lean)
     for step in range(4):
         for bb in mb.buckets:
             bb.out.fill_(-5.0)
-        mb.step(G)
+        mb.step(G, (1, 0, 1), mode, None, 1 if lean else 0, 1.0)
         if step in (0, 3):
             torch.cuda.synchronize()
             for i, (bb, one) in enumerate(zip(mb.buckets, ones)):
